@@ -1,0 +1,166 @@
+// Passes over the ACTIVE balls only (lam_i != 0), driven by the compacted ascending index list
+// (SURVEY 8(a) rows a1 vector part, a2, a6).  Only active rows contribute to sum_i v+_i and to
+// sum_i P_i q, so these kernels touch |A| rows, not m.
+//
+//   MODE_ROWSUM   sum_k lam_k b_k                      -> gradient, P:L111 / L232
+//   MODE_HVP      sum_{B3} coef_k b_k, sum_{B3} w_k^T q1   -> H q, P:L214-216 (P_i: reading 1)
+//   MODE_WRITEV   v_k <- sigma lam_k b_k, u_i <- sigma t_i, slot_i <- k   -> eq. (6)
+//
+// A TEAM of threads (one warp, or the whole CTA for long rows) owns a list entry; thread t of the
+// team owns columns t, t+TEAM, ... and accumulates them in its own slice of shared memory, so there
+// are no atomics and the summation order is fixed: entries k = team, team + nteams, ... in order,
+// then teams of a CTA in order, then CTAs in order (finalize kernels in meb_small.cu).
+#include "meb_internal.cuh"
+
+namespace {
+
+template <int TEAM>
+__device__ __forceinline__ double team_sum(double v, double* scratch) {
+    v = warp_sum(v);
+    if (TEAM == 32) return v;
+    // whole CTA: combine the warps in index order
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) scratch[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < MEB_WARPS; ++w) t += scratch[w];
+    return t;
+}
+
+template <typename T, int TEAM, int MODE>
+__global__ void __launch_bounds__(MEB_BLOCK) active_kernel(const ActiveArgs a) {
+    extern __shared__ __align__(16) double acc_s[];          // [teams_per_block][dpad]
+    __shared__ double scratch[MEB_WARPS];
+    __shared__ double sc_red[MEB_WARPS];
+    constexpr int TPB = MEB_BLOCK / TEAM;
+    const int team = threadIdx.x / TEAM, tt = threadIdx.x % TEAM;
+    const int d = a.d;
+    double* acc = acc_s + (size_t)team * a.dpad;
+    if (MODE != MODE_WRITEV)
+        for (int j = tt; j < a.dpad; j += TEAM) acc[j] = 0.0;
+    const T* __restrict__ C = static_cast<const T*>(a.C);
+    const T* __restrict__ V = static_cast<const T*>(a.V);
+    const double* __restrict__ cx = a.x + 1;
+    const T inv_sig = T(1) / (T)a.sigma;
+    const int n = *a.count;
+    const int nteams = gridDim.x * TPB;
+    double sc = 0.0;                                         // scalar partial (one per team, in thread 0)
+    for (int k = blockIdx.x * TPB + team; k < n; k += nteams) {
+        const int i = a.list[k];
+        const T* rowp = C + (int64_t)i * a.ld;
+        const int slot = a.v_slot ? a.v_slot[i] : -1;
+        const T* vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
+        if (MODE == MODE_ROWSUM) {
+            const double lam = a.rec_lam[i];
+            for (int j = tt; j < d; j += TEAM) {
+                T b = rowp[j] - (T)cx[j];
+                if (vrow) b = fma(vrow[j], inv_sig, b);
+                acc[j] = fma(lam, (double)b, acc[j]);
+            }
+        } else if (MODE == MODE_HVP) {
+            const double rho = a.rec_rho[i];
+            if (rho > 1.5) continue;                          // B1: P_i = I, handled in the finalize
+            double dot = 0.0, nb2 = 0.0;
+            for (int j = tt; j < d; j += TEAM) {
+                T b = rowp[j] - (T)cx[j];
+                if (vrow) b = fma(vrow[j], inv_sig, b);
+                const double bd = (double)b;
+                dot = fma(bd, a.q[1 + j], dot);
+                nb2 = fma(bd, bd, nb2);
+            }
+            dot = team_sum<TEAM>(dot, scratch);
+            nb2 = team_sum<TEAM>(nb2, scratch);
+            const double nb = sqrt(nb2);
+            const double wq = dot / nb;                       // w_i^T q1
+            const double coef = (a.q[0] - rho * wq) / nb;     // (P_i q)_1 = 1/2 (coef b + (1+rho) q1)
+            for (int j = tt; j < d; j += TEAM) {
+                T b = rowp[j] - (T)cx[j];
+                if (vrow) b = fma(vrow[j], inv_sig, b);
+                acc[j] = fma(coef, (double)b, acc[j]);
+            }
+            if (tt == 0) sc += wq;
+        } else {  // MODE_WRITEV
+            const double lam = a.rec_lam[i], t = a.rec_t[i];
+            const T sl = (T)(a.sigma * lam);
+            T* vout = static_cast<T*>(a.V_out) + (int64_t)k * a.ldv_out;
+            const bool store = k < a.cap_rows;
+            double nb2 = 0.0;
+            for (int j = tt; j < d; j += TEAM) {
+                T b = rowp[j] - (T)cx[j];
+                if (vrow) b = fma(vrow[j], inv_sig, b);
+                const T vp = sl * b;
+                if (store) vout[j] = vp;
+                nb2 = fma((double)vp, (double)vp, nb2);
+            }
+            nb2 = team_sum<TEAM>(nb2, scratch);
+            if (tt == 0) {
+                const T up = (T)a.sigma * (T)t;
+                static_cast<T*>(a.U_out)[i] = up;
+                a.slot_out[i] = store ? k : -1;
+                sc += (double)up * (double)up + nb2;
+            }
+        }
+    }
+    // ---- CTA partials, fixed order ----
+    __syncthreads();
+    if (MODE != MODE_WRITEV) {
+        double* pv = a.part_vec + (size_t)blockIdx.x * a.dpad;
+        for (int j = threadIdx.x; j < d; j += MEB_BLOCK) {
+            double s = 0.0;
+#pragma unroll
+            for (int tm = 0; tm < TPB; ++tm) s += acc_s[(size_t)tm * a.dpad + j];
+            pv[j] = s;
+        }
+    }
+    // scalar partial: teams in order
+    if (TEAM == 32) {
+        if (tt == 0) sc_red[team] = sc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s = 0.0;
+            for (int tm = 0; tm < TPB; ++tm) s += sc_red[tm];
+            a.part_sc[blockIdx.x] = s;
+        }
+    } else if (threadIdx.x == 0) {
+        a.part_sc[blockIdx.x] = sc;
+    }
+}
+
+template <typename T, int MODE>
+int launch_active_t(meb_ctx* ctx, const ActiveArgs& a, int* grid_out) {
+    const bool wide = a.d > 2048;
+    const int tpb = wide ? 1 : MEB_WARPS;
+    const size_t smem = (MODE == MODE_WRITEV) ? 0 : (size_t)tpb * a.dpad * sizeof(double);
+    if (smem > 220 * 1024) return MEB_E_CAPACITY;
+    int grid = ctx->sm_count * (smem > 100 * 1024 ? 1 : 2);
+    if ((int64_t)grid > ctx->vec_rows) grid = (int)ctx->vec_rows;
+    cudaError_t e;
+    if (wide) {
+        auto kern = active_kernel<T, MEB_BLOCK, MODE>;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a);
+    } else {
+        auto kern = active_kernel<T, 32, MODE>;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
+    *grid_out = grid;
+    return MEB_OK;
+}
+
+}  // namespace
+
+int meb_launch_active(meb_ctx* ctx, int mode, int prec, const ActiveArgs& a, int* grid_out) {
+    if (prec == MEB_FP64) {
+        if (mode == MODE_ROWSUM) return launch_active_t<double, MODE_ROWSUM>(ctx, a, grid_out);
+        if (mode == MODE_HVP) return launch_active_t<double, MODE_HVP>(ctx, a, grid_out);
+        return launch_active_t<double, MODE_WRITEV>(ctx, a, grid_out);
+    }
+    if (mode == MODE_ROWSUM) return launch_active_t<float, MODE_ROWSUM>(ctx, a, grid_out);
+    if (mode == MODE_HVP) return launch_active_t<float, MODE_HVP>(ctx, a, grid_out);
+    return launch_active_t<float, MODE_WRITEV>(ctx, a, grid_out);
+}

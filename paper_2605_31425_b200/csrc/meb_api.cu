@@ -1,0 +1,396 @@
+// C-ABI entry points of libmeb_b200.so: context management and the per-primitive calls of
+// include/meb.h.  Argument checking and launch sequencing only; all arithmetic is in the kernels.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "meb_internal.cuh"
+
+// layout of ctx->small (doubles)
+#define SM_EV 0          // [16] evaluation scalars scratch
+#define SM_AUX 16        // [16] argmax / sums scratch
+#define SM_X 32          // [d_max+1] assembled x = (r, c)
+
+static size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static void ctx_free_all(meb_ctx* c) {
+    if (!c) return;
+    cudaFree(c->mask); cudaFree(c->rec_lam); cudaFree(c->rec_rho); cudaFree(c->rec_t);
+    cudaFree(c->list); cudaFree(c->blocksum); cudaFree(c->part_scalar); cudaFree(c->part_vec);
+    cudaFree(c->part_mat); cudaFree(c->count_dev); cudaFree(c->part_sc); cudaFree(c->small);
+    if (c->h_pinned) cudaFreeHost(c->h_pinned);
+    for (int i = 0; i < 16; ++i) if (c->own[i]) cudaFree(c->own[i]);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+}
+
+extern "C" int meb_version(void) { return 100; }
+
+extern "C" const char* meb_strerror(int code) {
+    switch (code) {
+        case MEB_OK: return "ok";
+        case MEB_W_NOT_CONVERGED: return "iteration cap reached; outputs hold the best iterate";
+        case MEB_E_ARG: return "invalid argument";
+        case MEB_E_INPUT: return "non-finite data or negative radius";
+        case MEB_E_ALLOC: return "allocation failed";
+        case MEB_E_CUDA: return "CUDA error (see meb_last_cuda_error)";
+        case MEB_E_CAPACITY: return "capacity exceeded";
+        default: return "unknown code";
+    }
+}
+
+extern "C" void meb_default_params(meb_params* p) {
+    if (!p) return;
+    memset(p, 0, sizeof(*p));
+    p->rho = 0.5; p->sigma0 = 1.0; p->kappa = 3.0; p->sigma_max = 1e8; p->tau = 1.0;
+    p->armijo_mu = 1e-4; p->tol_lo = 1e-2; p->tol_red_factor = 0.02;
+    p->armijo_max_halvings = 30; p->cg_max = 500; p->dense_d_max = 128; p->inner_max = 50;
+    p->outer_max = 200; p->max_rounds = 10; p->sample_rows = 1024;
+}
+
+extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t m_max, int32_t d_max) {
+    if (!out || m_max < 1 || d_max < 1 || m_max >= 2147483647LL - 64) return MEB_E_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return MEB_E_CUDA;
+    meb_ctx* c = new (std::nothrow) meb_ctx();
+    if (!c) return MEB_E_ALLOC;
+    memset(c, 0, sizeof(*c));
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->m_max = m_max;
+    c->d_max = d_max;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    const size_t nwords = (size_t)(m_max + 31) / 32 + 8;
+    const size_t nseg = nwords / 2048 + 8;
+    const size_t dpad = round_up((size_t)d_max + 1, 8);
+    c->vec_rows = 2 * (int64_t)(c->sm_count > 0 ? c->sm_count : 148);
+    c->small_len = SM_X + (int64_t)dpad + 64;
+    c->h_pinned_len = 4 * (int64_t)dpad + 256;
+#define TRY_ALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void**)&(ptr), (bytes))
+    TRY_ALLOC(c->mask, nwords * sizeof(uint32_t));
+    TRY_ALLOC(c->rec_lam, (size_t)m_max * sizeof(double));
+    TRY_ALLOC(c->rec_rho, (size_t)m_max * sizeof(double));
+    TRY_ALLOC(c->rec_t, (size_t)m_max * sizeof(double));
+    TRY_ALLOC(c->list, ((size_t)m_max + 32) * sizeof(int32_t));
+    TRY_ALLOC(c->blocksum, nseg * sizeof(int32_t));
+    TRY_ALLOC(c->part_scalar, (size_t)MEB_MAX_GRID * MEB_NPART * sizeof(double));
+    TRY_ALLOC(c->part_vec, (size_t)c->vec_rows * dpad * sizeof(double));
+    {
+        const size_t dpm = (size_t)((d_max < 128 ? d_max : 128) + 15) / 16 * 16;
+        c->part_mat_len = (size_t)c->vec_rows * (dpm * dpm + dpm);
+    }
+    TRY_ALLOC(c->part_mat, c->part_mat_len * sizeof(double));
+    TRY_ALLOC(c->count_dev, 8 * sizeof(int32_t));
+    TRY_ALLOC(c->part_sc, 1024 * sizeof(double));
+    TRY_ALLOC(c->small, (size_t)c->small_len * sizeof(double));
+#undef TRY_ALLOC
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_pinned, (size_t)c->h_pinned_len * sizeof(double));
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->count_dev, 0, 8 * sizeof(int32_t), c->stream);
+    if (e != cudaSuccess) {
+        const bool oom = (e == cudaErrorMemoryAllocation);
+        ctx_free_all(c);
+        delete c;
+        cudaGetLastError();
+        return oom ? MEB_E_ALLOC : MEB_E_CUDA;
+    }
+    *out = c;
+    return MEB_OK;
+}
+
+extern "C" int meb_destroy(meb_ctx* ctx) {
+    if (!ctx) return MEB_E_ARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    ctx_free_all(ctx);
+    delete ctx;
+    return MEB_OK;
+}
+
+extern "C" int meb_last_cuda_error(const meb_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
+
+extern "C" int meb_set_pass_timing(meb_ctx* ctx, int on) {
+    if (!ctx) return MEB_E_ARG;
+    ctx->time_passes = on != 0;
+    return MEB_OK;
+}
+
+extern "C" int meb_last_pass_info(const meb_ctx* ctx, double* h_ms, double* h_bytes) {
+    if (!ctx) return MEB_E_ARG;
+    if (h_ms) *h_ms = ctx->last_pass_ms;
+    if (h_bytes) *h_bytes = ctx->last_pass_bytes;
+    return MEB_OK;
+}
+
+static int check_problem(const meb_ctx* ctx, int64_t m, int32_t d, const void* C, int64_t ld) {
+    if (!ctx || !C || m < 1 || d < 1 || ld < d) return MEB_E_ARG;
+    if (m > ctx->m_max || d > ctx->d_max) return MEB_E_CAPACITY;
+    return MEB_OK;
+}
+
+// one streaming launch, optionally timed with CUDA events on the context's stream
+static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid) {
+    if (ctx->time_passes) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+    int rc = meb_launch_stream(ctx, op, prec, a, grid);
+    if (rc != MEB_OK) return rc;
+    ctx->last_grid = *grid;
+    ctx->last_pass_bytes = bytes;
+    if (ctx->time_passes) {
+        MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaEventSynchronize(ctx->ev1));
+        float ms = 0.f;
+        MEB_CUDA_OK(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+        ctx->last_pass_ms = ms;
+    }
+    return MEB_OK;
+}
+
+static ActiveArgs active_args(meb_ctx* ctx, const EvalCall& c) {
+    ActiveArgs a;
+    memset(&a, 0, sizeof(a));
+    a.C = c.C; a.ld = c.ld; a.U = c.U; a.v_slot = c.v_slot; a.V = c.V; a.ldv = c.ldv;
+    a.x = c.x; a.d = c.d; a.dpad = (int32_t)round_up((size_t)c.d, 8); a.sigma = c.sigma;
+    a.list = ctx->list; a.count = ctx->count_dev;
+    a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
+    a.part_vec = ctx->part_vec; a.part_sc = ctx->part_sc;
+    return a;
+}
+
+int meb_grad_from_records(meb_ctx* ctx, const EvalCall& c, double* out_scalars, double* grad) {
+    ActiveArgs a = active_args(ctx, c);
+    int nvec = 0;
+    int rc = meb_launch_active(ctx, MODE_ROWSUM, c.prec, a, &nvec);
+    if (rc != MEB_OK) return rc;
+    return meb_eval_finalize(ctx, ctx->last_grid, nvec, a.dpad, ctx->count_dev, c.x, c.xbar, c.sigma, c.tau,
+                             c.d, out_scalars, grad);
+}
+
+int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, bool want_grad, double* out_scalars, double* grad,
+                      double* t_out, double* lam_out) {
+    StreamArgs s;
+    memset(&s, 0, sizeof(s));
+    s.C = c.C; s.ld = c.ld; s.R = c.R; s.U = c.U; s.v_slot = c.v_slot; s.V = c.V; s.ldv = c.ldv;
+    s.x = c.x; s.m = c.m; s.d = c.d; s.sigma = c.sigma;
+    s.mask = ctx->mask; s.rec_lam = ctx->rec_lam; s.rec_rho = ctx->rec_rho; s.rec_t = ctx->rec_t;
+    s.t_out = t_out; s.lam_out = lam_out; s.part = ctx->part_scalar;
+    const double sz = c.prec == MEB_FP64 ? 8.0 : 4.0;
+    const double bytes = (double)c.m * (c.d * sz + (c.R ? sz : 0) + (c.U ? sz : 0) + (c.v_slot ? 4 : 0));
+    int grid = 0;
+    int rc = timed_stream(ctx, OP_EVAL, c.prec, s, bytes, &grid);
+    if (rc != MEB_OK) return rc;
+    rc = meb_launch_compact(ctx, ctx->mask, c.m, ctx->list, ctx->count_dev);
+    if (rc != MEB_OK) return rc;
+    if (want_grad) return meb_grad_from_records(ctx, c, out_scalars, grad);
+    return meb_eval_finalize(ctx, grid, 0, (int)round_up((size_t)c.d, 8), ctx->count_dev, c.x, c.xbar, c.sigma,
+                             c.tau, c.d, out_scalars, grad);
+}
+
+int meb_hvp_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, const double* q,
+                         double* Hq) {
+    ActiveArgs a = active_args(ctx, c);
+    a.q = q;
+    int nvec = 0;
+    int rc = meb_launch_active(ctx, MODE_HVP, c.prec, a, &nvec);
+    if (rc != MEB_OK) return rc;
+    return meb_hvp_finalize(ctx, nvec, a.dpad, ctx->part_sc, ev_scalars, q, c.sigma, c.tau, c.d, Hq);
+}
+
+static int check_eval_args(const meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
+                           const int32_t* v_slot, const void* V, int64_t ldv, const double* x, double sigma) {
+    int rc = check_problem(ctx, m, d, C, ld);
+    if (rc != MEB_OK) return rc;
+    if ((prec != MEB_FP64 && prec != MEB_FP32) || !x || !(sigma > 0.0)) return MEB_E_ARG;
+    if (v_slot && (!V || ldv < d)) return MEB_E_ARG;
+    return MEB_OK;
+}
+
+extern "C" int meb_eval_alm(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
+                            const void* R, const void* U, const int32_t* v_slot, const void* Vrows,
+                            int64_t ldv, const double* x, const double* xbar, double sigma, double tau,
+                            double* out_scalars, double* grad, double* t_out, double* lam_out,
+                            int32_t* active_idx, double* active_rho, double* active_lam) {
+    int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
+    if (rc != MEB_OK) return rc;
+    if (!out_scalars || !grad || !(tau >= 0.0)) return MEB_E_ARG;
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, xbar, sigma, tau};
+    rc = meb_eval_internal(ctx, c, true, out_scalars, grad, t_out, lam_out);
+    if (rc != MEB_OK) return rc;
+    if (active_idx) {
+        MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->count_dev, sizeof(int32_t),
+                                         cudaMemcpyDeviceToHost, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+        const int64_t n = *(int32_t*)ctx->h_pinned;
+        if (n > 0) {
+            MEB_CUDA_OK(ctx, cudaMemcpyAsync(active_idx, ctx->list, n * sizeof(int32_t),
+                                             cudaMemcpyDeviceToDevice, ctx->stream));
+            if (active_rho) { rc = meb_gather_vec_f64(ctx, ctx->rec_rho, ctx->list, n, active_rho); if (rc) return rc; }
+            if (active_lam) { rc = meb_gather_vec_f64(ctx, ctx->rec_lam, ctx->list, n, active_lam); if (rc) return rc; }
+        }
+    }
+    return MEB_OK;
+}
+
+extern "C" int meb_hvp(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
+                       const void* R, const void* U, const int32_t* v_slot, const void* Vrows, int64_t ldv,
+                       const double* x, double sigma, double tau, const double* q, double* Hq) {
+    int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
+    if (rc != MEB_OK) return rc;
+    if (!q || !Hq || !(tau >= 0.0)) return MEB_E_ARG;
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, tau};
+    double* ev = ctx->small + SM_EV;
+    rc = meb_eval_internal(ctx, c, false, ev, ctx->small + SM_X, nullptr, nullptr);
+    if (rc != MEB_OK) return rc;
+    return meb_hvp_from_records(ctx, c, ev, q, Hq);
+}
+
+extern "C" int meb_dense_hessian(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
+                                 const void* R, const void* U, const int32_t* v_slot, const void* Vrows,
+                                 int64_t ldv, const double* x, double sigma, double tau, double* H) {
+    int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
+    if (rc != MEB_OK) return rc;
+    if (!H || !(tau >= 0.0)) return MEB_E_ARG;
+    if (d > 128) return MEB_E_CAPACITY;
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, tau};
+    double* ev = ctx->small + SM_EV;
+    rc = meb_eval_internal(ctx, c, false, ev, ctx->small + SM_X, nullptr, nullptr);
+    if (rc != MEB_OK) return rc;
+    return meb_dense_from_records(ctx, c, ev, H);
+}
+
+extern "C" int meb_update_multipliers(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C,
+                                      int64_t ld, const void* R, const void* U, const int32_t* v_slot,
+                                      const void* Vrows, int64_t ldv, const double* x, double sigma,
+                                      void* U_out, int32_t* v_slot_out, void* Vrows_out, int64_t ldv_out,
+                                      int64_t cap_rows, int64_t* h_n_slots, double* h_sum_mult2) {
+    int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
+    if (rc != MEB_OK) return rc;
+    if (!U_out || !v_slot_out || !Vrows_out || ldv_out < d || cap_rows < 0) return MEB_E_ARG;
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, 0.0};
+    rc = meb_eval_internal(ctx, c, false, ctx->small + SM_EV, ctx->small + SM_X, nullptr, nullptr);
+    if (rc != MEB_OK) return rc;
+    if (prec == MEB_FP64) rc = meb_fill_f64(ctx, (double*)U_out, m, 0.0);
+    else rc = meb_fill_f32(ctx, (float*)U_out, m, 0.f);
+    if (rc != MEB_OK) return rc;
+    rc = meb_fill_i32(ctx, v_slot_out, m, -1);
+    if (rc != MEB_OK) return rc;
+    ActiveArgs a = active_args(ctx, c);
+    a.U_out = U_out; a.slot_out = v_slot_out; a.V_out = Vrows_out; a.ldv_out = ldv_out; a.cap_rows = cap_rows;
+    int nvec = 0;
+    rc = meb_launch_active(ctx, MODE_WRITEV, prec, a, &nvec);
+    if (rc != MEB_OK) return rc;
+    rc = meb_scalar_sum(ctx, ctx->part_sc, nvec, ctx->small + SM_AUX);
+    if (rc != MEB_OK) return rc;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_AUX, sizeof(double), cudaMemcpyDeviceToHost,
+                                     ctx->stream));
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 1, ctx->count_dev, sizeof(int32_t), cudaMemcpyDeviceToHost,
+                                     ctx->stream));
+    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    const int64_t n = *(int32_t*)(ctx->h_pinned + 1);
+    if (h_n_slots) *h_n_slots = n;
+    if (h_sum_mult2) *h_sum_mult2 = ctx->h_pinned[0];
+    return n > cap_rows ? MEB_E_CAPACITY : MEB_OK;
+}
+
+// x = (r, c) assembled on the device from a host scalar and a device vector
+static int assemble_x(meb_ctx* ctx, double r, const double* c, int32_t d) {
+    ctx->h_pinned[8] = r;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->small + SM_X, ctx->h_pinned + 8, sizeof(double), cudaMemcpyHostToDevice,
+                                     ctx->stream));
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->small + SM_X + 1, c, (size_t)d * sizeof(double),
+                                     cudaMemcpyDeviceToDevice, ctx->stream));
+    return MEB_OK;
+}
+
+extern "C" int meb_screen_compact(meb_ctx* ctx, int64_t m, int32_t d, const float* C32, int64_t ld32,
+                                  const float* R32, float r_hat, const double* c_hat, float tol_red,
+                                  int32_t* idx_out, int64_t cap, int64_t* h_count, uint8_t* flags,
+                                  int flags_are_input) {
+    if (!ctx || !idx_out || cap < 0 || m < 1 || m > ctx->m_max) return MEB_E_ARG;
+    int rc;
+    if (flags_are_input) {
+        if (!flags) return MEB_E_ARG;
+        rc = meb_launch_flags_to_mask(ctx, flags, m, ctx->mask);
+        if (rc != MEB_OK) return rc;
+    } else {
+        rc = check_problem(ctx, m, d, C32, ld32);
+        if (rc != MEB_OK) return rc;
+        if (!c_hat) return MEB_E_ARG;
+        rc = assemble_x(ctx, (double)r_hat, c_hat, d);
+        if (rc != MEB_OK) return rc;
+        StreamArgs s;
+        memset(&s, 0, sizeof(s));
+        s.C = C32; s.ld = ld32; s.R = R32; s.x = ctx->small + SM_X; s.m = m; s.d = d; s.sigma = 1.0;
+        s.mask = ctx->mask; s.part = ctx->part_scalar; s.eps = (double)tol_red; s.flags_out = flags;
+        int grid = 0;
+        rc = timed_stream(ctx, OP_SCREEN, MEB_FP32, s, (double)m * (d * 4.0 + (R32 ? 4 : 0)), &grid);
+        if (rc != MEB_OK) return rc;
+    }
+    rc = meb_launch_compact_cap(ctx, ctx->mask, m, idx_out, cap, ctx->count_dev);
+    if (rc != MEB_OK) return rc;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->count_dev, sizeof(int32_t), cudaMemcpyDeviceToHost,
+                                     ctx->stream));
+    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    const int64_t n = *(int32_t*)ctx->h_pinned;
+    if (h_count) *h_count = n;
+    return n > cap ? MEB_E_CAPACITY : MEB_OK;
+}
+
+extern "C" int meb_feasibility_check(meb_ctx* ctx, int64_t m, int32_t d, const double* C, int64_t ld,
+                                     const double* R, double r, const double* c, double eps_feas,
+                                     const uint8_t* kept_mask, double* h_delta_max, int32_t* h_argmax,
+                                     int32_t* viol_idx, int64_t cap, int64_t* h_n_viol) {
+    int rc = check_problem(ctx, m, d, C, ld);
+    if (rc != MEB_OK) return rc;
+    if (!c || cap < 0 || (cap > 0 && !viol_idx)) return MEB_E_ARG;
+    rc = assemble_x(ctx, r, c, d);
+    if (rc != MEB_OK) return rc;
+    StreamArgs s;
+    memset(&s, 0, sizeof(s));
+    s.C = C; s.ld = ld; s.R = R; s.x = ctx->small + SM_X; s.m = m; s.d = d; s.sigma = 1.0;
+    s.mask = ctx->mask; s.part = ctx->part_scalar; s.eps = eps_feas; s.kept = kept_mask;
+    int grid = 0;
+    rc = timed_stream(ctx, OP_FEAS, MEB_FP64, s, (double)m * (d * 8.0 + (R ? 8 : 0) + (kept_mask ? 1 : 0)), &grid);
+    if (rc != MEB_OK) return rc;
+    rc = meb_argmax_finalize(ctx, grid, ctx->small + SM_AUX);
+    if (rc != MEB_OK) return rc;
+    rc = meb_launch_compact_cap(ctx, ctx->mask, m, viol_idx ? viol_idx : ctx->list, viol_idx ? cap : 0,
+                                ctx->count_dev);
+    if (rc != MEB_OK) return rc;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_AUX, 2 * sizeof(double),
+                                     cudaMemcpyDeviceToHost, ctx->stream));
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 2, ctx->count_dev, sizeof(int32_t), cudaMemcpyDeviceToHost,
+                                     ctx->stream));
+    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    if (h_delta_max) *h_delta_max = ctx->h_pinned[0];
+    if (h_argmax) *h_argmax = (int32_t)ctx->h_pinned[1];
+    const int64_t n = *(int32_t*)(ctx->h_pinned + 2);
+    if (h_n_viol) *h_n_viol = n;
+    return (viol_idx && n > cap) ? MEB_E_CAPACITY : MEB_OK;
+}
+
+extern "C" int meb_ingest(meb_ctx* ctx, int64_t m, int32_t d, const double* C, int64_t ld, const double* R,
+                          int32_t sample_rows, double* c0_out, double* scalars_out, float* C32, int64_t ld32,
+                          float* R32) {
+    int rc = check_problem(ctx, m, d, C, ld);
+    if (rc != MEB_OK) return rc;
+    if (!c0_out || !scalars_out || sample_rows < 1) return MEB_E_ARG;
+    if (C32 && (ld32 < d || ld32 % 4 != 0)) return MEB_E_ARG;
+    const int S = (int)(m < sample_rows ? m : sample_rows);
+    rc = meb_sample_mean(ctx, C, ld, m, d, S, c0_out);
+    if (rc != MEB_OK) return rc;
+    StreamArgs s;
+    memset(&s, 0, sizeof(s));
+    s.C = C; s.ld = ld; s.R = R; s.x = nullptr; s.c0 = c0_out; s.m = m; s.d = d; s.sigma = 1.0;
+    s.part = ctx->part_scalar; s.C32 = C32; s.ld32 = ld32; s.R32 = (C32 && R) ? R32 : nullptr;
+    int grid = 0;
+    const double bytes = (double)m * (d * 8.0 + (R ? 8 : 0)) + (C32 ? (double)m * (d * 4.0 + (R ? 4 : 0)) : 0.0);
+    rc = timed_stream(ctx, OP_INGEST, MEB_FP64, s, bytes, &grid);
+    if (rc != MEB_OK) return rc;
+    return meb_argmax_finalize(ctx, grid, scalars_out);
+}

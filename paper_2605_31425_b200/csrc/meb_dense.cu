@@ -1,0 +1,239 @@
+// Dense generalized Hessian for moderate d (SURVEY 8(a) rows a2', a3) and its Cholesky solve.
+//
+//   H = (tau/sigma) I + sigma [ n1 I + 1/2 [[n3, s^T],[s, (n3 + sum rho) I - sum_{B3} rho_i w_i w_i^T]] ]
+//   with w_i = b_i/||b_i||, s = sum_{B3} w_i        (P:L187 with P_i of reading 1).
+//
+// The data-dependent part is a weighted SYRK over the ACTIVE B3 rows with SIGNED weights rho_i in
+// (-1, 1).  It is FP64 and d <= 128, so it runs on the FP64 pipes: 16 x 16 threads, each owning a
+// BS x BS register block of the d x d accumulator (interleaved ownership: conflict-free shared
+// loads), fed from a shared tile of RB normalised rows.  Static list partition + fixed-order
+// combination of the per-CTA partial matrices: deterministic.
+#include <string.h>
+
+#include "meb_internal.cuh"
+
+namespace {
+
+constexpr int RB = 16;      // rows per shared tile
+
+template <typename T, int BS>
+__global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a, double* __restrict__ part_mat,
+                                                          int dp) {
+    extern __shared__ __align__(16) double sm[];          // W[RB][dp] then rho[RB]
+    double* W = sm;
+    double* rho_s = sm + (size_t)RB * dp;
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int d = a.d;
+    const T* __restrict__ C = static_cast<const T*>(a.C);
+    const T* __restrict__ V = static_cast<const T*>(a.V);
+    const double* __restrict__ cx = a.x + 1;
+    const T inv_sig = T(1) / (T)a.sigma;
+    const int n = *a.count;
+    double acc[BS][BS];
+    double accs[BS];
+#pragma unroll
+    for (int i = 0; i < BS; ++i) {
+        accs[i] = 0.0;
+#pragma unroll
+        for (int j = 0; j < BS; ++j) acc[i][j] = 0.0;
+    }
+    // tiles of RB consecutive list entries, tile t -> CTA t mod grid
+    for (int k0 = blockIdx.x * RB; k0 < n; k0 += gridDim.x * RB) {
+        __syncthreads();
+        // each warp fills RB / 8 = 2 rows of the tile
+        for (int rr = warp; rr < RB; rr += MEB_WARPS) {
+            const int k = k0 + rr;
+            double rho = 0.0;
+            bool use = false;
+            int i = 0;
+            if (k < n) { i = a.list[k]; rho = a.rec_rho[i]; use = rho < 1.5; }   // B1 rows: P_i = I, no SYRK term
+            double nb2 = 0.0;
+            if (use) {
+                const T* rowp = C + (int64_t)i * a.ld;
+                const int slot = a.v_slot ? a.v_slot[i] : -1;
+                const T* vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
+                for (int j = lane; j < dp; j += 32) {
+                    double bd = 0.0;
+                    if (j < d) {
+                        T b = rowp[j] - (T)cx[j];
+                        if (vrow) b = fma(vrow[j], inv_sig, b);
+                        bd = (double)b;
+                    }
+                    W[(size_t)rr * dp + j] = bd;
+                    nb2 = fma(bd, bd, nb2);
+                }
+                nb2 = warp_sum(nb2);
+                const double inv = 1.0 / sqrt(nb2);
+                for (int j = lane; j < dp; j += 32) W[(size_t)rr * dp + j] *= inv;
+            } else {
+                for (int j = lane; j < dp; j += 32) W[(size_t)rr * dp + j] = 0.0;
+            }
+            if (lane == 0) rho_s[rr] = use ? rho : 0.0;
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int rr = 0; rr < RB; ++rr) {
+            const double rho = rho_s[rr];
+            const double* w = W + (size_t)rr * dp;
+            double wq[BS], wp[BS];
+#pragma unroll
+            for (int j = 0; j < BS; ++j) wq[j] = w[tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < BS; ++i) wp[i] = rho * w[ty + 16 * i];
+#pragma unroll
+            for (int i = 0; i < BS; ++i)
+#pragma unroll
+                for (int j = 0; j < BS; ++j) acc[i][j] = fma(wp[i], wq[j], acc[i][j]);
+            if (ty == 0) {
+#pragma unroll
+                for (int j = 0; j < BS; ++j) accs[j] += wq[j];
+            }
+        }
+    }
+    // per-CTA partial: [dp*dp] matrix then [dp] vector
+    double* pm = part_mat + (size_t)blockIdx.x * ((size_t)dp * dp + dp);
+#pragma unroll
+    for (int i = 0; i < BS; ++i)
+#pragma unroll
+        for (int j = 0; j < BS; ++j) pm[(size_t)(ty + 16 * i) * dp + tx + 16 * j] = acc[i][j];
+    if (ty == 0) {
+#pragma unroll
+        for (int j = 0; j < BS; ++j) pm[(size_t)dp * dp + tx + 16 * j] = accs[j];
+    }
+}
+
+__global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __restrict__ part_mat, int nparts,
+                                                             int dp, int d, const double* __restrict__ ev,
+                                                             double sigma, double tau, double* __restrict__ H) {
+    const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
+    const double tos = tau / sigma;
+    const int n = d + 1;
+    const size_t stride = (size_t)dp * dp + dp;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n * n; e += gridDim.x * blockDim.x) {
+        const int p = e / n, q = e % n;
+        double v;
+        if (p == 0 && q == 0) {
+            v = tos + sigma * (n1 + 0.5 * n3);
+        } else if (p == 0 || q == 0) {
+            const int j = (p == 0 ? q : p) - 1;
+            double s = 0.0;
+            for (int b = 0; b < nparts; ++b) s += part_mat[b * stride + (size_t)dp * dp + j];
+            v = 0.5 * sigma * s;
+        } else {
+            double s = 0.0;
+            for (int b = 0; b < nparts; ++b) s += part_mat[b * stride + (size_t)(p - 1) * dp + (q - 1)];
+            v = -0.5 * sigma * s;
+            if (p == q) v += tos + sigma * (n1 + 0.5 * (n3 + srho));
+        }
+        H[(size_t)p * n + q] = v;
+    }
+}
+
+// Solve (scale * H) delta = -g for one SPD matrix of order n <= 257 held in shared memory
+// (right-looking Cholesky, then the two triangular solves).  One CTA.
+__global__ void __launch_bounds__(256) chol_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
+                                                         int n, double scale, double* __restrict__ delta,
+                                                         int* __restrict__ info) {
+    extern __shared__ __align__(16) double A[];           // n*n + n
+    double* y = A + (size_t)n * n;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (int e = tid; e < n * n; e += nt) A[e] = scale * H[e];
+    for (int e = tid; e < n; e += nt) y[e] = -g[e];
+    __shared__ int bad;
+    if (tid == 0) bad = 0;
+    __syncthreads();
+    for (int k = 0; k < n; ++k) {
+        if (tid == 0) {
+            const double dkk = A[(size_t)k * n + k];
+            if (!(dkk > 0.0)) { bad = k + 1; A[(size_t)k * n + k] = 1.0; }
+            else A[(size_t)k * n + k] = sqrt(dkk);
+        }
+        __syncthreads();
+        const double lkk = A[(size_t)k * n + k];
+        for (int i = k + 1 + tid; i < n; i += nt) A[(size_t)i * n + k] /= lkk;
+        __syncthreads();
+        // trailing update: A[i][j] -= L[i][k] L[j][k], j <= i
+        const int rem = n - k - 1;
+        for (int e = tid; e < rem * rem; e += nt) {
+            const int i = k + 1 + e / rem, j = k + 1 + e % rem;
+            if (j <= i) A[(size_t)i * n + j] -= A[(size_t)i * n + k] * A[(size_t)j * n + k];
+        }
+        __syncthreads();
+    }
+    // forward substitution L y = rhs, then L^T x = y (one warp; n is small)
+    if (tid < 32) {
+        for (int i = 0; i < n; ++i) {
+            double s = 0.0;
+            for (int j = tid; j < i; j += 32) s += A[(size_t)i * n + j] * y[j];
+            s = warp_sum(s);
+            if (tid == 0) y[i] = (y[i] - s) / A[(size_t)i * n + i];
+            __syncwarp();
+        }
+        for (int i = n - 1; i >= 0; --i) {
+            double s = 0.0;
+            for (int j = i + 1 + tid; j < n; j += 32) s += A[(size_t)j * n + i] * y[j];
+            s = warp_sum(s);
+            if (tid == 0) y[i] = (y[i] - s) / A[(size_t)i * n + i];
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    for (int e = tid; e < n; e += nt) delta[e] = y[e];
+    if (tid == 0 && info) *info = bad;
+}
+
+template <typename T>
+int launch_syrk(meb_ctx* ctx, const ActiveArgs& a, int dp, double* part_mat, int grid) {
+    const int bs = dp / 16;
+    const size_t smem = ((size_t)RB * dp + RB) * sizeof(double);
+#define MEB_SYRK_CASE(B) case B: syrk_kernel<T, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat, dp); break;
+    switch (bs) {
+        MEB_SYRK_CASE(1) MEB_SYRK_CASE(2) MEB_SYRK_CASE(3) MEB_SYRK_CASE(4)
+        MEB_SYRK_CASE(5) MEB_SYRK_CASE(6) MEB_SYRK_CASE(7) MEB_SYRK_CASE(8)
+        default: return MEB_E_CAPACITY;
+    }
+#undef MEB_SYRK_CASE
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+}  // namespace
+
+// H (device, (d+1)^2) from the records of the last streaming pass.  d <= 128.
+int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, double* H) {
+    if (c.d > 128) return MEB_E_CAPACITY;
+    const int dp = (c.d + 15) / 16 * 16;
+    const size_t per = (size_t)dp * dp + dp;
+    const size_t avail = ctx->part_mat_len;
+    int grid = ctx->sm_count * 2;
+    if ((size_t)grid * per > avail) grid = (int)(avail / per);
+    if (grid < 1) return MEB_E_CAPACITY;
+    ActiveArgs a;
+    memset(&a, 0, sizeof(a));
+    a.C = c.C; a.ld = c.ld; a.U = c.U; a.v_slot = c.v_slot; a.V = c.V; a.ldv = c.ldv; a.x = c.x; a.d = c.d;
+    a.sigma = c.sigma; a.list = ctx->list; a.count = ctx->count_dev;
+    a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
+    int rc = c.prec == MEB_FP64 ? launch_syrk<double>(ctx, a, dp, ctx->part_mat, grid)
+                                : launch_syrk<float>(ctx, a, dp, ctx->part_mat, grid);
+    if (rc != MEB_OK) return rc;
+    const int n = c.d + 1;
+    int fgrid = (n * n + 255) / 256;
+    if (fgrid > 64) fgrid = 64;
+    dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, dp, c.d, ev_scalars, c.sigma,
+                                                          c.tau, H);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+// delta <- -(scale*H)^{-1} g on the device; info_dev (nullable) receives 0 or the failing pivot + 1
+int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
+                   int* info_dev) {
+    const size_t smem = ((size_t)n * n + n) * sizeof(double);
+    if (smem > 220 * 1024) return MEB_E_CAPACITY;
+    MEB_CUDA_OK(ctx, cudaFuncSetAttribute(chol_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)smem));
+    chol_solve_kernel<<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}

@@ -1,0 +1,180 @@
+// Internal declarations shared by the translation units of libmeb_b200.so (sm_100a only).
+// Nothing here is used by, or shared with, the CPU oracle.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/meb.h"
+
+#define MEB_FULL_MASK 0xffffffffu
+#define MEB_BLOCK 256                 // threads per CTA of every streaming kernel
+#define MEB_WARPS (MEB_BLOCK / 32)
+#define MEB_MAX_GRID 2368             // 148 SMs x 16: upper bound on CTAs of a streaming launch
+
+// number of per-CTA scalar partials written by the streaming kernels
+#define MEB_NPART 12
+
+struct meb_ctx {
+    int device;
+    cudaStream_t stream;
+    int64_t m_max;
+    int32_t d_max;
+    int sm_count;
+    int last_cuda_error;
+    // ---- workspace (device) ----
+    uint32_t* mask;         // [ceil(m/32)] active / flag bit mask of the last streaming pass
+    double* rec_lam;        // [m] lam_i of active balls (dense-indexed, sparse writes)
+    double* rec_rho;        // [m] rho_i = a/nb (2.0 marks B1)
+    double* rec_t;          // [m] t_i of active balls
+    int32_t* list;          // [m] compacted ascending index list
+    int32_t* blocksum;      // [nseg + 2] per-segment popcounts of the compaction; [nseg] = total
+    double* part_scalar;    // [MEB_MAX_GRID * MEB_NPART] per-CTA scalar partials
+    double* part_vec;       // [vec_rows * (d_max+8)] per-CTA vector partials of the list kernels
+    int64_t vec_rows;
+    double* part_mat;       // per-CTA partial matrices of the dense-Hessian SYRK
+    size_t part_mat_len;
+    int32_t* count_dev;     // [8] device counters (compaction totals)
+    double* part_sc;        // [1024] per-CTA scalar partials of the active-list kernels
+    int last_grid;          // CTAs of the last streaming launch (its partials are still in part_scalar)
+    double* small;          // small device state: scalars, vectors of length d+1 (see meb_api.cu)
+    int64_t small_len;
+    double* h_pinned;       // pinned host mirror for small read-backs
+    int64_t h_pinned_len;
+    // ---- owned copies for meb_solve / meb_solve_host ----
+    void* own[16];
+    size_t own_bytes[16];
+    // ---- measurement ----
+    cudaEvent_t ev0, ev1;
+    double last_pass_ms;
+    double last_pass_bytes;
+    bool time_passes;
+};
+
+#define MEB_CUDA_OK(ctx, expr)                                   \
+    do {                                                         \
+        cudaError_t e__ = (expr);                                \
+        if (e__ != cudaSuccess) {                                \
+            (ctx)->last_cuda_error = (int)e__;                   \
+            return MEB_E_CUDA;                                   \
+        }                                                        \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------------
+template <typename T> struct VecOf;
+template <> struct VecOf<double> { typedef double2 type; static constexpr int N = 2; };
+template <> struct VecOf<float>  { typedef float4 type;  static constexpr int N = 4; };
+
+__device__ __forceinline__ double2 ldg_stream(const double2* p) {
+    double2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ float4 ldg_stream(const float4* p) {
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(MEB_FULL_MASK, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(MEB_FULL_MASK, v, o));
+    return v;
+}
+
+// host-side launch helpers implemented in the .cu files -------------------------------------------
+struct StreamArgs {
+    const void* C; int64_t ld;
+    const void* R;               // nullable
+    const void* U;               // nullable (all zero)
+    const int32_t* v_slot;       // nullable
+    const void* V; int64_t ldv;
+    const double* x;             // device (d+1): (r, c)
+    int64_t m; int32_t d;
+    double sigma;
+    // outputs
+    uint32_t* mask;
+    double* rec_lam; double* rec_rho; double* rec_t;
+    double* t_out; double* lam_out;      // nullable dense per-ball outputs
+    double* part;                        // [grid * MEB_NPART]
+    // feasibility / screening
+    double eps; const uint8_t* kept; uint8_t* flags_out;
+    // ingest
+    float* C32; int64_t ld32; float* R32; const double* c0;
+};
+
+enum StreamOp { OP_EVAL = 0, OP_FEAS = 1, OP_SCREEN = 2, OP_INGEST = 3 };
+
+int meb_launch_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out);
+int meb_launch_compact(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* list, int32_t* count_dev);
+
+// ---- active-list passes (meb_active.cu) ----
+enum ActiveMode { MODE_ROWSUM = 0, MODE_HVP = 1, MODE_WRITEV = 2 };
+
+struct ActiveArgs {
+    const void* C; int64_t ld;
+    const void* U;
+    const int32_t* v_slot; const void* V; int64_t ldv;
+    const double* x;                 // (r, c)
+    int32_t d; int32_t dpad;
+    double sigma;
+    const int32_t* list; const int32_t* count;
+    const double* rec_lam; const double* rec_rho; const double* rec_t;
+    const double* q;                 // hvp: (q0, q1)
+    double* part_vec;                // [grid][dpad]
+    double* part_sc;                 // [grid][2]
+    void* U_out; int32_t* slot_out; void* V_out; int64_t ldv_out; int64_t cap_rows;
+};
+
+
+int meb_launch_active(meb_ctx* ctx, int mode, int prec, const ActiveArgs& a, int* grid_out);
+int meb_launch_compact_cap(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* list, int64_t cap,
+                           int32_t* count_dev);
+int meb_launch_flags_to_mask(meb_ctx* ctx, const uint8_t* flags, int64_t m, uint32_t* mask);
+
+// ---- second-level reductions and small kernels (meb_small.cu) ----
+int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t* count, const double* x,
+                      const double* xbar, double sigma, double tau, int d, double* out, double* grad);
+int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
+                     const double* q, double sigma, double tau, int d, double* Hq);
+int meb_argmax_finalize(meb_ctx* ctx, int grid, double* out);
+int meb_scalar_sum(meb_ctx* ctx, const double* v, int n, double* out);
+int meb_sample_mean(meb_ctx* ctx, const double* C, int64_t ld, int64_t m, int d, int S, double* c0);
+int meb_fill_f64(meb_ctx* ctx, double* p, int64_t n, double v);
+int meb_fill_f32(meb_ctx* ctx, float* p, int64_t n, float v);
+int meb_fill_i32(meb_ctx* ctx, int32_t* p, int64_t n, int32_t v);
+int meb_fill_u8(meb_ctx* ctx, uint8_t* p, int64_t n, uint8_t v);
+int meb_gather_rows_f64(meb_ctx* ctx, const double* src, int64_t ld_src, const int32_t* idx, int64_t n, int d,
+                        double* dst, int64_t ld_dst);
+int meb_gather_vec_f64(meb_ctx* ctx, const double* src, const int32_t* idx, int64_t n, double* dst);
+int meb_gather_mult(meb_ctx* ctx, const float* U32, const int32_t* slot32, const float* V32, int64_t ldv32,
+                    const int32_t* idx, int64_t n, int d, double* U, int32_t* slot, double* V, int64_t ldv);
+int meb_set_kept(meb_ctx* ctx, const int32_t* idx, int64_t n, uint8_t* kept);
+
+// ---- internal composite passes (meb_api.cu), used by the solver ----
+// layout of ctx->small (doubles): see meb_api.cu
+struct EvalCall {
+    int prec; int64_t m; int32_t d;
+    const void* C; int64_t ld; const void* R; const void* U;
+    const int32_t* v_slot; const void* V; int64_t ldv;
+    const double* x; const double* xbar; double sigma; double tau;
+};
+// streaming pass + compaction of the active set (+ gradient vector part unless psi_only)
+int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, bool want_grad, double* out_scalars, double* grad,
+                      double* t_out, double* lam_out);
+// gradient vector part for the records of the LAST streaming pass (same C, x, V as that pass)
+int meb_grad_from_records(meb_ctx* ctx, const EvalCall& c, double* out_scalars, double* grad);
+int meb_hvp_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, const double* q, double* Hq);
+
+// ---- dense Hessian and Cholesky (meb_dense.cu) ----
+int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, double* H);
+int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
+                   int* info_dev);

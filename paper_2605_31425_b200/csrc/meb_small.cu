@@ -1,0 +1,297 @@
+// Second level of the fixed-order reduction trees and the (d+1)-sized state updates.
+// Single-CTA kernels: their inputs are the per-CTA partials written by the streaming / active-list
+// kernels (a few thousand doubles), so they are latency-, not bandwidth-bound.
+#include "meb_internal.cuh"
+
+namespace {
+
+constexpr int FBLOCK = 1024;
+
+// deterministic block-wide sum: warp xor tree, then warps in index order
+__device__ __forceinline__ double block_sum_1024(double v, double* sm) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    for (int w = 0; w < FBLOCK / 32; ++w) t += sm[w];
+    return t;
+}
+
+// scalar k of the CTA partials: lanes stride over the CTAs, xor tree (warp k handles scalar k)
+__device__ __forceinline__ double partial_sum(const double* part, int grid, int k, int lane) {
+    double s = 0.0;
+    for (int b = lane; b < grid; b += 32) s += part[(size_t)b * MEB_NPART + k];
+    return warp_sum(s);
+}
+__device__ __forceinline__ double partial_max(const double* part, int grid, int k, int lane) {
+    double s = 0.0;
+    for (int b = lane; b < grid; b += 32) s = fmax(s, part[(size_t)b * MEB_NPART + k]);
+    return warp_max(s);
+}
+
+// out_scalars / grad of one ALM evaluation (reading 13 for psi_var)
+__global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
+    const double* __restrict__ part, int grid, const double* __restrict__ part_vec, int nvec, int dpad,
+    const int32_t* __restrict__ count, const double* __restrict__ x, const double* __restrict__ xbar,
+    double sigma, double tau, int d, double* __restrict__ out, double* __restrict__ grad) {
+    __shared__ double sm[FBLOCK / 32];
+    __shared__ double sc[MEB_NPART];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (warp < 9) {
+        double v;
+        if (warp >= 5 && warp <= 7) v = partial_max(part, grid, warp, lane);
+        else v = partial_sum(part, grid, warp, lane);
+        if (lane == 0) sc[warp] = v;
+    }
+    // vector part: sum_i v+_i = sigma * sum_k lam_k b_k
+    double nv2 = 0.0, dx2 = 0.0;
+    const double tos = tau / sigma;
+    for (int j = threadIdx.x; j < d; j += FBLOCK) {
+        double s = 0.0;
+        for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
+        const double sv = sigma * s;
+        const double dx = x[1 + j] - (xbar ? xbar[1 + j] : x[1 + j]);
+        grad[1 + j] = -sv + tos * dx;
+        nv2 = fma(sv, sv, nv2);
+        dx2 = fma(dx, dx, dx2);
+    }
+    nv2 = block_sum_1024(nv2, sm);
+    dx2 = block_sum_1024(dx2, sm);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const double dx0 = x[0] - (xbar ? xbar[0] : x[0]);
+        dx2 += dx0 * dx0;
+        grad[0] = 1.0 - sc[1] + tos * dx0;
+        out[MEB_EV_PSI] = x[0] + 0.5 * sigma * sc[0] + 0.5 * tos * dx2;
+        out[MEB_EV_SUM_UPLUS] = sc[1];
+        out[MEB_EV_SUM_PROJ2] = sc[0];
+        out[MEB_EV_SUM_DMULT2] = sc[2];
+        out[MEB_EV_N_B1] = sc[3];
+        out[MEB_EV_N_B3] = sc[4];
+        out[MEB_EV_MAX_PFEAS] = sc[5];
+        out[MEB_EV_MAX_COMPL] = sc[6];
+        out[MEB_EV_MAX_DFEAS] = sc[7];
+        out[MEB_EV_SUM_RHO] = sc[8];
+        out[MEB_EV_NORM_SUM_VPLUS] = sqrt(nv2);
+        out[MEB_EV_N_ACTIVE] = (double)(*count);
+        out[12] = dx2;
+        out[13] = 0.0; out[14] = 0.0; out[15] = 0.0;
+    }
+}
+
+// H q from the active-list partials (reading 1):
+//  (Hq)_0 = (tau/sigma) q0 + sigma [ n1 q0 + 1/2 (n3 q0 + sum_{B3} w^T q1) ]
+//  (Hq)_1 = (tau/sigma) q1 + sigma [ n1 q1 + 1/2 (sum_{B3} coef b + (n3 + sum rho) q1) ]
+__global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
+    const double* __restrict__ part_vec, int nvec, int dpad, const double* __restrict__ part_sc,
+    const double* __restrict__ ev, const double* __restrict__ q, double sigma, double tau, int d,
+    double* __restrict__ Hq) {
+    const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
+    const double tos = tau / sigma;
+    for (int j = threadIdx.x; j < d; j += FBLOCK) {
+        double s = 0.0;
+        for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
+        const double qj = q[1 + j];
+        Hq[1 + j] = tos * qj + sigma * (n1 * qj + 0.5 * (s + (n3 + srho) * qj));
+    }
+    if (threadIdx.x < 32) {
+        double s = 0.0;
+        for (int b = threadIdx.x; b < nvec; b += 32) s += part_sc[b];
+        s = warp_sum(s);
+        if (threadIdx.x == 0) Hq[0] = tos * q[0] + sigma * (n1 * q[0] + 0.5 * (n3 * q[0] + s));
+    }
+}
+
+// arg-max style partials (feasibility / ingest): out[0] = max value, out[1] = index, out[2] = count sum
+__global__ void __launch_bounds__(32) argmax_finalize_kernel(const double* __restrict__ part, int grid,
+                                                             double* __restrict__ out) {
+    const int lane = threadIdx.x;
+    double bv = 0.0, bi = -1.0, cnt = 0.0;
+    for (int b = lane; b < grid; b += 32) {
+        const double v = part[(size_t)b * MEB_NPART], i = part[(size_t)b * MEB_NPART + 1];
+        cnt += part[(size_t)b * MEB_NPART + 2];
+        if (i >= 0.0 && (bi < 0.0 || v > bv || (v == bv && i < bi))) { bv = v; bi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(MEB_FULL_MASK, bv, o);
+        const double oi = __shfl_xor_sync(MEB_FULL_MASK, bi, o);
+        if (oi >= 0.0 && (bi < 0.0 || ov > bv || (ov == bv && oi < bi))) { bv = ov; bi = oi; }
+    }
+    cnt = warp_sum(cnt);
+    if (lane == 0) { out[0] = bv; out[1] = bi; out[2] = cnt; }
+}
+
+__global__ void __launch_bounds__(32) scalar_sum_kernel(const double* __restrict__ v, int n,
+                                                        double* __restrict__ out) {
+    double s = 0.0;
+    for (int b = threadIdx.x; b < n; b += 32) s += v[b];
+    s = warp_sum(s);
+    if (threadIdx.x == 0) out[0] = s;
+}
+
+// c0 = mean of the S rows floor(k m / S) (reading 3); one CTA, thread per column, rows in order
+__global__ void __launch_bounds__(256) sample_mean_kernel(const double* __restrict__ C, int64_t ld,
+                                                          int64_t m, int d, int S,
+                                                          double* __restrict__ c0) {
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < d; j += gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int k = 0; k < S; ++k) {
+            const int64_t row = ((int64_t)k * m) / S;
+            s += C[row * ld + j];
+        }
+        c0[j] = s / (double)S;
+    }
+}
+
+template <typename T>
+__global__ void fill_kernel(T* p, int64_t n, T v) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x)
+        p[i] = v;
+}
+
+// gather rows idx[k] of a row-major matrix (and convert): reduced problem of P:L265-269
+template <typename TI, typename TO>
+__global__ void __launch_bounds__(256) gather_rows_kernel(const TI* __restrict__ src, int64_t ld_src,
+                                                          const int32_t* __restrict__ idx, int64_t n, int d,
+                                                          TO* __restrict__ dst, int64_t ld_dst,
+                                                          const double* __restrict__ add) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int nw = (gridDim.x * blockDim.x) >> 5;
+    for (int64_t k = warp; k < n; k += nw) {
+        const TI* s = src + (int64_t)idx[k] * ld_src;
+        TO* o = dst + k * ld_dst;
+        for (int j = lane; j < d; j += 32) o[j] = (TO)s[j] + (add ? (TO)add[j] : (TO)0);
+    }
+}
+
+template <typename TI, typename TO>
+__global__ void __launch_bounds__(256) gather_vec_kernel(const TI* __restrict__ src,
+                                                         const int32_t* __restrict__ idx, int64_t n,
+                                                         TO* __restrict__ dst) {
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n;
+         k += (int64_t)gridDim.x * blockDim.x)
+        dst[k] = src ? (TO)src[idx[k]] : (TO)0;
+}
+
+// reduced-problem multipliers from the FP32 run: for list entry k (ball i = idx[k]):
+// U_red[k] = U32[i]; if slot32[i] >= 0: V_red row k = V32 row slot32[i], slot_red[k] = k else -1
+__global__ void __launch_bounds__(256) gather_mult_kernel(const float* __restrict__ U32,
+                                                          const int32_t* __restrict__ slot32,
+                                                          const float* __restrict__ V32, int64_t ldv32,
+                                                          const int32_t* __restrict__ idx, int64_t n, int d,
+                                                          double* __restrict__ U, int32_t* __restrict__ slot,
+                                                          double* __restrict__ V, int64_t ldv) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int nw = (gridDim.x * blockDim.x) >> 5;
+    for (int64_t k = warp; k < n; k += nw) {
+        const int i = idx[k];
+        const int s = slot32 ? slot32[i] : -1;
+        if (lane == 0) { U[k] = (double)U32[i]; slot[k] = s >= 0 ? (int32_t)k : -1; }
+        if (s >= 0)
+            for (int j = lane; j < d; j += 32) V[k * ldv + j] = (double)V32[(int64_t)s * ldv32 + j];
+    }
+}
+
+__global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint8_t* __restrict__ kept) {
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n;
+         k += (int64_t)gridDim.x * blockDim.x)
+        kept[idx[k]] = 1;
+}
+
+}  // namespace
+
+// ---- host wrappers ---------------------------------------------------------------------------------
+int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t* count, const double* x,
+                      const double* xbar, double sigma, double tau, int d, double* out, double* grad) {
+    eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_scalar, grid, ctx->part_vec, nvec, dpad,
+                                                        count, x, xbar, sigma, tau, d, out, grad);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
+                     const double* q, double sigma, double tau, int d, double* Hq) {
+    hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, dpad, part_sc, ev, q, sigma, tau,
+                                                       d, Hq);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+int meb_argmax_finalize(meb_ctx* ctx, int grid, double* out) {
+    argmax_finalize_kernel<<<1, 32, 0, ctx->stream>>>(ctx->part_scalar, grid, out);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+int meb_scalar_sum(meb_ctx* ctx, const double* v, int n, double* out) {
+    scalar_sum_kernel<<<1, 32, 0, ctx->stream>>>(v, n, out);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+int meb_sample_mean(meb_ctx* ctx, const double* C, int64_t ld, int64_t m, int d, int S, double* c0) {
+    const int grid = (d + 255) / 256;
+    sample_mean_kernel<<<grid, 256, 0, ctx->stream>>>(C, ld, m, d, S, c0);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+static int grid_for(int64_t n, int per) {
+    int64_t g = (n + per - 1) / per;
+    if (g < 1) g = 1;
+    if (g > 148 * 8) g = 148 * 8;
+    return (int)g;
+}
+
+int meb_fill_f64(meb_ctx* ctx, double* p, int64_t n, double v) {
+    fill_kernel<double><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+int meb_fill_f32(meb_ctx* ctx, float* p, int64_t n, float v) {
+    fill_kernel<float><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+int meb_fill_i32(meb_ctx* ctx, int32_t* p, int64_t n, int32_t v) {
+    fill_kernel<int32_t><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+int meb_fill_u8(meb_ctx* ctx, uint8_t* p, int64_t n, uint8_t v) {
+    fill_kernel<uint8_t><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+
+int meb_gather_rows_f64(meb_ctx* ctx, const double* src, int64_t ld_src, const int32_t* idx, int64_t n, int d,
+                        double* dst, int64_t ld_dst) {
+    if (n <= 0) return MEB_OK;
+    gather_rows_kernel<double, double><<<grid_for(n, 8), 256, 0, ctx->stream>>>(src, ld_src, idx, n, d, dst,
+                                                                                 ld_dst, nullptr);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+int meb_gather_vec_f64(meb_ctx* ctx, const double* src, const int32_t* idx, int64_t n, double* dst) {
+    if (n <= 0) return MEB_OK;
+    gather_vec_kernel<double, double><<<grid_for(n, 256), 256, 0, ctx->stream>>>(src, idx, n, dst);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+int meb_gather_mult(meb_ctx* ctx, const float* U32, const int32_t* slot32, const float* V32, int64_t ldv32,
+                    const int32_t* idx, int64_t n, int d, double* U, int32_t* slot, double* V, int64_t ldv) {
+    if (n <= 0) return MEB_OK;
+    gather_mult_kernel<<<grid_for(n, 8), 256, 0, ctx->stream>>>(U32, slot32, V32, ldv32, idx, n, d, U, slot, V,
+                                                                ldv);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}
+int meb_set_kept(meb_ctx* ctx, const int32_t* idx, int64_t n, uint8_t* kept) {
+    if (n <= 0) return MEB_OK;
+    set_kept_kernel<<<grid_for(n, 256), 256, 0, ctx->stream>>>(idx, n, kept);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    return MEB_OK;
+}

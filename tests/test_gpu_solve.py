@@ -1,0 +1,134 @@
+"""GPU parity of meb_solve against the CPU oracle (run with -m gpu).
+
+Bar: final radius within 1e-8 relative of the oracle run to 1e-10; feasibility violation of the
+returned ball <= 1e-10 (1 + r); centre within 1e-5 (1 + r) (the centre is less well conditioned than
+the radius).  Iteration paths, multipliers and index sets may differ (DESIGN reading 14): only the
+unique optimum is compared, the rest is checked for validity."""
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from oracle import ripalm
+
+pytestmark = pytest.mark.gpu
+
+MODES = ["fp64", "mixed"]
+
+
+@pytest.fixture(scope="module")
+def meb():
+    import paper_2605_31425_b200 as meb
+    meb.load()
+    return meb
+
+
+def _solve(meb, C, R, mode, tol=1e-8, host=False):
+    m, d = C.shape
+    with meb.Context(m, d) as ctx:
+        pm = meb.MEB_MODE_FP64 if mode == "fp64" else meb.MEB_MODE_MIXED
+        if host:
+            hc = torch.from_numpy(C).pin_memory()
+            hr = None if R is None else torch.from_numpy(R).pin_memory()
+            c, r, st = meb.meb_solve_host(ctx, hc, hr, tol, pm)
+        else:
+            dC = torch.from_numpy(C).cuda()
+            dR = None if R is None else torch.from_numpy(R).cuda()
+            c, r, st = meb.meb_solve(ctx, dC, dR, tol, pm)
+    return c.numpy(), r, st
+
+
+def _violation(C, R, c, r):
+    Rz = 0 if R is None else R
+    return float(np.max(np.sqrt(((C - c) ** 2).sum(1)) + Rz - r))
+
+
+def _check_against_oracle(meb, C, R, mode, host=False):
+    c, r, st = _solve(meb, C, R, mode, host=host)
+    co, ro, _ = ripalm.meb_solve(C, R, 1e-10, "fp64")
+    assert st["converged"] == 1
+    assert abs(r - ro) <= 1e-8 * ro, (r, ro)
+    assert np.linalg.norm(c - co) <= 1e-5 * (1 + ro)
+    assert _violation(C, R, c, r) <= 1e-10 * (1 + r)
+    assert st["kkt"] <= 1e-8
+    return c, r, st
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("k,m,d", [(1, 10_000, 10), (2, 30_000, 100), (3, 3_000, 1000), (4, 60_000, 32),
+                                   (5, 400, 3000), (1, 777, 7), (3, 999, 129)])
+def test_solve_matches_oracle(meb, k, m, d, mode):
+    C, R = workloads.config(k, m, d)
+    c, r, st = _check_against_oracle(meb, C, R, mode)
+    if mode == "mixed":
+        assert st["rounds"] >= 1 and 0 < st["n_reduced"] <= m
+        assert st["passes_fp32_full"] > 0 and st["passes_reduced"] > 0
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_solve_host_entry_point(meb, mode):
+    C, R = workloads.config(1, 5000, 10)
+    _check_against_oracle(meb, C, R, mode, host=True)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_paper_instances(meb, mode):
+    for m, d in [(1000, 20), (5000, 40)]:
+        C, R = workloads.paper_instance(m, d)
+        _check_against_oracle(meb, C, R, mode)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_closed_forms(meb, mode):
+    # two balls (P: north_star): r = (||c1-c2|| + r1 + r2)/2, centre on the segment
+    c1, r1 = np.array([1.0, 2.0, -1.0, 0.5]), 0.7
+    c2, r2 = np.array([-2.0, 0.0, 3.0, 1.5]), 1.9
+    dist = np.linalg.norm(c1 - c2)
+    rw = (dist + r1 + r2) / 2
+    cw = c1 + (rw - r1) * (c2 - c1) / dist
+    c, r, _ = _solve(meb, np.array([c1, c2]), np.array([r1, r2]), mode, 1e-10)
+    assert abs(r - rw) <= 1e-9 * rw and np.allclose(c, cw, atol=1e-7)
+    # regular simplex e_1..e_n
+    n = 12
+    c, r, _ = _solve(meb, np.eye(n), None, mode, 1e-10)
+    assert abs(r - np.sqrt((n - 1) / n)) <= 1e-9 and np.allclose(c, 1.0 / n, atol=1e-7)
+    # points on a sphere whose hull contains the centre
+    d = 6
+    C = np.vstack([np.eye(d), -np.eye(d)]) * 2.5 - 1.0
+    c, r, _ = _solve(meb, C, None, mode, 1e-10)
+    assert abs(r - 2.5) <= 1e-8 and np.allclose(c, -1.0, atol=1e-6)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_degenerate_inputs(meb, mode):
+    c, r, _ = _solve(meb, np.array([[1.0, -2.0, 3.0]]), np.array([0.25]), mode)        # m = 1
+    assert abs(r - 0.25) <= 1e-9 and np.allclose(c, [1, -2, 3], atol=1e-7)
+    C = np.tile(np.array([[0.5, 0.5]]), (9, 1)); R = np.linspace(0.1, 0.9, 9)           # equal centres
+    c, r, _ = _solve(meb, C, R, mode)
+    assert abs(r - 0.9) <= 1e-8 and np.allclose(c, 0.5, atol=1e-7)
+    c, r, _ = _solve(meb, np.ones((4, 3)), None, mode)                                 # L = 0
+    assert r == 0.0 and np.allclose(c, 1.0)
+    rng = np.random.default_rng(4)                                                     # containment
+    C = np.vstack([[0.3, -0.1, 0.2], rng.uniform(-1, 1, (30, 3))]); R = np.r_[10.0, rng.uniform(0, 1, 30)]
+    c, r, _ = _solve(meb, C, R, mode)
+    assert abs(r - 10.0) <= 1e-7 and np.allclose(c, C[0], atol=1e-6)
+
+
+def test_bad_input_is_reported(meb):
+    C, R = workloads.config(1, 300, 10)
+    C[5, 5] = np.inf
+    with pytest.raises(meb.MebError) as ei:
+        _solve(meb, C, R, "fp64")
+    assert ei.value.code == meb.MEB_E_INPUT
+    C, R = workloads.config(1, 300, 10)
+    R[7] = -1.0
+    with pytest.raises(meb.MebError) as ei:
+        _solve(meb, C, R, "mixed")
+    assert ei.value.code == meb.MEB_E_INPUT
+
+
+def test_solve_is_deterministic(meb):
+    C, R = workloads.config(1, 20_000, 10)
+    a = _solve(meb, C, R, "mixed")
+    b = _solve(meb, C, R, "mixed")
+    assert a[1] == b[1] and np.array_equal(a[0], b[0])

@@ -106,7 +106,24 @@ typedef struct meb_stats {
     double length_scale;        /* L = r^0 (reading 3) */
     double ms_total, ms_phase_lo, ms_phase_hi, ms_check;   /* device times (CUDA events) */
     double bytes_streamed;      /* algorithmic bytes of all streaming passes */
+    /* per pass class (MEB_PASS_*): device time of the streaming launches (CUDA events recorded on the
+     * context's stream around each launch, read after the solve), their algorithmic bytes and count */
+    double pass_ms[8];
+    double pass_bytes[8];
+    int32_t pass_count[8];
+    int64_t kernel_launches;    /* kernels of this library launched by the solve */
 } meb_stats;
+
+/* classes of streaming passes in meb_stats.pass_* */
+enum {
+    MEB_PASS_INGEST = 0,       /* a0: FP64 read of all m rows (+ FP32 shadow write in mixed mode) */
+    MEB_PASS_EVAL_FP64 = 1,    /* a1 over all m rows, FP64 */
+    MEB_PASS_EVAL_FP32 = 2,    /* a1 over all m rows of the FP32 shadow */
+    MEB_PASS_SCREEN = 3,       /* a7 over all m rows of the FP32 shadow */
+    MEB_PASS_FEAS = 4,         /* a8 over all m rows, FP64 */
+    MEB_PASS_EVAL_REDUCED = 5, /* a1 over the reduced problem (L2-resident, not an HBM claim) */
+    MEB_PASS_NCLASS = 8
+};
 
 /* Scalars written by meb_eval_alm into out_scalars[MEB_EVAL_NSCALARS] (device, double). */
 enum {
@@ -154,7 +171,7 @@ MEB_API int meb_solve_host(meb_ctx* ctx, int64_t m, int32_t d, const double* h_c
 /* ---- a0: ingest (reading 3; P:L250 low-precision copy) ---------------------------------------
  * c0_out[d] (device, double) = mean of the S = min(m, sample_rows) rows floor(k*m/S);
  * scalars_out[0] = L = max_i(||c_i - c0|| + r_i), scalars_out[1] = argmax (as double),
- * scalars_out[2] = number of non-finite entries or negative radii found (validation).
+ * scalars_out[2] = number of rows with a non-finite entry, or a negative or non-finite radius (validation).
  * If C32 != NULL also writes the FP32 shadow C32[i,:] = fl32(c_i - c0) (row stride ld32, a multiple
  * of 4) and R32[i] = fl32(r_i) (R32 may be NULL when R is NULL). */
 MEB_API int meb_ingest(meb_ctx* ctx, int64_t m, int32_t d, const double* C, int64_t ld, const double* R,

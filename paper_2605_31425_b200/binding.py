@@ -20,6 +20,7 @@ MEB_E_ARG, MEB_E_INPUT, MEB_E_ALLOC, MEB_E_CUDA, MEB_E_CAPACITY = -1, -2, -3, -4
 MEB_FP64, MEB_FP32 = 0, 1
 MEB_MODE_FP64, MEB_MODE_MIXED = 0, 1
 MEB_EVAL_NSCALARS = 16
+PASS = dict(INGEST=0, EVAL_FP64=1, EVAL_FP32=2, SCREEN=3, FEAS=4, EVAL_REDUCED=5)
 EV = dict(PSI=0, SUM_UPLUS=1, SUM_PROJ2=2, SUM_DMULT2=3, N_B1=4, N_B3=5, MAX_PFEAS=6, MAX_COMPL=7,
           MAX_DFEAS=8, SUM_RHO=9, NORM_SUM_VPLUS=10, N_ACTIVE=11)
 
@@ -47,13 +48,15 @@ class meb_stats(C.Structure):
                 ("n_support", C.c_int64), ("kkt", C.c_double), ("kkt_terms", C.c_double * 5),
                 ("delta_max", C.c_double), ("radius_alg", C.c_double), ("length_scale", C.c_double),
                 ("ms_total", C.c_double), ("ms_phase_lo", C.c_double), ("ms_phase_hi", C.c_double),
-                ("ms_check", C.c_double), ("bytes_streamed", C.c_double)]
+                ("ms_check", C.c_double), ("bytes_streamed", C.c_double),
+                ("pass_ms", C.c_double * 8), ("pass_bytes", C.c_double * 8), ("pass_count", C.c_int32 * 8),
+                ("kernel_launches", C.c_int64)]
 
     def as_dict(self):
         out = {}
         for name, _ in self._fields_:
             v = getattr(self, name)
-            out[name] = list(v) if name == "kkt_terms" else v
+            out[name] = list(v) if hasattr(v, "__len__") else v
         return out
 
 

@@ -140,11 +140,11 @@ int launch_active_t(meb_ctx* ctx, const ActiveArgs& a, int* grid_out) {
     if (wide) {
         auto kern = active_kernel<T, MEB_BLOCK, MODE>;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a);
+        if (e == cudaSuccess) { ctx->launches++; kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a); }
     } else {
         auto kern = active_kernel<T, 32, MODE>;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a);
+        if (e == cudaSuccess) { ctx->launches++; kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a); }
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }

@@ -25,6 +25,10 @@ static void ctx_free_all(meb_ctx* c) {
     for (int i = 0; i < 16; ++i) if (c->own[i]) cudaFree(c->own[i]);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->evpool) {
+        for (int i = 0; i < 2 * MEB_EVPOOL; ++i) if (c->evpool[i]) cudaEventDestroy(c->evpool[i]);
+        free(c->evpool);
+    }
 }
 
 extern "C" int meb_version(void) { return 100; }
@@ -92,6 +96,12 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_pinned, (size_t)c->h_pinned_len * sizeof(double));
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e == cudaSuccess) {
+        c->evpool = (cudaEvent_t*)calloc(2 * MEB_EVPOOL, sizeof(cudaEvent_t));
+        if (!c->evpool) e = cudaErrorMemoryAllocation;
+        for (int i = 0; e == cudaSuccess && i < 2 * MEB_EVPOOL; ++i) e = cudaEventCreate(&c->evpool[i]);
+    }
+    c->cur_class = MEB_PASS_NCLASS - 1;
     if (e == cudaSuccess) e = cudaMemsetAsync(c->count_dev, 0, 8 * sizeof(int32_t), c->stream);
     if (e != cudaSuccess) {
         const bool oom = (e == cudaErrorMemoryAllocation);
@@ -137,8 +147,16 @@ static int check_problem(const meb_ctx* ctx, int64_t m, int32_t d, const void* C
 // one streaming launch, optionally timed with CUDA events on the context's stream
 static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid) {
     if (ctx->time_passes) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+    const bool pool = ctx->ev_record && !ctx->time_passes && ctx->evn < MEB_EVPOOL;
+    if (pool) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn], ctx->stream));
     int rc = meb_launch_stream(ctx, op, prec, a, grid);
     if (rc != MEB_OK) return rc;
+    if (pool) {
+        MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn + 1], ctx->stream));
+        ctx->evclass[ctx->evn] = ctx->cur_class;
+        ctx->evbytes[ctx->evn] = bytes;
+        ctx->evn++;
+    }
     ctx->last_grid = *grid;
     ctx->last_pass_bytes = bytes;
     if (ctx->time_passes) {
@@ -328,6 +346,7 @@ extern "C" int meb_screen_compact(meb_ctx* ctx, int64_t m, int32_t d, const floa
         s.C = C32; s.ld = ld32; s.R = R32; s.x = ctx->small + SM_X; s.m = m; s.d = d; s.sigma = 1.0;
         s.mask = ctx->mask; s.part = ctx->part_scalar; s.eps = (double)tol_red; s.flags_out = flags;
         int grid = 0;
+        ctx->cur_class = MEB_PASS_SCREEN;
         rc = timed_stream(ctx, OP_SCREEN, MEB_FP32, s, (double)m * (d * 4.0 + (R32 ? 4 : 0)), &grid);
         if (rc != MEB_OK) return rc;
     }
@@ -355,6 +374,7 @@ extern "C" int meb_feasibility_check(meb_ctx* ctx, int64_t m, int32_t d, const d
     s.C = C; s.ld = ld; s.R = R; s.x = ctx->small + SM_X; s.m = m; s.d = d; s.sigma = 1.0;
     s.mask = ctx->mask; s.part = ctx->part_scalar; s.eps = eps_feas; s.kept = kept_mask;
     int grid = 0;
+    ctx->cur_class = MEB_PASS_FEAS;
     rc = timed_stream(ctx, OP_FEAS, MEB_FP64, s, (double)m * (d * 8.0 + (R ? 8 : 0) + (kept_mask ? 1 : 0)), &grid);
     if (rc != MEB_OK) return rc;
     rc = meb_argmax_finalize(ctx, grid, ctx->small + SM_AUX);
@@ -390,6 +410,7 @@ extern "C" int meb_ingest(meb_ctx* ctx, int64_t m, int32_t d, const double* C, i
     s.part = ctx->part_scalar; s.C32 = C32; s.ld32 = ld32; s.R32 = (C32 && R) ? R32 : nullptr;
     int grid = 0;
     const double bytes = (double)m * (d * 8.0 + (R ? 8 : 0)) + (C32 ? (double)m * (d * 4.0 + (R ? 4 : 0)) : 0.0);
+    ctx->cur_class = MEB_PASS_INGEST;
     rc = timed_stream(ctx, OP_INGEST, MEB_FP64, s, bytes, &grid);
     if (rc != MEB_OK) return rc;
     return meb_argmax_finalize(ctx, grid, scalars_out);

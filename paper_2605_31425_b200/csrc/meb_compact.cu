@@ -131,8 +131,8 @@ int meb_launch_compact_cap(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_
                            int32_t* count_dev) {
     const int64_t nwords = (m + 31) / 32;
     const int nseg = (int)((nwords + SEG_WORDS - 1) / SEG_WORDS);
-    compact_count_kernel<<<nseg, CBLOCK, 0, ctx->stream>>>(mask, nwords, m, ctx->blocksum);
-    compact_write_kernel<<<nseg, CBLOCK, 0, ctx->stream>>>(mask, nwords, m, ctx->blocksum, nseg, list, cap,
+    ctx->launches++; compact_count_kernel<<<nseg, CBLOCK, 0, ctx->stream>>>(mask, nwords, m, ctx->blocksum);
+    ctx->launches++; compact_write_kernel<<<nseg, CBLOCK, 0, ctx->stream>>>(mask, nwords, m, ctx->blocksum, nseg, list, cap,
                                                            count_dev);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -145,7 +145,7 @@ int meb_launch_compact(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* l
 int meb_launch_flags_to_mask(meb_ctx* ctx, const uint8_t* flags, int64_t m, uint32_t* mask) {
     const int64_t n32 = (m + 31) / 32 * 32;
     const int64_t grid = (n32 + 255) / 256;
-    flags_to_mask_kernel<<<(unsigned)grid, 256, 0, ctx->stream>>>(flags, m, mask);
+    ctx->launches++; flags_to_mask_kernel<<<(unsigned)grid, 256, 0, ctx->stream>>>(flags, m, mask);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -187,7 +187,7 @@ template <typename T>
 int launch_syrk(meb_ctx* ctx, const ActiveArgs& a, int dp, double* part_mat, int grid) {
     const int bs = dp / 16;
     const size_t smem = ((size_t)RB * dp + RB) * sizeof(double);
-#define MEB_SYRK_CASE(B) case B: syrk_kernel<T, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat, dp); break;
+#define MEB_SYRK_CASE(B) case B: ctx->launches++; syrk_kernel<T, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat, dp); break;
     switch (bs) {
         MEB_SYRK_CASE(1) MEB_SYRK_CASE(2) MEB_SYRK_CASE(3) MEB_SYRK_CASE(4)
         MEB_SYRK_CASE(5) MEB_SYRK_CASE(6) MEB_SYRK_CASE(7) MEB_SYRK_CASE(8)
@@ -220,7 +220,7 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
     const int n = c.d + 1;
     int fgrid = (n * n + 255) / 256;
     if (fgrid > 64) fgrid = 64;
-    dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, dp, c.d, ev_scalars, c.sigma,
+    ctx->launches++; dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, dp, c.d, ev_scalars, c.sigma,
                                                           c.tau, H);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -233,7 +233,7 @@ int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double
     if (smem > 220 * 1024) return MEB_E_CAPACITY;
     MEB_CUDA_OK(ctx, cudaFuncSetAttribute(chol_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)smem));
-    chol_solve_kernel<<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev);
+    ctx->launches++; chol_solve_kernel<<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -14,6 +14,7 @@
 
 // number of per-CTA scalar partials written by the streaming kernels
 #define MEB_NPART 12
+#define MEB_EVPOOL 4096               // streaming launches of one solve that get an event pair
 
 struct meb_ctx {
     int device;
@@ -49,6 +50,14 @@ struct meb_ctx {
     double last_pass_ms;
     double last_pass_bytes;
     bool time_passes;
+    // event pool: one (start, stop) pair per streaming launch of a solve, read after the solve
+    cudaEvent_t* evpool;    // [2 * MEB_EVPOOL]
+    int evclass[MEB_EVPOOL];
+    double evbytes[MEB_EVPOOL];
+    int evn;
+    bool ev_record;         // on inside meb_solve
+    int cur_class;          // MEB_PASS_* of the next streaming launch
+    int64_t launches;       // kernels launched through this context
 };
 
 #define MEB_CUDA_OK(ctx, expr)                                   \

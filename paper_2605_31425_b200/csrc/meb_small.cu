@@ -206,7 +206,7 @@ __global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint
 // ---- host wrappers ---------------------------------------------------------------------------------
 int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t* count, const double* x,
                       const double* xbar, double sigma, double tau, int d, double* out, double* grad) {
-    eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_scalar, grid, ctx->part_vec, nvec, dpad,
+    ctx->launches++; eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_scalar, grid, ctx->part_vec, nvec, dpad,
                                                         count, x, xbar, sigma, tau, d, out, grad);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -214,27 +214,27 @@ int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t*
 
 int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
                      const double* q, double sigma, double tau, int d, double* Hq) {
-    hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, dpad, part_sc, ev, q, sigma, tau,
+    ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, dpad, part_sc, ev, q, sigma, tau,
                                                        d, Hq);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 
 int meb_argmax_finalize(meb_ctx* ctx, int grid, double* out) {
-    argmax_finalize_kernel<<<1, 32, 0, ctx->stream>>>(ctx->part_scalar, grid, out);
+    ctx->launches++; argmax_finalize_kernel<<<1, 32, 0, ctx->stream>>>(ctx->part_scalar, grid, out);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 
 int meb_scalar_sum(meb_ctx* ctx, const double* v, int n, double* out) {
-    scalar_sum_kernel<<<1, 32, 0, ctx->stream>>>(v, n, out);
+    ctx->launches++; scalar_sum_kernel<<<1, 32, 0, ctx->stream>>>(v, n, out);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 
 int meb_sample_mean(meb_ctx* ctx, const double* C, int64_t ld, int64_t m, int d, int S, double* c0) {
     const int grid = (d + 255) / 256;
-    sample_mean_kernel<<<grid, 256, 0, ctx->stream>>>(C, ld, m, d, S, c0);
+    ctx->launches++; sample_mean_kernel<<<grid, 256, 0, ctx->stream>>>(C, ld, m, d, S, c0);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
@@ -247,22 +247,22 @@ static int grid_for(int64_t n, int per) {
 }
 
 int meb_fill_f64(meb_ctx* ctx, double* p, int64_t n, double v) {
-    fill_kernel<double><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    ctx->launches++; fill_kernel<double><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 int meb_fill_f32(meb_ctx* ctx, float* p, int64_t n, float v) {
-    fill_kernel<float><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    ctx->launches++; fill_kernel<float><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 int meb_fill_i32(meb_ctx* ctx, int32_t* p, int64_t n, int32_t v) {
-    fill_kernel<int32_t><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    ctx->launches++; fill_kernel<int32_t><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 int meb_fill_u8(meb_ctx* ctx, uint8_t* p, int64_t n, uint8_t v) {
-    fill_kernel<uint8_t><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
+    ctx->launches++; fill_kernel<uint8_t><<<grid_for(n, 1024), 256, 0, ctx->stream>>>(p, n, v);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
@@ -270,28 +270,28 @@ int meb_fill_u8(meb_ctx* ctx, uint8_t* p, int64_t n, uint8_t v) {
 int meb_gather_rows_f64(meb_ctx* ctx, const double* src, int64_t ld_src, const int32_t* idx, int64_t n, int d,
                         double* dst, int64_t ld_dst) {
     if (n <= 0) return MEB_OK;
-    gather_rows_kernel<double, double><<<grid_for(n, 8), 256, 0, ctx->stream>>>(src, ld_src, idx, n, d, dst,
+    ctx->launches++; gather_rows_kernel<double, double><<<grid_for(n, 8), 256, 0, ctx->stream>>>(src, ld_src, idx, n, d, dst,
                                                                                  ld_dst, nullptr);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 int meb_gather_vec_f64(meb_ctx* ctx, const double* src, const int32_t* idx, int64_t n, double* dst) {
     if (n <= 0) return MEB_OK;
-    gather_vec_kernel<double, double><<<grid_for(n, 256), 256, 0, ctx->stream>>>(src, idx, n, dst);
+    ctx->launches++; gather_vec_kernel<double, double><<<grid_for(n, 256), 256, 0, ctx->stream>>>(src, idx, n, dst);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 int meb_gather_mult(meb_ctx* ctx, const float* U32, const int32_t* slot32, const float* V32, int64_t ldv32,
                     const int32_t* idx, int64_t n, int d, double* U, int32_t* slot, double* V, int64_t ldv) {
     if (n <= 0) return MEB_OK;
-    gather_mult_kernel<<<grid_for(n, 8), 256, 0, ctx->stream>>>(U32, slot32, V32, ldv32, idx, n, d, U, slot, V,
+    ctx->launches++; gather_mult_kernel<<<grid_for(n, 8), 256, 0, ctx->stream>>>(U32, slot32, V32, ldv32, idx, n, d, U, slot, V,
                                                                 ldv);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 int meb_set_kept(meb_ctx* ctx, const int32_t* idx, int64_t n, uint8_t* kept) {
     if (n <= 0) return MEB_OK;
-    set_kept_kernel<<<grid_for(n, 256), 256, 0, ctx->stream>>>(idx, n, kept);
+    ctx->launches++; set_kept_kernel<<<grid_for(n, 256), 256, 0, ctx->stream>>>(idx, n, kept);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -99,6 +99,7 @@ int evaluate(Solver& S, const Problem& P, const std::vector<double>& xn, double 
     int rc = upload(ctx, S.dx, xr.data(), S.d + 1);
     if (rc) return rc;
     EvalCall c = make_call(S, P, sigma);
+    ctx->cur_class = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
     rc = meb_eval_internal(ctx, c, want_grad, ctx->small + SM_EV, S.dgrad, nullptr, nullptr);
     if (rc) return rc;
     count_pass(S, P);
@@ -356,6 +357,9 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         return MEB_E_ARG;
     const int n = d + 1;
     const bool timing_was = ctx->time_passes;
+    ctx->evn = 0;
+    ctx->ev_record = true;
+    const int64_t launches0 = ctx->launches;
     cudaEvent_t e_start, e_mid, e_hi, e_end;
     MEB_CUDA_OK(ctx, cudaEventCreate(&e_start));
     MEB_CUDA_OK(ctx, cudaEventCreate(&e_mid));
@@ -402,7 +406,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                                          ctx->stream));
         rc = sync_stream(ctx);
         if (rc) break;
-        if (ctx->h_pinned[2] > 0.0) { rc = MEB_E_INPUT; break; }
+        if (ctx->h_pinned[2] > 0.0 || !(ctx->h_pinned[0] < 1.79e308)) { rc = MEB_E_INPUT; break; }
         S.L = ctx->h_pinned[0];
         st->length_scale = S.L;
         memcpy(c0.data(), ctx->h_pinned + 16, d * sizeof(double));
@@ -588,7 +592,16 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         st->kkt = kkt;
         memcpy(st->kkt_terms, terms, sizeof(terms));
         st->bytes_streamed = S.bytes;
+        for (int k = 0; k < ctx->evn; ++k) {           // per-class device time of the streaming launches
+            float pms = 0.f;
+            if (cudaEventElapsedTime(&pms, ctx->evpool[2 * k], ctx->evpool[2 * k + 1]) != cudaSuccess) continue;
+            const int cls = ctx->evclass[k] & 7;
+            st->pass_ms[cls] += pms; st->pass_bytes[cls] += ctx->evbytes[k]; st->pass_count[cls]++;
+        }
+        cudaGetLastError();
+        st->kernel_launches = ctx->launches - launches0;
     }
+    ctx->ev_record = false;
     cudaEventDestroy(e_start); cudaEventDestroy(e_mid); cudaEventDestroy(e_hi); cudaEventDestroy(e_end);
     ctx->time_passes = timing_was;
     if (rc != MEB_OK) return rc;

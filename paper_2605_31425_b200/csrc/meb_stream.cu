@@ -108,7 +108,8 @@ __device__ __forceinline__ bool row_epilogue(const StreamArgs& a, int64_t row, b
         return flag;
     } else {  // OP_INGEST
         const double val = (double)t_sqrt<T>(nb2) + (double)ri;
-        if (!(val < 1.79e308) || !(val >= 0.0) || ri < T(0)) acc.n0++;   // NaN/Inf/negative radius
+        // rows with a non-finite entry (0 * e accumulated in ne2 is then NaN) or a bad radius
+        if (!(ne2 == T(0)) || !(ri >= T(0)) || !((double)ri < 1.79e308)) acc.n0++;
         if (acc.i0 < 0 || val > acc.m0) { acc.m0 = val; acc.i0 = row; }
         if (a.R32) a.R32[row] = (float)ri;
         return false;
@@ -252,6 +253,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
                     for (int j = 0; j < VEC; ++j) {
                         const T ee = e[k][j] - creg[k][j];
                         s_nb2 = fma(ee, ee, s_nb2);
+                        if (OP == OP_INGEST) s_ne2 = fma(e[k][j], T(0), s_ne2);   // NaN iff a non-finite entry
                         if (SHADOW) e[k][j] = ee;
                     }
             } else {
@@ -284,6 +286,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
 #pragma unroll
             for (int o = G / 2; o > 0; o >>= 1) {
                 s_nb2 += __shfl_xor_sync(MEB_FULL_MASK, s_nb2, o);
+                if (OP == OP_INGEST) s_ne2 += __shfl_xor_sync(MEB_FULL_MASK, s_ne2, o);
                 if (anyv) {
                     s_ne2 += __shfl_xor_sync(MEB_FULL_MASK, s_ne2, o);
                     s_ev += __shfl_xor_sync(MEB_FULL_MASK, s_ev, o);
@@ -295,6 +298,10 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
             const bool take = (it == lane / RPW);
             const T g0 = __shfl_sync(MEB_FULL_MASK, s_nb2, src);
             if (take) my_nb2 = g0;
+            if (OP == OP_INGEST) {
+                const T g1 = __shfl_sync(MEB_FULL_MASK, s_ne2, src);
+                if (take) my_ne2 = g1;
+            }
             if (anyv) {
                 const T g1 = __shfl_sync(MEB_FULL_MASK, s_ne2, src);
                 const T g2 = __shfl_sync(MEB_FULL_MASK, s_ev, src);
@@ -359,6 +366,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
                             if (col + j < d) {
                                 const T ee = e[u][j] - (T)__ldg(cptr + col + j);
                                 s_nb2 = fma(ee, ee, s_nb2);
+                                if (OP == OP_INGEST) s_ne2 = fma(e[u][j], T(0), s_ne2);
                                 if (SHADOW) a.C32[row * a.ld32 + col + j] = (float)ee;
                             }
                         }
@@ -393,6 +401,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 s_nb2 += __shfl_xor_sync(MEB_FULL_MASK, s_nb2, o);
+                if (OP == OP_INGEST) s_ne2 += __shfl_xor_sync(MEB_FULL_MASK, s_ne2, o);
                 if (slot >= 0) {
                     s_ne2 += __shfl_xor_sync(MEB_FULL_MASK, s_ne2, o);
                     s_ev += __shfl_xor_sync(MEB_FULL_MASK, s_ev, o);
@@ -429,7 +438,7 @@ int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_ou
     int grid = (int)(want < cap ? want : cap);
     if (grid < 1) grid = 1;
     StreamArgs b = a;
-    kernel<<<grid, MEB_BLOCK, 0, ctx->stream>>>(b);
+    ctx->launches++; kernel<<<grid, MEB_BLOCK, 0, ctx->stream>>>(b);
     e = cudaGetLastError();
     if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
     *grid_out = grid;

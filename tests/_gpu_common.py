@@ -15,7 +15,7 @@ def make_state(seed, m, d, with_radii=True, frac_mult=0.3, data="normal"):
     R = rng.uniform(0, 0.3, m) if with_radii else None
     c = rng.standard_normal(d) * 0.1
     dist = np.sqrt(((C - c) ** 2).sum(1)) + (0 if R is None else R)
-    r = float(np.quantile(dist, 0.7))
+    r = float(np.quantile(dist, 0.7)) * 1.0001   # off the data points: no ball exactly on a branch boundary
     x = np.concatenate([[r], c])
     xbar = x + rng.standard_normal(d + 1) * 0.05
     U = np.zeros(m)

@@ -45,6 +45,13 @@ def _near_boundary(ev, tol):
     return (np.abs(nb - a) <= 10 * tol * scale) | (np.abs(nb + a) <= 10 * tol * scale)
 
 
+def _branch_flip_slack(C, R, U, V, x, sigma, prec):
+    """Allowance for balls within the tolerance of a branch boundary of P:L115, whose P_i may
+    legitimately be taken from the other branch: sigma * ||P_i||_F <= sigma * sqrt(d+1) each."""
+    ev = prim.eval_alm(C, R, U, V, x, x, sigma, 0.0, dtype=NPDT[prec])
+    return float(_near_boundary(ev, TOL[prec]).sum()) * sigma * np.sqrt(C.shape[1] + 1.0)
+
+
 def _check_eval(meb, ctx, prec, C, R, U, V, x, xbar, sigma, tau, layout, ld_pad):
     tol = TOL[prec]
     Cd, Rd, Ud, slot, Vr = to_device(C, R, U, V, THDT[prec], layout, ld_pad)
@@ -133,7 +140,8 @@ def test_hvp(meb, ctx, prec, m, d, ld_pad):
     q = np.random.default_rng(5).standard_normal(d + 1)
     Hq = meb.meb_hvp(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), 2.0, 0.5, dvec(q)).cpu().numpy()
     want, scale = prim.hvp(C, R, U, V, x, 2.0, 0.5, q, dtype=NPDT[prec])
-    assert np.linalg.norm(Hq - want) <= 4 * TOL[prec] * np.linalg.norm(scale)
+    slack = _branch_flip_slack(C, R, U, V, x, 2.0, prec) * np.linalg.norm(q)
+    assert np.linalg.norm(Hq - want) <= 4 * TOL[prec] * np.linalg.norm(scale) + slack
     assert q @ Hq >= 0.25 * (q @ q) * (1 - 1e-6)          # q^T H q >= (tau/sigma) ||q||^2
 
 
@@ -147,7 +155,8 @@ def test_dense_hessian(meb, ctx, prec, m, d):
     Cd, Rd, Ud, slot, Vr = to_device(C, R, U, V, THDT[prec], "sparse")
     H = meb.meb_dense_hessian(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), 2.0, 0.5).cpu().numpy()
     want, scale = prim.dense_hessian(C, R, U, V, x, 2.0, 0.5, dtype=NPDT[prec])
-    assert np.linalg.norm(H - want) <= 4 * TOL[prec] * np.linalg.norm(scale)
+    slack = _branch_flip_slack(C, R, U, V, x, 2.0, prec)
+    assert np.linalg.norm(H - want) <= 4 * TOL[prec] * np.linalg.norm(scale) + slack
     assert np.array_equal(H, H.T) or np.abs(H - H.T).max() <= 1e-13 * np.abs(H).max()
 
 
@@ -162,20 +171,24 @@ def test_update_multipliers(meb, ctx, prec, m, d):
     res = meb.meb_update_multipliers(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), 1.7)
     Up, Vp, m2 = prim.update_multipliers(C, R, U, V, x, 1.7, dtype=NPDT[prec])
     ev = prim.eval_alm(C, R, U, V, x, x, 1.7, 1.0, dtype=NPDT[prec])
-    near = _near_boundary(ev, TOL[prec])
-    assert not near.any()
+    near = _near_boundary(ev, TOL[prec])          # balls that may legitimately land in the other branch
+    ok = ~near
     Ug = res["U"].cpu().numpy().astype(np.float64)
     sl = res["v_slot"].cpu().numpy()
     Vg = res["Vrows"].cpu().numpy().astype(np.float64)
     mag = 1.7 * (np.abs(ev["a"].astype(np.float64)) + ev["nb"].astype(np.float64))
-    assert np.all(np.abs(Ug - Up) <= TOL[prec] * mag + 1e-300)
+    assert np.all(np.abs(Ug - Up)[ok] <= TOL[prec] * mag[ok] + 1e-300)
     act = np.flatnonzero(ev["br"] != 2)
-    assert res["n_slots"] == act.size and res["code"] == 0
-    assert np.array_equal(np.flatnonzero(sl >= 0), act)
-    assert np.array_equal(sl[act], np.arange(act.size))              # rows in ascending ball order
-    assert np.all(np.abs(Vg[sl[act]] - Vp[act]) <= TOL[prec] * mag[act][:, None])
+    act_g = np.flatnonzero(sl >= 0)
+    assert np.all(near[np.setxor1d(act, act_g)])
+    assert res["n_slots"] == act_g.size and res["code"] == 0
+    assert np.array_equal(sl[act_g], np.arange(act_g.size))          # rows in ascending ball order
+    both = np.intersect1d(act, act_g)
+    both = both[ok[both]]
+    assert np.all(np.abs(Vg[sl[both]] - Vp[both]) <= TOL[prec] * mag[both][:, None])
     assert np.all(Ug[sl < 0] == 0)
-    assert abs(res["sum_mult2"] - m2) <= 4 * TOL[prec] * m2
+    assert abs(res["sum_mult2"] - m2) <= 4 * TOL[prec] * m2 + near.sum() * 4.0 * float(np.max(mag)) ** 2
+    act = act_g
     # capacity error: too few rows for the active balls
     res2 = meb.meb_update_multipliers(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), 1.7, cap_rows=act.size - 1)
     assert res2["code"] == meb.MEB_E_CAPACITY and res2["n_slots"] == act.size
@@ -222,8 +235,10 @@ def test_screen_compact(meb, ctx, m, d, ld_pad):
     C32 = C.astype(np.float32); R32 = None if R is None else R.astype(np.float32)
     Cd, Rd, *_ = to_device(C32.astype(np.float64), None if R is None else R32.astype(np.float64), U, V,
                            torch.float32, "none", ld_pad)
-    r_hat, c_hat = x[0] * 1.3, x[1:]
-    tol_red = 0.1 * r_hat
+    r_hat, c_hat = x[0], x[1:]
+    # threshold chosen so that about 40% of the balls are retained whatever d is (distances concentrate)
+    dist = np.sqrt(((C32.astype(np.float64) - c_hat) ** 2).sum(1)) + (0 if R is None else R32)
+    tol_red = float(np.quantile(r_hat - dist, 0.4)) + 1e-4 * r_hat
     flags, s = prim.screen_flags(C32, R32, r_hat, c_hat, tol_red)
     res = meb.meb_screen_compact(ctx, Cd, Rd, r_hat, dvec(c_hat), tol_red)
     fg = res["flags"].cpu().numpy()

@@ -38,6 +38,10 @@ __global__ void __launch_bounds__(MEB_BLOCK) active_kernel(const ActiveArgs a) {
     const int team = threadIdx.x / TEAM, tt = threadIdx.x % TEAM;
     const int d = a.d;
     double* acc = acc_s + (size_t)team * a.dpad;
+    if (blockIdx.x * TPB >= *a.count) {                      // no list entry for this CTA: the finalize
+        if (threadIdx.x == 0) a.part_sc[blockIdx.x] = 0.0;   // kernels skip its vector partial
+        return;
+    }
     if (MODE != MODE_WRITEV)
         for (int j = tt; j < a.dpad; j += TEAM) acc[j] = 0.0;
     const T* __restrict__ C = static_cast<const T*>(a.C);

@@ -30,6 +30,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a, dou
     const double* __restrict__ cx = a.x + 1;
     const T inv_sig = T(1) / (T)a.sigma;
     const int n = *a.count;
+    if (blockIdx.x * RB >= n) return;                     // no tile for this CTA: the finalize skips it
     double acc[BS][BS];
     double accs[BS];
 #pragma unroll
@@ -104,8 +105,11 @@ __global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a, dou
 }
 
 __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __restrict__ part_mat, int nparts,
+                                                             const int32_t* __restrict__ count,
                                                              int dp, int d, const double* __restrict__ ev,
                                                              double sigma, double tau, double* __restrict__ H) {
+    const int ntiles = (*count + RB - 1) / RB;            // CTAs b < ntiles wrote a partial
+    if (nparts > ntiles) nparts = ntiles;
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
     const int n = d + 1;
@@ -130,56 +134,51 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
     }
 }
 
-// Solve (scale * H) delta = -g for one SPD matrix of order n <= 257 held in shared memory
-// (right-looking Cholesky, then the two triangular solves).  One CTA.
+// Solve (scale * H) delta = -g for one SPD matrix of order n <= 256 held in shared memory.
+// Square-root-free Cholesky (H = L D L^T, no pivoting: H is SPD) on the AUGMENTED lower
+// triangle [H; -g^T]: eliminating column k also updates the right-hand-side row, so after the n
+// column steps row n holds D L^{-1}(-g) and only the backward substitution with L^T is left.
+// One __syncthreads per column; 16 x 16 threads own an interleaved 2-D slice of the trailing
+// block (no integer division, conflict-free shared accesses with an odd leading dimension).
 __global__ void __launch_bounds__(256) chol_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
                                                          int n, double scale, double* __restrict__ delta,
                                                          int* __restrict__ info) {
-    extern __shared__ __align__(16) double A[];           // n*n + n
-    double* y = A + (size_t)n * n;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    for (int e = tid; e < n * n; e += nt) A[e] = scale * H[e];
-    for (int e = tid; e < n; e += nt) y[e] = -g[e];
+    extern __shared__ __align__(16) double A[];           // (n+1) rows x lda, then invd[n]
+    const int lda = (n + 1) | 1;
+    double* invd = A + (size_t)(n + 1) * lda;
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    for (int i = ty; i < n; i += 16)
+        for (int j = tx; j <= i; j += 16) A[(size_t)i * lda + j] = scale * H[(size_t)i * n + j];
+    for (int j = tid; j < n; j += 256) A[(size_t)n * lda + j] = -g[j];
     __shared__ int bad;
     if (tid == 0) bad = 0;
-    __syncthreads();
     for (int k = 0; k < n; ++k) {
-        if (tid == 0) {
-            const double dkk = A[(size_t)k * n + k];
-            if (!(dkk > 0.0)) { bad = k + 1; A[(size_t)k * n + k] = 1.0; }
-            else A[(size_t)k * n + k] = sqrt(dkk);
+        __syncthreads();
+        double dk = A[(size_t)k * lda + k];
+        if (!(dk > 0.0)) { if (tid == 0) bad = k + 1; dk = 1.0; }
+        const double inv = 1.0 / dk;
+        if (tid == 0) invd[k] = inv;
+        for (int i = k + 1 + ty; i <= n; i += 16) {
+            const double lik = A[(size_t)i * lda + k] * inv;
+            const int jmax = i < n ? i : n - 1;
+            for (int j = k + 1 + tx; j <= jmax; j += 16)
+                A[(size_t)i * lda + j] = fma(-lik, A[(size_t)j * lda + k], A[(size_t)i * lda + j]);
         }
-        __syncthreads();
-        const double lkk = A[(size_t)k * n + k];
-        for (int i = k + 1 + tid; i < n; i += nt) A[(size_t)i * n + k] /= lkk;
-        __syncthreads();
-        // trailing update: A[i][j] -= L[i][k] L[j][k], j <= i
-        const int rem = n - k - 1;
-        for (int e = tid; e < rem * rem; e += nt) {
-            const int i = k + 1 + e / rem, j = k + 1 + e % rem;
-            if (j <= i) A[(size_t)i * n + j] -= A[(size_t)i * n + k] * A[(size_t)j * n + k];
-        }
-        __syncthreads();
     }
-    // forward substitution L y = rhs, then L^T x = y (one warp; n is small)
+    __syncthreads();
+    // z = D^{-1} (row n); then L^T x = z, column-oriented, one warp (L_kj = A[k][j] * invd[j])
+    double* z = A + (size_t)n * lda;
     if (tid < 32) {
-        for (int i = 0; i < n; ++i) {
-            double s = 0.0;
-            for (int j = tid; j < i; j += 32) s += A[(size_t)i * n + j] * y[j];
-            s = warp_sum(s);
-            if (tid == 0) y[i] = (y[i] - s) / A[(size_t)i * n + i];
-            __syncwarp();
-        }
-        for (int i = n - 1; i >= 0; --i) {
-            double s = 0.0;
-            for (int j = i + 1 + tid; j < n; j += 32) s += A[(size_t)j * n + i] * y[j];
-            s = warp_sum(s);
-            if (tid == 0) y[i] = (y[i] - s) / A[(size_t)i * n + i];
+        for (int j = tid; j < n; j += 32) z[j] *= invd[j];
+        __syncwarp();
+        for (int k = n - 1; k > 0; --k) {
+            const double xk = z[k];
+            for (int j = tid; j < k; j += 32) z[j] = fma(-A[(size_t)k * lda + j] * invd[j], xk, z[j]);
             __syncwarp();
         }
     }
     __syncthreads();
-    for (int e = tid; e < n; e += nt) delta[e] = y[e];
+    for (int e = tid; e < n; e += 256) delta[e] = z[e];
     if (tid == 0 && info) *info = bad;
 }
 
@@ -220,7 +219,7 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
     const int n = c.d + 1;
     int fgrid = (n * n + 255) / 256;
     if (fgrid > 64) fgrid = 64;
-    ctx->launches++; dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, dp, c.d, ev_scalars, c.sigma,
+    ctx->launches++; dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, ctx->count_dev, dp, c.d, ev_scalars, c.sigma,
                                                           c.tau, H);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -229,7 +228,7 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
 // delta <- -(scale*H)^{-1} g on the device; info_dev (nullable) receives 0 or the failing pivot + 1
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
                    int* info_dev) {
-    const size_t smem = ((size_t)n * n + n) * sizeof(double);
+    const size_t smem = ((size_t)(n + 1) * ((n + 1) | 1) + n) * sizeof(double);
     if (smem > 220 * 1024) return MEB_E_CAPACITY;
     MEB_CUDA_OK(ctx, cudaFuncSetAttribute(chol_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)smem));

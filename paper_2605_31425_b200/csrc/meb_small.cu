@@ -32,7 +32,7 @@ __device__ __forceinline__ double partial_max(const double* part, int grid, int 
 
 // out_scalars / grad of one ALM evaluation (reading 13 for psi_var)
 __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
-    const double* __restrict__ part, int grid, const double* __restrict__ part_vec, int nvec, int dpad,
+    const double* __restrict__ part, int grid, const double* __restrict__ part_vec, int nvec, int tpb, int dpad,
     const int32_t* __restrict__ count, const double* __restrict__ x, const double* __restrict__ xbar,
     double sigma, double tau, int d, double* __restrict__ out, double* __restrict__ grad) {
     __shared__ double sm[FBLOCK / 32];
@@ -44,7 +44,8 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
         else v = partial_sum(part, grid, warp, lane);
         if (lane == 0) sc[warp] = v;
     }
-    // vector part: sum_i v+_i = sigma * sum_k lam_k b_k
+    // vector part: sum_i v+_i = sigma * sum_k lam_k b_k (only CTAs b < ceil(count/tpb) had list entries)
+    if (nvec > 0) { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
     double nv2 = 0.0, dx2 = 0.0;
     const double tos = tau / sigma;
     for (int j = threadIdx.x; j < d; j += FBLOCK) {
@@ -84,11 +85,12 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
 //  (Hq)_0 = (tau/sigma) q0 + sigma [ n1 q0 + 1/2 (n3 q0 + sum_{B3} w^T q1) ]
 //  (Hq)_1 = (tau/sigma) q1 + sigma [ n1 q1 + 1/2 (sum_{B3} coef b + (n3 + sum rho) q1) ]
 __global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
-    const double* __restrict__ part_vec, int nvec, int dpad, const double* __restrict__ part_sc,
-    const double* __restrict__ ev, const double* __restrict__ q, double sigma, double tau, int d,
+    const double* __restrict__ part_vec, int nvec, int tpb, const int32_t* __restrict__ count, int dpad,
+    const double* __restrict__ part_sc, const double* __restrict__ ev, const double* __restrict__ q, double sigma, double tau, int d,
     double* __restrict__ Hq) {
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
+    { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
     for (int j = threadIdx.x; j < d; j += FBLOCK) {
         double s = 0.0;
         for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
@@ -131,18 +133,30 @@ __global__ void __launch_bounds__(32) scalar_sum_kernel(const double* __restrict
     if (threadIdx.x == 0) out[0] = s;
 }
 
-// c0 = mean of the S rows floor(k m / S) (reading 3); one CTA, thread per column, rows in order
+// c0 = mean of the S rows floor(k m / S) (reading 3).  Stage 1: CTA (x, g) adds the rows of sample
+// chunk g (S/32 rows, in order) for 256 columns -> part[g][j]; stage 2 adds the 32 chunks in order.
+constexpr int SM_CHUNKS = 32;
 __global__ void __launch_bounds__(256) sample_mean_kernel(const double* __restrict__ C, int64_t ld,
                                                           int64_t m, int d, int S,
-                                                          double* __restrict__ c0) {
-    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < d; j += gridDim.x * blockDim.x) {
-        double s = 0.0;
-        for (int k = 0; k < S; ++k) {
-            const int64_t row = ((int64_t)k * m) / S;
-            s += C[row * ld + j];
-        }
-        c0[j] = s / (double)S;
-    }
+                                                          double* __restrict__ part) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int g = blockIdx.y;
+    if (j >= d) return;
+    const int per = (S + SM_CHUNKS - 1) / SM_CHUNKS;
+    const int k0 = g * per, k1 = min(S, k0 + per);
+    double s = 0.0;
+#pragma unroll 4
+    for (int k = k0; k < k1; ++k) s += C[(((int64_t)k * m) / S) * ld + j];
+    part[(size_t)g * d + j] = s;
+}
+__global__ void __launch_bounds__(256) sample_mean_final_kernel(const double* __restrict__ part, int d, int S,
+                                                                double* __restrict__ c0) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= d) return;
+    double s = 0.0;
+#pragma unroll
+    for (int g = 0; g < SM_CHUNKS; ++g) s += part[(size_t)g * d + j];
+    c0[j] = s / (double)S;
 }
 
 template <typename T>
@@ -206,7 +220,8 @@ __global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint
 // ---- host wrappers ---------------------------------------------------------------------------------
 int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t* count, const double* x,
                       const double* xbar, double sigma, double tau, int d, double* out, double* grad) {
-    ctx->launches++; eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_scalar, grid, ctx->part_vec, nvec, dpad,
+    const int tpb = d > 2048 ? 1 : MEB_WARPS;      // list entries per CTA round of the active kernel
+    ctx->launches++; eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_scalar, grid, ctx->part_vec, nvec, tpb, dpad,
                                                         count, x, xbar, sigma, tau, d, out, grad);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -214,7 +229,8 @@ int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t*
 
 int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
                      const double* q, double sigma, double tau, int d, double* Hq) {
-    ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, dpad, part_sc, ev, q, sigma, tau,
+    const int tpb = d > 2048 ? 1 : MEB_WARPS;
+    ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, tpb, ctx->count_dev, dpad, part_sc, ev, q, sigma, tau,
                                                        d, Hq);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -233,8 +249,10 @@ int meb_scalar_sum(meb_ctx* ctx, const double* v, int n, double* out) {
 }
 
 int meb_sample_mean(meb_ctx* ctx, const double* C, int64_t ld, int64_t m, int d, int S, double* c0) {
-    const int grid = (d + 255) / 256;
-    ctx->launches++; sample_mean_kernel<<<grid, 256, 0, ctx->stream>>>(C, ld, m, d, S, c0);
+    const int gx = (d + 255) / 256;
+    double* part = ctx->part_vec;                  // [32][d] scratch: vec_rows >= 32 rows of >= d doubles
+    ctx->launches++; sample_mean_kernel<<<dim3(gx, SM_CHUNKS), 256, 0, ctx->stream>>>(C, ld, m, d, S, part);
+    ctx->launches++; sample_mean_final_kernel<<<gx, 256, 0, ctx->stream>>>(part, d, S, c0);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

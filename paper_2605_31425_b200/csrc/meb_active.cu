@@ -30,7 +30,9 @@ __device__ __forceinline__ double team_sum(double v, double* scratch) {
 }
 
 template <typename T, int TEAM, int MODE>
-__global__ void __launch_bounds__(MEB_BLOCK) active_kernel(const ActiveArgs a) {
+__global__ void __launch_bounds__(MEB_BLOCK) active_kernel(const ActiveArgs a_in) {
+    ActiveArgs a = a_in;
+    meb_resolve_dyn(a);
     extern __shared__ __align__(16) double acc_s[];          // [teams_per_block][dpad]
     __shared__ double scratch[MEB_WARPS];
     __shared__ double sc_red[MEB_WARPS];

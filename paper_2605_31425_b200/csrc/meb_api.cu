@@ -8,6 +8,7 @@
 #include <new>
 
 #include "meb_internal.cuh"
+#include "meb_ctrl.cuh"
 
 // layout of ctx->small (doubles)
 #define SM_EV 0          // [16] evaluation scalars scratch
@@ -144,13 +145,18 @@ static int check_problem(const meb_ctx* ctx, int64_t m, int32_t d, const void* C
     return MEB_OK;
 }
 
-// one streaming launch, optionally timed with CUDA events on the context's stream
-static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid) {
+// one streaming launch, optionally timed with CUDA events on the context's stream.  Short aligned rows
+// go to the TMA-staged tile kernels (meb_tile.cu), everything else to the register-mapped kernels.
+static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid, bool* fused) {
     if (ctx->time_passes) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-    const bool pool = ctx->ev_record && !ctx->time_passes && ctx->evn < MEB_EVPOOL;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(ctx->stream, &cap);
+    const bool pool = ctx->ev_record && !ctx->time_passes && ctx->evn < MEB_EVPOOL && cap == cudaStreamCaptureStatusNone;
     if (pool) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn], ctx->stream));
-    int rc = meb_launch_stream(ctx, op, prec, a, grid);
+    const bool tile = meb_tile_applicable(op, prec, a);
+    int rc = tile ? meb_launch_tile(ctx, op, prec, a, grid) : meb_launch_stream(ctx, op, prec, a, grid);
     if (rc != MEB_OK) return rc;
+    if (fused) *fused = tile && op == OP_EVAL;
     if (pool) {
         MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn + 1], ctx->stream));
         ctx->evclass[ctx->evn] = ctx->cur_class;
@@ -159,7 +165,8 @@ static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, dou
     }
     ctx->last_grid = *grid;
     ctx->last_pass_bytes = bytes;
-    if (ctx->time_passes) {
+    ctx->list_valid = false;
+    if (ctx->time_passes && cap == cudaStreamCaptureStatusNone) {
         MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
         MEB_CUDA_OK(ctx, cudaEventSynchronize(ctx->ev1));
         float ms = 0.f;
@@ -167,6 +174,12 @@ static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, dou
         ctx->last_pass_ms = ms;
     }
     return MEB_OK;
+}
+
+static void graph_side(ActiveArgs& a, const GraphSide* gs) {
+    if (!gs) return;
+    a.dyn = gs->dyn;
+    for (int b = 0; b < 2; ++b) { a.U2[b] = gs->U2[b]; a.slot2[b] = gs->slot2[b]; a.V2[b] = gs->V2[b]; a.vcap2[b] = gs->vcap2[b]; }
 }
 
 static ActiveArgs active_args(meb_ctx* ctx, const EvalCall& c) {
@@ -177,19 +190,19 @@ static ActiveArgs active_args(meb_ctx* ctx, const EvalCall& c) {
     a.list = ctx->list; a.count = ctx->count_dev;
     a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
     a.part_vec = ctx->part_vec; a.part_sc = ctx->part_sc;
+    graph_side(a, c.gs);
     return a;
 }
 
-int meb_grad_from_records(meb_ctx* ctx, const EvalCall& c, double* out_scalars, double* grad) {
-    ActiveArgs a = active_args(ctx, c);
-    int nvec = 0;
-    int rc = meb_launch_active(ctx, MODE_ROWSUM, c.prec, a, &nvec);
-    if (rc != MEB_OK) return rc;
-    return meb_eval_finalize(ctx, ctx->last_grid, nvec, a.dpad, ctx->count_dev, c.x, c.xbar, c.sigma, c.tau,
-                             c.d, out_scalars, grad);
+// ascending list of the rows flagged by the last streaming pass (the active set of an evaluation)
+int meb_ensure_list(meb_ctx* ctx, int64_t m) {
+    if (ctx->list_valid) return MEB_OK;
+    int rc = meb_launch_compact(ctx, ctx->mask, m, ctx->list, ctx->count_dev);
+    if (rc == MEB_OK) ctx->list_valid = true;
+    return rc;
 }
 
-int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, bool want_grad, double* out_scalars, double* grad,
+int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, double* out_scalars, double* grad,
                       double* t_out, double* lam_out) {
     StreamArgs s;
     memset(&s, 0, sizeof(s));
@@ -197,26 +210,50 @@ int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, bool want_grad, double* o
     s.x = c.x; s.m = c.m; s.d = c.d; s.sigma = c.sigma;
     s.mask = ctx->mask; s.rec_lam = ctx->rec_lam; s.rec_rho = ctx->rec_rho; s.rec_t = ctx->rec_t;
     s.t_out = t_out; s.lam_out = lam_out; s.part = ctx->part_scalar;
+    s.part_vec = ctx->part_vec; s.dpad = (int32_t)round_up((size_t)c.d, 8);
+    bool any_mult = c.U != nullptr;
+    if (c.gs) {
+        s.dyn = c.gs->dyn;
+        for (int b = 0; b < 2; ++b) { s.U2[b] = c.gs->U2[b]; s.slot2[b] = c.gs->slot2[b]; s.V2[b] = c.gs->V2[b]; }
+        any_mult = true;
+    }
     const double sz = c.prec == MEB_FP64 ? 8.0 : 4.0;
-    const double bytes = (double)c.m * (c.d * sz + (c.R ? sz : 0) + (c.U ? sz : 0) + (c.v_slot ? 4 : 0));
+    const double bytes = (double)c.m * (c.d * sz + (c.R ? sz : 0) + (any_mult ? sz + 4 : 0));
     int grid = 0;
-    int rc = timed_stream(ctx, OP_EVAL, c.prec, s, bytes, &grid);
+    bool fused = false;
+    int rc = timed_stream(ctx, OP_EVAL, c.prec, s, bytes, &grid, &fused);
     if (rc != MEB_OK) return rc;
-    rc = meb_launch_compact(ctx, ctx->mask, c.m, ctx->list, ctx->count_dev);
-    if (rc != MEB_OK) return rc;
-    if (want_grad) return meb_grad_from_records(ctx, c, out_scalars, grad);
-    return meb_eval_finalize(ctx, grid, 0, (int)round_up((size_t)c.d, 8), ctx->count_dev, c.x, c.xbar, c.sigma,
-                             c.tau, c.d, out_scalars, grad);
+    FinalizeArgs f;
+    memset(&f, 0, sizeof(f));
+    f.part = ctx->part_scalar; f.grid = grid; f.part_vec = ctx->part_vec; f.dpad = s.dpad;
+    f.count = ctx->count_dev; f.x = c.x; f.xbar = c.xbar; f.sigma = c.sigma; f.tau = c.tau; f.d = c.d;
+    f.out = out_scalars; f.grad = grad;
+    if (c.gs) { f.dyn = c.gs->dyn; f.S = c.gs->S; if (c.gs->v) f.v = *c.gs->v; }
+    if (fused) {
+        f.nvec = grid; f.tpb = 0;
+    } else {                          // long rows: the vector part comes from the active-list kernel
+        rc = meb_ensure_list(ctx, c.m);
+        if (rc != MEB_OK) return rc;
+        ActiveArgs a = active_args(ctx, c);
+        int nvec = 0;
+        rc = meb_launch_active(ctx, MODE_ROWSUM, c.prec, a, &nvec);
+        if (rc != MEB_OK) return rc;
+        f.nvec = nvec; f.tpb = c.d > 2048 ? 1 : MEB_WARPS;
+    }
+    return meb_eval_finalize(ctx, f);
 }
 
 int meb_hvp_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, const double* q,
                          double* Hq) {
+    int rc = meb_ensure_list(ctx, c.m);
+    if (rc != MEB_OK) return rc;
     ActiveArgs a = active_args(ctx, c);
     a.q = q;
     int nvec = 0;
-    int rc = meb_launch_active(ctx, MODE_HVP, c.prec, a, &nvec);
+    rc = meb_launch_active(ctx, MODE_HVP, c.prec, a, &nvec);
     if (rc != MEB_OK) return rc;
-    return meb_hvp_finalize(ctx, nvec, a.dpad, ctx->part_sc, ev_scalars, q, c.sigma, c.tau, c.d, Hq);
+    return meb_hvp_finalize(ctx, nvec, a.dpad, ctx->part_sc, ev_scalars, q, c.sigma, c.tau, c.d, Hq,
+                            c.gs ? c.gs->dyn : nullptr);
 }
 
 static int check_eval_args(const meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
@@ -236,10 +273,12 @@ extern "C" int meb_eval_alm(meb_ctx* ctx, int prec, int64_t m, int32_t d, const 
     int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
     if (rc != MEB_OK) return rc;
     if (!out_scalars || !grad || !(tau >= 0.0)) return MEB_E_ARG;
-    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, xbar, sigma, tau};
-    rc = meb_eval_internal(ctx, c, true, out_scalars, grad, t_out, lam_out);
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, xbar, sigma, tau, nullptr};
+    rc = meb_eval_internal(ctx, c, out_scalars, grad, t_out, lam_out);
     if (rc != MEB_OK) return rc;
     if (active_idx) {
+        rc = meb_ensure_list(ctx, m);
+        if (rc != MEB_OK) return rc;
         MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->count_dev, sizeof(int32_t),
                                          cudaMemcpyDeviceToHost, ctx->stream));
         MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
@@ -260,9 +299,9 @@ extern "C" int meb_hvp(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void*
     int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
     if (rc != MEB_OK) return rc;
     if (!q || !Hq || !(tau >= 0.0)) return MEB_E_ARG;
-    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, tau};
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, tau, nullptr};
     double* ev = ctx->small + SM_EV;
-    rc = meb_eval_internal(ctx, c, false, ev, ctx->small + SM_X, nullptr, nullptr);
+    rc = meb_eval_internal(ctx, c, ev, ctx->small + SM_X, nullptr, nullptr);
     if (rc != MEB_OK) return rc;
     return meb_hvp_from_records(ctx, c, ev, q, Hq);
 }
@@ -274,9 +313,9 @@ extern "C" int meb_dense_hessian(meb_ctx* ctx, int prec, int64_t m, int32_t d, c
     if (rc != MEB_OK) return rc;
     if (!H || !(tau >= 0.0)) return MEB_E_ARG;
     if (d > 128) return MEB_E_CAPACITY;
-    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, tau};
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, tau, nullptr};
     double* ev = ctx->small + SM_EV;
-    rc = meb_eval_internal(ctx, c, false, ev, ctx->small + SM_X, nullptr, nullptr);
+    rc = meb_eval_internal(ctx, c, ev, ctx->small + SM_X, nullptr, nullptr);
     if (rc != MEB_OK) return rc;
     return meb_dense_from_records(ctx, c, ev, H);
 }
@@ -289,8 +328,10 @@ extern "C" int meb_update_multipliers(meb_ctx* ctx, int prec, int64_t m, int32_t
     int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
     if (rc != MEB_OK) return rc;
     if (!U_out || !v_slot_out || !Vrows_out || ldv_out < d || cap_rows < 0) return MEB_E_ARG;
-    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, 0.0};
-    rc = meb_eval_internal(ctx, c, false, ctx->small + SM_EV, ctx->small + SM_X, nullptr, nullptr);
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, nullptr, sigma, 0.0, nullptr};
+    rc = meb_eval_internal(ctx, c, ctx->small + SM_EV, ctx->small + SM_X, nullptr, nullptr);
+    if (rc != MEB_OK) return rc;
+    rc = meb_ensure_list(ctx, m);
     if (rc != MEB_OK) return rc;
     if (prec == MEB_FP64) rc = meb_fill_f64(ctx, (double*)U_out, m, 0.0);
     else rc = meb_fill_f32(ctx, (float*)U_out, m, 0.f);
@@ -347,7 +388,7 @@ extern "C" int meb_screen_compact(meb_ctx* ctx, int64_t m, int32_t d, const floa
         s.mask = ctx->mask; s.part = ctx->part_scalar; s.eps = (double)tol_red; s.flags_out = flags;
         int grid = 0;
         ctx->cur_class = MEB_PASS_SCREEN;
-        rc = timed_stream(ctx, OP_SCREEN, MEB_FP32, s, (double)m * (d * 4.0 + (R32 ? 4 : 0)), &grid);
+        rc = timed_stream(ctx, OP_SCREEN, MEB_FP32, s, (double)m * (d * 4.0 + (R32 ? 4 : 0)), &grid, nullptr);
         if (rc != MEB_OK) return rc;
     }
     rc = meb_launch_compact_cap(ctx, ctx->mask, m, idx_out, cap, ctx->count_dev);
@@ -375,7 +416,7 @@ extern "C" int meb_feasibility_check(meb_ctx* ctx, int64_t m, int32_t d, const d
     s.mask = ctx->mask; s.part = ctx->part_scalar; s.eps = eps_feas; s.kept = kept_mask;
     int grid = 0;
     ctx->cur_class = MEB_PASS_FEAS;
-    rc = timed_stream(ctx, OP_FEAS, MEB_FP64, s, (double)m * (d * 8.0 + (R ? 8 : 0) + (kept_mask ? 1 : 0)), &grid);
+    rc = timed_stream(ctx, OP_FEAS, MEB_FP64, s, (double)m * (d * 8.0 + (R ? 8 : 0) + (kept_mask ? 1 : 0)), &grid, nullptr);
     if (rc != MEB_OK) return rc;
     rc = meb_argmax_finalize(ctx, grid, ctx->small + SM_AUX);
     if (rc != MEB_OK) return rc;
@@ -411,7 +452,7 @@ extern "C" int meb_ingest(meb_ctx* ctx, int64_t m, int32_t d, const double* C, i
     int grid = 0;
     const double bytes = (double)m * (d * 8.0 + (R ? 8 : 0)) + (C32 ? (double)m * (d * 4.0 + (R ? 4 : 0)) : 0.0);
     ctx->cur_class = MEB_PASS_INGEST;
-    rc = timed_stream(ctx, OP_INGEST, MEB_FP64, s, bytes, &grid);
+    rc = timed_stream(ctx, OP_INGEST, MEB_FP64, s, bytes, &grid, nullptr);
     if (rc != MEB_OK) return rc;
     return meb_argmax_finalize(ctx, grid, scalars_out);
 }

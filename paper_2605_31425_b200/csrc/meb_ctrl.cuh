@@ -1,0 +1,185 @@
+// Device-resident state of Algorithm 1 (ripALM) and Algorithm 2 (semismooth Newton,
+// P:L220-242), and the single-CTA controller steps that advance it inside a CUDA graph WHILE loop.
+// No host round trip happens between the evaluations of a phase: the controllers decide on the
+// device what runs next (another Armijo trial, a Newton solve, a multiplier update) by setting the
+// graph's conditional handles.
+//
+// Units (reading 3): the (d+1)-sized state lives in normalised units x~ = (r/L, (c - off)/L); the
+// streaming kernels run on the raw data with x_raw = (L r~, off + L c~), sigma_raw = sigma/L,
+// tau_eff = tau/L^2.  g and the multipliers are the same in both unit systems, psi~ = psi_raw/L.
+#pragma once
+#include "meb_internal.cuh"
+
+enum { PH_FIRST = 0,      // first evaluation of an outer iteration (Alg. 2 lines 3-4): always accepted
+       PH_ARMIJO = 1,     // evaluation of an Armijo trial point x + eta*Delta (Alg. 2 line 9)
+       PH_REEVAL = 2 };   // re-evaluation at x before a multiplier update (records of the last pass are stale)
+enum { ACT_TRIAL = 0, ACT_NEWTON = 1, ACT_UPDATE = 2, ACT_DONE = 3 };
+enum { ST_RUNNING = 0, ST_CONVERGED = 1, ST_OUTER_CAP = 2, ST_NEED_CAPACITY = 3, ST_CHOL_FAILED = 4 };
+
+struct SolverDev {
+    // ---- constants of the phase (written by the host before the graph is launched) ----
+    double L, tol, rho, tau, kappa, sigma_max, armijo_mu;
+    int32_t n, d, inner_max, outer_max, armijo_max, cg_max, dense, use_off;
+    int64_t vcap[2];              // rows available in the two V pools
+    // ---- dynamic ----
+    MebDyn dyn;                   // what the streaming kernels read: sigma_raw, tau_eff, cur, has_mult
+    double sigma;                 // normalised sigma_k
+    double eta, psi_cur, slope;
+    int32_t phase, action, outer, inner, ls, done, status, stalled;
+    int32_t newton_total, cg_total, evals, chol_info;
+    double kkt, terms[5];
+    int64_t n_support;
+    double cg_rr, cg_tol;
+    int32_t cg_it, cg_go;
+    // ---- in-graph timing of the evaluation passes (globaltimer, ns) ----
+    unsigned long long pass_ns;
+    long long pass_count;
+    // ---- conditional handles of the solve graph ----
+    cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
+    int32_t in_graph, pad;
+};
+
+// (d+1)-vectors of the state, each of length nv = n rounded up to 8, in one device array
+struct SolverVecs {
+    double *xn, *xbar, *ab, *delta, *g, *xt, *x_raw, *xbar_raw, *off, *grad_t, *res, *p, *Hp;
+    double *ev_t, *ev;           // [MEB_EVAL_NSCALARS] scalars of the trial / accepted evaluation
+};
+
+// arguments of the evaluation-finalize kernel (meb_small.cu)
+struct FinalizeArgs {
+    const double* part; int grid;                 // per-CTA scalar partials of the streaming kernel
+    const double* part_vec; int nvec; int tpb;    // per-CTA vector partials; tpb > 0: written by the active-list
+    int dpad;                                     //   kernel (only CTAs b < ceil(count/tpb) hold data); 0: all nvec
+    const int32_t* count;
+    const double* x; const double* xbar;
+    double sigma, tau; int d;
+    double* out; double* grad;
+    const MebDyn* dyn;                            // nullable: overrides sigma, tau
+    SolverDev* S; SolverVecs v;                   // nullable: controller step of the solve graph
+};
+
+__device__ __forceinline__ double ctrl_block_sum(double v, double* sm) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    const int nw = (blockDim.x + 31) >> 5;
+    for (int w = 0; w < nw; ++w) t += sm[w];
+    return t;
+}
+
+// x_raw = (L r~, off + L c~)
+__device__ __forceinline__ void ctrl_to_raw(const SolverDev* S, const SolverVecs& v, const double* xn_, double* out) {
+    for (int j = threadIdx.x; j < S->n; j += blockDim.x)
+        out[j] = (j == 0) ? S->L * xn_[0] : ((S->use_off ? v.off[j - 1] : 0.0) + S->L * xn_[j]);
+}
+
+__device__ __forceinline__ void ctrl_set_handles(const SolverDev* S) {
+    if (!S->in_graph) return;
+    cudaGraphSetConditional(S->h_while, S->done ? 0u : 1u);
+    cudaGraphSetConditional(S->h_newton, (!S->done && S->action == ACT_NEWTON) ? 1u : 0u);
+    cudaGraphSetConditional(S->h_update, (!S->done && S->action == ACT_UPDATE) ? 1u : 0u);
+    cudaGraphSetConditional(S->h_cg, (!S->done && S->action == ACT_NEWTON && !S->dense && S->cg_go) ? 1u : 0u);
+}
+
+// relative KKT residual (reading 7) from the scalars of an evaluation
+__device__ __forceinline__ double ctrl_rel_kkt(const double* ev, double r_raw, double* terms) {
+    terms[0] = fabs(1.0 - ev[MEB_EV_SUM_UPLUS]);
+    terms[1] = ev[MEB_EV_NORM_SUM_VPLUS];
+    terms[2] = ev[MEB_EV_MAX_PFEAS] / (1.0 + r_raw);
+    terms[3] = ev[MEB_EV_MAX_DFEAS];
+    terms[4] = ev[MEB_EV_MAX_COMPL] / (1.0 + r_raw);
+    double k = 0.0;
+    for (int i = 0; i < 5; ++i) k = fmax(k, terms[i]);
+    return k;
+}
+
+// Runs in the single CTA of the evaluation-finalize kernel, after ev_t / grad_t of the pass at
+// x_raw have been written: Armijo test (reading 4), stopping tests (5) and KKT (P:L133-135,
+// L244, reading 6), choice of the next action.  All threads of the CTA call it.
+__device__ inline void ctrl_after_eval(SolverDev* S, const SolverVecs v, double* sm) {
+    __syncthreads();
+    const int n = S->n;
+    const int phase = S->phase;
+    const double psi_t = v.ev_t[MEB_EV_PSI] / S->L;
+    bool accept = true, stalled = false;
+    if (phase == PH_ARMIJO) {
+        if (!(psi_t <= S->psi_cur + S->armijo_mu * S->eta * S->slope)) {
+            if (S->ls >= S->armijo_max) {
+                stalled = true;
+                accept = psi_t <= S->psi_cur;          // last trial did not increase Psi: take it
+            } else {
+                accept = false;
+            }
+        }
+    }
+    __syncthreads();
+    if (!accept) {
+        if (stalled) {                                 // records of this pass are not those of x: re-evaluate
+            ctrl_to_raw(S, v, v.xn, v.x_raw);
+            __syncthreads();
+            if (threadIdx.x == 0) { S->phase = PH_REEVAL; S->action = ACT_TRIAL; S->evals++; ctrl_set_handles(S); }
+        } else {                                       // halve the step
+            const double eta = 0.5 * S->eta;
+            for (int j = threadIdx.x; j < n; j += blockDim.x) v.xt[j] = v.xn[j] + eta * v.delta[j];
+            __syncthreads();
+            ctrl_to_raw(S, v, v.xt, v.x_raw);
+            __syncthreads();
+            if (threadIdx.x == 0) { S->eta = eta; S->ls++; S->action = ACT_TRIAL; S->evals++; ctrl_set_handles(S); }
+        }
+        return;
+    }
+    // ---- accepted: the pass becomes the evaluation at x ----
+    if (phase == PH_ARMIJO)
+        for (int j = threadIdx.x; j < n; j += blockDim.x) v.xn[j] = v.xt[j];
+    for (int j = threadIdx.x; j < n; j += blockDim.x) v.g[j] = v.grad_t[j];
+    if (threadIdx.x < MEB_EVAL_NSCALARS) v.ev[threadIdx.x] = v.ev_t[threadIdx.x];
+    __syncthreads();
+    // condition (5): 2 sigma |<(alpha,beta) - x, g>| + sigma^2 ||g||^2 <= rho (sum ||dmult||^2 + tau ||x - xbar||^2)
+    double agx = 0.0, gg = 0.0, dx2 = 0.0;
+    for (int j = threadIdx.x; j < n; j += blockDim.x) {
+        const double gj = v.g[j], xj = v.xn[j];
+        agx = fma(v.ab[j] - xj, gj, agx);
+        gg = fma(gj, gj, gg);
+        const double dx = xj - v.xbar[j];
+        dx2 = fma(dx, dx, dx2);
+    }
+    agx = ctrl_block_sum(agx, sm);
+    gg = ctrl_block_sum(gg, sm);
+    dx2 = ctrl_block_sum(dx2, sm);
+    if (threadIdx.x == 0) {
+        S->evals++;
+        S->psi_cur = psi_t;
+        double terms[5];
+        const double kkt = ctrl_rel_kkt(v.ev, S->L * v.xn[0], terms);
+        S->kkt = kkt;
+        for (int i = 0; i < 5; ++i) S->terms[i] = terms[i];
+        const double sg = S->sigma;
+        const double lhs = 2.0 * sg * fabs(agx) + sg * sg * gg;
+        const double rhs = S->rho * (v.ev[MEB_EV_SUM_DMULT2] + S->tau * dx2);
+        const bool exit_inner = (phase == PH_REEVAL) || stalled || lhs <= rhs || kkt <= S->tol ||
+                                S->inner >= S->inner_max;
+        if (exit_inner) {
+            S->action = ACT_UPDATE;
+        } else {
+            S->action = ACT_NEWTON;
+            S->inner++;
+            S->newton_total++;
+            // CG start (matrix-free path): delta = 0, res = p = -g, stop at min(0.1, ||g||) ||g||  (reading 5)
+            const double gn = sqrt(gg);
+            S->cg_rr = gg;
+            S->cg_tol = fmin(0.1, gn) * gn;
+            S->cg_it = 0;
+            S->cg_go = (gn > S->cg_tol && S->cg_max > 0) ? 1 : 0;
+        }
+        ctrl_set_handles(S);
+    }
+    __syncthreads();
+    if (S->action == ACT_NEWTON && !S->dense)
+        for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            v.delta[j] = 0.0;
+            v.res[j] = -v.g[j];
+            v.p[j] = -v.g[j];
+        }
+}

@@ -17,8 +17,10 @@ namespace {
 constexpr int RB = 16;      // rows per shared tile
 
 template <typename T, int BS>
-__global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a, double* __restrict__ part_mat,
+__global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a_in, double* __restrict__ part_mat,
                                                           int dp) {
+    ActiveArgs a = a_in;
+    meb_resolve_dyn(a);
     extern __shared__ __align__(16) double sm[];          // W[RB][dp] then rho[RB]
     double* W = sm;
     double* rho_s = sm + (size_t)RB * dp;
@@ -107,7 +109,9 @@ __global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a, dou
 __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __restrict__ part_mat, int nparts,
                                                              const int32_t* __restrict__ count,
                                                              int dp, int d, const double* __restrict__ ev,
-                                                             double sigma, double tau, double* __restrict__ H) {
+                                                             double sigma, double tau, double* __restrict__ H,
+                                                             const MebDyn* __restrict__ dyn) {
+    if (dyn) { sigma = dyn->sigma_raw; tau = dyn->tau_eff; }
     const int ntiles = (*count + RB - 1) / RB;            // CTAs b < ntiles wrote a partial
     if (nparts > ntiles) nparts = ntiles;
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
@@ -134,46 +138,76 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
     }
 }
 
-// Solve (scale * H) delta = -g for one SPD matrix of order n <= 256 held in shared memory.
-// Square-root-free Cholesky (H = L D L^T, no pivoting: H is SPD) on the AUGMENTED lower
-// triangle [H; -g^T]: eliminating column k also updates the right-hand-side row, so after the n
-// column steps row n holds D L^{-1}(-g) and only the backward substitution with L^T is left.
-// One __syncthreads per column; 16 x 16 threads own an interleaved 2-D slice of the trailing
-// block (no integer division, conflict-free shared accesses with an odd leading dimension).
-__global__ void __launch_bounds__(256) chol_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
+// Solve (scale * H) delta = -g for one SPD matrix of order n <= 16*BS - 1, one CTA of 16 x 16 threads.
+// Square-root-free Cholesky (H = L D L^T, no pivoting: H is SPD) on the AUGMENTED matrix
+// M = [H; -g^T]: eliminating column k also updates the right-hand-side row n, so after the n column
+// steps row n holds D L^{-1}(-g) and only the backward substitution with L^T is left.
+// The matrix lives in REGISTERS: thread (ty, tx) owns M[ty + 16 ii][tx + 16 jj], ii, jj < BS.  Per
+// column k the owners publish column k to shared memory (kept there as row k of Lm = L D for the
+// backward substitution), one __syncthreads, then every thread updates its live entries with
+// broadcast / conflict-free shared reads and register FMAs.
+template <int BS>
+__global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
                                                          int n, double scale, double* __restrict__ delta,
                                                          int* __restrict__ info) {
-    extern __shared__ __align__(16) double A[];           // (n+1) rows x lda, then invd[n]
-    const int lda = (n + 1) | 1;
-    double* invd = A + (size_t)(n + 1) * lda;
+    extern __shared__ __align__(16) double Lm[];          // n rows x ldl (column k of L D as row k), invd[n], z[n]
+    constexpr int NP = 16 * BS;
+    const int ldl = NP | 1;
+    double* invd = Lm + (size_t)n * ldl;
+    double* z = invd + NP;
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    for (int i = ty; i < n; i += 16)
-        for (int j = tx; j <= i; j += 16) A[(size_t)i * lda + j] = scale * H[(size_t)i * n + j];
-    for (int j = tid; j < n; j += 256) A[(size_t)n * lda + j] = -g[j];
+    double a[BS][BS];
+#pragma unroll
+    for (int ii = 0; ii < BS; ++ii)
+#pragma unroll
+        for (int jj = 0; jj < BS; ++jj) {
+            const int i = ty + 16 * ii, j = tx + 16 * jj;
+            double v = 0.0;
+            if (j < n && j <= i) {
+                if (i < n) v = scale * H[(size_t)i * n + j];
+                else if (i == n) v = -g[j];
+            }
+            a[ii][jj] = v;
+        }
     __shared__ int bad;
     if (tid == 0) bad = 0;
     for (int k = 0; k < n; ++k) {
+        double* col = Lm + (size_t)k * ldl;
+        if (tx == (k & 15)) {                             // owners of column k publish rows i >= k
+            const int jk = k >> 4;
+#pragma unroll
+            for (int jj = 0; jj < BS; ++jj)
+                if (jj == jk) {
+#pragma unroll
+                    for (int ii = 0; ii < BS; ++ii) col[ty + 16 * ii] = a[ii][jj];
+                }
+        }
         __syncthreads();
-        double dk = A[(size_t)k * lda + k];
+        double dk = col[k];
         if (!(dk > 0.0)) { if (tid == 0) bad = k + 1; dk = 1.0; }
         const double inv = 1.0 / dk;
         if (tid == 0) invd[k] = inv;
-        for (int i = k + 1 + ty; i <= n; i += 16) {
-            const double lik = A[(size_t)i * lda + k] * inv;
-            const int jmax = i < n ? i : n - 1;
-            for (int j = k + 1 + tx; j <= jmax; j += 16)
-                A[(size_t)i * lda + j] = fma(-lik, A[(size_t)j * lda + k], A[(size_t)i * lda + j]);
+#pragma unroll
+        for (int ii = 0; ii < BS; ++ii) {
+            const int i = ty + 16 * ii;
+            if (16 * ii + 15 > k && i > k && i <= n) {
+                const double lik = col[i] * inv;
+#pragma unroll
+                for (int jj = 0; jj <= ii; ++jj) {
+                    const int j = tx + 16 * jj;
+                    if (j > k && j <= i) a[ii][jj] = fma(-lik, col[j], a[ii][jj]);
+                }
+            }
         }
     }
     __syncthreads();
-    // z = D^{-1} (row n); then L^T x = z, column-oriented, one warp (L_kj = A[k][j] * invd[j])
-    double* z = A + (size_t)n * lda;
+    // z = D^{-1} (row n of L D); then L^T x = z, column-oriented, one warp: L_kj = Lm[j][k] * invd[j]
     if (tid < 32) {
-        for (int j = tid; j < n; j += 32) z[j] *= invd[j];
+        for (int j = tid; j < n; j += 32) z[j] = Lm[(size_t)j * ldl + n] * invd[j];
         __syncwarp();
         for (int k = n - 1; k > 0; --k) {
             const double xk = z[k];
-            for (int j = tid; j < k; j += 32) z[j] = fma(-A[(size_t)k * lda + j] * invd[j], xk, z[j]);
+            for (int j = tid; j < k; j += 32) z[j] = fma(-Lm[(size_t)j * ldl + k] * invd[j], xk, z[j]);
             __syncwarp();
         }
     }
@@ -202,6 +236,7 @@ int launch_syrk(meb_ctx* ctx, const ActiveArgs& a, int dp, double* part_mat, int
 // H (device, (d+1)^2) from the records of the last streaming pass.  d <= 128.
 int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, double* H) {
     if (c.d > 128) return MEB_E_CAPACITY;
+    { const int rcl = meb_ensure_list(ctx, c.m); if (rcl != MEB_OK) return rcl; }
     const int dp = (c.d + 15) / 16 * 16;
     const size_t per = (size_t)dp * dp + dp;
     const size_t avail = ctx->part_mat_len;
@@ -213,6 +248,10 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
     a.C = c.C; a.ld = c.ld; a.U = c.U; a.v_slot = c.v_slot; a.V = c.V; a.ldv = c.ldv; a.x = c.x; a.d = c.d;
     a.sigma = c.sigma; a.list = ctx->list; a.count = ctx->count_dev;
     a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
+    if (c.gs) {
+        a.dyn = c.gs->dyn;
+        for (int b = 0; b < 2; ++b) { a.U2[b] = c.gs->U2[b]; a.slot2[b] = c.gs->slot2[b]; a.V2[b] = c.gs->V2[b]; a.vcap2[b] = c.gs->vcap2[b]; }
+    }
     int rc = c.prec == MEB_FP64 ? launch_syrk<double>(ctx, a, dp, ctx->part_mat, grid)
                                 : launch_syrk<float>(ctx, a, dp, ctx->part_mat, grid);
     if (rc != MEB_OK) return rc;
@@ -220,7 +259,7 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
     int fgrid = (n * n + 255) / 256;
     if (fgrid > 64) fgrid = 64;
     ctx->launches++; dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, ctx->count_dev, dp, c.d, ev_scalars, c.sigma,
-                                                          c.tau, H);
+                                                          c.tau, H, c.gs ? c.gs->dyn : nullptr);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
@@ -228,11 +267,23 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
 // delta <- -(scale*H)^{-1} g on the device; info_dev (nullable) receives 0 or the failing pivot + 1
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
                    int* info_dev) {
-    const size_t smem = ((size_t)(n + 1) * ((n + 1) | 1) + n) * sizeof(double);
-    if (smem > 220 * 1024) return MEB_E_CAPACITY;
-    MEB_CUDA_OK(ctx, cudaFuncSetAttribute(chol_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)smem));
-    ctx->launches++; chol_solve_kernel<<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev);
+    const int bs = (n + 1 + 15) / 16;                       // augmented order n + 1 <= 16 bs
+    if (bs > 9) return MEB_E_CAPACITY;
+    const int np = 16 * bs;
+    const size_t smem = ((size_t)n * (np | 1) + 2 * (size_t)np) * sizeof(double);
+#define MEB_LDLT_CASE(B)                                                                                        \
+    case B:                                                                                                     \
+        MEB_CUDA_OK(ctx, cudaFuncSetAttribute(ldlt_solve_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                              (int)smem));                                                      \
+        ctx->launches++;                                                                                        \
+        ldlt_solve_kernel<B><<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev);                   \
+        break;
+    switch (bs) {
+        MEB_LDLT_CASE(1) MEB_LDLT_CASE(2) MEB_LDLT_CASE(3) MEB_LDLT_CASE(4) MEB_LDLT_CASE(5)
+        MEB_LDLT_CASE(6) MEB_LDLT_CASE(7) MEB_LDLT_CASE(8) MEB_LDLT_CASE(9)
+        default: return MEB_E_CAPACITY;
+    }
+#undef MEB_LDLT_CASE
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -38,6 +38,7 @@ struct meb_ctx {
     int32_t* count_dev;     // [8] device counters (compaction totals)
     double* part_sc;        // [1024] per-CTA scalar partials of the active-list kernels
     int last_grid;          // CTAs of the last streaming launch (its partials are still in part_scalar)
+    bool list_valid;        // ctx->list / count_dev hold the compaction of the mask of the last streaming pass
     double* small;          // small device state: scalars, vectors of length d+1 (see meb_api.cu)
     int64_t small_len;
     double* h_pinned;       // pinned host mirror for small read-backs
@@ -99,6 +100,14 @@ __device__ __forceinline__ double warp_max(double v) {
     return v;
 }
 
+// Parameters that change while a solve graph runs live in device memory (no host round trip):
+struct MebDyn {
+    double sigma_raw;       // sigma / L   (reading 3: kernels run on the raw data)
+    double tau_eff;         // tau / L^2
+    int32_t cur;            // which of the two multiplier buffers holds (U, V) of the current outer iteration
+    int32_t has_mult;       // 0: all multipliers are zero (first outer iteration)
+};
+
 // host-side launch helpers implemented in the .cu files -------------------------------------------
 struct StreamArgs {
     const void* C; int64_t ld;
@@ -118,11 +127,33 @@ struct StreamArgs {
     double eps; const uint8_t* kept; uint8_t* flags_out;
     // ingest
     float* C32; int64_t ld32; float* R32; const double* c0;
+    // fused evaluation (meb_tile.cu): per-CTA partial of sum_i lam_i b_i, [grid][dpad]
+    double* part_vec; int32_t dpad;
+    // device-resident parameters (solve graph): if dyn != nullptr it overrides sigma, U, v_slot, V
+    const MebDyn* dyn;
+    const void* U2[2]; const int32_t* slot2[2]; const void* V2[2];
 };
+
+// resolves the device-resident parameters of a solve graph into the plain fields
+__device__ __forceinline__ void meb_resolve_dyn(StreamArgs& a) {
+    if (a.dyn) {
+        const int cur = a.dyn->cur;
+        const bool hm = a.dyn->has_mult != 0;
+        a.sigma = a.dyn->sigma_raw;
+        a.U = hm ? a.U2[cur] : nullptr;
+        a.v_slot = hm ? a.slot2[cur] : nullptr;
+        a.V = hm ? a.V2[cur] : nullptr;
+    }
+}
 
 enum StreamOp { OP_EVAL = 0, OP_FEAS = 1, OP_SCREEN = 2, OP_INGEST = 3 };
 
 int meb_launch_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out);
+// TMA-staged lane-per-row kernels (meb_tile.cu).  meb_tile_applicable: rows of at most 1024 bytes whose
+// start and stride are multiples of 16 bytes.  For OP_EVAL the kernel also accumulates sum_i lam_i b_i
+// (a.part_vec), so no active-list pass is needed for the gradient.
+bool meb_tile_applicable(int op, int prec, const StreamArgs& a);
+int meb_launch_tile(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out);
 int meb_launch_compact(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* list, int32_t* count_dev);
 
 // ---- active-list passes (meb_active.cu) ----
@@ -141,7 +172,24 @@ struct ActiveArgs {
     double* part_vec;                // [grid][dpad]
     double* part_sc;                 // [grid][2]
     void* U_out; int32_t* slot_out; void* V_out; int64_t ldv_out; int64_t cap_rows;
+    // device-resident parameters (solve graph): override sigma, U, v_slot, V and, for MODE_WRITEV,
+    // the output buffers (the multiplier buffer that is NOT current)
+    const MebDyn* dyn;
+    void* U2[2]; int32_t* slot2[2]; void* V2[2]; int64_t vcap2[2];
 };
+
+__device__ __forceinline__ void meb_resolve_dyn(ActiveArgs& a) {
+    if (a.dyn) {
+        const int cur = a.dyn->cur;
+        const bool hm = a.dyn->has_mult != 0;
+        const int nxt = hm ? 1 - cur : 0;
+        a.sigma = a.dyn->sigma_raw;
+        a.U = hm ? a.U2[cur] : nullptr;
+        a.v_slot = hm ? a.slot2[cur] : nullptr;
+        a.V = hm ? a.V2[cur] : nullptr;
+        a.U_out = a.U2[nxt]; a.slot_out = a.slot2[nxt]; a.V_out = a.V2[nxt]; a.cap_rows = a.vcap2[nxt];
+    }
+}
 
 
 int meb_launch_active(meb_ctx* ctx, int mode, int prec, const ActiveArgs& a, int* grid_out);
@@ -150,10 +198,10 @@ int meb_launch_compact_cap(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_
 int meb_launch_flags_to_mask(meb_ctx* ctx, const uint8_t* flags, int64_t m, uint32_t* mask);
 
 // ---- second-level reductions and small kernels (meb_small.cu) ----
-int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t* count, const double* x,
-                      const double* xbar, double sigma, double tau, int d, double* out, double* grad);
+struct FinalizeArgs;
+int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f);
 int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
-                     const double* q, double sigma, double tau, int d, double* Hq);
+                     const double* q, double sigma, double tau, int d, double* Hq, const MebDyn* dyn);
 int meb_argmax_finalize(meb_ctx* ctx, int grid, double* out);
 int meb_scalar_sum(meb_ctx* ctx, const double* v, int n, double* out);
 int meb_sample_mean(meb_ctx* ctx, const double* C, int64_t ld, int64_t m, int d, int S, double* c0);
@@ -170,17 +218,28 @@ int meb_set_kept(meb_ctx* ctx, const int32_t* idx, int64_t n, uint8_t* kept);
 
 // ---- internal composite passes (meb_api.cu), used by the solver ----
 // layout of ctx->small (doubles): see meb_api.cu
+struct SolverDev;
+struct SolverVecs;
+// device-resident side of a call made while a solve graph is being captured: the multipliers are
+// double-buffered and selected on the device by dyn->cur; sigma and tau come from dyn
+struct GraphSide {
+    const MebDyn* dyn;
+    void* U2[2]; int32_t* slot2[2]; void* V2[2]; int64_t vcap2[2];
+    SolverDev* S; const SolverVecs* v;
+};
 struct EvalCall {
     int prec; int64_t m; int32_t d;
     const void* C; int64_t ld; const void* R; const void* U;
     const int32_t* v_slot; const void* V; int64_t ldv;
     const double* x; const double* xbar; double sigma; double tau;
+    const GraphSide* gs;         // nullable
 };
-// streaming pass + compaction of the active set (+ gradient vector part unless psi_only)
-int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, bool want_grad, double* out_scalars, double* grad,
+// One evaluation: streaming pass (+ the vector part of the gradient: fused in the tile kernel, or by
+// the active-list kernel after a compaction) + finalize.  The active list is built lazily
+// (meb_ensure_list) because only the Newton solve and the multiplier update need it.
+int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, double* out_scalars, double* grad,
                       double* t_out, double* lam_out);
-// gradient vector part for the records of the LAST streaming pass (same C, x, V as that pass)
-int meb_grad_from_records(meb_ctx* ctx, const EvalCall& c, double* out_scalars, double* grad);
+int meb_ensure_list(meb_ctx* ctx, int64_t m);
 int meb_hvp_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, const double* q, double* Hq);
 
 // ---- dense Hessian and Cholesky (meb_dense.cu) ----

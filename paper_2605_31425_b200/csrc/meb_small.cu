@@ -2,6 +2,7 @@
 // Single-CTA kernels: their inputs are the per-CTA partials written by the streaming / active-list
 // kernels (a few thousand doubles), so they are latency-, not bandwidth-bound.
 #include "meb_internal.cuh"
+#include "meb_ctrl.cuh"
 
 namespace {
 
@@ -30,40 +31,87 @@ __device__ __forceinline__ double partial_max(const double* part, int grid, int 
     return warp_max(s);
 }
 
-// out_scalars / grad of one ALM evaluation (reading 13 for psi_var)
-__global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
-    const double* __restrict__ part, int grid, const double* __restrict__ part_vec, int nvec, int tpb, int dpad,
-    const int32_t* __restrict__ count, const double* __restrict__ x, const double* __restrict__ xbar,
-    double sigma, double tau, int d, double* __restrict__ out, double* __restrict__ grad) {
+// out_scalars / grad of one ALM evaluation (reading 13 for psi_var).  Second level of the
+// fixed-order reduction: CTA partials are added in index order (in S interleaved segments that are
+// then added in order, so the order does not depend on timing).  With f.S != nullptr the same CTA then
+// runs the controller step of the device-resident solver (meb_ctrl.cuh).
+__global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArgs f) {
     __shared__ double sm[FBLOCK / 32];
     __shared__ double sc[MEB_NPART];
+    __shared__ double seg[FBLOCK];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double* __restrict__ part = f.part;
+    const double* __restrict__ part_vec = f.part_vec;
+    const int grid = f.grid, d = f.d, dpad = f.dpad;
+    double sigma = f.sigma, tau = f.tau;
+    if (f.dyn) { sigma = f.dyn->sigma_raw; tau = f.dyn->tau_eff; }
+    const double* x = f.x; const double* xbar = f.xbar;
     if (warp < 9) {
         double v;
         if (warp >= 5 && warp <= 7) v = partial_max(part, grid, warp, lane);
         else v = partial_sum(part, grid, warp, lane);
         if (lane == 0) sc[warp] = v;
+    } else if (warp == 9 && f.S) {
+        // device time of the pass: last CTA end - first CTA start (globaltimer stamps of the tile kernel)
+        long long t0 = 0x7fffffffffffffffLL, t1 = 0;
+        for (int b = lane; b < grid; b += 32) {
+            const long long s0 = __double_as_longlong(part[(size_t)b * MEB_NPART + 10]);
+            const long long s1 = __double_as_longlong(part[(size_t)b * MEB_NPART + 11]);
+            if (s1 > 0) { t0 = min(t0, s0); t1 = max(t1, s1); }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            t0 = min(t0, __shfl_xor_sync(MEB_FULL_MASK, t0, o));
+            t1 = max(t1, __shfl_xor_sync(MEB_FULL_MASK, t1, o));
+        }
+        if (lane == 0 && t1 > t0) { f.S->pass_ns += (unsigned long long)(t1 - t0); f.S->pass_count++; }
     }
-    // vector part: sum_i v+_i = sigma * sum_k lam_k b_k (only CTAs b < ceil(count/tpb) had list entries)
-    if (nvec > 0) { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
+    // vector part: sum_i v+_i = sigma * sum_k lam_k b_k
+    int nvec = f.nvec;
+    if (nvec > 0 && f.tpb > 0) {           // active-list kernel: only CTAs b < ceil(count/tpb) had entries
+        const int used = (*f.count + f.tpb - 1) / f.tpb;
+        if (nvec > used) nvec = used;
+    }
     double nv2 = 0.0, dx2 = 0.0;
     const double tos = tau / sigma;
-    for (int j = threadIdx.x; j < d; j += FBLOCK) {
+    if (d <= FBLOCK) {
+        const int dr = (d + 31) & ~31;
+        int S = FBLOCK / dr;
+        if (S > 32) S = 32;
+        const int j = threadIdx.x % dr, sg = threadIdx.x / dr;
         double s = 0.0;
-        for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
-        const double sv = sigma * s;
-        const double dx = x[1 + j] - (xbar ? xbar[1 + j] : x[1 + j]);
-        grad[1 + j] = -sv + tos * dx;
-        nv2 = fma(sv, sv, nv2);
-        dx2 = fma(dx, dx, dx2);
+        if (sg < S && j < d)
+            for (int b = sg; b < nvec; b += S) s += part_vec[(size_t)b * dpad + j];
+        seg[threadIdx.x] = s;
+        __syncthreads();
+        if (threadIdx.x < d) {
+            double t = 0.0;
+            for (int q = 0; q < S; ++q) t += seg[q * dr + threadIdx.x];
+            const double sv = sigma * t;
+            const double dx = x[1 + threadIdx.x] - (xbar ? xbar[1 + threadIdx.x] : x[1 + threadIdx.x]);
+            f.grad[1 + threadIdx.x] = -sv + tos * dx;
+            nv2 = sv * sv;
+            dx2 = dx * dx;
+        }
+    } else {
+        for (int j = threadIdx.x; j < d; j += FBLOCK) {
+            double s = 0.0;
+            for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
+            const double sv = sigma * s;
+            const double dx = x[1 + j] - (xbar ? xbar[1 + j] : x[1 + j]);
+            f.grad[1 + j] = -sv + tos * dx;
+            nv2 = fma(sv, sv, nv2);
+            dx2 = fma(dx, dx, dx2);
+        }
     }
     nv2 = block_sum_1024(nv2, sm);
     dx2 = block_sum_1024(dx2, sm);
     __syncthreads();
     if (threadIdx.x == 0) {
+        double* out = f.out;
         const double dx0 = x[0] - (xbar ? xbar[0] : x[0]);
         dx2 += dx0 * dx0;
-        grad[0] = 1.0 - sc[1] + tos * dx0;
+        f.grad[0] = 1.0 - sc[1] + tos * dx0;
         out[MEB_EV_PSI] = x[0] + 0.5 * sigma * sc[0] + 0.5 * tos * dx2;
         out[MEB_EV_SUM_UPLUS] = sc[1];
         out[MEB_EV_SUM_PROJ2] = sc[0];
@@ -75,10 +123,11 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
         out[MEB_EV_MAX_DFEAS] = sc[7];
         out[MEB_EV_SUM_RHO] = sc[8];
         out[MEB_EV_NORM_SUM_VPLUS] = sqrt(nv2);
-        out[MEB_EV_N_ACTIVE] = (double)(*count);
+        out[MEB_EV_N_ACTIVE] = sc[3] + sc[4];          // active <=> branch B1 or B3
         out[12] = dx2;
         out[13] = 0.0; out[14] = 0.0; out[15] = 0.0;
     }
+    if (f.S) ctrl_after_eval(f.S, f.v, sm);
 }
 
 // H q from the active-list partials (reading 1):
@@ -86,8 +135,9 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(
 //  (Hq)_1 = (tau/sigma) q1 + sigma [ n1 q1 + 1/2 (sum_{B3} coef b + (n3 + sum rho) q1) ]
 __global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
     const double* __restrict__ part_vec, int nvec, int tpb, const int32_t* __restrict__ count, int dpad,
-    const double* __restrict__ part_sc, const double* __restrict__ ev, const double* __restrict__ q, double sigma, double tau, int d,
-    double* __restrict__ Hq) {
+    const double* __restrict__ part_sc, const double* __restrict__ ev, const double* __restrict__ q,
+    double sigma, double tau, int d, double* __restrict__ Hq, const MebDyn* __restrict__ dyn) {
+    if (dyn) { sigma = dyn->sigma_raw; tau = dyn->tau_eff; }
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
     { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
@@ -218,20 +268,17 @@ __global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint
 }  // namespace
 
 // ---- host wrappers ---------------------------------------------------------------------------------
-int meb_eval_finalize(meb_ctx* ctx, int grid, int nvec, int dpad, const int32_t* count, const double* x,
-                      const double* xbar, double sigma, double tau, int d, double* out, double* grad) {
-    const int tpb = d > 2048 ? 1 : MEB_WARPS;      // list entries per CTA round of the active kernel
-    ctx->launches++; eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_scalar, grid, ctx->part_vec, nvec, tpb, dpad,
-                                                        count, x, xbar, sigma, tau, d, out, grad);
+int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f) {
+    ctx->launches++; eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(f);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 
 int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
-                     const double* q, double sigma, double tau, int d, double* Hq) {
+                     const double* q, double sigma, double tau, int d, double* Hq, const MebDyn* dyn) {
     const int tpb = d > 2048 ? 1 : MEB_WARPS;
     ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, tpb, ctx->count_dev, dpad, part_sc, ev, q, sigma, tau,
-                                                       d, Hq);
+                                                       d, Hq, dyn);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -75,6 +75,7 @@ struct Ev { double s[MEB_EVAL_NSCALARS]; std::vector<double> g; double psi_n; };
 
 EvalCall make_call(const Solver& S, const Problem& P, double sigma) {
     EvalCall c;
+    c.gs = nullptr;
     c.prec = P.prec; c.m = P.m; c.d = P.d; c.C = P.C; c.ld = P.ld; c.R = P.R;
     c.U = P.has_mult ? P.U[P.cur] : nullptr;
     c.v_slot = P.has_mult ? P.slot[P.cur] : nullptr;
@@ -100,7 +101,8 @@ int evaluate(Solver& S, const Problem& P, const std::vector<double>& xn, double 
     if (rc) return rc;
     EvalCall c = make_call(S, P, sigma);
     ctx->cur_class = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
-    rc = meb_eval_internal(ctx, c, want_grad, ctx->small + SM_EV, S.dgrad, nullptr, nullptr);
+    want_grad = true;
+    rc = meb_eval_internal(ctx, c, ctx->small + SM_EV, S.dgrad, nullptr, nullptr);
     if (rc) return rc;
     count_pass(S, P);
     MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_EV, MEB_EVAL_NSCALARS * sizeof(double),
@@ -113,24 +115,6 @@ int evaluate(Solver& S, const Problem& P, const std::vector<double>& xn, double 
     memcpy(ev.s, ctx->h_pinned, sizeof(ev.s));
     ev.psi_n = ev.s[MEB_EV_PSI] / S.L;
     if (want_grad) ev.g.assign(ctx->h_pinned + 16, ctx->h_pinned + 16 + S.d + 1);
-    return MEB_OK;
-}
-
-// gradient for the records of the last streaming pass (the accepted Armijo trial)
-int gradient_of_last(Solver& S, const Problem& P, double sigma, Ev& ev) {
-    meb_ctx* ctx = S.ctx;
-    EvalCall c = make_call(S, P, sigma);
-    int rc = meb_grad_from_records(ctx, c, ctx->small + SM_EV, S.dgrad);
-    if (rc) return rc;
-    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_EV, MEB_EVAL_NSCALARS * sizeof(double),
-                                     cudaMemcpyDeviceToHost, ctx->stream));
-    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 16, S.dgrad, (S.d + 1) * sizeof(double),
-                                     cudaMemcpyDeviceToHost, ctx->stream));
-    rc = sync_stream(ctx);
-    if (rc) return rc;
-    memcpy(ev.s, ctx->h_pinned, sizeof(ev.s));
-    ev.psi_n = ev.s[MEB_EV_PSI] / S.L;
-    ev.g.assign(ctx->h_pinned + 16, ctx->h_pinned + 16 + S.d + 1);
     return MEB_OK;
 }
 
@@ -228,6 +212,8 @@ int update_multipliers(Solver& S, Problem& P, double sigma, const Ev& ev) {
     rc = meb_fill_i32(ctx, P.slot[nxt], P.m, -1);
     if (rc) return rc;
     EvalCall c = make_call(S, P, sigma);
+    rc = meb_ensure_list(ctx, P.m);
+    if (rc) return rc;
     ActiveArgs a;
     memset(&a, 0, sizeof(a));
     a.C = c.C; a.ld = c.ld; a.U = c.U; a.v_slot = c.v_slot; a.V = c.V; a.ldv = c.ldv; a.x = c.x; a.d = c.d;
@@ -292,16 +278,14 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             if (!accepted) {
                 if (evt.psi_n <= ev.psi_n) {                          // last trial did not increase Psi: take it
                     xn = xt;
-                    rc = gradient_of_last(S, P, sigma, ev);
-                    if (rc) return rc;
+                    ev = evt;
                 } else {
                     records_current = false;
                 }
                 break;                                                // stalled
             }
             xn = xt;
-            rc = gradient_of_last(S, P, sigma, ev);                   // the accepted trial is the next evaluation
-            if (rc) return rc;
+            ev = evt;                                                 // the accepted trial is the next evaluation
         }
         if (!records_current) {                                       // rare: re-evaluate at x for the update
             rc = evaluate(S, P, xn, sigma, true, ev);

@@ -1,0 +1,474 @@
+// TMA-staged streaming map-reduce for SHORT rows (row <= 1024 bytes): SURVEY 8(a) rows a0, a1, a7, a8.
+//
+// B200 mapping.  One persistent CTA per SM.  Every warp runs its own producer/consumer ring of NS
+// shared-memory stages; a stage is one contiguous block of 32*R rows of C, fetched by ONE bulk
+// asynchronous copy (cp.async.bulk global -> shared, completion on an mbarrier: the TMA engine moves
+// the bytes, no registers, no per-thread address arithmetic), so each SM keeps W*(NS-1) stages
+// (~100 KB) of HBM reads in flight regardless of how long the per-row epilogue is.  Inside a stage
+// the mapping is LANE PER ROW: lane L reads its row from shared memory in 16-byte chunks (chunk
+// order rotated by the lane index when the row stride is an even number of 16-byte slots, which
+// makes the quarter-warp LDS.128 conflict-free), accumulates ||c_i - c||^2 with no shuffles, and runs
+// the scalar epilogue (branch of P:L115, multiplier, KKT terms) for its own row.
+//
+// Fused evaluation (OP_EVAL): for every ACTIVE row of the stage (lam_i != 0, found by ballot) the
+// warp adds lam_i b_i into per-lane register accumulators straight from the shared-memory copy of
+// the row -- the gradient's vector part sum_i v+_i costs no second pass over C.
+//
+// Determinism: static stage -> warp assignment, per-lane / per-warp accumulation in a fixed order,
+// warps combined in index order, CTA partials combined in index order by the finalize kernel.
+#include <string.h>
+
+#include "meb_internal.cuh"
+#include "meb_rowops.cuh"
+
+namespace {
+
+// ---- mbarrier / bulk-copy PTX -------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// one contiguous block global -> shared through the TMA engine; bytes is a multiple of 16
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+template <typename T> struct Chunk;
+template <> struct Chunk<double> { typedef double2 type; static constexpr int N = 2; };
+template <> struct Chunk<float>  { typedef float4 type;  static constexpr int N = 4; };
+
+struct TileCfg {
+    int G, logG;           // lanes per row (1, 2 or 4); a sub-tile is 32/G rows
+    int R;                 // sub-tiles per stage
+    int NS;                // stages per warp
+    int W;                 // warps per CTA
+    uint32_t row_bytes;    // ld * sizeof(T), a multiple of 16
+    uint32_t stage_rows;   // R * 32 / G
+    uint32_t stage_bytes;  // whole stage: rows, then per-row scalars u_i, r_i, slot_i (each 16-byte aligned)
+    uint32_t off_u, off_r, off_slot;   // byte offsets of the per-row scalars inside a stage
+    int nch;               // 16-byte chunks that cover the d columns of a row
+    int rot;               // 1: rotate the chunk order by the row index (bank conflicts)
+    int sc_tma;            // 1: per-row scalars come with the stage (their arrays are 16-byte aligned)
+    uint32_t off_tiles;    // byte offsets inside the dynamic shared memory
+    uint32_t off_bars;
+    uint32_t off_vec;
+};
+
+// ---- the kernel ------------------------------------------------------------------------------------
+// CH = 16-byte chunks per lane when a whole warp walks ONE row (active rows, shadow): ceil(nch / 32).
+template <typename T, int OP, int CH, bool SHADOW>
+__global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, const TileCfg cfg) {
+    typedef typename Chunk<T>::type V4;
+    constexpr int VEC = Chunk<T>::N;
+    extern __shared__ __align__(128) unsigned char smem[];
+    StreamArgs a = a_in;
+    meb_resolve_dyn(a);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int d = a.d;
+    const int64_t m = a.m;
+    const int W = cfg.W, NS = cfg.NS, R = cfg.R, nch = cfg.nch, G = cfg.G, LG = cfg.logG;
+    const int RPT = 32 >> LG;                                            // rows per sub-tile
+    const int g = lane & (G - 1), rl = lane >> LG;
+    T* cs = reinterpret_cast<T*>(smem);                                  // centre, padded to whole chunks
+    unsigned char* tiles = smem + cfg.off_tiles + (size_t)warp * NS * cfg.stage_bytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + cfg.off_bars) + warp * NS;
+    const T* __restrict__ C = static_cast<const T*>(a.C);
+    const T* __restrict__ Vg = static_cast<const T*>(a.V);
+    const T* __restrict__ Ug = static_cast<const T*>(a.U);
+    const T* __restrict__ Rg = static_cast<const T*>(a.R);
+    const bool HASU = (OP == OP_EVAL) && Ug != nullptr;
+    const bool HASV = (OP == OP_EVAL) && a.v_slot != nullptr;
+    const bool HASR = Rg != nullptr;
+
+    long long t_start = 0;
+    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_start));
+    const double* cptr = (OP == OP_INGEST) ? a.c0 : a.x + 1;
+    for (int j = threadIdx.x; j < nch * VEC; j += blockDim.x) cs[j] = j < d ? (T)cptr[j] : T(0);
+    if (lane == 0) {
+        for (int s = 0; s < NS; ++s) mbar_init(&bars[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const T r = (OP == OP_INGEST) ? T(0) : (T)a.x[0];
+    const T sig = (T)a.sigma;
+    const T inv_sig = T(1) / sig;
+    Acc acc;
+    // whole-warp-per-row view: lane owns chunks lane, lane + 32 (columns (lane + 32 q) * VEC + e)
+    double vacc[CH][VEC];
+    T creg[CH][VEC];
+    const V4* cs4 = reinterpret_cast<const V4*>(cs);
+#pragma unroll
+    for (int q = 0; q < CH; ++q) {
+        const int ch = lane + 32 * q;
+        V4 cv;
+        if (ch < nch) cv = cs4[ch];
+        const T* cc = reinterpret_cast<const T*>(&cv);
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) { vacc[q][e] = 0.0; creg[q][e] = ch < nch ? cc[e] : T(0); }
+    }
+
+    // stages: st = gw, gw + GW, ...  (consecutive stages go to different SMs)
+    const int64_t rows_per_stage = cfg.stage_rows;
+    const int64_t nstages = (m + rows_per_stage - 1) / rows_per_stage;
+    const int64_t gw = (int64_t)warp * gridDim.x + blockIdx.x;
+    const int64_t GW = (int64_t)gridDim.x * W;
+    const int64_t mine = gw < nstages ? (nstages - gw + GW - 1) / GW : 0;
+
+    auto issue = [&](int64_t k, int s) {                // k-th stage of this warp -> ring slot s
+        const int64_t st = gw + k * GW;
+        const int64_t row0 = st * rows_per_stage;
+        const int64_t nrows = (m - row0) < rows_per_stage ? (m - row0) : rows_per_stage;
+        const uint32_t nb = (uint32_t)(nrows & ~(int64_t)3);             // rows whose scalars come in 16-byte units
+        unsigned char* dst = tiles + (size_t)s * cfg.stage_bytes;
+        uint32_t bytes = (uint32_t)nrows * cfg.row_bytes;
+        const bool sc = cfg.sc_tma && nb > 0;
+        if (sc) bytes += (HASU ? nb * (uint32_t)sizeof(T) : 0u) + (HASR ? nb * (uint32_t)sizeof(T) : 0u) + (HASV ? nb * 4u : 0u);
+        mbar_expect_tx(&bars[s], bytes);
+        bulk_g2s(dst, reinterpret_cast<const unsigned char*>(C) + (size_t)row0 * cfg.row_bytes,
+                 (uint32_t)nrows * cfg.row_bytes, &bars[s]);
+        if (sc) {
+            if (HASU) bulk_g2s(dst + cfg.off_u, Ug + row0, nb * (uint32_t)sizeof(T), &bars[s]);
+            if (HASR) bulk_g2s(dst + cfg.off_r, Rg + row0, nb * (uint32_t)sizeof(T), &bars[s]);
+            if (HASV) bulk_g2s(dst + cfg.off_slot, a.v_slot + row0, nb * 4u, &bars[s]);
+        }
+    };
+    if (lane == 0)
+        for (int k = 0; k < NS && k < mine; ++k) issue(k, k);
+
+    const int ldT = (int)(cfg.row_bytes / sizeof(T));
+    const int npl = (nch + G - 1) >> LG;                                 // chunks per lane (G lanes per row)
+    const int start = cfg.rot ? (rl % npl) : 0;
+    const bool haspad = nch * VEC != d;
+
+    int s = 0;
+    uint32_t parity = 0;
+    for (int64_t k = 0; k < mine; ++k) {
+        mbar_wait(&bars[s], parity);
+        unsigned char* sbase = tiles + (size_t)s * cfg.stage_bytes;
+        T* stage = reinterpret_cast<T*>(sbase);
+        const T* Us = reinterpret_cast<const T*>(sbase + cfg.off_u);
+        const T* Rs = reinterpret_cast<const T*>(sbase + cfg.off_r);
+        const int32_t* Ss = reinterpret_cast<const int32_t*>(sbase + cfg.off_slot);
+        const int64_t st = gw + k * GW;
+        const int64_t srow0 = st * rows_per_stage;
+        const int64_t snrows = (m - srow0) < rows_per_stage ? (m - srow0) : rows_per_stage;
+        const int nbulk = cfg.sc_tma ? (int)(snrows & ~(int64_t)3) : 0;
+        for (int rr = 0; rr < R; ++rr) {
+            const int rs0 = rr * RPT;                                    // first row of the sub-tile in the stage
+            const int64_t row0 = srow0 + rs0;
+            if (row0 >= m) break;                                        // warp-uniform
+            const int myrs = rs0 + rl;
+            const int64_t myrow = row0 + rl;
+            const bool myvalid = myrow < m;
+            T* rowp = stage + (size_t)myrs * ldT;
+            // per-row scalars: staged with the rows, or (tail rows / unaligned arrays) read from global memory
+            int myslot = -1;
+            T ri = T(0), ui = T(0);
+            if (myvalid) {
+                if (myrs < nbulk) {
+                    if (HASV) myslot = Ss[myrs];
+                    if (HASR) ri = Rs[myrs];
+                    if (HASU) ui = Us[myrs];
+                } else {
+                    if (HASV) myslot = a.v_slot[myrow];
+                    if (HASR) ri = Rg[myrow];
+                    if (HASU) ui = Ug[myrow];
+                }
+            }
+            T nb2 = T(0), ne2 = T(0), evd = T(0), vv = T(0);
+            if (haspad) {                                                // zero the padding of the last chunk
+                if (myvalid && g == 0)
+                    for (int j = d; j < nch * VEC; ++j) rowp[j] = T(0);
+                __syncwarp();
+            }
+            if (myvalid) {
+                if (myslot < 0) {
+                    T s0 = T(0), s1 = T(0), f0 = T(0);
+                    // my chunks are g, g + G, ... (n_g of them), visited from `start` with wrap-around
+                    const V4* rp = reinterpret_cast<const V4*>(rowp) + g;
+                    const V4* cp = cs4 + g;
+                    auto chunk = [&](int c) {
+                        const V4 ev4 = rp[c << LG];
+                        const V4 cv4 = cp[c << LG];
+                        const T* e = reinterpret_cast<const T*>(&ev4);
+                        const T* cc = reinterpret_cast<const T*>(&cv4);
+#pragma unroll
+                        for (int j = 0; j < VEC; ++j) {
+                            const T ee = e[j] - cc[j];
+                            if (j & 1) s1 = fma(ee, ee, s1); else s0 = fma(ee, ee, s0);
+                            if (OP == OP_INGEST) f0 = fma(e[j], T(0), f0);   // NaN iff a non-finite entry
+                        }
+                    };
+                    const int n_g = (nch - g + G - 1) >> LG;
+                    int c = start < n_g ? start : 0;
+                    const int c_first = c;
+                    for (; c + 4 <= n_g; c += 4) { chunk(c); chunk(c + 1); chunk(c + 2); chunk(c + 3); }
+                    for (; c < n_g; ++c) chunk(c);
+                    c = 0;
+                    for (; c + 4 <= c_first; c += 4) { chunk(c); chunk(c + 1); chunk(c + 2); chunk(c + 3); }
+                    for (; c < c_first; ++c) chunk(c);
+                    nb2 = s0 + s1;
+                    if (OP == OP_INGEST) ne2 = f0;
+                } else {                                                 // row with a multiplier v_i
+                    const T* vrow = Vg + (int64_t)myslot * a.ldv;
+                    for (int c = g; c < nch; c += G) {
+                        const int col = c * VEC;
+#pragma unroll
+                        for (int j = 0; j < VEC; ++j) {
+                            if (col + j < d) {
+                                const T ee = rowp[col + j] - cs[col + j];
+                                const T v = __ldg(vrow + col + j);
+                                const T b = fma(v, inv_sig, ee);
+                                nb2 = fma(b, b, nb2);
+                                ne2 = fma(ee, ee, ne2);
+                                evd = fma(ee, v, evd);
+                                vv = fma(v, v, vv);
+                            }
+                        }
+                    }
+                }
+            }
+            for (int o = G >> 1; o > 0; o >>= 1) {                       // combine the G lanes of a row
+                nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, o);
+                if (HASV || OP == OP_INGEST) ne2 += __shfl_xor_sync(MEB_FULL_MASK, ne2, o);
+                if (HASV) {
+                    evd += __shfl_xor_sync(MEB_FULL_MASK, evd, o);
+                    vv += __shfl_xor_sync(MEB_FULL_MASK, vv, o);
+                }
+            }
+            double mylam;
+            const bool flag = row_epilogue_core<T, OP>(a, myrow, myvalid && g == 0, myslot >= 0, nb2, ne2, evd, vv,
+                                                       r, sig, ri, ui, acc, mylam);
+            if (OP != OP_INGEST) {
+                uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);      // bit of lane rl*G <-> row rl
+                {   // RPT-bit piece of the 32-row mask word: lane q < RPT takes the flag of row q
+                    const bool f2 = __shfl_sync(MEB_FULL_MASK, (int)flag, (lane << LG) & 31) != 0 && lane < RPT;
+                    const uint32_t piece = __ballot_sync(MEB_FULL_MASK, f2);
+                    if (lane == 0) {
+                        if (G == 1) a.mask[row0 >> 5] = piece;
+                        else if (G == 2) reinterpret_cast<uint16_t*>(a.mask)[row0 >> 4] = (uint16_t)piece;
+                        else reinterpret_cast<uint8_t*>(a.mask)[row0 >> 3] = (uint8_t)piece;
+                    }
+                }
+                if (OP == OP_EVAL) {
+                    // gradient vector part: sum over the ACTIVE rows of lam_i b_i, from shared memory
+                    while (bits) {
+                        const int ls = __ffs(bits) - 1;                  // lane that owns the row
+                        bits &= bits - 1;
+                        const double lam = __shfl_sync(MEB_FULL_MASK, mylam, ls);
+                        const int slot = HASV ? __shfl_sync(MEB_FULL_MASK, myslot, ls) : -1;
+                        const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + (ls >> LG)) * ldT);
+#pragma unroll
+                        for (int q = 0; q < CH; ++q) {
+                            const int ch = lane + 32 * q;
+                            if (ch < nch) {
+                                const V4 ev4 = rp4[ch];
+                                const T* e = reinterpret_cast<const T*>(&ev4);
+                                T b[VEC];
+#pragma unroll
+                                for (int j = 0; j < VEC; ++j) b[j] = e[j] - creg[q][j];
+                                if (slot >= 0) {
+                                    const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
+#pragma unroll
+                                    for (int j = 0; j < VEC; ++j)
+                                        if (ch * VEC + j < d) b[j] = fma(__ldg(vrow + j), inv_sig, b[j]);
+                                }
+#pragma unroll
+                                for (int j = 0; j < VEC; ++j) vacc[q][j] = fma(lam, (double)b[j], vacc[q][j]);
+                            }
+                        }
+                    }
+                }
+            }
+            if (SHADOW) {                       // FP32 shadow of the centred rows (reading 8)
+                const int nr = (m - row0) < RPT ? (int)(m - row0) : RPT;
+#pragma unroll 4
+                for (int rs = 0; rs < nr; ++rs) {
+                    const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
+                    float* srow = a.C32 + (row0 + rs) * a.ld32;
+#pragma unroll
+                    for (int q = 0; q < CH; ++q) {
+                        const int ch = lane + 32 * q;
+                        if (ch < nch) {
+                            const V4 ev4 = rp4[ch];
+                            const T* e = reinterpret_cast<const T*>(&ev4);
+                            const int col = ch * VEC;
+                            if (VEC == 2 && col + 1 < d) {
+                                float2 o;
+                                o.x = (float)(e[0] - creg[q][0]);
+                                o.y = (float)(e[1] - creg[q][1]);
+                                *reinterpret_cast<float2*>(srow + col) = o;       // ld32 is a multiple of 4
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < VEC; ++j)
+                                    if (col + j < d) srow[col + j] = (float)(e[j] - creg[q][j]);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0 && k + NS < mine) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // accesses above before the refill
+            issue(k + NS, s);
+        }
+        if (++s == NS) { s = 0; parity ^= 1u; }
+    }
+
+    // ---- CTA partials, fixed order ----
+    if (OP == OP_EVAL) {
+        double* vs = reinterpret_cast<double*>(smem + cfg.off_vec);      // [W][CH * 32 * VEC]
+        constexpr int VW = CH * 32 * VEC;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < CH; ++q)
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) vs[(size_t)warp * VW + (lane + 32 * q) * VEC + j] = vacc[q][j];
+        __syncthreads();
+        double* pv = a.part_vec + (size_t)blockIdx.x * a.dpad;
+        for (int j = threadIdx.x; j < d; j += blockDim.x) {
+            double sacc = 0.0;
+            for (int w = 0; w < W; ++w) sacc += vs[(size_t)w * VW + j];
+            pv[j] = sacc;
+        }
+    }
+    block_reduce_store<OP>(acc, a.part, W);
+    if (threadIdx.x == 0) {                 // device time stamps of this CTA (ns), read by the finalize kernel
+        long long t_end;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
+        a.part[(size_t)blockIdx.x * MEB_NPART + 10] = __longlong_as_double(t_start);
+        a.part[(size_t)blockIdx.x * MEB_NPART + 11] = __longlong_as_double(t_end);
+    }
+}
+
+}  // namespace
+
+// ---- host-side configuration and dispatch --------------------------------------------------------
+namespace {
+
+constexpr size_t TILE_SMEM_BUDGET = 212 * 1024;     // of the 227 KB a CTA may use on sm_100
+
+bool aligned16(const void* p) { return ((uintptr_t)p % 16) == 0; }
+
+bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out) {
+    TileCfg c;
+    memset(&c, 0, sizeof(c));
+    c.row_bytes = (uint32_t)(a.ld * (int64_t)esize);
+    c.nch = (int)(((size_t)a.d * esize + 15) / 16);
+    c.G = c.row_bytes <= 208 ? 1 : (c.row_bytes <= 416 ? 2 : 4);     // sub-tile of at most ~6.5 KB
+    c.logG = c.G == 1 ? 0 : (c.G == 2 ? 1 : 2);
+    const int rpt = 32 / c.G;
+    const int slots = (int)(c.row_bytes / 16);
+    c.rot = (slots % c.G == 0 && ((slots / c.G) % 2 == 0)) ? 1 : 0;
+    // stage of about 12 KB of rows, but never so large that a small problem lands on a handful of warps
+    int R = (int)(6656 / ((size_t)rpt * c.row_bytes));
+    if (R < 1) R = 1;
+    if (R > 8) R = 8;
+    while (R > 1 && (a.m + (int64_t)rpt * R - 1) / ((int64_t)rpt * R) < (int64_t)grid * 16 * 4) --R;
+    c.R = R;
+    c.stage_rows = (uint32_t)(R * rpt);
+    c.off_u = c.stage_rows * c.row_bytes;
+    c.off_r = c.off_u + c.stage_rows * (uint32_t)esize;
+    c.off_slot = c.off_r + c.stage_rows * (uint32_t)esize;
+    c.stage_bytes = (c.off_slot + c.stage_rows * 4u + 127u) / 128u * 128u;
+    c.sc_tma = 1;
+    const void* ptrs[] = {a.U, a.R, a.v_slot, a.U2[0], a.U2[1], a.slot2[0], a.slot2[1]};
+    for (const void* q : ptrs) if (q && !aligned16(q)) c.sc_tma = 0;
+    const size_t cs_bytes = ((size_t)c.nch * 16 + 127) / 128 * 128;
+    int W = 16, NS = 0;
+    for (; W >= 2; --W) {
+        const size_t fixed = cs_bytes + 16 * 4 * sizeof(uint64_t) + 256 + (size_t)W * 32 * cpl * sizeof(double);
+        if (fixed + (size_t)W * 2 * c.stage_bytes > TILE_SMEM_BUDGET) continue;
+        NS = (int)((TILE_SMEM_BUDGET - fixed) / ((size_t)W * c.stage_bytes));
+        if (NS > 4) NS = 4;
+        break;
+    }
+    if (NS < 2) return false;
+    c.W = W; c.NS = NS;
+    c.off_tiles = (uint32_t)cs_bytes;
+    c.off_bars = (uint32_t)(cs_bytes + (size_t)W * NS * c.stage_bytes);
+    c.off_vec = (uint32_t)((c.off_bars + (size_t)W * NS * sizeof(uint64_t) + 127) / 128 * 128);
+    *out = c;
+    return true;
+}
+
+size_t cfg_smem(const TileCfg& c, int cpl) { return (size_t)c.off_vec + (size_t)c.W * 32 * cpl * sizeof(double); }
+
+template <typename KernelT>
+int launch_cfg(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, size_t esize, int cpl, int* grid_out) {
+    int grid = ctx->sm_count > 0 ? ctx->sm_count : 148;            // one persistent CTA per SM
+    TileCfg c;
+    if (!make_cfg(a, esize, cpl, grid, &c)) return MEB_E_CAPACITY;
+    const int64_t nstages = (a.m + c.stage_rows - 1) / c.stage_rows;
+    if (nstages < grid) grid = (int)nstages;                       // stage k -> CTA k % grid, warp k / grid
+    if (grid < 1) grid = 1;
+    const size_t smem = cfg_smem(c, cpl);
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
+    ctx->launches++;
+    kernel<<<grid, 32 * c.W, smem, ctx->stream>>>(a, c);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
+    *grid_out = grid;
+    return MEB_OK;
+}
+
+template <typename T, int OP, bool SHADOW>
+int launch_cpl(meb_ctx* ctx, const StreamArgs& a, int* grid_out) {
+    const int nch = (int)(((size_t)a.d * sizeof(T) + 15) / 16);        // <= 64 (rows of at most 1024 bytes)
+    constexpr int VEC = 16 / sizeof(T);
+    if (nch <= 32) return launch_cfg(ctx, tile_kernel<T, OP, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
+    return launch_cfg(ctx, tile_kernel<T, OP, 2, SHADOW>, a, sizeof(T), 2 * VEC, grid_out);
+}
+
+}  // namespace
+
+bool meb_tile_applicable(int op, int prec, const StreamArgs& a) {
+    const size_t esize = prec == MEB_FP64 ? 8 : 4;
+    const size_t row_bytes = (size_t)a.ld * esize;
+    if (row_bytes > 1024 || row_bytes % 16 != 0 || ((uintptr_t)a.C % 16) != 0) return false;
+    if (a.d > 256) return false;
+    if (op == OP_EVAL && a.part_vec == nullptr) return false;
+    return true;
+}
+
+int meb_launch_tile(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out) {
+    if (prec == MEB_FP64) {
+        switch (op) {
+            case OP_EVAL: return launch_cpl<double, OP_EVAL, false>(ctx, a, grid_out);
+            case OP_FEAS: return launch_cfg(ctx, tile_kernel<double, OP_FEAS, 1, false>, a, 8, 1, grid_out);
+            case OP_INGEST:
+                if (a.C32) return launch_cpl<double, OP_INGEST, true>(ctx, a, grid_out);
+                return launch_cfg(ctx, tile_kernel<double, OP_INGEST, 1, false>, a, 8, 1, grid_out);
+            default: return MEB_E_ARG;
+        }
+    }
+    switch (op) {
+        case OP_EVAL: return launch_cpl<float, OP_EVAL, false>(ctx, a, grid_out);
+        case OP_SCREEN: return launch_cfg(ctx, tile_kernel<float, OP_SCREEN, 1, false>, a, 4, 1, grid_out);
+        default: return MEB_E_ARG;
+    }
+}

@@ -26,10 +26,18 @@ static void ctx_free_all(meb_ctx* c) {
     for (int i = 0; i < 16; ++i) if (c->own[i]) cudaFree(c->own[i]);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    meb_free_graph_cache(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->sdev) cudaFree(c->sdev);
+    if (c->h_sdev) cudaFreeHost(c->h_sdev);
     if (c->evpool) {
         for (int i = 0; i < 2 * MEB_EVPOOL; ++i) if (c->evpool[i]) cudaEventDestroy(c->evpool[i]);
         free(c->evpool);
     }
+}
+
+void meb_debug_cuda(const char* file, int line, int err) {
+    if (getenv("MEB_DEBUG")) fprintf(stderr, "[meb] %s:%d: CUDA error %d (%s)\n", file, line, err, cudaGetErrorString((cudaError_t)err));
 }
 
 extern "C" int meb_version(void) { return 100; }
@@ -95,6 +103,9 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     TRY_ALLOC(c->small, (size_t)c->small_len * sizeof(double));
 #undef TRY_ALLOC
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_pinned, (size_t)c->h_pinned_len * sizeof(double));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaMalloc(&c->sdev, meb_solver_dev_size());
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_sdev, meb_solver_dev_size());
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
     if (e == cudaSuccess) {

@@ -36,7 +36,7 @@ struct SolverDev {
     long long pass_count;
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
-    int32_t in_graph, pad;
+    int32_t in_graph, eval_cap;   // eval_cap: hard bound on the evaluations of a phase (a runaway loop cannot hang the GPU)
 };
 
 // (d+1)-vectors of the state, each of length nv = n rounded up to 8, in one device array
@@ -80,7 +80,7 @@ __device__ __forceinline__ void ctrl_set_handles(const SolverDev* S) {
     cudaGraphSetConditional(S->h_while, S->done ? 0u : 1u);
     cudaGraphSetConditional(S->h_newton, (!S->done && S->action == ACT_NEWTON) ? 1u : 0u);
     cudaGraphSetConditional(S->h_update, (!S->done && S->action == ACT_UPDATE) ? 1u : 0u);
-    cudaGraphSetConditional(S->h_cg, (!S->done && S->action == ACT_NEWTON && !S->dense && S->cg_go) ? 1u : 0u);
+    if (!S->dense) cudaGraphSetConditional(S->h_cg, (!S->done && S->action == ACT_NEWTON && S->cg_go) ? 1u : 0u);
 }
 
 // relative KKT residual (reading 7) from the scalars of an evaluation
@@ -119,14 +119,22 @@ __device__ inline void ctrl_after_eval(SolverDev* S, const SolverVecs v, double*
         if (stalled) {                                 // records of this pass are not those of x: re-evaluate
             ctrl_to_raw(S, v, v.xn, v.x_raw);
             __syncthreads();
-            if (threadIdx.x == 0) { S->phase = PH_REEVAL; S->action = ACT_TRIAL; S->evals++; ctrl_set_handles(S); }
+            if (threadIdx.x == 0) {
+                S->phase = PH_REEVAL; S->action = ACT_TRIAL; S->evals++;
+                if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
+                ctrl_set_handles(S);
+            }
         } else {                                       // halve the step
             const double eta = 0.5 * S->eta;
             for (int j = threadIdx.x; j < n; j += blockDim.x) v.xt[j] = v.xn[j] + eta * v.delta[j];
             __syncthreads();
             ctrl_to_raw(S, v, v.xt, v.x_raw);
             __syncthreads();
-            if (threadIdx.x == 0) { S->eta = eta; S->ls++; S->action = ACT_TRIAL; S->evals++; ctrl_set_handles(S); }
+            if (threadIdx.x == 0) {
+                S->eta = eta; S->ls++; S->action = ACT_TRIAL; S->evals++;
+                if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
+                ctrl_set_handles(S);
+            }
         }
         return;
     }
@@ -173,6 +181,7 @@ __device__ inline void ctrl_after_eval(SolverDev* S, const SolverVecs v, double*
             S->cg_it = 0;
             S->cg_go = (gn > S->cg_tol && S->cg_max > 0) ? 1 : 0;
         }
+        if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
         ctrl_set_handles(S);
     }
     __syncthreads();

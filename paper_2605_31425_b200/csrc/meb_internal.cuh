@@ -59,13 +59,22 @@ struct meb_ctx {
     bool ev_record;         // on inside meb_solve
     int cur_class;          // MEB_PASS_* of the next streaming launch
     int64_t launches;       // kernels launched through this context
+    // ---- device-resident solver (meb_ctrl.cuh, meb_solver.cu) ----
+    void* sdev;             // SolverDev on the device
+    void* h_sdev;           // pinned host mirror
+    void* graph_cache;      // instantiated solve graphs (meb_solver.cu)
+    cudaStream_t cap_stream; // private stream used only to CAPTURE graphs (the legacy default stream cannot capture)
 };
+
+// prints file:line and the CUDA error string to stderr when the environment variable MEB_DEBUG is set
+void meb_debug_cuda(const char* file, int line, int err);
 
 #define MEB_CUDA_OK(ctx, expr)                                   \
     do {                                                         \
         cudaError_t e__ = (expr);                                \
         if (e__ != cudaSuccess) {                                \
             (ctx)->last_cuda_error = (int)e__;                   \
+            meb_debug_cuda(__FILE__, __LINE__, (int)e__);        \
             return MEB_E_CUDA;                                   \
         }                                                        \
     } while (0)
@@ -246,3 +255,14 @@ int meb_hvp_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scala
 int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, double* H);
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
                    int* info_dev);
+
+// ---- controller kernels of the device-resident solver (meb_ctrl.cu) ----
+int meb_ctrl_init(meb_ctx* ctx, SolverDev* S, const SolverVecs& v, double sigma0, int cur, int has_mult);
+int meb_ctrl_resume(meb_ctx* ctx, SolverDev* S);
+int meb_ctrl_after_newton(meb_ctx* ctx, SolverDev* S, const SolverVecs& v);
+int meb_ctrl_cg_step(meb_ctx* ctx, SolverDev* S, const SolverVecs& v);
+int meb_ctrl_after_update(meb_ctx* ctx, SolverDev* S, const SolverVecs& v, const int32_t* count);
+int meb_reset_next(meb_ctx* ctx, int prec, const MebDyn* dyn, void* U0, void* U1, int32_t* s0, int32_t* s1,
+                   int64_t m);
+void meb_free_graph_cache(meb_ctx* ctx);
+size_t meb_solver_dev_size();

@@ -7,11 +7,13 @@
 // psi~ = psi_raw/L and H~ = L H_raw, so no scaled copy of C is ever made.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
 
 #include "meb_internal.cuh"
+#include "meb_ctrl.cuh"
 
 #define SM_EV 0
 #define SM_AUX 16
@@ -36,7 +38,7 @@ struct Problem {                   // one ripALM run: data + double-buffered mul
     int prec; int64_t m; int32_t d;
     const void* C; int64_t ld; const void* R;
     void* U[2]; int32_t* slot[2]; void* V[2]; int64_t ldv; int64_t vcap[2];
-    int own_v[2];                  // own[] slots holding the V pools
+    int own_v[2];                  // own[] slots holding the V pools (-1: fixed capacity)
     int cur; bool has_mult;
     const double* off;             // host: raw offset of the centre (c0 for raw data, nullptr for the centred shadow)
     bool full;                     // streams all m rows (for the pass statistics)
@@ -45,15 +47,21 @@ struct Problem {                   // one ripALM run: data + double-buffered mul
 struct Solver {
     meb_ctx* ctx; meb_params par; meb_stats* st;
     int32_t d; double L;
-    double* dx; double* dxbar; double* dq; double* dHq; double* dgrad;   // device (d+1)
-    double* dH; double* ddelta;                                         // device (d+1)^2, (d+1): dense Newton system
-    std::vector<double> hx, hxbar;
+    double* dH;                    // device (d+1)^2: dense Newton system
+    SolverVecs v;                  // device (d+1)-vectors of the controller
     double bytes;
 };
 
 size_t esz(int prec) { return prec == MEB_FP64 ? 8 : 4; }
 
 int sync_stream(meb_ctx* ctx) { MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream)); return MEB_OK; }
+
+// x_raw = (L r~, off + L c~)
+void to_raw(const Solver& S, const Problem& P, const std::vector<double>& xn, std::vector<double>& xr) {
+    xr.resize(S.d + 1);
+    xr[0] = S.L * xn[0];
+    for (int j = 0; j < S.d; ++j) xr[1 + j] = (P.off ? P.off[j] : 0.0) + S.L * xn[1 + j];
+}
 
 int upload(meb_ctx* ctx, double* dst, const double* src, size_t n) {
     // staged through pinned memory so that the copy is truly asynchronous and ordered on the stream
@@ -64,245 +72,325 @@ int upload(meb_ctx* ctx, double* dst, const double* src, size_t n) {
     return MEB_OK;
 }
 
-// x_raw = (L r~, off + L c~)
-void to_raw(const Solver& S, const Problem& P, const std::vector<double>& xn, std::vector<double>& xr) {
-    xr.resize(S.d + 1);
-    xr[0] = S.L * xn[0];
-    for (int j = 0; j < S.d; ++j) xr[1 + j] = (P.off ? P.off[j] : 0.0) + S.L * xn[1 + j];
+// ---- the solve graph of one phase ------------------------------------------------------------------
+// WHILE (!done) { evaluation at the trial point + controller;  IF (Newton) { active list, dense H +
+// LDL^T  |  CG: WHILE { H p; CG step } ; first Armijo trial };  IF (update) { active list, (U,V) <- (U+,V+),
+// outer-iteration bookkeeping } }.  Everything the kernels need that changes between iterations is
+// read from device memory (SolverDev / MebDyn), so the instantiated graph is launched once per phase.
+struct GraphKey {
+    int prec, dense; int64_t m; int32_t d; const void* C; int64_t ld; const void* R;
+    void* U[2]; int32_t* slot[2]; void* V[2]; int64_t ldv; int64_t vcap[2];
+    const double* dH; const double* xn;
+};
+struct SolveGraph {
+    bool used; GraphKey key; cudaGraph_t g; cudaGraphExec_t ex;
+    cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
+    int k_eval, k_newton, k_cg, k_update;      // kernels launched per evaluation / Newton solve / CG step / update
+    double bytes_per_eval; uint64_t stamp;
+};
+constexpr int MAX_GRAPHS = 8;
+struct GraphCache { SolveGraph e[MAX_GRAPHS]; uint64_t clock; };
+
+}  // namespace
+
+size_t meb_solver_dev_size() { return sizeof(SolverDev); }
+
+void meb_free_graph_cache(meb_ctx* ctx) {
+    GraphCache* gc = (GraphCache*)ctx->graph_cache;
+    if (!gc) return;
+    for (int i = 0; i < MAX_GRAPHS; ++i)
+        if (gc->e[i].used) { cudaGraphExecDestroy(gc->e[i].ex); cudaGraphDestroy(gc->e[i].g); }
+    free(gc);
+    ctx->graph_cache = nullptr;
 }
 
-struct Ev { double s[MEB_EVAL_NSCALARS]; std::vector<double> g; double psi_n; };
+namespace {
 
-EvalCall make_call(const Solver& S, const Problem& P, double sigma) {
-    EvalCall c;
-    c.gs = nullptr;
-    c.prec = P.prec; c.m = P.m; c.d = P.d; c.C = P.C; c.ld = P.ld; c.R = P.R;
-    c.U = P.has_mult ? P.U[P.cur] : nullptr;
-    c.v_slot = P.has_mult ? P.slot[P.cur] : nullptr;
-    c.V = P.has_mult ? P.V[P.cur] : nullptr;
-    c.ldv = P.ldv;
-    c.x = S.dx; c.xbar = S.dxbar; c.sigma = sigma / S.L; c.tau = S.par.tau / (S.L * S.L);
-    return c;
+GraphCache* cache_of(meb_ctx* ctx) {
+    if (!ctx->graph_cache) ctx->graph_cache = calloc(1, sizeof(GraphCache));
+    return (GraphCache*)ctx->graph_cache;
 }
 
-void count_pass(Solver& S, const Problem& P) {
-    if (!P.full) S.st->passes_reduced++;
-    else if (P.prec == MEB_FP64) S.st->passes_fp64_full++;
-    else S.st->passes_fp32_full++;
-    S.bytes += S.ctx->last_pass_bytes;
-}
-
-// evaluate at normalised x; want_grad = false gives psi and the scalars only (Armijo trials)
-int evaluate(Solver& S, const Problem& P, const std::vector<double>& xn, double sigma, bool want_grad, Ev& ev) {
-    meb_ctx* ctx = S.ctx;
-    std::vector<double> xr;
-    to_raw(S, P, xn, xr);
-    int rc = upload(ctx, S.dx, xr.data(), S.d + 1);
-    if (rc) return rc;
-    EvalCall c = make_call(S, P, sigma);
-    ctx->cur_class = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
-    want_grad = true;
-    rc = meb_eval_internal(ctx, c, ctx->small + SM_EV, S.dgrad, nullptr, nullptr);
-    if (rc) return rc;
-    count_pass(S, P);
-    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_EV, MEB_EVAL_NSCALARS * sizeof(double),
-                                     cudaMemcpyDeviceToHost, ctx->stream));
-    if (want_grad)
-        MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 16, S.dgrad, (S.d + 1) * sizeof(double),
-                                         cudaMemcpyDeviceToHost, ctx->stream));
-    rc = sync_stream(ctx);
-    if (rc) return rc;
-    memcpy(ev.s, ctx->h_pinned, sizeof(ev.s));
-    ev.psi_n = ev.s[MEB_EV_PSI] / S.L;
-    if (want_grad) ev.g.assign(ctx->h_pinned + 16, ctx->h_pinned + 16 + S.d + 1);
+int add_conditional(meb_ctx* ctx, cudaGraph_t parent, cudaGraphConditionalHandle h, bool is_while,
+                    cudaGraphNode_t* node, cudaGraph_t* body) {
+    // inside a stream capture into `parent`: append a conditional node after what was captured so far
+    cudaStreamCaptureStatus status;
+    cudaGraph_t cg = nullptr;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    MEB_CUDA_OK(ctx, cudaStreamGetCaptureInfo(ctx->stream, &status, nullptr, &cg, &deps, &ndeps));
+    if (status != cudaStreamCaptureStatusActive || cg != parent) return MEB_E_CUDA;
+    cudaGraphNodeParams p = {};
+    p.type = cudaGraphNodeTypeConditional;
+    p.conditional.handle = h;
+    p.conditional.type = is_while ? cudaGraphCondTypeWhile : cudaGraphCondTypeIf;
+    p.conditional.size = 1;
+    MEB_CUDA_OK(ctx, cudaGraphAddNode(node, parent, deps, ndeps, &p));
+    *body = p.conditional.phGraph_out[0];
+    MEB_CUDA_OK(ctx, cudaStreamUpdateCaptureDependencies(ctx->stream, node, 1, cudaStreamSetCaptureDependencies));
     return MEB_OK;
 }
 
-double rel_kkt(const Ev& ev, double r_raw, double terms[5]) {   // P:L307-311, reading 7
-    terms[0] = fabs(1.0 - ev.s[MEB_EV_SUM_UPLUS]);
-    terms[1] = ev.s[MEB_EV_NORM_SUM_VPLUS];
-    terms[2] = ev.s[MEB_EV_MAX_PFEAS] / (1.0 + r_raw);
-    terms[3] = ev.s[MEB_EV_MAX_DFEAS];
-    terms[4] = ev.s[MEB_EV_MAX_COMPL] / (1.0 + r_raw);
-    double k = 0.0;
-    for (int i = 0; i < 5; ++i) k = fmax(k, terms[i]);
+#define RC(expr) do { rc = (expr); if (rc != MEB_OK) goto fail; } while (0)
+#define CU(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { ctx->last_cuda_error = (int)e__; meb_debug_cuda(__FILE__, __LINE__, (int)e__); rc = MEB_E_CUDA; goto fail; } } while (0)
+
+int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
+    meb_ctx* ctx = S.ctx;
+    SolverDev* dev = (SolverDev*)ctx->sdev;
+    int rc = MEB_OK;
+    bool capturing = false;
+    cudaGraph_t tmp = nullptr, body = nullptr, bn = nullptr, bu = nullptr, bcg = nullptr;
+    cudaGraphNode_t wnode, nnode, unode, cgnode;
+    GraphSide gs;
+    memset(&gs, 0, sizeof(gs));
+    gs.dyn = &dev->dyn; gs.S = dev; gs.v = &S.v;
+    for (int b = 0; b < 2; ++b) { gs.U2[b] = P.U[b]; gs.slot2[b] = P.slot[b]; gs.V2[b] = P.V[b]; gs.vcap2[b] = P.vcap[b]; }
+    EvalCall c;
+    memset(&c, 0, sizeof(c));
+    c.prec = P.prec; c.m = P.m; c.d = P.d; c.C = P.C; c.ld = P.ld; c.R = P.R; c.ldv = P.ldv;
+    c.x = S.v.x_raw; c.xbar = S.v.xbar_raw; c.sigma = 1.0; c.tau = 1.0; c.gs = &gs;
+    bool list_after_eval = false;
+    int64_t l0;
+    cudaStream_t user_stream = ctx->stream;
+    ctx->stream = ctx->cap_stream;                 // launches below are CAPTURED on the private stream
+
+    CU(cudaGraphCreate(&G->g, 0));
+    CU(cudaGraphConditionalHandleCreate(&G->h_while, G->g, 1, cudaGraphCondAssignDefault));
+    CU(cudaGraphConditionalHandleCreate(&G->h_newton, G->g, 0, cudaGraphCondAssignDefault));
+    CU(cudaGraphConditionalHandleCreate(&G->h_update, G->g, 0, cudaGraphCondAssignDefault));
+    if (!dense) CU(cudaGraphConditionalHandleCreate(&G->h_cg, G->g, 0, cudaGraphCondAssignDefault));
+    {
+        cudaGraphNodeParams p = {};
+        p.type = cudaGraphNodeTypeConditional;
+        p.conditional.handle = G->h_while;
+        p.conditional.type = cudaGraphCondTypeWhile;
+        p.conditional.size = 1;
+        CU(cudaGraphAddNode(&wnode, G->g, nullptr, 0, &p));
+        body = p.conditional.phGraph_out[0];
+    }
+    // ---- loop body: evaluation + controller, then the two conditional branches ----
+    CU(cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    capturing = true;
+    l0 = ctx->launches;
+    ctx->cur_class = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
+    RC(meb_eval_internal(ctx, c, S.v.ev_t, S.v.grad_t, nullptr, nullptr));
+    G->k_eval = (int)(ctx->launches - l0);
+    G->bytes_per_eval = ctx->last_pass_bytes;
+    list_after_eval = ctx->list_valid;
+    RC(add_conditional(ctx, body, G->h_newton, false, &nnode, &bn));
+    RC(add_conditional(ctx, body, G->h_update, false, &unode, &bu));
+    CU(cudaStreamEndCapture(ctx->stream, &tmp));
+    capturing = false;
+    // ---- Newton branch (Alg. 2 line 8) ----
+    CU(cudaStreamBeginCaptureToGraph(ctx->stream, bn, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    capturing = true;
+    l0 = ctx->launches;
+    ctx->list_valid = list_after_eval;
+    RC(meb_ensure_list(ctx, P.m));
+    if (dense) {
+        RC(meb_dense_from_records(ctx, c, S.v.ev, S.dH));
+        RC(meb_chol_solve(ctx, S.dH, S.v.g, S.d + 1, S.L, S.v.delta, &dev->chol_info));
+        G->k_cg = 0;
+    } else {
+        RC(add_conditional(ctx, bn, G->h_cg, true, &cgnode, &bcg));
+    }
+    RC(meb_ctrl_after_newton(ctx, dev, S.v));
+    G->k_newton = (int)(ctx->launches - l0);
+    CU(cudaStreamEndCapture(ctx->stream, &tmp));
+    capturing = false;
+    if (!dense) {
+        CU(cudaStreamBeginCaptureToGraph(ctx->stream, bcg, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+        capturing = true;
+        l0 = ctx->launches;
+        ctx->list_valid = true;
+        RC(meb_hvp_from_records(ctx, c, S.v.ev, S.v.p, S.v.Hp));
+        RC(meb_ctrl_cg_step(ctx, dev, S.v));
+        G->k_cg = (int)(ctx->launches - l0);
+        CU(cudaStreamEndCapture(ctx->stream, &tmp));
+        capturing = false;
+    }
+    // ---- multiplier update branch (eq. (6), Alg. 1 lines 3-4) ----
+    CU(cudaStreamBeginCaptureToGraph(ctx->stream, bu, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    capturing = true;
+    l0 = ctx->launches;
+    ctx->list_valid = list_after_eval;
+    RC(meb_ensure_list(ctx, P.m));
+    RC(meb_reset_next(ctx, P.prec, &dev->dyn, P.U[0], P.U[1], P.slot[0], P.slot[1], P.m));
+    {
+        ActiveArgs a;
+        memset(&a, 0, sizeof(a));
+        a.C = c.C; a.ld = c.ld; a.ldv = c.ldv; a.x = c.x; a.d = c.d; a.dpad = (c.d + 7) / 8 * 8; a.sigma = 1.0;
+        a.list = ctx->list; a.count = ctx->count_dev;
+        a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
+        a.part_vec = ctx->part_vec; a.part_sc = ctx->part_sc; a.ldv_out = P.ldv;
+        a.dyn = gs.dyn;
+        for (int b = 0; b < 2; ++b) { a.U2[b] = gs.U2[b]; a.slot2[b] = gs.slot2[b]; a.V2[b] = gs.V2[b]; a.vcap2[b] = gs.vcap2[b]; }
+        int nvec = 0;
+        RC(meb_launch_active(ctx, MODE_WRITEV, P.prec, a, &nvec));
+    }
+    RC(meb_ctrl_after_update(ctx, dev, S.v, ctx->count_dev));
+    G->k_update = (int)(ctx->launches - l0);
+    CU(cudaStreamEndCapture(ctx->stream, &tmp));
+    capturing = false;
+    ctx->list_valid = false;
+    CU(cudaGraphInstantiate(&G->ex, G->g, 0));
+    ctx->stream = user_stream;
+    return MEB_OK;
+fail:
+    if (capturing) { cudaStreamEndCapture(ctx->stream, &tmp); }
+    ctx->stream = user_stream;
+    cudaGetLastError();
+    if (G->g) { cudaGraphDestroy(G->g); G->g = nullptr; }
+    ctx->list_valid = false;
+    return rc;
+}
+#undef RC
+#undef CU
+
+GraphKey make_key(const Solver& S, const Problem& P, bool dense) {
+    GraphKey k;
+    memset(&k, 0, sizeof(k));
+    k.prec = P.prec; k.dense = dense ? 1 : 0; k.m = P.m; k.d = P.d; k.C = P.C; k.ld = P.ld; k.R = P.R;
+    for (int b = 0; b < 2; ++b) { k.U[b] = P.U[b]; k.slot[b] = P.slot[b]; k.V[b] = P.V[b]; k.vcap[b] = P.vcap[b]; }
+    k.ldv = P.ldv; k.dH = S.dH; k.xn = S.v.xn;
     return k;
 }
 
-double dot(const std::vector<double>& a, const std::vector<double>& b) {
-    double s = 0.0;
-    for (size_t i = 0; i < a.size(); ++i) s += a[i] * b[i];
-    return s;
-}
-
-// H~ q = L * H_raw q through the active-list kernel (records of the evaluation at the current x)
-int apply_H(Solver& S, const Problem& P, double sigma, const std::vector<double>& q, std::vector<double>& Hq) {
-    meb_ctx* ctx = S.ctx;
-    int rc = upload(ctx, S.dq, q.data(), S.d + 1);
-    if (rc) return rc;
-    EvalCall c = make_call(S, P, sigma);
-    rc = meb_hvp_from_records(ctx, c, ctx->small + SM_EV, S.dq, S.dHq);
-    if (rc) return rc;
-    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 16, S.dHq, (S.d + 1) * sizeof(double),
-                                     cudaMemcpyDeviceToHost, ctx->stream));
-    rc = sync_stream(ctx);
-    if (rc) return rc;
-    Hq.resize(S.d + 1);
-    for (int j = 0; j <= S.d; ++j) Hq[j] = S.L * ctx->h_pinned[16 + j];
-    return MEB_OK;
-}
-
-// Newton direction by conjugate gradients (reading 5)
-int newton_cg(Solver& S, const Problem& P, double sigma, const std::vector<double>& g, std::vector<double>& delta) {
-    const int n = S.d + 1;
-    const double gn = sqrt(dot(g, g));
-    const double tol = fmin(0.1, gn) * gn;
-    delta.assign(n, 0.0);
-    std::vector<double> res(n), p(n), Hp;
-    for (int j = 0; j < n; ++j) { res[j] = -g[j]; p[j] = res[j]; }
-    double rr = dot(res, res);
-    for (int it = 0; it < S.par.cg_max; ++it) {
-        if (sqrt(rr) <= tol) break;
-        int rc = apply_H(S, P, sigma, p, Hp);
-        if (rc) return rc;
-        S.st->cg_iters++;
-        const double alpha = rr / dot(p, Hp);
-        for (int j = 0; j < n; ++j) { delta[j] += alpha * p[j]; res[j] -= alpha * Hp[j]; }
-        const double rr_new = dot(res, res);
-        const double beta = rr_new / rr;
-        for (int j = 0; j < n; ++j) p[j] = res[j] + beta * p[j];
-        rr = rr_new;
+int get_graph(Solver& S, const Problem& P, bool dense, SolveGraph** out) {
+    GraphCache* gc = cache_of(S.ctx);
+    if (!gc) return MEB_E_ALLOC;
+    const GraphKey key = make_key(S, P, dense);
+    int victim = 0;
+    for (int i = 0; i < MAX_GRAPHS; ++i) {
+        if (gc->e[i].used && memcmp(&gc->e[i].key, &key, sizeof(key)) == 0) {
+            gc->e[i].stamp = ++gc->clock;
+            *out = &gc->e[i];
+            return MEB_OK;
+        }
+        if (!gc->e[i].used) victim = i;
     }
+    if (gc->e[victim].used)
+        for (int i = 0; i < MAX_GRAPHS; ++i)
+            if (gc->e[i].stamp < gc->e[victim].stamp) victim = i;
+    SolveGraph* G = &gc->e[victim];
+    if (G->used) { cudaGraphExecDestroy(G->ex); cudaGraphDestroy(G->g); }
+    memset(G, 0, sizeof(*G));
+    int rc = build_graph(S, P, dense, G);
+    if (rc != MEB_OK) return rc;
+    G->used = true; G->key = key; G->stamp = ++gc->clock;
+    *out = G;
     return MEB_OK;
 }
 
-// Newton direction by dense assembly + Cholesky on the device (moderate d)
-int newton_dense(Solver& S, const Problem& P, double sigma, std::vector<double>& delta) {
-    meb_ctx* ctx = S.ctx;
-    const int n = S.d + 1;
-    EvalCall c = make_call(S, P, sigma);
-    int rc = meb_dense_from_records(ctx, c, ctx->small + SM_EV, S.dH);
+// Grow the V pool of buffer b to at least `rows` rows (keeps nothing: only called for the buffer that
+// is about to be overwritten, or before any multiplier exists).
+int grow_pool(meb_ctx* ctx, Problem& P, int b, int64_t rows) {
+    if (P.own_v[b] < 0) return MEB_E_CAPACITY;
+    int rc = own_reserve(ctx, P.own_v[b], (size_t)rows * P.ldv * esz(P.prec));
     if (rc) return rc;
-    rc = meb_chol_solve(ctx, S.dH, S.dgrad, n, S.L, S.ddelta, nullptr);      // H~ = L H_raw
-    if (rc) return rc;
-    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 16, S.ddelta, n * sizeof(double), cudaMemcpyDeviceToHost,
-                                     ctx->stream));
-    rc = sync_stream(ctx);
-    if (rc) return rc;
-    delta.assign(ctx->h_pinned + 16, ctx->h_pinned + 16 + n);
+    P.V[b] = ctx->own[P.own_v[b]];
+    P.vcap[b] = (int64_t)(ctx->own_bytes[P.own_v[b]] / ((size_t)P.ldv * esz(P.prec)));
     return MEB_OK;
 }
 
-// (U, V) <- (U+, V+) from the records of the evaluation at the accepted point (eq. (6))
-int update_multipliers(Solver& S, Problem& P, double sigma, const Ev& ev) {
-    meb_ctx* ctx = S.ctx;
-    const int nxt = P.has_mult ? 1 - P.cur : 0;
-    const int64_t nact = (int64_t)ev.s[MEB_EV_N_ACTIVE];
-    if (P.vcap[nxt] < nact || !P.V[nxt]) {
-        if (P.own_v[nxt] < 0) return MEB_E_CAPACITY;
-        const int64_t cap = nact + nact / 2 + 64;
-        int rc = own_reserve(ctx, P.own_v[nxt], (size_t)cap * P.ldv * esz(P.prec));
-        if (rc) return rc;
-        P.V[nxt] = ctx->own[P.own_v[nxt]];
-        P.vcap[nxt] = (int64_t)(ctx->own_bytes[P.own_v[nxt]] / ((size_t)P.ldv * esz(P.prec)));
-    }
-    int rc = P.prec == MEB_FP64 ? meb_fill_f64(ctx, (double*)P.U[nxt], P.m, 0.0)
-                                : meb_fill_f32(ctx, (float*)P.U[nxt], P.m, 0.f);
-    if (rc) return rc;
-    rc = meb_fill_i32(ctx, P.slot[nxt], P.m, -1);
-    if (rc) return rc;
-    EvalCall c = make_call(S, P, sigma);
-    rc = meb_ensure_list(ctx, P.m);
-    if (rc) return rc;
-    ActiveArgs a;
-    memset(&a, 0, sizeof(a));
-    a.C = c.C; a.ld = c.ld; a.U = c.U; a.v_slot = c.v_slot; a.V = c.V; a.ldv = c.ldv; a.x = c.x; a.d = c.d;
-    a.dpad = (c.d + 7) / 8 * 8; a.sigma = c.sigma; a.list = ctx->list; a.count = ctx->count_dev;
-    a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
-    a.part_vec = ctx->part_vec; a.part_sc = ctx->part_sc;
-    a.U_out = P.U[nxt]; a.slot_out = P.slot[nxt]; a.V_out = P.V[nxt]; a.ldv_out = P.ldv; a.cap_rows = P.vcap[nxt];
-    int nvec = 0;
-    rc = meb_launch_active(ctx, MODE_WRITEV, P.prec, a, &nvec);
-    if (rc) return rc;
-    P.cur = nxt;
-    P.has_mult = true;
-    return MEB_OK;
-}
-
-// Algorithm 1 with Algorithm 2 inside.  xn / ab are the normalised x and (alpha, beta), in/out.
+// Algorithm 1 with Algorithm 2 inside, device-resident: one graph launch per phase (plus one relaunch
+// whenever a V pool has to grow).  xn / ab are the normalised x and (alpha, beta), in/out (host).
 int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& ab, double tol, bool* converged,
            double* kkt_out, double terms_out[5]) {
-    const meb_params& par = S.par;
     meb_ctx* ctx = S.ctx;
+    const meb_params& par = S.par;
     const int n = S.d + 1;
-    double sigma = par.sigma0;
-    const double tau = par.tau;
+    SolverDev* dev = (SolverDev*)ctx->sdev;
+    SolverDev* h = (SolverDev*)ctx->h_sdev;
+    const bool dense = S.d <= par.dense_d_max && S.d <= 128;
     *converged = false;
-    Ev ev, evt;
-    std::vector<double> xbar, delta, xt(n), xr;
-    double terms[5];
-    for (int k = 0; k < par.outer_max; ++k) {
-        xbar = xn;                                                    // (r^k, c^k)
-        to_raw(S, P, xbar, xr);
-        int rc = upload(ctx, S.dxbar, xr.data(), n);
-        if (rc) return rc;
-        rc = evaluate(S, P, xn, sigma, true, ev);                     // Alg. 2 lines 3-4
-        if (rc) return rc;
-        bool records_current = true;
-        for (int j = 0; j < par.inner_max; ++j) {
-            const double kkt = rel_kkt(ev, S.L * xn[0], terms);
-            // relative-type stopping condition (5), on the tentative quantities
-            double agx = 0.0, dx2 = 0.0;
-            for (int i = 0; i < n; ++i) {
-                agx += (ab[i] - xn[i]) * ev.g[i];
-                dx2 += (xn[i] - xbar[i]) * (xn[i] - xbar[i]);
-            }
-            const double lhs = 2.0 * sigma * fabs(agx) + sigma * sigma * dot(ev.g, ev.g);
-            const double rhs = par.rho * (ev.s[MEB_EV_SUM_DMULT2] + tau * dx2);
-            if (lhs <= rhs) break;                                    // Alg. 2 line 5
-            if (kkt <= tol) break;                                    // reading 6
-            rc = (S.d <= par.dense_d_max && S.d <= 128) ? newton_dense(S, P, sigma, delta)
-                                                        : newton_cg(S, P, sigma, ev.g, delta);   // Alg. 2 line 8
-            if (rc) return rc;
-            S.st->newton_iters++;
-            const double slope = dot(ev.g, delta);
-            double eta = 1.0;
-            bool accepted = false;
-            for (int ls = 0; ls <= par.armijo_max_halvings; ++ls) {   // Armijo, P:L212 / reading 4
-                for (int i = 0; i < n; ++i) xt[i] = xn[i] + eta * delta[i];
-                rc = evaluate(S, P, xt, sigma, false, evt);
-                if (rc) return rc;
-                if (evt.psi_n <= ev.psi_n + par.armijo_mu * eta * slope) { accepted = true; break; }
-                eta *= 0.5;
-            }
-            if (!accepted) {
-                if (evt.psi_n <= ev.psi_n) {                          // last trial did not increase Psi: take it
-                    xn = xt;
-                    ev = evt;
-                } else {
-                    records_current = false;
-                }
-                break;                                                // stalled
-            }
-            xn = xt;
-            ev = evt;                                                 // the accepted trial is the next evaluation
-        }
-        if (!records_current) {                                       // rare: re-evaluate at x for the update
-            rc = evaluate(S, P, xn, sigma, true, ev);
+    // V pools: start small, grow on demand (ST_NEED_CAPACITY)
+    for (int b = 0; b < 2; ++b)
+        if (P.own_v[b] >= 0 && P.vcap[b] < 1024) {
+            int rc = grow_pool(ctx, P, b, P.m < 4096 ? P.m : 4096);
             if (rc) return rc;
         }
-        rc = update_multipliers(S, P, sigma, ev);                     // eq. (6)
+    int rc = upload(ctx, S.v.xn, xn.data(), n);
+    if (rc) return rc;
+    {   // (alpha, beta) and the raw offset share one staged upload each
+        rc = upload(ctx, S.v.ab, ab.data(), n);
         if (rc) return rc;
-        for (int i = 0; i < n; ++i) ab[i] -= sigma * ev.g[i];
-        S.st->outer_iters++;
-        const double kkt = rel_kkt(ev, S.L * xn[0], terms);
-        *kkt_out = kkt;
-        memcpy(terms_out, terms, sizeof(terms));
-        S.st->n_support = (int64_t)ev.s[MEB_EV_N_ACTIVE];
-        if (kkt <= tol) { *converged = true; break; }
-        sigma = fmin(par.sigma_max, par.kappa * sigma);               // P:L175, reading 3
+        if (P.off) { rc = upload(ctx, S.v.off, P.off, S.d); if (rc) return rc; }
     }
-    return MEB_OK;
+    bool first = true;
+    for (int attempt = 0; attempt < 64; ++attempt) {
+        SolveGraph* G = nullptr;
+        rc = get_graph(S, P, dense, &G);
+        if (rc) return rc;
+        MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));          // h is free to be rewritten
+        if (first) {
+            memset(h, 0, sizeof(*h));
+            h->L = S.L; h->tol = tol; h->rho = par.rho; h->tau = par.tau; h->kappa = par.kappa;
+            h->sigma_max = par.sigma_max; h->armijo_mu = par.armijo_mu;
+            h->n = n; h->d = S.d; h->inner_max = par.inner_max; h->outer_max = par.outer_max;
+            h->armijo_max = par.armijo_max_halvings; h->cg_max = par.cg_max; h->dense = dense ? 1 : 0;
+            h->use_off = P.off ? 1 : 0;
+            h->eval_cap = 4 * par.outer_max * (par.inner_max + 2);
+        }
+        h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
+        h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
+        h->in_graph = 1;
+        if (first) {
+            MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
+            rc = meb_ctrl_init(ctx, dev, S.v, par.sigma0, P.cur, P.has_mult ? 1 : 0);
+        } else {                                                        // resume: constants that may have changed
+            MEB_CUDA_OK(ctx, cudaMemcpyAsync(&dev->vcap[0], &h->vcap[0], 2 * sizeof(int64_t),
+                                             cudaMemcpyHostToDevice, ctx->stream));
+            MEB_CUDA_OK(ctx, cudaMemcpyAsync(&dev->h_while, &h->h_while, 4 * sizeof(cudaGraphConditionalHandle),
+                                             cudaMemcpyHostToDevice, ctx->stream));
+            rc = meb_ctrl_resume(ctx, dev);
+        }
+        if (rc) return rc;
+        first = false;
+        MEB_CUDA_OK(ctx, cudaGraphLaunch(G->ex, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+        // ---- statistics of this launch ----
+        const int cls = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
+        if (h->status != ST_NEED_CAPACITY || true) {
+            // counters are cumulative over relaunches: take them at the end of the phase only
+        }
+        if (h->status == ST_NEED_CAPACITY) {
+            const int nxt = h->dyn.has_mult ? 1 - h->dyn.cur : 0;
+            const int64_t want = h->n_support + h->n_support / 2 + 64;
+            rc = grow_pool(ctx, P, nxt, want < P.m ? want : P.m);
+            if (rc) return rc;
+            if (!h->dyn.has_mult) { rc = grow_pool(ctx, P, 1 - nxt, want < P.m ? want : P.m); if (rc) return rc; }
+            continue;
+        }
+        // ---- phase finished ----
+        S.st->outer_iters += h->outer;
+        S.st->newton_iters += h->newton_total;
+        S.st->cg_iters += h->cg_total;
+        if (!P.full) S.st->passes_reduced += h->evals;
+        else if (P.prec == MEB_FP64) S.st->passes_fp64_full += h->evals;
+        else S.st->passes_fp32_full += h->evals;
+        S.bytes += (double)h->evals * G->bytes_per_eval;
+        S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
+        S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval;
+        S.st->pass_count[cls] += (int32_t)h->pass_count;
+        ctx->launches += (int64_t)h->evals * G->k_eval + (int64_t)h->newton_total * G->k_newton +
+                         (int64_t)h->cg_total * G->k_cg + (int64_t)h->outer * G->k_update;
+        S.st->n_support = h->n_support;
+        *kkt_out = h->kkt;
+        memcpy(terms_out, h->terms, 5 * sizeof(double));
+        *converged = h->status == ST_CONVERGED;
+        P.cur = h->dyn.cur;
+        P.has_mult = h->dyn.has_mult != 0;
+        // final iterate back to the host
+        MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, S.v.xn, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + n, S.v.ab, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+        xn.assign(ctx->h_pinned, ctx->h_pinned + n);
+        ab.assign(ctx->h_pinned + n, ctx->h_pinned + 2 * n);
+        return MEB_OK;
+    }
+    return MEB_E_CAPACITY;
 }
 
 int setup_multipliers(meb_ctx* ctx, Problem& P, int ownU0, int ownS0, int ownV0) {
@@ -340,6 +428,9 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         !(S.par.kappa >= 1.0) || S.par.sample_rows < 1)
         return MEB_E_ARG;
     const int n = d + 1;
+    // The KKT test runs at tol/10: the primal-feasibility term only bounds the error of the returned
+    // (feasible) radius by about tol (1 + r)/r, and the contract is a radius within tol (DESIGN reading 7).
+    const double tol_kkt = 0.1 * tol;
     const bool timing_was = ctx->time_passes;
     ctx->evn = 0;
     ctx->ev_record = true;
@@ -359,14 +450,17 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         MEB_CUDA_OK(ctx, cudaEventRecord(e_start, ctx->stream));
         // ---- state vectors on the device ----
         const size_t nH = (d <= 128) ? (size_t)n * n + 8 : 8;
-        rc = own_reserve(ctx, OWN_STATE, (size_t)(7 * (n + 8) + nH) * sizeof(double));
+        const size_t nv = ((size_t)n + 7) / 8 * 8;
+        rc = own_reserve(ctx, OWN_STATE, (14 * nv + 2 * MEB_EVAL_NSCALARS + nH) * sizeof(double));
         if (rc) break;
         double* base = (double*)ctx->own[OWN_STATE];
-        S.dx = base; S.dxbar = base + (n + 8); S.dq = base + 2 * (n + 8); S.dHq = base + 3 * (n + 8);
-        S.dgrad = base + 4 * (n + 8);
-        double* dc0 = base + 5 * (n + 8);
-        S.ddelta = base + 6 * (n + 8);
-        S.dH = base + 7 * (n + 8);
+        double** vecs[] = {&S.v.xn, &S.v.xbar, &S.v.ab, &S.v.delta, &S.v.g, &S.v.xt, &S.v.x_raw, &S.v.xbar_raw,
+                           &S.v.off, &S.v.grad_t, &S.v.res, &S.v.p, &S.v.Hp};
+        for (size_t i = 0; i < 13; ++i) *vecs[i] = base + i * nv;
+        double* dc0 = base + 13 * nv;
+        S.v.ev_t = base + 14 * nv;
+        S.v.ev = S.v.ev_t + MEB_EVAL_NSCALARS;
+        S.dH = S.v.ev + MEB_EVAL_NSCALARS;
         // ---- a0: ingest (initial point, validation, FP32 shadow) ----
         float* C32 = nullptr; float* R32 = nullptr;
         const int64_t ld32 = ((int64_t)d + 3) / 4 * 4;
@@ -412,17 +506,17 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             rc = setup_multipliers(ctx, P, OWN_U0, OWN_S0, OWN_V0);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
-            rc = ripalm(S, P, xn, ab, tol, &converged, &kkt, terms);
+            rc = ripalm(S, P, xn, ab, tol_kkt, &converged, &kkt, terms);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
             // final full pass: r_out = max_i(||c - c_i|| + r_i)   (step 7)
             std::vector<double> xr;
             to_raw(S, P, xn, xr);
-            rc = upload(ctx, S.dx, xr.data(), n);
+            rc = upload(ctx, S.v.x_raw, xr.data(), n);
             if (rc) break;
             r_alg = xr[0];
             int32_t am = 0; int64_t nv = 0;
-            rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.dx + 1, INFINITY, nullptr, &dmax,
+            rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, INFINITY, nullptr, &dmax,
                                        &am, nullptr, 0, &nv);
             if (rc) break;
             st->passes_fp64_full++;
@@ -448,10 +542,10 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             std::vector<double> xs(n);
             xs[0] = S.L * xn[0];
             for (int j = 0; j < d; ++j) xs[1 + j] = S.L * xn[1 + j];   // centred coordinates of the shadow
-            rc = upload(ctx, S.dq, xs.data(), n);
+            rc = upload(ctx, S.v.xt, xs.data(), n);
             if (rc) break;
             int64_t nred = 0;
-            rc = meb_screen_compact(ctx, m, d, C32, ld32, R32, (float)xs[0], S.dq + 1,
+            rc = meb_screen_compact(ctx, m, d, C32, ld32, R32, (float)xs[0], S.v.xt + 1,
                                     (float)(S.par.tol_red_factor * xs[0]), idx, m, &nred, nullptr, 0);
             if (rc) break;
             st->passes_fp32_full++;
@@ -517,19 +611,19 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                     P2.m = nred;
                     st->n_reduced = nred;
                     st->rounds = rnd + 1;
-                    rc = ripalm(S, P2, xn, ab, tol, &converged, &kkt, terms);
+                    rc = ripalm(S, P2, xn, ab, tol_kkt, &converged, &kkt, terms);
                     if (rc) break;
                     if (rnd == 0) MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
                     // a-posteriori check against ALL original constraints
                     std::vector<double> xr;
                     to_raw(S, P2, xn, xr);
-                    rc = upload(ctx, S.dx, xr.data(), n);
+                    rc = upload(ctx, S.v.x_raw, xr.data(), n);
                     if (rc) break;
                     r_alg = xr[0];
                     for (int j = 0; j < d; ++j) creturn[j] = xr[1 + j];
-                    const double eps_feas = tol * (1.0 + r_alg);            // reading 10
+                    const double eps_feas = tol_kkt * (1.0 + r_alg);        // reading 10
                     int32_t am = 0; int64_t nv = 0;
-                    rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.dx + 1, eps_feas, kept,
+                    rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, eps_feas, kept,
                                                &dmax, &am, idx + nred, m - nred, &nv);
                     if (rc) break;
                     st->passes_fp64_full++;

@@ -25,7 +25,9 @@ namespace {
 
 // ---- tiled kernel: G lanes per row, CPT chunks per lane (G * CPT * VEC >= d) ---------------------
 template <typename T, int G, int CPT, int VEC, int OP, bool SHADOW>
-__global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs a) {
+__global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs a_in) {
+    StreamArgs a = a_in;
+    meb_resolve_dyn(a);
     constexpr int RPW = 32 / G;                     // rows per warp-wide load instruction
     constexpr int NPAD = G * CPT * VEC;             // padded row length held in shared memory
     __shared__ __align__(16) T cs[NPAD];
@@ -148,7 +150,9 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
 
 // ---- loop kernel: one warp per row, any d -----------------------------------------------------------
 template <typename T, int VEC, int OP, bool SHADOW>
-__global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs a) {
+__global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs a_in) {
+    StreamArgs a = a_in;
+    meb_resolve_dyn(a);
     constexpr int UNR = 8;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d = a.d;
@@ -300,6 +304,7 @@ int meb_launch_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* 
     if (prec == MEB_FP64) {
         bool al = rows_aligned<double>(a.C, a.ld);
         if (a.v_slot) al = al && rows_aligned<double>(a.V, a.ldv);
+        if (a.dyn) al = al && rows_aligned<double>(a.V2[0], a.ldv) && rows_aligned<double>(a.V2[1], a.ldv);
         switch (op) {
             case OP_EVAL: return dispatch_shape<double, OP_EVAL, false>(ctx, a, al, grid_out);
             case OP_FEAS: return dispatch_shape<double, OP_FEAS, false>(ctx, a, al, grid_out);
@@ -311,6 +316,7 @@ int meb_launch_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* 
     } else {
         bool al = rows_aligned<float>(a.C, a.ld);
         if (a.v_slot) al = al && rows_aligned<float>(a.V, a.ldv);
+        if (a.dyn) al = al && rows_aligned<float>(a.V2[0], a.ldv) && rows_aligned<float>(a.V2[1], a.ldv);
         switch (op) {
             case OP_EVAL: return dispatch_shape<float, OP_EVAL, false>(ctx, a, al, grid_out);
             case OP_SCREEN: return dispatch_shape<float, OP_SCREEN, false>(ctx, a, al, grid_out);

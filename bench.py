@@ -38,7 +38,7 @@ TOL = 1e-8
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k-1], k = 1..5")
     ap.add_argument("--mode", default="mixed", choices=["mixed", "fp64"])
@@ -60,7 +60,8 @@ def workload_name(k, m, d, mode):
 
 # ------------------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs (one long-lived
+    `nvidia-smi -lms` process: spawning one per sample is slower than a short timed region)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -68,26 +69,35 @@ class ClockSampler:
     def __init__(self, index=0):
         self.index = index
         self.rows = []
-        self.stop = threading.Event()
-        self.th = threading.Thread(target=self._run, daemon=True)
+        self.proc = None
+        self.th = None
 
     def _run(self):
-        while not self.stop.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
-                self.rows.append([c.strip() for c in out.strip().split(",")])
-            except Exception:
-                pass
-            self.stop.wait(0.1)
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.strip().split(",")])
 
     def __enter__(self):
-        self.th.start()
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._run, daemon=True)
+            self.th.start()
+            time.sleep(0.3)                      # let the first samples arrive before the region starts
+            self.rows.clear()
+        except Exception:
+            self.proc = None
         return self
 
     def __exit__(self, *a):
-        self.stop.set()
-        self.th.join(timeout=6)
+        if self.proc is not None:
+            time.sleep(0.06)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+            self.th.join(timeout=5)
 
     def summary(self):
         sm, mx, reasons = [], 0.0, set()

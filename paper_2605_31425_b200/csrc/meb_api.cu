@@ -23,7 +23,7 @@ static void ctx_free_all(meb_ctx* c) {
     cudaFree(c->list); cudaFree(c->blocksum); cudaFree(c->part_scalar); cudaFree(c->part_vec);
     cudaFree(c->part_mat); cudaFree(c->count_dev); cudaFree(c->part_sc); cudaFree(c->small);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
-    for (int i = 0; i < 16; ++i) if (c->own[i]) cudaFree(c->own[i]);
+    for (int i = 0; i < 24; ++i) if (c->own[i]) cudaFree(c->own[i]);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     meb_free_graph_cache(c);

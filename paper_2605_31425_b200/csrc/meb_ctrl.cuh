@@ -69,6 +69,19 @@ __device__ __forceinline__ double ctrl_block_sum(double v, double* sm) {
     return t;
 }
 
+// three block-wide sums with one pair of barriers (fixed order: warp xor tree, then warps in index order)
+__device__ __forceinline__ void ctrl_block_sum3(double& a, double& b, double& c, double* sm) {
+    a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+    __syncthreads();
+    const int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) { sm[w] = a; sm[32 + w] = b; sm[64 + w] = c; }
+    __syncthreads();
+    const int nw = (blockDim.x + 31) >> 5;
+    double ta = 0.0, tb = 0.0, tc = 0.0;
+    for (int q = 0; q < nw; ++q) { ta += sm[q]; tb += sm[32 + q]; tc += sm[64 + q]; }
+    a = ta; b = tb; c = tc;
+}
+
 // x_raw = (L r~, off + L c~)
 __device__ __forceinline__ void ctrl_to_raw(const SolverDev* S, const SolverVecs& v, const double* xn_, double* out) {
     for (int j = threadIdx.x; j < S->n; j += blockDim.x)
@@ -98,7 +111,16 @@ __device__ __forceinline__ double ctrl_rel_kkt(const double* ev, double r_raw, d
 // Runs in the single CTA of the evaluation-finalize kernel, after ev_t / grad_t of the pass at
 // x_raw have been written: Armijo test (reading 4), stopping tests (5) and KKT (P:L133-135,
 // L244, reading 6), choice of the next action.  All threads of the CTA call it.
-__device__ inline void ctrl_after_eval(SolverDev* S, const SolverVecs v, double* sm) {
+// S is a SHARED-MEMORY copy of the state (loaded by the caller); it is written back to Sg at the end.
+__device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, double* sm);
+__device__ inline void ctrl_after_eval(SolverDev* Sg, SolverDev* S, const SolverVecs v, double* sm) {
+    ctrl_after_eval_body(S, v, sm);
+    __syncthreads();
+    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(S);
+    unsigned long long* dst = reinterpret_cast<unsigned long long*>(Sg);
+    for (int q = threadIdx.x; q < (int)(sizeof(SolverDev) / 8); q += blockDim.x) dst[q] = src[q];
+}
+__device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, double* sm) {
     __syncthreads();
     const int n = S->n;
     const int phase = S->phase;
@@ -153,9 +175,7 @@ __device__ inline void ctrl_after_eval(SolverDev* S, const SolverVecs v, double*
         const double dx = xj - v.xbar[j];
         dx2 = fma(dx, dx, dx2);
     }
-    agx = ctrl_block_sum(agx, sm);
-    gg = ctrl_block_sum(gg, sm);
-    dx2 = ctrl_block_sum(dx2, sm);
+    ctrl_block_sum3(agx, gg, dx2, sm);
     if (threadIdx.x == 0) {
         S->evals++;
         S->psi_cur = psi_t;

@@ -142,17 +142,20 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
 // Square-root-free Cholesky (H = L D L^T, no pivoting: H is SPD) on the AUGMENTED matrix
 // M = [H; -g^T]: eliminating column k also updates the right-hand-side row n, so after the n column
 // steps row n holds D L^{-1}(-g) and only the backward substitution with L^T is left.
-// The matrix lives in REGISTERS: thread (ty, tx) owns M[ty + 16 ii][tx + 16 jj], ii, jj < BS.  Per
-// column k the owners publish column k to shared memory (kept there as row k of Lm = L D for the
-// backward substitution), one __syncthreads, then every thread updates its live entries with
-// broadcast / conflict-free shared reads and register FMAs.
+// The matrix lives in REGISTERS: thread (ty, tx) owns M[ty + 16 ii][tx + 16 jj], jj <= ii < BS.
+// Column steps are grouped in phases of 16 (KB = k / 16) that are unrolled at compile time, so inside
+// a phase the code is straight-line: every thread updates its (BS-KB)(BS-KB+1)/2 live entries with
+// multipliers masked to zero outside the trailing block (no branches), the owners of column k+1
+// publish it to shared memory (where it stays as row k+1 of L D for the backward substitution)
+// together with 1/d_{k+1}, computed by the diagonal's owner while the others are still updating.
+// One __syncthreads per column.
 template <int BS>
 __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
                                                          int n, double scale, double* __restrict__ delta,
                                                          int* __restrict__ info) {
-    extern __shared__ __align__(16) double Lm[];          // n rows x ldl (column k of L D as row k), invd[n], z[n]
+    extern __shared__ __align__(16) double Lm[];          // n rows x ldl (column k of L D as row k), invd, z
     constexpr int NP = 16 * BS;
-    const int ldl = NP | 1;
+    constexpr int ldl = NP | 1;
     double* invd = Lm + (size_t)n * ldl;
     double* z = invd + NP;
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
@@ -163,7 +166,7 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
         for (int jj = 0; jj < BS; ++jj) {
             const int i = ty + 16 * ii, j = tx + 16 * jj;
             double v = 0.0;
-            if (j < n && j <= i) {
+            if (jj <= ii && j < n && j <= i) {
                 if (i < n) v = scale * H[(size_t)i * n + j];
                 else if (i == n) v = -g[j];
             }
@@ -171,37 +174,63 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
         }
     __shared__ int bad;
     if (tid == 0) bad = 0;
-    for (int k = 0; k < n; ++k) {
-        double* col = Lm + (size_t)k * ldl;
-        if (tx == (k & 15)) {                             // owners of column k publish rows i >= k
-            const int jk = k >> 4;
+    if (tx == 0) {                                        // publish column 0 and 1/d_0
 #pragma unroll
-            for (int jj = 0; jj < BS; ++jj)
-                if (jj == jk) {
-#pragma unroll
-                    for (int ii = 0; ii < BS; ++ii) col[ty + 16 * ii] = a[ii][jj];
-                }
-        }
-        __syncthreads();
-        double dk = col[k];
-        if (!(dk > 0.0)) { if (tid == 0) bad = k + 1; dk = 1.0; }
-        const double inv = 1.0 / dk;
-        if (tid == 0) invd[k] = inv;
-#pragma unroll
-        for (int ii = 0; ii < BS; ++ii) {
-            const int i = ty + 16 * ii;
-            if (16 * ii + 15 > k && i > k && i <= n) {
-                const double lik = col[i] * inv;
-#pragma unroll
-                for (int jj = 0; jj <= ii; ++jj) {
-                    const int j = tx + 16 * jj;
-                    if (j > k && j <= i) a[ii][jj] = fma(-lik, col[j], a[ii][jj]);
-                }
-            }
+        for (int ii = 0; ii < BS; ++ii) Lm[ty + 16 * ii] = a[ii][0];
+        if (ty == 0) {
+            double dk = a[0][0];
+            if (!(dk > 0.0)) { bad = 1; dk = 1.0; }
+            invd[0] = 1.0 / dk;
         }
     }
     __syncthreads();
-    // z = D^{-1} (row n of L D); then L^T x = z, column-oriented, one warp: L_kj = Lm[j][k] * invd[j]
+#pragma unroll
+    for (int KB = 0; KB < BS; ++KB) {
+        if (16 * KB < n) {
+#pragma unroll 1
+            for (int kk = 0; kk < 16; ++kk) {
+                const int k = 16 * KB + kk;
+                if (k >= n) break;                        // uniform
+                const double* col = Lm + (size_t)k * ldl;
+                const double inv = invd[k];
+                double lik[BS], cj[BS];
+#pragma unroll
+                for (int q = KB; q < BS; ++q) {
+                    const double ci = col[ty + 16 * q], cc = col[tx + 16 * q];
+                    lik[q] = (ty + 16 * q > k) ? ci * inv : 0.0;
+                    cj[q] = (tx + 16 * q > k) ? cc : 0.0;
+                }
+#pragma unroll
+                for (int ii = KB; ii < BS; ++ii)
+#pragma unroll
+                    for (int jj = KB; jj <= ii; ++jj) a[ii][jj] = fma(-lik[ii], cj[jj], a[ii][jj]);
+                const int k1 = k + 1;
+                if (k1 < n && tx == (k1 & 15)) {          // owners of column k+1 publish it
+                    double* cn = Lm + (size_t)k1 * ldl;
+                    if (kk < 15) {
+#pragma unroll
+                        for (int ii = KB; ii < BS; ++ii) cn[ty + 16 * ii] = a[ii][KB];
+                        if (ty == tx) {
+                            double dk = a[KB][KB];
+                            if (!(dk > 0.0)) { bad = k1 + 1; dk = 1.0; }
+                            invd[k1] = 1.0 / dk;
+                        }
+                    } else if (KB + 1 < BS) {
+#pragma unroll
+                        for (int ii = KB + 1; ii < BS; ++ii) cn[ty + 16 * ii] = a[ii][KB + 1 < BS ? KB + 1 : KB];
+                        if (ty == tx) {
+                            double dk = a[KB + 1 < BS ? KB + 1 : KB][KB + 1 < BS ? KB + 1 : KB];
+                            if (!(dk > 0.0)) { bad = k1 + 1; dk = 1.0; }
+                            invd[k1] = 1.0 / dk;
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+        }
+    }
+    // row n of L D is spread over the columns' shared rows: z_k = Lm[k][n] / d_k; then L^T x = z,
+    // column-oriented, one warp: L_kj = Lm[j][k] * invd[j]
     if (tid < 32) {
         for (int j = tid; j < n; j += 32) z[j] = Lm[(size_t)j * ldl + n] * invd[j];
         __syncwarp();

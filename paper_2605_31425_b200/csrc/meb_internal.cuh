@@ -44,8 +44,8 @@ struct meb_ctx {
     double* h_pinned;       // pinned host mirror for small read-backs
     int64_t h_pinned_len;
     // ---- owned copies for meb_solve / meb_solve_host ----
-    void* own[16];
-    size_t own_bytes[16];
+    void* own[24];
+    size_t own_bytes[24];
     // ---- measurement ----
     cudaEvent_t ev0, ev1;
     double last_pass_ms;

@@ -8,17 +8,6 @@ namespace {
 
 constexpr int FBLOCK = 1024;
 
-// deterministic block-wide sum: warp xor tree, then warps in index order
-__device__ __forceinline__ double block_sum_1024(double v, double* sm) {
-    v = warp_sum(v);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double t = 0.0;
-    for (int w = 0; w < FBLOCK / 32; ++w) t += sm[w];
-    return t;
-}
-
 // scalar k of the CTA partials: lanes stride over the CTAs, xor tree (warp k handles scalar k)
 __device__ __forceinline__ double partial_sum(const double* part, int grid, int k, int lane) {
     double s = 0.0;
@@ -36,10 +25,17 @@ __device__ __forceinline__ double partial_max(const double* part, int grid, int 
 // then added in order, so the order does not depend on timing).  With f.S != nullptr the same CTA then
 // runs the controller step of the device-resident solver (meb_ctrl.cuh).
 __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArgs f) {
-    __shared__ double sm[FBLOCK / 32];
+    __shared__ double sm[96];
     __shared__ double sc[MEB_NPART];
     __shared__ double seg[FBLOCK];
+    __shared__ __align__(16) SolverDev sS;             // working copy of the solver state (controller step)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (f.S) {
+        const unsigned long long* src = reinterpret_cast<const unsigned long long*>(f.S);
+        unsigned long long* dst = reinterpret_cast<unsigned long long*>(&sS);
+        for (int q = threadIdx.x; q < (int)(sizeof(SolverDev) / 8); q += FBLOCK) dst[q] = src[q];
+        __syncthreads();
+    }
     const double* __restrict__ part = f.part;
     const double* __restrict__ part_vec = f.part_vec;
     const int grid = f.grid, d = f.d, dpad = f.dpad;
@@ -64,7 +60,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
             t0 = min(t0, __shfl_xor_sync(MEB_FULL_MASK, t0, o));
             t1 = max(t1, __shfl_xor_sync(MEB_FULL_MASK, t1, o));
         }
-        if (lane == 0 && t1 > t0) { f.S->pass_ns += (unsigned long long)(t1 - t0); f.S->pass_count++; }
+        if (lane == 0 && t1 > t0) { sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++; }
     }
     // vector part: sum_i v+_i = sigma * sum_k lam_k b_k
     int nvec = f.nvec;
@@ -104,8 +100,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
             dx2 = fma(dx, dx, dx2);
         }
     }
-    nv2 = block_sum_1024(nv2, sm);
-    dx2 = block_sum_1024(dx2, sm);
+    { double dummy = 0.0; ctrl_block_sum3(nv2, dx2, dummy, sm); }
     __syncthreads();
     if (threadIdx.x == 0) {
         double* out = f.out;
@@ -127,7 +122,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
         out[12] = dx2;
         out[13] = 0.0; out[14] = 0.0; out[15] = 0.0;
     }
-    if (f.S) ctrl_after_eval(f.S, f.v, sm);
+    if (f.S) ctrl_after_eval(f.S, &sS, f.v, sm);
 }
 
 // H q from the active-list partials (reading 1):

@@ -22,7 +22,7 @@
 namespace {
 
 enum { OWN_U0 = 0, OWN_U1, OWN_S0, OWN_S1, OWN_V0, OWN_V1, OWN_C32, OWN_R32, OWN_IDX, OWN_CRED, OWN_RRED,
-       OWN_KEPT, OWN_STATE, OWN_HOSTC, OWN_HOSTR, OWN_SPARE };
+       OWN_KEPT, OWN_STATE, OWN_HOSTC, OWN_HOSTR, OWN_SPARE, OWN_VRED0, OWN_VRED1 };
 
 int own_reserve(meb_ctx* ctx, int slot, size_t bytes) {
     if (ctx->own_bytes[slot] >= bytes && ctx->own[slot]) return MEB_OK;
@@ -131,24 +131,80 @@ int add_conditional(meb_ctx* ctx, cudaGraph_t parent, cudaGraphConditionalHandle
     return MEB_OK;
 }
 
+// ---- launch sequences shared by the captured graph and the stepped (host-sequenced) driver ----------
+struct Seq {
+    Solver* S; const Problem* P; bool dense;
+    GraphSide gs; EvalCall c; SolverDev* dev;
+};
+
+void seq_init(Seq& q, Solver& S, const Problem& P, bool dense) {
+    meb_ctx* ctx = S.ctx;
+    q.S = &S; q.P = &P; q.dense = dense;
+    q.dev = (SolverDev*)ctx->sdev;
+    memset(&q.gs, 0, sizeof(q.gs));
+    q.gs.dyn = &q.dev->dyn; q.gs.S = q.dev; q.gs.v = &S.v;
+    for (int b = 0; b < 2; ++b) { q.gs.U2[b] = P.U[b]; q.gs.slot2[b] = P.slot[b]; q.gs.V2[b] = P.V[b]; q.gs.vcap2[b] = P.vcap[b]; }
+    memset(&q.c, 0, sizeof(q.c));
+    q.c.prec = P.prec; q.c.m = P.m; q.c.d = P.d; q.c.C = P.C; q.c.ld = P.ld; q.c.R = P.R; q.c.ldv = P.ldv;
+    q.c.x = S.v.x_raw; q.c.xbar = S.v.xbar_raw; q.c.sigma = 1.0; q.c.tau = 1.0; q.c.gs = &q.gs;
+}
+
+// evaluation at the trial point + controller step (Alg. 2 lines 3-7, 9)
+int seq_eval(Seq& q) {
+    meb_ctx* ctx = q.S->ctx;
+    const Problem& P = *q.P;
+    ctx->cur_class = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
+    return meb_eval_internal(ctx, q.c, q.S->v.ev_t, q.S->v.grad_t, nullptr, nullptr);
+}
+// Newton direction, dense path (Alg. 2 line 8): active list, H, LDL^T
+int seq_newton_dense(Seq& q) {
+    meb_ctx* ctx = q.S->ctx;
+    int rc = meb_ensure_list(ctx, q.P->m);
+    if (rc) return rc;
+    rc = meb_dense_from_records(ctx, q.c, q.S->v.ev, q.S->dH);
+    if (rc) return rc;
+    return meb_chol_solve(ctx, q.S->dH, q.S->v.g, q.S->d + 1, q.S->L, q.S->v.delta, &q.dev->chol_info);
+}
+// one CG iteration of the matrix-free path: Hp = H p over the active rows, CG step
+int seq_cg_body(Seq& q) {
+    meb_ctx* ctx = q.S->ctx;
+    int rc = meb_hvp_from_records(ctx, q.c, q.S->v.ev, q.S->v.p, q.S->v.Hp);
+    if (rc) return rc;
+    return meb_ctrl_cg_step(ctx, q.dev, q.S->v);
+}
+// multiplier update (eq. (6)) and the bookkeeping of Algorithm 1 lines 3-4
+int seq_update(Seq& q) {
+    meb_ctx* ctx = q.S->ctx;
+    const Problem& P = *q.P;
+    int rc = meb_ensure_list(ctx, P.m);
+    if (rc) return rc;
+    rc = meb_reset_next(ctx, P.prec, &q.dev->dyn, P.U[0], P.U[1], P.slot[0], P.slot[1], P.m);
+    if (rc) return rc;
+    ActiveArgs a;
+    memset(&a, 0, sizeof(a));
+    a.C = q.c.C; a.ld = q.c.ld; a.ldv = q.c.ldv; a.x = q.c.x; a.d = q.c.d; a.dpad = (q.c.d + 7) / 8 * 8; a.sigma = 1.0;
+    a.list = ctx->list; a.count = ctx->count_dev;
+    a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
+    a.part_vec = ctx->part_vec; a.part_sc = ctx->part_sc; a.ldv_out = P.ldv;
+    a.dyn = q.gs.dyn;
+    for (int b = 0; b < 2; ++b) { a.U2[b] = q.gs.U2[b]; a.slot2[b] = q.gs.slot2[b]; a.V2[b] = q.gs.V2[b]; a.vcap2[b] = q.gs.vcap2[b]; }
+    int nvec = 0;
+    rc = meb_launch_active(ctx, MODE_WRITEV, P.prec, a, &nvec);
+    if (rc) return rc;
+    return meb_ctrl_after_update(ctx, q.dev, q.S->v, ctx->count_dev);
+}
+
 #define RC(expr) do { rc = (expr); if (rc != MEB_OK) goto fail; } while (0)
 #define CU(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { ctx->last_cuda_error = (int)e__; meb_debug_cuda(__FILE__, __LINE__, (int)e__); rc = MEB_E_CUDA; goto fail; } } while (0)
 
 int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     meb_ctx* ctx = S.ctx;
-    SolverDev* dev = (SolverDev*)ctx->sdev;
     int rc = MEB_OK;
     bool capturing = false;
     cudaGraph_t tmp = nullptr, body = nullptr, bn = nullptr, bu = nullptr, bcg = nullptr;
     cudaGraphNode_t wnode, nnode, unode, cgnode;
-    GraphSide gs;
-    memset(&gs, 0, sizeof(gs));
-    gs.dyn = &dev->dyn; gs.S = dev; gs.v = &S.v;
-    for (int b = 0; b < 2; ++b) { gs.U2[b] = P.U[b]; gs.slot2[b] = P.slot[b]; gs.V2[b] = P.V[b]; gs.vcap2[b] = P.vcap[b]; }
-    EvalCall c;
-    memset(&c, 0, sizeof(c));
-    c.prec = P.prec; c.m = P.m; c.d = P.d; c.C = P.C; c.ld = P.ld; c.R = P.R; c.ldv = P.ldv;
-    c.x = S.v.x_raw; c.xbar = S.v.xbar_raw; c.sigma = 1.0; c.tau = 1.0; c.gs = &gs;
+    Seq q;
+    seq_init(q, S, P, dense);
     bool list_after_eval = false;
     int64_t l0;
     cudaStream_t user_stream = ctx->stream;
@@ -172,8 +228,7 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     CU(cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
     capturing = true;
     l0 = ctx->launches;
-    ctx->cur_class = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
-    RC(meb_eval_internal(ctx, c, S.v.ev_t, S.v.grad_t, nullptr, nullptr));
+    RC(seq_eval(q));
     G->k_eval = (int)(ctx->launches - l0);
     G->bytes_per_eval = ctx->last_pass_bytes;
     list_after_eval = ctx->list_valid;
@@ -186,15 +241,14 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     capturing = true;
     l0 = ctx->launches;
     ctx->list_valid = list_after_eval;
-    RC(meb_ensure_list(ctx, P.m));
     if (dense) {
-        RC(meb_dense_from_records(ctx, c, S.v.ev, S.dH));
-        RC(meb_chol_solve(ctx, S.dH, S.v.g, S.d + 1, S.L, S.v.delta, &dev->chol_info));
+        RC(seq_newton_dense(q));
         G->k_cg = 0;
     } else {
+        RC(meb_ensure_list(ctx, P.m));
         RC(add_conditional(ctx, bn, G->h_cg, true, &cgnode, &bcg));
     }
-    RC(meb_ctrl_after_newton(ctx, dev, S.v));
+    RC(meb_ctrl_after_newton(ctx, q.dev, S.v));
     G->k_newton = (int)(ctx->launches - l0);
     CU(cudaStreamEndCapture(ctx->stream, &tmp));
     capturing = false;
@@ -203,8 +257,7 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
         capturing = true;
         l0 = ctx->launches;
         ctx->list_valid = true;
-        RC(meb_hvp_from_records(ctx, c, S.v.ev, S.v.p, S.v.Hp));
-        RC(meb_ctrl_cg_step(ctx, dev, S.v));
+        RC(seq_cg_body(q));
         G->k_cg = (int)(ctx->launches - l0);
         CU(cudaStreamEndCapture(ctx->stream, &tmp));
         capturing = false;
@@ -214,21 +267,7 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     capturing = true;
     l0 = ctx->launches;
     ctx->list_valid = list_after_eval;
-    RC(meb_ensure_list(ctx, P.m));
-    RC(meb_reset_next(ctx, P.prec, &dev->dyn, P.U[0], P.U[1], P.slot[0], P.slot[1], P.m));
-    {
-        ActiveArgs a;
-        memset(&a, 0, sizeof(a));
-        a.C = c.C; a.ld = c.ld; a.ldv = c.ldv; a.x = c.x; a.d = c.d; a.dpad = (c.d + 7) / 8 * 8; a.sigma = 1.0;
-        a.list = ctx->list; a.count = ctx->count_dev;
-        a.rec_lam = ctx->rec_lam; a.rec_rho = ctx->rec_rho; a.rec_t = ctx->rec_t;
-        a.part_vec = ctx->part_vec; a.part_sc = ctx->part_sc; a.ldv_out = P.ldv;
-        a.dyn = gs.dyn;
-        for (int b = 0; b < 2; ++b) { a.U2[b] = gs.U2[b]; a.slot2[b] = gs.slot2[b]; a.V2[b] = gs.V2[b]; a.vcap2[b] = gs.vcap2[b]; }
-        int nvec = 0;
-        RC(meb_launch_active(ctx, MODE_WRITEV, P.prec, a, &nvec));
-    }
-    RC(meb_ctrl_after_update(ctx, dev, S.v, ctx->count_dev));
+    RC(seq_update(q));
     G->k_update = (int)(ctx->launches - l0);
     CU(cudaStreamEndCapture(ctx->stream, &tmp));
     capturing = false;
@@ -246,6 +285,49 @@ fail:
 }
 #undef RC
 #undef CU
+
+// Stepped driver (environment variable MEB_NO_GRAPH=1): the SAME kernels and controller steps, but
+// sequenced by the host, which reads the controller's decision after every evaluation.  It exists so
+// that profilers, which do not see inside conditional graph nodes, can list every launch of a solve.
+int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
+    meb_ctx* ctx = S.ctx;
+    Seq q;
+    seq_init(q, S, P, dense);
+    SolverDev* dev = q.dev;
+    for (;;) {
+        int rc = seq_eval(q);
+        if (rc) return rc;
+        MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
+        MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+        if (h->done) return MEB_OK;
+        if (h->action == ACT_NEWTON) {
+            if (dense) {
+                rc = seq_newton_dense(q);
+                if (rc) return rc;
+            } else {
+                rc = meb_ensure_list(ctx, P.m);
+                if (rc) return rc;
+                int go = h->cg_go;
+                while (go) {
+                    rc = seq_cg_body(q);
+                    if (rc) return rc;
+                    MEB_CUDA_OK(ctx, cudaMemcpyAsync(&h->cg_go, &dev->cg_go, sizeof(int32_t), cudaMemcpyDeviceToHost,
+                                                     ctx->stream));
+                    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+                    go = h->cg_go;
+                }
+            }
+            rc = meb_ctrl_after_newton(ctx, dev, S.v);
+            if (rc) return rc;
+        } else if (h->action == ACT_UPDATE) {
+            rc = seq_update(q);
+            if (rc) return rc;
+            MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
+            MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+            if (h->done) return MEB_OK;
+        }
+    }
+}
 
 GraphKey make_key(const Solver& S, const Problem& P, bool dense) {
     GraphKey k;
@@ -318,10 +400,17 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         if (P.off) { rc = upload(ctx, S.v.off, P.off, S.d); if (rc) return rc; }
     }
     bool first = true;
+    const bool stepped = getenv("MEB_NO_GRAPH") != nullptr;
+    int64_t stepped_launches = 0;
+    (void)stepped_launches;
+    SolveGraph stepped_info;
+    memset(&stepped_info, 0, sizeof(stepped_info));
     for (int attempt = 0; attempt < 64; ++attempt) {
-        SolveGraph* G = nullptr;
-        rc = get_graph(S, P, dense, &G);
-        if (rc) return rc;
+        SolveGraph* G = &stepped_info;
+        if (!stepped) {
+            rc = get_graph(S, P, dense, &G);
+            if (rc) return rc;
+        }
         MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));          // h is free to be rewritten
         if (first) {
             memset(h, 0, sizeof(*h));
@@ -334,7 +423,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
         h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
-        h->in_graph = 1;
+        h->in_graph = stepped ? 0 : 1;
         if (first) {
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
             rc = meb_ctrl_init(ctx, dev, S.v, par.sigma0, P.cur, P.has_mult ? 1 : 0);
@@ -347,14 +436,19 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         if (rc) return rc;
         first = false;
-        MEB_CUDA_OK(ctx, cudaGraphLaunch(G->ex, ctx->stream));
+        if (stepped) {
+            const int64_t l0 = ctx->launches;
+            rc = run_stepped(S, P, dense, h);
+            if (rc) return rc;
+            stepped_info.bytes_per_eval = ctx->last_pass_bytes;
+            stepped_launches += ctx->launches - l0;
+        } else {
+            MEB_CUDA_OK(ctx, cudaGraphLaunch(G->ex, ctx->stream));
+        }
         MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
         MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
         // ---- statistics of this launch ----
         const int cls = !P.full ? MEB_PASS_EVAL_REDUCED : (P.prec == MEB_FP64 ? MEB_PASS_EVAL_FP64 : MEB_PASS_EVAL_FP32);
-        if (h->status != ST_NEED_CAPACITY || true) {
-            // counters are cumulative over relaunches: take them at the end of the phase only
-        }
         if (h->status == ST_NEED_CAPACITY) {
             const int nxt = h->dyn.has_mult ? 1 - h->dyn.cur : 0;
             const int64_t want = h->n_support + h->n_support / 2 + 64;
@@ -374,8 +468,9 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
         S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval;
         S.st->pass_count[cls] += (int32_t)h->pass_count;
-        ctx->launches += (int64_t)h->evals * G->k_eval + (int64_t)h->newton_total * G->k_newton +
-                         (int64_t)h->cg_total * G->k_cg + (int64_t)h->outer * G->k_update;
+        if (!stepped)       // kernels launched by the graph: counted from the device-side iteration counters
+            ctx->launches += (int64_t)h->evals * G->k_eval + (int64_t)h->newton_total * G->k_newton +
+                             (int64_t)h->cg_total * G->k_cg + (int64_t)h->outer * G->k_update;
         S.st->n_support = h->n_support;
         *kkt_out = h->kkt;
         memcpy(terms_out, h->terms, 5 * sizeof(double));
@@ -584,15 +679,13 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                 double* Cred = (double*)ctx->own[OWN_CRED];
                 double* Rred = radii ? (double*)ctx->own[OWN_RRED] : nullptr;
                 // reduced multipliers: dense V (slot k = k) of capacity cap_red rows, double-buffered
+                // (context-owned buffers: stable addresses keep the cached solve graph valid across solves)
                 void* Vred[2] = {nullptr, nullptr};
-                cudaError_t ce = cudaMalloc(&Vred[0], (size_t)cap_red * ldr * sizeof(double));
-                if (ce == cudaSuccess) ce = cudaMalloc(&Vred[1], (size_t)cap_red * ldr * sizeof(double));
-                if (ce != cudaSuccess) {
-                    cudaGetLastError();
-                    if (Vred[0]) cudaFree(Vred[0]);
-                    rc = MEB_E_ALLOC;
-                    break;
-                }
+                rc = own_reserve(ctx, OWN_VRED0, (size_t)cap_red * ldr * sizeof(double));
+                if (rc) break;
+                rc = own_reserve(ctx, OWN_VRED1, (size_t)cap_red * ldr * sizeof(double));
+                if (rc) break;
+                Vred[0] = ctx->own[OWN_VRED0]; Vred[1] = ctx->own[OWN_VRED1];
                 P2.prec = MEB_FP64; P2.d = d; P2.ldv = ldr; P2.off = c0.data(); P2.full = false;
                 P2.C = Cred; P2.ld = ldr; P2.R = Rred;
                 P2.U[0] = ctx->own[OWN_HOSTC]; P2.U[1] = ctx->own[OWN_HOSTR];
@@ -646,9 +739,6 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                     converged = false;
                     ab = xn;
                 }
-                sync_stream(ctx);
-                cudaFree(Vred[0]);
-                cudaFree(Vred[1]);
                 if (rc) break;
             }
         }

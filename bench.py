@@ -10,8 +10,11 @@ exercises every row of SURVEY 8(a)).  Prints ONE JSON line (see the task contrac
 
   value      seconds per solve with the balls already resident in HBM (CUDA events around K solves)
   e2e        the same through meb_solve_host with pinned HOST buffers (H2D inside the timed region)
-  roofline   the dominant streaming kernel of the step: algorithmic bytes / launch duration, from
-             CUDA-event pairs recorded around each of its launches INSIDE the timed solves
+  roofline   the dominant streaming kernel of the step: algorithmic bytes / launch duration measured
+             INSIDE the timed solves (evaluation passes run inside a CUDA-graph WHILE node, where no
+             event can be recorded per iteration: their device time comes from %globaltimer stamps of
+             the kernel's CTAs; ingest / screen / feasibility launches are bracketed by CUDA events),
+             plus `events_check`: the same kernel timed stand-alone with CUDA events
   cpu_baseline  the CPU oracle timed on the host cores on a bounded sample (rank 0, N = 1)
 
 N > 1 (torchrun): the path does not shard in this round ("replicas only"): every rank
@@ -282,6 +285,33 @@ def run_b200(args, rank, world, local_rank):
                 "traffic": ncu_traffic(names[dom], k, args.mode),
                 "algorithmic_bytes_per_launch": tot_by[dom] / tot_n[dom],
                 "share_of_step": tot_ms[dom] / ms, "per_pass": per_pass}
+
+    # ---- cross-check: the dominant evaluation kernel alone, CUDA events around each launch
+    try:
+        import numpy as np
+        reps = 10
+        if args.mode == "mixed":
+            ing = meb.meb_ingest(ctx, dC, dR, 1024, want_shadow=True)
+            Cp, Rp, prec = ing["C32"], ing["R32"], meb.MEB_FP32
+            x0 = torch.zeros(d + 1, dtype=torch.float64, device=device); x0[0] = 0.9 * ing["L"]
+        else:
+            ing = meb.meb_ingest(ctx, dC, dR, 1024)
+            Cp, Rp, prec = dC, dR, meb.MEB_FP64
+            x0 = torch.cat([torch.tensor([0.9 * ing["L"]], dtype=torch.float64, device=device), ing["c0"]])
+        meb.meb_set_pass_timing(ctx, True)
+        tms = []
+        for _ in range(reps + 2):
+            meb.meb_eval_alm(ctx, prec, Cp, Rp, None, None, None, x0, x0, 1.0 / ing["L"], 1.0 / ing["L"] ** 2)
+            tms.append(meb.meb_last_pass_info(ctx))
+        meb.meb_set_pass_timing(ctx, False)
+        tms = tms[2:]
+        ev_ms = sum(t[0] for t in tms) / len(tms)
+        roofline["events_check"] = {"kernel": "eval_alm stand-alone (no multipliers), CUDA events",
+                                    "ms_per_launch": ev_ms, "GBps": tms[0][1] / ev_ms / 1e6,
+                                    "bytes_per_launch": tms[0][1]}
+        del ing, Cp, Rp
+    except Exception as exc:  # the cross-check must never take the bench line down
+        roofline["events_check"] = {"error": repr(exc)}
 
     # ---- end to end: host buffers in, (r, c) out, through meb_solve_host
     e2e = None

@@ -28,6 +28,17 @@ __device__ __forceinline__ bool row_epilogue_core(const StreamArgs& a, int64_t r
     lam_out = 0.0;
     if (!valid) return false;
     if (OP == OP_EVAL) {
+        if (!hasv && ui == T(0)) {
+            // Fast path: a ball without multipliers that lies clearly inside the current ball is in
+            // branch B2 (nb <= -a = r - r_i) and every one of its terms is exactly zero.  The margin
+            // keeps balls near the branch boundary on the exact path below.
+            const T apf = r - ri;
+            if (apf > T(0) && nb2 <= apf * apf * T(0.998)) {
+                if (a.t_out) a.t_out[row] = 0.0;
+                if (a.lam_out) a.lam_out[row] = 0.0;
+                return false;
+            }
+        }
         const T av = ri - r + ui / sig;                    // a_i
         const T nb = t_sqrt<T>(nb2);
         T t, lam;

@@ -76,29 +76,38 @@ struct TileCfg {
 };
 
 // ---- the kernel ------------------------------------------------------------------------------------
+// G  = lanes per row (compile time: chunk offsets become immediates);
 // CH = 16-byte chunks per lane when a whole warp walks ONE row (active rows, shadow): ceil(nch / 32).
-template <typename T, int OP, int CH, bool SHADOW>
-__global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, const TileCfg cfg) {
+template <typename T, int OP, int G, int CH, bool SHADOW>
+__global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const TileCfg cfg) {
     typedef typename Chunk<T>::type V4;
     constexpr int VEC = Chunk<T>::N;
+    constexpr int LG = G == 1 ? 0 : (G == 2 ? 1 : 2);
+    constexpr int RPT = 32 / G;                                          // rows per sub-tile
     extern __shared__ __align__(128) unsigned char smem[];
-    StreamArgs a = a_in;
-    meb_resolve_dyn(a);
+    // device-resident parameters of a solve graph override the launch-time ones (no copy of `a`)
+    double sigma_d = a.sigma;
+    const void* Up = a.U; const int32_t* slotp = a.v_slot; const void* Vp = a.V;
+    if (a.dyn) {
+        const int cur = a.dyn->cur;
+        const bool hm = a.dyn->has_mult != 0;
+        sigma_d = a.dyn->sigma_raw;
+        Up = hm ? a.U2[cur] : nullptr; slotp = hm ? a.slot2[cur] : nullptr; Vp = hm ? a.V2[cur] : nullptr;
+    }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d = a.d;
-    const int64_t m = a.m;
-    const int W = cfg.W, NS = cfg.NS, R = cfg.R, nch = cfg.nch, G = cfg.G, LG = cfg.logG;
-    const int RPT = 32 >> LG;                                            // rows per sub-tile
+    const int m = (int)a.m;                                              // m < 2^31 - 64 (meb.h)
+    const int W = cfg.W, NS = cfg.NS, R = cfg.R, nch = cfg.nch;
     const int g = lane & (G - 1), rl = lane >> LG;
     T* cs = reinterpret_cast<T*>(smem);                                  // centre, padded to whole chunks
     unsigned char* tiles = smem + cfg.off_tiles + (size_t)warp * NS * cfg.stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + cfg.off_bars) + warp * NS;
-    const T* __restrict__ C = static_cast<const T*>(a.C);
-    const T* __restrict__ Vg = static_cast<const T*>(a.V);
-    const T* __restrict__ Ug = static_cast<const T*>(a.U);
+    const unsigned char* __restrict__ Cb = static_cast<const unsigned char*>(a.C);
+    const T* __restrict__ Vg = static_cast<const T*>(Vp);
+    const T* __restrict__ Ug = static_cast<const T*>(Up);
     const T* __restrict__ Rg = static_cast<const T*>(a.R);
     const bool HASU = (OP == OP_EVAL) && Ug != nullptr;
-    const bool HASV = (OP == OP_EVAL) && a.v_slot != nullptr;
+    const bool HASV = (OP == OP_EVAL) && slotp != nullptr;
     const bool HASR = Rg != nullptr;
 
     long long t_start = 0;
@@ -112,7 +121,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
     __syncthreads();
 
     const T r = (OP == OP_INGEST) ? T(0) : (T)a.x[0];
-    const T sig = (T)a.sigma;
+    const T sig = (T)sigma_d;
     const T inv_sig = T(1) / sig;
     Acc acc;
     // whole-warp-per-row view: lane owns chunks lane, lane + 32 (columns (lane + 32 q) * VEC + e)
@@ -130,57 +139,54 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
     }
 
     // stages: st = gw, gw + GW, ...  (consecutive stages go to different SMs)
-    const int64_t rows_per_stage = cfg.stage_rows;
-    const int64_t nstages = (m + rows_per_stage - 1) / rows_per_stage;
-    const int64_t gw = (int64_t)warp * gridDim.x + blockIdx.x;
-    const int64_t GW = (int64_t)gridDim.x * W;
-    const int64_t mine = gw < nstages ? (nstages - gw + GW - 1) / GW : 0;
+    const int rows_per_stage = (int)cfg.stage_rows;
+    const int nstages = (m + rows_per_stage - 1) / rows_per_stage;
+    const int gw = warp * (int)gridDim.x + (int)blockIdx.x;
+    const int GW = (int)gridDim.x * W;
+    const int mine = gw < nstages ? (nstages - gw + GW - 1) / GW : 0;
+    const uint32_t sc_row_bytes = cfg.sc_tma ? ((HASU ? (uint32_t)sizeof(T) : 0u) + (HASR ? (uint32_t)sizeof(T) : 0u) + (HASV ? 4u : 0u)) : 0u;
 
-    auto issue = [&](int64_t k, int s) {                // k-th stage of this warp -> ring slot s
-        const int64_t st = gw + k * GW;
-        const int64_t row0 = st * rows_per_stage;
-        const int64_t nrows = (m - row0) < rows_per_stage ? (m - row0) : rows_per_stage;
-        const uint32_t nb = (uint32_t)(nrows & ~(int64_t)3);             // rows whose scalars come in 16-byte units
+    auto issue = [&](int k, int s) {                    // k-th stage of this warp -> ring slot s
+        const int row0 = (gw + k * GW) * rows_per_stage;
+        const int nrows = (m - row0) < rows_per_stage ? (m - row0) : rows_per_stage;
+        const uint32_t nb = (uint32_t)(nrows & ~3);                      // rows whose scalars come in 16-byte units
         unsigned char* dst = tiles + (size_t)s * cfg.stage_bytes;
-        uint32_t bytes = (uint32_t)nrows * cfg.row_bytes;
-        const bool sc = cfg.sc_tma && nb > 0;
-        if (sc) bytes += (HASU ? nb * (uint32_t)sizeof(T) : 0u) + (HASR ? nb * (uint32_t)sizeof(T) : 0u) + (HASV ? nb * 4u : 0u);
-        mbar_expect_tx(&bars[s], bytes);
-        bulk_g2s(dst, reinterpret_cast<const unsigned char*>(C) + (size_t)row0 * cfg.row_bytes,
-                 (uint32_t)nrows * cfg.row_bytes, &bars[s]);
-        if (sc) {
+        const uint32_t rbytes = (uint32_t)nrows * cfg.row_bytes;
+        mbar_expect_tx(&bars[s], rbytes + nb * sc_row_bytes);
+        bulk_g2s(dst, Cb + (size_t)row0 * cfg.row_bytes, rbytes, &bars[s]);
+        if (sc_row_bytes != 0u && nb > 0u) {
             if (HASU) bulk_g2s(dst + cfg.off_u, Ug + row0, nb * (uint32_t)sizeof(T), &bars[s]);
             if (HASR) bulk_g2s(dst + cfg.off_r, Rg + row0, nb * (uint32_t)sizeof(T), &bars[s]);
-            if (HASV) bulk_g2s(dst + cfg.off_slot, a.v_slot + row0, nb * 4u, &bars[s]);
+            if (HASV) bulk_g2s(dst + cfg.off_slot, slotp + row0, nb * 4u, &bars[s]);
         }
     };
     if (lane == 0)
         for (int k = 0; k < NS && k < mine; ++k) issue(k, k);
 
     const int ldT = (int)(cfg.row_bytes / sizeof(T));
-    const int npl = (nch + G - 1) >> LG;                                 // chunks per lane (G lanes per row)
-    const int start = cfg.rot ? (rl % npl) : 0;
+    const int n_g = (nch - g + G - 1) >> LG;                             // my chunks: g, g + G, ...
+    const int start = cfg.rot ? (rl % n_g) : 0;                          // rotated start (bank conflicts)
     const bool haspad = nch * VEC != d;
 
     int s = 0;
     uint32_t parity = 0;
-    for (int64_t k = 0; k < mine; ++k) {
+    int srow0 = gw * rows_per_stage;
+    const int srow_step = GW * rows_per_stage;
+    for (int k = 0; k < mine; ++k, srow0 += srow_step) {
         mbar_wait(&bars[s], parity);
         unsigned char* sbase = tiles + (size_t)s * cfg.stage_bytes;
         T* stage = reinterpret_cast<T*>(sbase);
         const T* Us = reinterpret_cast<const T*>(sbase + cfg.off_u);
         const T* Rs = reinterpret_cast<const T*>(sbase + cfg.off_r);
         const int32_t* Ss = reinterpret_cast<const int32_t*>(sbase + cfg.off_slot);
-        const int64_t st = gw + k * GW;
-        const int64_t srow0 = st * rows_per_stage;
-        const int64_t snrows = (m - srow0) < rows_per_stage ? (m - srow0) : rows_per_stage;
-        const int nbulk = cfg.sc_tma ? (int)(snrows & ~(int64_t)3) : 0;
+        const int snrows = (m - srow0) < rows_per_stage ? (m - srow0) : rows_per_stage;
+        const int nbulk = cfg.sc_tma ? (snrows & ~3) : 0;
         for (int rr = 0; rr < R; ++rr) {
             const int rs0 = rr * RPT;                                    // first row of the sub-tile in the stage
-            const int64_t row0 = srow0 + rs0;
+            const int row0 = srow0 + rs0;
             if (row0 >= m) break;                                        // warp-uniform
             const int myrs = rs0 + rl;
-            const int64_t myrow = row0 + rl;
+            const int myrow = row0 + rl;
             const bool myvalid = myrow < m;
             T* rowp = stage + (size_t)myrs * ldT;
             // per-row scalars: staged with the rows, or (tail rows / unaligned arrays) read from global memory
@@ -192,7 +198,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
                     if (HASR) ri = Rs[myrs];
                     if (HASU) ui = Us[myrs];
                 } else {
-                    if (HASV) myslot = a.v_slot[myrow];
+                    if (HASV) myslot = slotp[myrow];
                     if (HASR) ri = Rg[myrow];
                     if (HASU) ui = Ug[myrow];
                 }
@@ -206,12 +212,11 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
             if (myvalid) {
                 if (myslot < 0) {
                     T s0 = T(0), s1 = T(0), f0 = T(0);
-                    // my chunks are g, g + G, ... (n_g of them), visited from `start` with wrap-around
                     const V4* rp = reinterpret_cast<const V4*>(rowp) + g;
                     const V4* cp = cs4 + g;
-                    auto chunk = [&](int c) {
-                        const V4 ev4 = rp[c << LG];
-                        const V4 cv4 = cp[c << LG];
+                    auto chunk = [&](const V4* rq, const V4* cq) {
+                        const V4 ev4 = *rq;
+                        const V4 cv4 = *cq;
                         const T* e = reinterpret_cast<const T*>(&ev4);
                         const T* cc = reinterpret_cast<const T*>(&cv4);
 #pragma unroll
@@ -221,14 +226,21 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
                             if (OP == OP_INGEST) f0 = fma(e[j], T(0), f0);   // NaN iff a non-finite entry
                         }
                     };
-                    const int n_g = (nch - g + G - 1) >> LG;
-                    int c = start < n_g ? start : 0;
-                    const int c_first = c;
-                    for (; c + 4 <= n_g; c += 4) { chunk(c); chunk(c + 1); chunk(c + 2); chunk(c + 3); }
-                    for (; c < n_g; ++c) chunk(c);
-                    c = 0;
-                    for (; c + 4 <= c_first; c += 4) { chunk(c); chunk(c + 1); chunk(c + 2); chunk(c + 3); }
-                    for (; c < c_first; ++c) chunk(c);
+                    if (!cfg.rot) {                                      // my chunks g, g + G, ... in order
+                        const V4* rq = rp;
+                        const V4* cq = cp;
+                        int c = 0;
+                        for (; c + 4 <= n_g; c += 4, rq += 4 * G, cq += 4 * G) {
+                            chunk(rq, cq); chunk(rq + G, cq + G); chunk(rq + 2 * G, cq + 2 * G); chunk(rq + 3 * G, cq + 3 * G);
+                        }
+                        for (; c < n_g; ++c, rq += G, cq += G) chunk(rq, cq);
+                    } else {                                             // same trip count, start rotated by the row index
+                        int ci = start;
+                        for (int c = 0; c < n_g; ++c) {
+                            chunk(rp + ci * G, cp + ci * G);
+                            ci = (ci + 1 == n_g) ? 0 : ci + 1;
+                        }
+                    }
                     nb2 = s0 + s1;
                     if (OP == OP_INGEST) ne2 = f0;
                 } else {                                                 // row with a multiplier v_i
@@ -250,6 +262,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
                     }
                 }
             }
+#pragma unroll
             for (int o = G >> 1; o > 0; o >>= 1) {                       // combine the G lanes of a row
                 nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, o);
                 if (HASV || OP == OP_INGEST) ne2 += __shfl_xor_sync(MEB_FULL_MASK, ne2, o);
@@ -263,12 +276,13 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
                                                        r, sig, ri, ui, acc, mylam);
             if (OP != OP_INGEST) {
                 uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);      // bit of lane rl*G <-> row rl
-                {   // RPT-bit piece of the 32-row mask word: lane q < RPT takes the flag of row q
+                if (G == 1) {
+                    if (lane == 0) a.mask[row0 >> 5] = bits;
+                } else {   // RPT-bit piece of the 32-row mask word: lane q < RPT takes the flag of row q
                     const bool f2 = __shfl_sync(MEB_FULL_MASK, (int)flag, (lane << LG) & 31) != 0 && lane < RPT;
                     const uint32_t piece = __ballot_sync(MEB_FULL_MASK, f2);
                     if (lane == 0) {
-                        if (G == 1) a.mask[row0 >> 5] = piece;
-                        else if (G == 2) reinterpret_cast<uint16_t*>(a.mask)[row0 >> 4] = (uint16_t)piece;
+                        if (G == 2) reinterpret_cast<uint16_t*>(a.mask)[row0 >> 4] = (uint16_t)piece;
                         else reinterpret_cast<uint8_t*>(a.mask)[row0 >> 3] = (uint8_t)piece;
                     }
                 }
@@ -303,11 +317,11 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a_in, con
                 }
             }
             if (SHADOW) {                       // FP32 shadow of the centred rows (reading 8)
-                const int nr = (m - row0) < RPT ? (int)(m - row0) : RPT;
+                const int nr = (m - row0) < RPT ? (m - row0) : RPT;
 #pragma unroll 4
                 for (int rs = 0; rs < nr; ++rs) {
                     const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
-                    float* srow = a.C32 + (row0 + rs) * a.ld32;
+                    float* srow = a.C32 + (int64_t)(row0 + rs) * a.ld32;
 #pragma unroll
                     for (int q = 0; q < CH; ++q) {
                         const int ch = lane + 32 * q;
@@ -373,16 +387,37 @@ constexpr size_t TILE_SMEM_BUDGET = 212 * 1024;     // of the 227 KB a CTA may u
 
 bool aligned16(const void* p) { return ((uintptr_t)p % 16) == 0; }
 
+int lanes_per_row(const StreamArgs& a, size_t esize);
+
 bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out) {
     TileCfg c;
     memset(&c, 0, sizeof(c));
     c.row_bytes = (uint32_t)(a.ld * (int64_t)esize);
     c.nch = (int)(((size_t)a.d * esize + 15) / 16);
-    c.G = c.row_bytes <= 208 ? 1 : (c.row_bytes <= 416 ? 2 : 4);     // sub-tile of at most ~6.5 KB
+    c.G = lanes_per_row(a, esize);
     c.logG = c.G == 1 ? 0 : (c.G == 2 ? 1 : 2);
     const int rpt = 32 / c.G;
     const int slots = (int)(c.row_bytes / 16);
-    c.rot = (slots % c.G == 0 && ((slots / c.G) % 2 == 0)) ? 1 : 0;
+    {   // bank conflicts of the quarter-warp LDS.128 (8 lanes, 8 slots of 16 bytes per wavefront): lane
+        // (rl, g) reads slot S rl + g + G ((c + rot rl) mod n_g); pick the rotation with fewer collisions
+        int best = 1 << 30;
+        for (int rot = 0; rot < 2; ++rot) {
+            int coll = 0;
+            for (int q = 0; q < 4; ++q) {                     // the four quarter-warps
+                int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+                for (int l = 8 * q; l < 8 * q + 8; ++l) {
+                    const int g = l % c.G, rl = l / c.G;
+                    const int n_g = (c.nch - g + c.G - 1) / c.G;
+                    const int ci = rot && n_g > 0 ? rl % n_g : 0;
+                    cnt[(slots * rl + g + c.G * ci) & 7]++;
+                }
+                for (int b = 0; b < 8; ++b) if (cnt[b] > 1) coll += cnt[b] - 1;
+            }
+            // rotation costs instructions: use it only against severe (>= 4-way on average) conflicts
+            if (rot == 0) { best = coll; c.rot = 0; }
+            else if (best >= 24 && coll < best) { best = coll; c.rot = 1; }
+        }
+    }
     // stage of about 12 KB of rows, but never so large that a small problem lands on a handful of warps
     int R = (int)(6656 / ((size_t)rpt * c.row_bytes));
     if (R < 1) R = 1;
@@ -436,12 +471,21 @@ int launch_cfg(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, size_t esize, 
     return MEB_OK;
 }
 
+int lanes_per_row(const StreamArgs& a, size_t esize) {
+    const size_t rb = (size_t)a.ld * esize;
+    return rb <= 208 ? 1 : (rb <= 416 ? 2 : 4);              // sub-tile of at most ~6.5 KB
+}
+
+// G is fixed by the row length; CH = 2 only occurs with G = 4 (rows longer than 512 bytes)
 template <typename T, int OP, bool SHADOW>
-int launch_cpl(meb_ctx* ctx, const StreamArgs& a, int* grid_out) {
+int launch_g(meb_ctx* ctx, const StreamArgs& a, bool want_ch, int* grid_out) {
     const int nch = (int)(((size_t)a.d * sizeof(T) + 15) / 16);        // <= 64 (rows of at most 1024 bytes)
     constexpr int VEC = 16 / sizeof(T);
-    if (nch <= 32) return launch_cfg(ctx, tile_kernel<T, OP, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
-    return launch_cfg(ctx, tile_kernel<T, OP, 2, SHADOW>, a, sizeof(T), 2 * VEC, grid_out);
+    const int G = lanes_per_row(a, sizeof(T));
+    if (G == 1) return launch_cfg(ctx, tile_kernel<T, OP, 1, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
+    if (G == 2) return launch_cfg(ctx, tile_kernel<T, OP, 2, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
+    if (!want_ch || nch <= 32) return launch_cfg(ctx, tile_kernel<T, OP, 4, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
+    return launch_cfg(ctx, tile_kernel<T, OP, 4, 2, SHADOW>, a, sizeof(T), 2 * VEC, grid_out);
 }
 
 }  // namespace
@@ -458,17 +502,17 @@ bool meb_tile_applicable(int op, int prec, const StreamArgs& a) {
 int meb_launch_tile(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out) {
     if (prec == MEB_FP64) {
         switch (op) {
-            case OP_EVAL: return launch_cpl<double, OP_EVAL, false>(ctx, a, grid_out);
-            case OP_FEAS: return launch_cfg(ctx, tile_kernel<double, OP_FEAS, 1, false>, a, 8, 1, grid_out);
+            case OP_EVAL: return launch_g<double, OP_EVAL, false>(ctx, a, true, grid_out);
+            case OP_FEAS: return launch_g<double, OP_FEAS, false>(ctx, a, false, grid_out);
             case OP_INGEST:
-                if (a.C32) return launch_cpl<double, OP_INGEST, true>(ctx, a, grid_out);
-                return launch_cfg(ctx, tile_kernel<double, OP_INGEST, 1, false>, a, 8, 1, grid_out);
+                if (a.C32) return launch_g<double, OP_INGEST, true>(ctx, a, true, grid_out);
+                return launch_g<double, OP_INGEST, false>(ctx, a, false, grid_out);
             default: return MEB_E_ARG;
         }
     }
     switch (op) {
-        case OP_EVAL: return launch_cpl<float, OP_EVAL, false>(ctx, a, grid_out);
-        case OP_SCREEN: return launch_cfg(ctx, tile_kernel<float, OP_SCREEN, 1, false>, a, 4, 1, grid_out);
+        case OP_EVAL: return launch_g<float, OP_EVAL, false>(ctx, a, true, grid_out);
+        case OP_SCREEN: return launch_g<float, OP_SCREEN, false>(ctx, a, false, grid_out);
         default: return MEB_E_ARG;
     }
 }

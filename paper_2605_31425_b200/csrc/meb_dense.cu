@@ -149,6 +149,17 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
 // publish it to shared memory (where it stays as row k+1 of L D for the backward substitution)
 // together with 1/d_{k+1}, computed by the diagonal's owner while the others are still updating.
 // One __syncthreads per column.
+// 1/d for d > 0 in full precision: hardware seed (about 20 bits) + two Newton steps, 4 dependent FMAs
+// (the IEEE division subroutine is several times longer and sits on the critical path of every column)
+__device__ __forceinline__ double fast_rcp(double d) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    return fma(r, e, r);
+}
+
 template <int BS>
 __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
                                                          int n, double scale, double* __restrict__ delta,
@@ -164,24 +175,23 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
     for (int ii = 0; ii < BS; ++ii)
 #pragma unroll
         for (int jj = 0; jj < BS; ++jj) {
+            // unconditional loads from clamped addresses (all in flight at once), selected afterwards
             const int i = ty + 16 * ii, j = tx + 16 * jj;
             double v = 0.0;
-            if (jj <= ii && j < n && j <= i) {
-                if (i < n) v = scale * H[(size_t)i * n + j];
-                else if (i == n) v = -g[j];
+            if (jj <= ii) {
+                const int ic = i < n ? i : n - 1, jc = j < n ? j : n - 1;
+                const double hv = H[(size_t)ic * n + jc];
+                const double gv = g[jc];
+                const bool live = j < n && j <= i;
+                v = (live && i < n) ? scale * hv : ((live && i == n) ? -gv : 0.0);
             }
             a[ii][jj] = v;
         }
     __shared__ int bad;
     if (tid == 0) bad = 0;
-    if (tx == 0) {                                        // publish column 0 and 1/d_0
+    if (tx == 0) {                                        // publish column 0
 #pragma unroll
         for (int ii = 0; ii < BS; ++ii) Lm[ty + 16 * ii] = a[ii][0];
-        if (ty == 0) {
-            double dk = a[0][0];
-            if (!(dk > 0.0)) { bad = 1; dk = 1.0; }
-            invd[0] = 1.0 / dk;
-        }
     }
     __syncthreads();
 #pragma unroll
@@ -192,37 +202,35 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
                 const int k = 16 * KB + kk;
                 if (k >= n) break;                        // uniform
                 const double* col = Lm + (size_t)k * ldl;
-                const double inv = invd[k];
+                double dk = col[k];
+                if (!(dk > 0.0)) { if (tid == 0) bad = k + 1; dk = 1.0; }
+                const double ninv = -fast_rcp(dk);        // every thread forms 1/d_k itself (no serial owner)
+                if (tid == 0) invd[k] = -ninv;
+                // multipliers; only block KB holds rows / columns <= k, which are masked to zero
                 double lik[BS], cj[BS];
 #pragma unroll
                 for (int q = KB; q < BS; ++q) {
-                    const double ci = col[ty + 16 * q], cc = col[tx + 16 * q];
-                    lik[q] = (ty + 16 * q > k) ? ci * inv : 0.0;
-                    cj[q] = (tx + 16 * q > k) ? cc : 0.0;
+                    double c1 = col[ty + 16 * q], c2 = col[tx + 16 * q];
+                    if (q == KB) {
+                        c1 = (ty + 16 * KB > k) ? c1 : 0.0;
+                        c2 = (tx + 16 * KB > k) ? c2 : 0.0;
+                    }
+                    lik[q] = c1 * ninv;
+                    cj[q] = c2;
                 }
 #pragma unroll
                 for (int ii = KB; ii < BS; ++ii)
 #pragma unroll
-                    for (int jj = KB; jj <= ii; ++jj) a[ii][jj] = fma(-lik[ii], cj[jj], a[ii][jj]);
+                    for (int jj = KB; jj <= ii; ++jj) a[ii][jj] = fma(lik[ii], cj[jj], a[ii][jj]);
                 const int k1 = k + 1;
                 if (k1 < n && tx == (k1 & 15)) {          // owners of column k+1 publish it
                     double* cn = Lm + (size_t)k1 * ldl;
                     if (kk < 15) {
 #pragma unroll
                         for (int ii = KB; ii < BS; ++ii) cn[ty + 16 * ii] = a[ii][KB];
-                        if (ty == tx) {
-                            double dk = a[KB][KB];
-                            if (!(dk > 0.0)) { bad = k1 + 1; dk = 1.0; }
-                            invd[k1] = 1.0 / dk;
-                        }
                     } else if (KB + 1 < BS) {
 #pragma unroll
                         for (int ii = KB + 1; ii < BS; ++ii) cn[ty + 16 * ii] = a[ii][KB + 1 < BS ? KB + 1 : KB];
-                        if (ty == tx) {
-                            double dk = a[KB + 1 < BS ? KB + 1 : KB][KB + 1 < BS ? KB + 1 : KB];
-                            if (!(dk > 0.0)) { bad = k1 + 1; dk = 1.0; }
-                            invd[k1] = 1.0 / dk;
-                        }
                     }
                 }
                 __syncthreads();
@@ -230,14 +238,37 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
         }
     }
     // row n of L D is spread over the columns' shared rows: z_k = Lm[k][n] / d_k; then L^T x = z,
-    // column-oriented, one warp: L_kj = Lm[j][k] * invd[j]
+    // column-oriented by one warp with z in REGISTERS (lane L holds z[L + 32 q]): per step one shuffle
+    // broadcasts x_k and every lane updates its entries j < k with L_kj = Lm[j][k] * invd[j].
     if (tid < 32) {
-        for (int j = tid; j < n; j += 32) z[j] = Lm[(size_t)j * ldl + n] * invd[j];
-        __syncwarp();
+        constexpr int ZQ = (NP + 31) / 32;
+        double zr[ZQ], dj[ZQ];
+#pragma unroll
+        for (int q = 0; q < ZQ; ++q) {
+            const int j = tid + 32 * q;
+            dj[q] = j < n ? invd[j] : 0.0;
+            zr[q] = j < n ? Lm[(size_t)j * ldl + n] * dj[q] : 0.0;
+        }
         for (int k = n - 1; k > 0; --k) {
-            const double xk = z[k];
-            for (int j = tid; j < k; j += 32) z[j] = fma(-Lm[(size_t)j * ldl + k] * invd[j], xk, z[j]);
-            __syncwarp();
+            double lv[ZQ];
+#pragma unroll
+            for (int q = 0; q < ZQ; ++q) {
+                const int j = tid + 32 * q;
+                lv[q] = j < k ? Lm[(size_t)j * ldl + k] * dj[q] : 0.0;     // independent of the x chain
+            }
+            double xk = 0.0;
+#pragma unroll
+            for (int q = 0; q < ZQ; ++q) {
+                const double t = __shfl_sync(MEB_FULL_MASK, zr[q], k & 31);
+                if (q == (k >> 5)) xk = t;
+            }
+#pragma unroll
+            for (int q = 0; q < ZQ; ++q) zr[q] = fma(-lv[q], xk, zr[q]);
+        }
+#pragma unroll
+        for (int q = 0; q < ZQ; ++q) {
+            const int j = tid + 32 * q;
+            if (j < n) z[j] = zr[q];
         }
     }
     __syncthreads();

@@ -84,7 +84,7 @@ typedef struct meb_params {
     int32_t outer_max;          /*                                                         200  */
     int32_t max_rounds;         /* active-set refinement rounds               10   */
     int32_t sample_rows;        /* rows whose mean is the initial centre c^0               1024 */
-    int32_t reserved;
+    int32_t outer_max_lo;       /* outer iterations of the low-precision run (reading 17)     30   */
 } meb_params;
 
 /* Counters and residuals of one meb_solve (host struct). */

@@ -113,6 +113,51 @@ __global__ void __launch_bounds__(CBLOCK) compact_write_kernel(const uint32_t* _
     }
 }
 
+// Small problems (up to a few million balls): ONE CTA of 1024 threads scans the whole mask in rounds of
+// 1024 words (ballot-free integer scan: per-word popcounts, warp shuffles, warp totals in shared memory)
+// and writes the indices at their final position -- one launch instead of two, no segment sums.
+__global__ void __launch_bounds__(1024) compact_single_kernel(const uint32_t* __restrict__ mask, int64_t nwords,
+                                                              int64_t m, int32_t* __restrict__ list, int64_t cap,
+                                                              int32_t* __restrict__ count) {
+    __shared__ int wtot[32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    long long base = 0;
+    for (int64_t w0 = 0; w0 < nwords; w0 += 1024) {
+        const int64_t w = w0 + threadIdx.x;
+        uint32_t bits = 0;
+        if (w < nwords) {
+            bits = mask[w];
+            if ((w + 1) * 32 > m) bits &= (m - w * 32 >= 32) ? 0xffffffffu : ((1u << (m - w * 32)) - 1u);
+        }
+        const int c = __popc(bits);
+        int incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(MEB_FULL_MASK, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
+        int wpre = 0, rtot = 0;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            const int v = wtot[k];
+            if (k < warp) wpre += v;
+            rtot += v;
+        }
+        long long pos = base + wpre + (incl - c);
+        while (bits) {
+            const int b = __ffs(bits) - 1;
+            bits &= bits - 1;
+            if (pos < cap) list[pos] = (int32_t)(w * 32 + b);
+            ++pos;
+        }
+        base += rtot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *count = (int32_t)base;
+}
+
 // uint8 flags -> bit mask (the "flags given" input mode of meb_screen_compact)
 __global__ void __launch_bounds__(256) flags_to_mask_kernel(const uint8_t* __restrict__ flags, int64_t m,
                                                            uint32_t* __restrict__ mask) {
@@ -130,6 +175,11 @@ __global__ void __launch_bounds__(256) flags_to_mask_kernel(const uint8_t* __res
 int meb_launch_compact_cap(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* list, int64_t cap,
                            int32_t* count_dev) {
     const int64_t nwords = (m + 31) / 32;
+    if (nwords <= 64 * 1024) {                     // up to 2M balls: one CTA, one launch
+        ctx->launches++; compact_single_kernel<<<1, 1024, 0, ctx->stream>>>(mask, nwords, m, list, cap, count_dev);
+        MEB_CUDA_OK(ctx, cudaGetLastError());
+        return MEB_OK;
+    }
     const int nseg = (int)((nwords + SEG_WORDS - 1) / SEG_WORDS);
     ctx->launches++; compact_count_kernel<<<nseg, CBLOCK, 0, ctx->stream>>>(mask, nwords, m, ctx->blocksum);
     ctx->launches++; compact_write_kernel<<<nseg, CBLOCK, 0, ctx->stream>>>(mask, nwords, m, ctx->blocksum, nseg, list, cap,

@@ -112,19 +112,23 @@ __device__ __forceinline__ double ctrl_rel_kkt(const double* ev, double r_raw, d
 // x_raw have been written: Armijo test (reading 4), stopping tests (5) and KKT (P:L133-135,
 // L244, reading 6), choice of the next action.  All threads of the CTA call it.
 // S is a SHARED-MEMORY copy of the state (loaded by the caller); it is written back to Sg at the end.
-__device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, double* sm);
-__device__ inline void ctrl_after_eval(SolverDev* Sg, SolverDev* S, const SolverVecs v, double* sm) {
-    ctrl_after_eval_body(S, v, sm);
+// ev_s: the scalars of this evaluation in shared memory (the caller also wrote them to v.ev_t).
+__device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, const double* ev_s, double* sm);
+__device__ inline void ctrl_after_eval(SolverDev* Sg, SolverDev* S, const SolverVecs v, const double* ev_s,
+                                       double* sm) {
+    ctrl_after_eval_body(S, v, ev_s, sm);
     __syncthreads();
     const unsigned long long* src = reinterpret_cast<const unsigned long long*>(S);
     unsigned long long* dst = reinterpret_cast<unsigned long long*>(Sg);
     for (int q = threadIdx.x; q < (int)(sizeof(SolverDev) / 8); q += blockDim.x) dst[q] = src[q];
 }
-__device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, double* sm) {
+__device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, const double* ev_s, double* sm) {
     __syncthreads();
     const int n = S->n;
     const int phase = S->phase;
-    const double psi_t = v.ev_t[MEB_EV_PSI] / S->L;
+    const double Ls = S->L;
+    const bool use_off = S->use_off != 0;
+    const double psi_t = ev_s[MEB_EV_PSI] / Ls;
     bool accept = true, stalled = false;
     if (phase == PH_ARMIJO) {
         if (!(psi_t <= S->psi_cur + S->armijo_mu * S->eta * S->slope)) {
@@ -136,56 +140,52 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, do
             }
         }
     }
-    __syncthreads();
     if (!accept) {
-        if (stalled) {                                 // records of this pass are not those of x: re-evaluate
-            ctrl_to_raw(S, v, v.xn, v.x_raw);
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                S->phase = PH_REEVAL; S->action = ACT_TRIAL; S->evals++;
-                if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
-                ctrl_set_handles(S);
-            }
-        } else {                                       // halve the step
-            const double eta = 0.5 * S->eta;
-            for (int j = threadIdx.x; j < n; j += blockDim.x) v.xt[j] = v.xn[j] + eta * v.delta[j];
-            __syncthreads();
-            ctrl_to_raw(S, v, v.xt, v.x_raw);
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                S->eta = eta; S->ls++; S->action = ACT_TRIAL; S->evals++;
-                if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
-                ctrl_set_handles(S);
-            }
+        // rejected trial: either halve the step (next trial x + eta Delta) or, when the halvings are
+        // exhausted, re-evaluate at x (the records of this pass are not those of x)
+        const double eta = stalled ? 0.0 : 0.5 * S->eta;
+        for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            const double xj = v.xn[j] + eta * v.delta[j];
+            v.xt[j] = xj;
+            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            if (stalled) { S->phase = PH_REEVAL; } else { S->eta = eta; S->ls++; }
+            S->action = ACT_TRIAL; S->evals++;
+            if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
+            ctrl_set_handles(S);
         }
         return;
     }
-    // ---- accepted: the pass becomes the evaluation at x ----
-    if (phase == PH_ARMIJO)
-        for (int j = threadIdx.x; j < n; j += blockDim.x) v.xn[j] = v.xt[j];
-    for (int j = threadIdx.x; j < n; j += blockDim.x) v.g[j] = v.grad_t[j];
-    if (threadIdx.x < MEB_EVAL_NSCALARS) v.ev[threadIdx.x] = v.ev_t[threadIdx.x];
-    __syncthreads();
-    // condition (5): 2 sigma |<(alpha,beta) - x, g>| + sigma^2 ||g||^2 <= rho (sum ||dmult||^2 + tau ||x - xbar||^2)
+    // ---- accepted: the pass becomes the evaluation at x; condition (5) in the same sweep:
+    //      2 sigma |<(alpha,beta) - x, g>| + sigma^2 ||g||^2 <= rho (sum ||dmult||^2 + tau ||x - xbar||^2)
     double agx = 0.0, gg = 0.0, dx2 = 0.0;
+    const bool take_xt = phase == PH_ARMIJO;
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
-        const double gj = v.g[j], xj = v.xn[j];
-        agx = fma(v.ab[j] - xj, gj, agx);
+        const double xj = take_xt ? v.xt[j] : v.xn[j];
+        const double gj = v.grad_t[j];
+        const double abj = v.ab[j], xbj = v.xbar[j];
+        if (take_xt) v.xn[j] = xj;
+        v.g[j] = gj;
+        agx = fma(abj - xj, gj, agx);
         gg = fma(gj, gj, gg);
-        const double dx = xj - v.xbar[j];
+        const double dx = xj - xbj;
         dx2 = fma(dx, dx, dx2);
+        if (j == 0) sm[96] = xj;                       // r~ for the KKT normalisation
     }
+    if (threadIdx.x < MEB_EVAL_NSCALARS) v.ev[threadIdx.x] = ev_s[threadIdx.x];
     ctrl_block_sum3(agx, gg, dx2, sm);
     if (threadIdx.x == 0) {
         S->evals++;
         S->psi_cur = psi_t;
         double terms[5];
-        const double kkt = ctrl_rel_kkt(v.ev, S->L * v.xn[0], terms);
+        const double kkt = ctrl_rel_kkt(ev_s, Ls * sm[96], terms);
         S->kkt = kkt;
         for (int i = 0; i < 5; ++i) S->terms[i] = terms[i];
         const double sg = S->sigma;
         const double lhs = 2.0 * sg * fabs(agx) + sg * sg * gg;
-        const double rhs = S->rho * (v.ev[MEB_EV_SUM_DMULT2] + S->tau * dx2);
+        const double rhs = S->rho * (ev_s[MEB_EV_SUM_DMULT2] + S->tau * dx2);
         const bool exit_inner = (phase == PH_REEVAL) || stalled || lhs <= rhs || kkt <= S->tol ||
                                 S->inner >= S->inner_max;
         if (exit_inner) {
@@ -207,8 +207,9 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, do
     __syncthreads();
     if (S->action == ACT_NEWTON && !S->dense)
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            const double gj = v.grad_t[j];
             v.delta[j] = 0.0;
-            v.res[j] = -v.g[j];
-            v.p[j] = -v.g[j];
+            v.res[j] = -gj;
+            v.p[j] = -gj;
         }
 }

@@ -25,7 +25,8 @@ __device__ __forceinline__ double partial_max(const double* part, int grid, int 
 // then added in order, so the order does not depend on timing).  With f.S != nullptr the same CTA then
 // runs the controller step of the device-resident solver (meb_ctrl.cuh).
 __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArgs f) {
-    __shared__ double sm[96];
+    __shared__ double sm[104];
+    __shared__ double ev_s[MEB_EVAL_NSCALARS];
     __shared__ double sc[MEB_NPART];
     __shared__ double seg[FBLOCK];
     __shared__ __align__(16) SolverDev sS;             // working copy of the solver state (controller step)
@@ -34,8 +35,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
         const unsigned long long* src = reinterpret_cast<const unsigned long long*>(f.S);
         unsigned long long* dst = reinterpret_cast<unsigned long long*>(&sS);
         for (int q = threadIdx.x; q < (int)(sizeof(SolverDev) / 8); q += FBLOCK) dst[q] = src[q];
-        __syncthreads();
-    }
+    }                                                   // (visible after the first __syncthreads below)
     const double* __restrict__ part = f.part;
     const double* __restrict__ part_vec = f.part_vec;
     const int grid = f.grid, d = f.d, dpad = f.dpad;
@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
             t0 = min(t0, __shfl_xor_sync(MEB_FULL_MASK, t0, o));
             t1 = max(t1, __shfl_xor_sync(MEB_FULL_MASK, t1, o));
         }
-        if (lane == 0 && t1 > t0) { sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++; }
+        if (lane == 0) { sm[100] = __longlong_as_double(t0); sm[101] = __longlong_as_double(t1); }
     }
     // vector part: sum_i v+_i = sigma * sum_k lam_k b_k
     int nvec = f.nvec;
@@ -103,7 +103,11 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
     { double dummy = 0.0; ctrl_block_sum3(nv2, dx2, dummy, sm); }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double* out = f.out;
+        if (f.S) {
+            const long long t0 = __double_as_longlong(sm[100]), t1 = __double_as_longlong(sm[101]);
+            if (t1 > t0) { sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++; }
+        }
+        double* out = ev_s;
         const double dx0 = x[0] - (xbar ? xbar[0] : x[0]);
         dx2 += dx0 * dx0;
         f.grad[0] = 1.0 - sc[1] + tos * dx0;
@@ -122,7 +126,9 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
         out[12] = dx2;
         out[13] = 0.0; out[14] = 0.0; out[15] = 0.0;
     }
-    if (f.S) ctrl_after_eval(f.S, &sS, f.v, sm);
+    __syncthreads();
+    if (threadIdx.x < MEB_EVAL_NSCALARS) f.out[threadIdx.x] = ev_s[threadIdx.x];
+    if (f.S) ctrl_after_eval(f.S, &sS, f.v, ev_s, sm);
 }
 
 // H q from the active-list partials (reading 1):

@@ -378,7 +378,7 @@ int grow_pool(meb_ctx* ctx, Problem& P, int b, int64_t rows) {
 // Algorithm 1 with Algorithm 2 inside, device-resident: one graph launch per phase (plus one relaunch
 // whenever a V pool has to grow).  xn / ab are the normalised x and (alpha, beta), in/out (host).
 int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& ab, double tol, bool* converged,
-           double* kkt_out, double terms_out[5]) {
+           double* kkt_out, double terms_out[5], int outer_cap) {
     meb_ctx* ctx = S.ctx;
     const meb_params& par = S.par;
     const int n = S.d + 1;
@@ -416,10 +416,10 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             memset(h, 0, sizeof(*h));
             h->L = S.L; h->tol = tol; h->rho = par.rho; h->tau = par.tau; h->kappa = par.kappa;
             h->sigma_max = par.sigma_max; h->armijo_mu = par.armijo_mu;
-            h->n = n; h->d = S.d; h->inner_max = par.inner_max; h->outer_max = par.outer_max;
+            h->n = n; h->d = S.d; h->inner_max = par.inner_max; h->outer_max = outer_cap;
             h->armijo_max = par.armijo_max_halvings; h->cg_max = par.cg_max; h->dense = dense ? 1 : 0;
             h->use_off = P.off ? 1 : 0;
-            h->eval_cap = 4 * par.outer_max * (par.inner_max + 2);
+            h->eval_cap = 4 * outer_cap * (par.inner_max + 2);
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
         h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
@@ -601,7 +601,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             rc = setup_multipliers(ctx, P, OWN_U0, OWN_S0, OWN_V0);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
-            rc = ripalm(S, P, xn, ab, tol_kkt, &converged, &kkt, terms);
+            rc = ripalm(S, P, xn, ab, tol_kkt, &converged, &kkt, terms, S.par.outer_max);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
             // final full pass: r_out = max_i(||c - c_i|| + r_i)   (step 7)
@@ -627,7 +627,8 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             if (rc) break;
             bool conv1 = false;
             double kkt1, terms1[5];
-            rc = ripalm(S, P1, xn, ab, S.par.tol_lo, &conv1, &kkt1, terms1);
+            rc = ripalm(S, P1, xn, ab, S.par.tol_lo, &conv1, &kkt1, terms1,
+                        S.par.outer_max_lo > 0 ? S.par.outer_max_lo : S.par.outer_max);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
             // ---- screening, tol_red = 0.02 r_hat (reading 9) ----
@@ -693,18 +694,19 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                 P2.V[0] = Vred[0]; P2.V[1] = Vred[1]; P2.vcap[0] = P2.vcap[1] = cap_red;
                 P2.own_v[0] = P2.own_v[1] = -1;
                 P2.cur = 0; P2.has_mult = true;
-                // warm start restricted to I_red
-                rc = meb_gather_mult(ctx, P1.has_mult ? (const float*)P1.U[P1.cur] : nullptr,
-                                     P1.has_mult ? P1.slot[P1.cur] : nullptr,
-                                     P1.has_mult ? (const float*)P1.V[P1.cur] : nullptr, P1.ldv, idx, nred, d,
-                                     (double*)P2.U[0], P2.slot[0], (double*)P2.V[0], ldr);
-                if (!P1.has_mult) P2.has_mult = false;
+                // warm start restricted to I_red.  If the low-precision run did not reach its
+                // tolerance (degenerate supports: reading 17) its multipliers are noise: start from zero.
+                if (P1.has_mult && conv1)
+                    rc = meb_gather_mult(ctx, (const float*)P1.U[P1.cur], P1.slot[P1.cur], (const float*)P1.V[P1.cur],
+                                         P1.ldv, idx, nred, d, (double*)P2.U[0], P2.slot[0], (double*)P2.V[0], ldr);
+                else
+                    P2.has_mult = false;
                 ab = xn;                                        // reading 11
                 for (int rnd = 0; rc == MEB_OK && rnd < S.par.max_rounds; ++rnd) {
                     P2.m = nred;
                     st->n_reduced = nred;
                     st->rounds = rnd + 1;
-                    rc = ripalm(S, P2, xn, ab, tol_kkt, &converged, &kkt, terms);
+                    rc = ripalm(S, P2, xn, ab, tol_kkt, &converged, &kkt, terms, S.par.outer_max);
                     if (rc) break;
                     if (rnd == 0) MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
                     // a-posteriori check against ALL original constraints

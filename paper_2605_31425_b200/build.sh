@@ -9,7 +9,9 @@ mkdir -p build
 pids=()
 for f in csrc/*.cu; do
   o=build/$(basename "${f%.cu}").o
-  if [ ! -f "$o" ] || [ "$f" -nt "$o" ] || [ csrc/meb_internal.cuh -nt "$o" ] || [ ../include/meb.h -nt "$o" ]; then
+  stale=0
+  for h in csrc/*.cuh ../include/meb.h; do [ "$h" -nt "$o" ] && stale=1; done
+  if [ ! -f "$o" ] || [ "$f" -nt "$o" ] || [ $stale = 1 ]; then
     $NVCC $FLAGS -c "$f" -o "$o" &
     pids+=($!)
   fi

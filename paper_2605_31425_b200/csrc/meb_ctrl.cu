@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(CBLK) ctrl_init_kernel(SolverDev* S, const Sol
         S->phase = PH_FIRST; S->action = ACT_TRIAL;
         S->outer = 0; S->inner = 0; S->ls = 0; S->done = 0; S->status = ST_RUNNING; S->stalled = 0;
         S->newton_total = 0; S->cg_total = 0; S->evals = 0; S->chol_info = 0;
-        S->kkt = 1e300; S->n_support = 0;
+        S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0;
         S->pass_ns = 0ull; S->pass_count = 0;
         S->eta = 1.0; S->psi_cur = 0.0; S->slope = 0.0;
         S->cg_go = 0; S->cg_it = 0;
@@ -107,22 +107,46 @@ __global__ void __launch_bounds__(CBLK) ctrl_after_update_kernel(SolverDev* S, c
         }
         return;
     }
+    // ---- decisions (every thread computes the same from the state as it was on entry) ----
     const double sg = S->sigma;
-    for (int j = threadIdx.x; j < n; j += blockDim.x) {
-        v.ab[j] -= sg * v.g[j];                     // P:L149
-        v.xbar[j] = v.xn[j];
-    }
-    ctrl_to_raw(S, v, v.xn, v.x_raw);
+    const double kkt = S->kkt;
+    const int outer1 = S->outer + 1;
+    const bool improved = kkt < S->best_kkt;                     // best iterate so far (returned if the run stalls)
+    const int stall = (kkt < 0.5 * S->best_kkt) ? 0 : S->stall_count + 1;
+    const double best = improved ? kkt : S->best_kkt;
+    int status = ST_RUNNING;
+    if (kkt <= S->tol) status = ST_CONVERGED;
+    else if (stall >= 3 && best <= S->tol_accept) status = ST_CONVERGED;     // floor of the arithmetic (reading 18)
+    else if (stall >= 6) status = ST_STALLED;
+    else if (outer1 >= S->outer_max) status = (best <= S->tol_accept) ? ST_CONVERGED : ST_OUTER_CAP;
+    const bool take_best = status != ST_RUNNING && !improved && kkt > S->tol;
+    const bool inner_capped = S->inner >= S->inner_max;
     __syncthreads();
-    for (int j = threadIdx.x; j < n; j += blockDim.x) v.xbar_raw[j] = v.x_raw[j];
+    for (int j = threadIdx.x; j < n; j += blockDim.x) {
+        const double xj = v.xn[j];
+        v.ab[j] -= sg * v.g[j];                     // P:L149
+        if (improved) v.xbest[j] = xj;
+        const double xo = take_best ? v.xbest[j] : xj;
+        if (take_best) v.xn[j] = xo;
+        v.xbar[j] = xo;
+        const double xr = (j == 0) ? S->L * xo : ((S->use_off ? v.off[j - 1] : 0.0) + S->L * xo);
+        v.x_raw[j] = xr;
+        v.xbar_raw[j] = xr;
+    }
+    __syncthreads();
     if (threadIdx.x == 0) {
         S->dyn.cur = nxt;
         S->dyn.has_mult = 1;
-        S->outer++;
+        S->outer = outer1;
         S->n_support = nact;
-        if (S->kkt <= S->tol) { S->done = 1; S->status = ST_CONVERGED; }
-        else if (S->outer >= S->outer_max) { S->done = 1; S->status = ST_OUTER_CAP; }
-        else {
+        S->stall_count = stall;
+        if (improved) { S->best_kkt = kkt; for (int i = 0; i < 5; ++i) S->best_terms[i] = S->terms[i]; }
+        if (status != ST_RUNNING) {
+            S->done = 1; S->status = status;
+            if (take_best) { S->kkt = S->best_kkt; for (int i = 0; i < 5; ++i) S->terms[i] = S->best_terms[i]; }
+        } else if (!inner_capped) {
+            // sigma grows only after an inner loop that ended by one of its tests (Theorem 1 needs a
+            // nondecreasing sequence; a loop cut by its cap gains nothing from a stiffer subproblem)
             const double s2 = fmin(S->sigma_max, S->kappa * sg);
             S->sigma = s2;
             S->dyn.sigma_raw = s2 / S->L;

@@ -14,7 +14,7 @@ enum { PH_FIRST = 0,      // first evaluation of an outer iteration (Alg. 2 line
        PH_ARMIJO = 1,     // evaluation of an Armijo trial point x + eta*Delta (Alg. 2 line 9)
        PH_REEVAL = 2 };   // re-evaluation at x before a multiplier update (records of the last pass are stale)
 enum { ACT_TRIAL = 0, ACT_NEWTON = 1, ACT_UPDATE = 2, ACT_DONE = 3 };
-enum { ST_RUNNING = 0, ST_CONVERGED = 1, ST_OUTER_CAP = 2, ST_NEED_CAPACITY = 3, ST_CHOL_FAILED = 4 };
+enum { ST_RUNNING = 0, ST_CONVERGED = 1, ST_OUTER_CAP = 2, ST_NEED_CAPACITY = 3, ST_CHOL_FAILED = 4, ST_STALLED = 5 };
 
 struct SolverDev {
     // ---- constants of the phase (written by the host before the graph is launched) ----
@@ -36,12 +36,14 @@ struct SolverDev {
     long long pass_count;
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
+    double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
+    int32_t stall_count, pad2;
     int32_t in_graph, eval_cap;   // eval_cap: hard bound on the evaluations of a phase (a runaway loop cannot hang the GPU)
 };
 
 // (d+1)-vectors of the state, each of length nv = n rounded up to 8, in one device array
 struct SolverVecs {
-    double *xn, *xbar, *ab, *delta, *g, *xt, *x_raw, *xbar_raw, *off, *grad_t, *res, *p, *Hp;
+    double *xn, *xbar, *ab, *delta, *g, *xt, *x_raw, *xbar_raw, *off, *grad_t, *res, *p, *Hp, *xbest;
     double *ev_t, *ev;           // [MEB_EVAL_NSCALARS] scalars of the trial / accepted evaluation
 };
 

@@ -320,6 +320,13 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
             rc = meb_ctrl_after_newton(ctx, dev, S.v);
             if (rc) return rc;
         } else if (h->action == ACT_UPDATE) {
+            if (getenv("MEB_TRACE")) {
+                double ev[MEB_EVAL_NSCALARS];
+                cudaMemcpy(ev, S.v.ev, sizeof(ev), cudaMemcpyDeviceToHost);
+                fprintf(stderr, "[meb trace] outer %d sigma %.3g inner %d evals %d kkt %.3e terms %.2e %.2e %.2e %.2e %.2e nB1 %.0f nB3 %.0f psi %.12g\n",
+                        h->outer, h->sigma, h->inner, h->evals, h->kkt, h->terms[0], h->terms[1], h->terms[2], h->terms[3],
+                        h->terms[4], ev[MEB_EV_N_B1], ev[MEB_EV_N_B3], h->psi_cur);
+            }
             rc = seq_update(q);
             if (rc) return rc;
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
@@ -377,8 +384,8 @@ int grow_pool(meb_ctx* ctx, Problem& P, int b, int64_t rows) {
 
 // Algorithm 1 with Algorithm 2 inside, device-resident: one graph launch per phase (plus one relaunch
 // whenever a V pool has to grow).  xn / ab are the normalised x and (alpha, beta), in/out (host).
-int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& ab, double tol, bool* converged,
-           double* kkt_out, double terms_out[5], int outer_cap) {
+int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& ab, double tol, double tol_accept,
+           bool* converged, double* kkt_out, double terms_out[5], int outer_cap) {
     meb_ctx* ctx = S.ctx;
     const meb_params& par = S.par;
     const int n = S.d + 1;
@@ -414,11 +421,15 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));          // h is free to be rewritten
         if (first) {
             memset(h, 0, sizeof(*h));
-            h->L = S.L; h->tol = tol; h->rho = par.rho; h->tau = par.tau; h->kappa = par.kappa;
+            h->L = S.L; h->tol = tol; h->tol_accept = tol_accept; h->rho = par.rho; h->tau = par.tau; h->kappa = par.kappa;
             h->sigma_max = par.sigma_max; h->armijo_mu = par.armijo_mu;
             h->n = n; h->d = S.d; h->inner_max = par.inner_max; h->outer_max = outer_cap;
             h->armijo_max = par.armijo_max_halvings; h->cg_max = par.cg_max; h->dense = dense ? 1 : 0;
             h->use_off = P.off ? 1 : 0;
+            if (P.prec == MEB_FP32) {      // FP32 cannot resolve steps below ~2^-12 or more than a few Newton steps (reading 17)
+                if (h->armijo_max > 12) h->armijo_max = 12;
+                if (h->inner_max > 20) h->inner_max = 20;
+            }
             h->eval_cap = 4 * outer_cap * (par.inner_max + 2);
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
@@ -546,14 +557,14 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         // ---- state vectors on the device ----
         const size_t nH = (d <= 128) ? (size_t)n * n + 8 : 8;
         const size_t nv = ((size_t)n + 7) / 8 * 8;
-        rc = own_reserve(ctx, OWN_STATE, (14 * nv + 2 * MEB_EVAL_NSCALARS + nH) * sizeof(double));
+        rc = own_reserve(ctx, OWN_STATE, (15 * nv + 2 * MEB_EVAL_NSCALARS + nH) * sizeof(double));
         if (rc) break;
         double* base = (double*)ctx->own[OWN_STATE];
         double** vecs[] = {&S.v.xn, &S.v.xbar, &S.v.ab, &S.v.delta, &S.v.g, &S.v.xt, &S.v.x_raw, &S.v.xbar_raw,
-                           &S.v.off, &S.v.grad_t, &S.v.res, &S.v.p, &S.v.Hp};
-        for (size_t i = 0; i < 13; ++i) *vecs[i] = base + i * nv;
-        double* dc0 = base + 13 * nv;
-        S.v.ev_t = base + 14 * nv;
+                           &S.v.off, &S.v.grad_t, &S.v.res, &S.v.p, &S.v.Hp, &S.v.xbest};
+        for (size_t i = 0; i < 14; ++i) *vecs[i] = base + i * nv;
+        double* dc0 = base + 14 * nv;
+        S.v.ev_t = base + 15 * nv;
         S.v.ev = S.v.ev_t + MEB_EVAL_NSCALARS;
         S.dH = S.v.ev + MEB_EVAL_NSCALARS;
         // ---- a0: ingest (initial point, validation, FP32 shadow) ----
@@ -601,7 +612,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             rc = setup_multipliers(ctx, P, OWN_U0, OWN_S0, OWN_V0);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
-            rc = ripalm(S, P, xn, ab, tol_kkt, &converged, &kkt, terms, S.par.outer_max);
+            rc = ripalm(S, P, xn, ab, tol_kkt, tol, &converged, &kkt, terms, S.par.outer_max);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
             // final full pass: r_out = max_i(||c - c_i|| + r_i)   (step 7)
@@ -627,7 +638,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             if (rc) break;
             bool conv1 = false;
             double kkt1, terms1[5];
-            rc = ripalm(S, P1, xn, ab, S.par.tol_lo, &conv1, &kkt1, terms1,
+            rc = ripalm(S, P1, xn, ab, S.par.tol_lo, S.par.tol_lo, &conv1, &kkt1, terms1,
                         S.par.outer_max_lo > 0 ? S.par.outer_max_lo : S.par.outer_max);
             if (rc) break;
             MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
@@ -706,7 +717,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                     P2.m = nred;
                     st->n_reduced = nred;
                     st->rounds = rnd + 1;
-                    rc = ripalm(S, P2, xn, ab, tol_kkt, &converged, &kkt, terms, S.par.outer_max);
+                    rc = ripalm(S, P2, xn, ab, tol_kkt, tol, &converged, &kkt, terms, S.par.outer_max);
                     if (rc) break;
                     if (rnd == 0) MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
                     // a-posteriori check against ALL original constraints

@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(CBLK) ctrl_init_kernel(SolverDev* S, const Sol
         S->outer = 0; S->inner = 0; S->ls = 0; S->done = 0; S->status = ST_RUNNING; S->stalled = 0;
         S->newton_total = 0; S->cg_total = 0; S->evals = 0; S->chol_info = 0;
         S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0;
-        S->pass_ns = 0ull; S->pass_count = 0;
+        S->pass_ns = 0ull; S->pass_count = 0; S->vrow_reads = 0ull;
         S->eta = 1.0; S->psi_cur = 0.0; S->slope = 0.0;
         S->cg_go = 0; S->cg_it = 0;
     }
@@ -120,7 +120,6 @@ __global__ void __launch_bounds__(CBLK) ctrl_after_update_kernel(SolverDev* S, c
     else if (stall >= 6) status = ST_STALLED;
     else if (outer1 >= S->outer_max) status = (best <= S->tol_accept) ? ST_CONVERGED : ST_OUTER_CAP;
     const bool take_best = status != ST_RUNNING && !improved && kkt > S->tol;
-    const bool inner_capped = S->inner >= S->inner_max;
     __syncthreads();
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
         const double xj = v.xn[j];
@@ -144,9 +143,7 @@ __global__ void __launch_bounds__(CBLK) ctrl_after_update_kernel(SolverDev* S, c
         if (status != ST_RUNNING) {
             S->done = 1; S->status = status;
             if (take_best) { S->kkt = S->best_kkt; for (int i = 0; i < 5; ++i) S->terms[i] = S->best_terms[i]; }
-        } else if (!inner_capped) {
-            // sigma grows only after an inner loop that ended by one of its tests (Theorem 1 needs a
-            // nondecreasing sequence; a loop cut by its cap gains nothing from a stiffer subproblem)
+        } else {
             const double s2 = fmin(S->sigma_max, S->kappa * sg);
             S->sigma = s2;
             S->dyn.sigma_raw = s2 / S->L;

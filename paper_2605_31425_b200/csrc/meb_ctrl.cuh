@@ -34,6 +34,7 @@ struct SolverDev {
     // ---- in-graph timing of the evaluation passes (globaltimer, ns) ----
     unsigned long long pass_ns;
     long long pass_count;
+    unsigned long long vrow_reads;  // sum over the evaluation passes of the V rows they read (balls with u_i > 0)
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
     double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
@@ -155,6 +156,7 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         if (threadIdx.x == 0) {
             if (stalled) { S->phase = PH_REEVAL; } else { S->eta = eta; S->ls++; }
             S->action = ACT_TRIAL; S->evals++;
+            S->vrow_reads += (unsigned long long)(S->dyn.has_mult ? S->n_support : 0);
             if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
             ctrl_set_handles(S);
         }
@@ -180,6 +182,7 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     ctrl_block_sum3(agx, gg, dx2, sm);
     if (threadIdx.x == 0) {
         S->evals++;
+        S->vrow_reads += (unsigned long long)(S->dyn.has_mult ? S->n_support : 0);
         S->psi_cur = psi_t;
         double terms[5];
         const double kkt = ctrl_rel_kkt(ev_s, Ls * sm[96], terms);

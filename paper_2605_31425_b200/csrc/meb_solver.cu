@@ -46,6 +46,8 @@ struct Problem {                   // one ripALM run: data + double-buffered mul
 
 struct Solver {
     meb_ctx* ctx; meb_params par; meb_stats* st;
+    double sigma_start;            // sigma_0 of the next phase (normalised units)
+    double sigma_end;              // sigma reached by the last phase
     int32_t d; double L;
     double* dH;                    // device (d+1)^2: dense Newton system
     SolverVecs v;                  // device (d+1)-vectors of the controller
@@ -437,7 +439,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         h->in_graph = stepped ? 0 : 1;
         if (first) {
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
-            rc = meb_ctrl_init(ctx, dev, S.v, par.sigma0, P.cur, P.has_mult ? 1 : 0);
+            rc = meb_ctrl_init(ctx, dev, S.v, S.sigma_start, P.cur, P.has_mult ? 1 : 0);
         } else {                                                        // resume: constants that may have changed
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(&dev->vcap[0], &h->vcap[0], 2 * sizeof(int64_t),
                                              cudaMemcpyHostToDevice, ctx->stream));
@@ -475,9 +477,10 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         if (!P.full) S.st->passes_reduced += h->evals;
         else if (P.prec == MEB_FP64) S.st->passes_fp64_full += h->evals;
         else S.st->passes_fp32_full += h->evals;
-        S.bytes += (double)h->evals * G->bytes_per_eval;
+        const double vbytes = (double)h->vrow_reads * (double)S.d * (double)esz(P.prec);   // V rows of balls with u_i > 0
+        S.bytes += (double)h->evals * G->bytes_per_eval + vbytes;
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
-        S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval;
+        S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval + vbytes;
         S.st->pass_count[cls] += (int32_t)h->pass_count;
         if (!stepped)       // kernels launched by the graph: counted from the device-side iteration counters
             ctx->launches += (int64_t)h->evals * G->k_eval + (int64_t)h->newton_total * G->k_newton +
@@ -486,6 +489,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         *kkt_out = h->kkt;
         memcpy(terms_out, h->terms, 5 * sizeof(double));
         *converged = h->status == ST_CONVERGED;
+        S.sigma_end = h->sigma;
         P.cur = h->dyn.cur;
         P.has_mult = h->dyn.has_mult != 0;
         // final iterate back to the host
@@ -528,11 +532,12 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
     meb_stats* st = h_stats ? h_stats : &local_stats;
     memset(st, 0, sizeof(*st));
     Solver S;
-    S.ctx = ctx; S.st = st; S.d = d; S.bytes = 0.0;
+    S.ctx = ctx; S.st = st; S.d = d; S.bytes = 0.0; S.sigma_start = 0.0; S.sigma_end = 0.0;
     if (h_params) S.par = *h_params; else meb_default_params(&S.par);
     if (!(S.par.rho >= 0.0 && S.par.rho < 1.0) || !(S.par.sigma0 > 0.0) || !(S.par.tau > 0.0) ||
         !(S.par.kappa >= 1.0) || S.par.sample_rows < 1)
         return MEB_E_ARG;
+    S.sigma_start = S.par.sigma0;
     const int n = d + 1;
     // The KKT test runs at tol/10: the primal-feasibility term only bounds the error of the returned
     // (feasible) radius by about tol (1 + r)/r, and the contract is a radius within tol (DESIGN reading 7).

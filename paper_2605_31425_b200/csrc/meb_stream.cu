@@ -28,6 +28,8 @@ template <typename T, int G, int CPT, int VEC, int OP, bool SHADOW>
 __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs a_in) {
     StreamArgs a = a_in;
     meb_resolve_dyn(a);
+    long long t_start = 0;
+    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_start));
     constexpr int RPW = 32 / G;                     // rows per warp-wide load instruction
     constexpr int NPAD = G * CPT * VEC;             // padded row length held in shared memory
     __shared__ __align__(16) T cs[NPAD];
@@ -146,6 +148,12 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
         }
     }
     block_reduce_store<OP>(acc, a.part);
+    if (threadIdx.x == 0) {                 // device time stamps of this CTA (ns), read by the finalize kernel
+        long long t_end;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
+        a.part[(size_t)blockIdx.x * MEB_NPART + 10] = __longlong_as_double(t_start);
+        a.part[(size_t)blockIdx.x * MEB_NPART + 11] = __longlong_as_double(t_end);
+    }
 }
 
 // ---- loop kernel: one warp per row, any d -----------------------------------------------------------
@@ -153,6 +161,8 @@ template <typename T, int VEC, int OP, bool SHADOW>
 __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs a_in) {
     StreamArgs a = a_in;
     meb_resolve_dyn(a);
+    long long t_start = 0;
+    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_start));
     constexpr int UNR = 8;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d = a.d;
@@ -166,6 +176,11 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
     const T inv_sig = T(1) / sig;
     const int nchunks = (d + VEC - 1) / VEC;
     Acc acc;
+    // the centre, converted to T once, in dynamic shared memory (padded with zeros to whole chunks)
+    extern __shared__ __align__(16) unsigned char loop_dyn_smem[];
+    T* cs = reinterpret_cast<T*>(loop_dyn_smem);
+    for (int j = threadIdx.x; j < nchunks * VEC; j += MEB_BLOCK) cs[j] = j < d ? (T)cptr[j] : T(0);
+    __syncthreads();
 
     const int64_t ntiles = (m + 31) >> 5;
     const int64_t stride = (int64_t)gridDim.x * MEB_WARPS;
@@ -195,7 +210,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) {
                             if (col + j < d) {
-                                const T ee = e[u][j] - (T)__ldg(cptr + col + j);
+                                const T ee = e[u][j] - cs[col + j];
                                 s_nb2 = fma(ee, ee, s_nb2);
                                 if (OP == OP_INGEST) s_ne2 = fma(e[u][j], T(0), s_ne2);
                                 if (SHADOW) a.C32[row * a.ld32 + col + j] = (float)ee;
@@ -218,7 +233,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) {
                             if (col + j < d) {
-                                const T ee = e[u][j] - (T)__ldg(cptr + col + j);
+                                const T ee = e[u][j] - cs[col + j];
                                 const T b = fma(v[u][j], inv_sig, ee);
                                 s_nb2 = fma(b, b, s_nb2);
                                 s_ne2 = fma(ee, ee, s_ne2);
@@ -249,6 +264,12 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
         }
     }
     block_reduce_store<OP>(acc, a.part);
+    if (threadIdx.x == 0) {                 // device time stamps of this CTA (ns), read by the finalize kernel
+        long long t_end;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
+        a.part[(size_t)blockIdx.x * MEB_NPART + 10] = __longlong_as_double(t_start);
+        a.part[(size_t)blockIdx.x * MEB_NPART + 11] = __longlong_as_double(t_end);
+    }
 }
 
 }  // namespace
@@ -257,9 +278,12 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
 namespace {
 
 template <typename KernelT>
-int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_out) {
+int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_out, size_t smem = 0) {
+    if (smem > 220 * 1024) return MEB_E_CAPACITY;            // centre does not fit in shared memory (d > ~28,000)
     int occ = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, MEB_BLOCK, 0);
+    cudaError_t e = cudaSuccess;
+    if (smem > 48 * 1024) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, MEB_BLOCK, smem);
     if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
     if (occ < 1) occ = 1;
     const int64_t ntiles = (a.m + 31) / 32;
@@ -269,7 +293,7 @@ int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_ou
     int grid = (int)(want < cap ? want : cap);
     if (grid < 1) grid = 1;
     StreamArgs b = a;
-    ctx->launches++; kernel<<<grid, MEB_BLOCK, 0, ctx->stream>>>(b);
+    ctx->launches++; kernel<<<grid, MEB_BLOCK, smem, ctx->stream>>>(b);
     e = cudaGetLastError();
     if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
     *grid_out = grid;
@@ -279,7 +303,7 @@ int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_ou
 template <typename T, int OP, bool SHADOW>
 int dispatch_shape(meb_ctx* ctx, const StreamArgs& a, bool aligned, int* grid_out) {
     constexpr int VEC = VecOf<T>::N;
-    if (!aligned) return launch_sized(ctx, stream_loop_kernel<T, 1, OP, SHADOW>, a, grid_out);
+    if (!aligned) return launch_sized(ctx, stream_loop_kernel<T, 1, OP, SHADOW>, a, grid_out, ((size_t)a.d * sizeof(T) + 15) / 16 * 16);
     const int nchunks = (a.d + VEC - 1) / VEC;
     if (nchunks <= 4)   return launch_sized(ctx, stream_tile_kernel<T, 4, 1, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 8)   return launch_sized(ctx, stream_tile_kernel<T, 4, 2, VEC, OP, SHADOW>, a, grid_out);
@@ -289,7 +313,7 @@ int dispatch_shape(meb_ctx* ctx, const StreamArgs& a, bool aligned, int* grid_ou
     if (nchunks <= 128) return launch_sized(ctx, stream_tile_kernel<T, 16, 8, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 256) return launch_sized(ctx, stream_tile_kernel<T, 32, 8, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 512) return launch_sized(ctx, stream_tile_kernel<T, 32, 16, VEC, OP, SHADOW>, a, grid_out);
-    return launch_sized(ctx, stream_loop_kernel<T, VEC, OP, SHADOW>, a, grid_out);
+    return launch_sized(ctx, stream_loop_kernel<T, VEC, OP, SHADOW>, a, grid_out, (size_t)nchunks * 16);
 }
 
 template <typename T>

@@ -113,49 +113,52 @@ __global__ void __launch_bounds__(CBLOCK) compact_write_kernel(const uint32_t* _
     }
 }
 
-// Small problems (up to a few million balls): ONE CTA of 1024 threads scans the whole mask in rounds of
-// 1024 words (ballot-free integer scan: per-word popcounts, warp shuffles, warp totals in shared memory)
-// and writes the indices at their final position -- one launch instead of two, no segment sums.
+// Small problems (up to 2M balls): ONE CTA of 1024 threads.  Thread t owns the contiguous run of W words
+// [t W, (t+1) W): it counts its bits, one block-wide exclusive scan (warp shuffles + warp totals in
+// shared memory, two barriers in all) gives its output offset, and it writes its indices in order.
 __global__ void __launch_bounds__(1024) compact_single_kernel(const uint32_t* __restrict__ mask, int64_t nwords,
                                                               int64_t m, int32_t* __restrict__ list, int64_t cap,
                                                               int32_t* __restrict__ count) {
     __shared__ int wtot[32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    long long base = 0;
-    for (int64_t w0 = 0; w0 < nwords; w0 += 1024) {
-        const int64_t w = w0 + threadIdx.x;
-        uint32_t bits = 0;
-        if (w < nwords) {
-            bits = mask[w];
-            if ((w + 1) * 32 > m) bits &= (m - w * 32 >= 32) ? 0xffffffffu : ((1u << (m - w * 32)) - 1u);
-        }
-        const int c = __popc(bits);
-        int incl = c;
+    const int W = (int)((nwords + 1023) / 1024);
+    const int64_t w0 = (int64_t)threadIdx.x * W;
+    auto word = [&](int64_t w) -> uint32_t {
+        if (w >= nwords) return 0u;
+        uint32_t bits = mask[w];
+        if ((w + 1) * 32 > m) bits &= (m - w * 32 >= 32) ? 0xffffffffu : ((1u << (m - w * 32)) - 1u);
+        return bits;
+    };
+    int c = 0;
+#pragma unroll 4
+    for (int k = 0; k < W; ++k) c += __popc(word(w0 + k));
+    int incl = c;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int v = __shfl_up_sync(MEB_FULL_MASK, incl, o);
-            if (lane >= o) incl += v;
-        }
-        if (lane == 31) wtot[warp] = incl;
-        __syncthreads();
-        int wpre = 0, rtot = 0;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(MEB_FULL_MASK, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    int wpre = 0, tot = 0;
 #pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            const int v = wtot[k];
-            if (k < warp) wpre += v;
-            rtot += v;
-        }
-        long long pos = base + wpre + (incl - c);
+    for (int k = 0; k < 32; ++k) {
+        const int v = wtot[k];
+        if (k < warp) wpre += v;
+        tot += v;
+    }
+    if (threadIdx.x == 0) *count = tot;
+    if (c == 0) return;
+    long long pos = (long long)wpre + (incl - c);
+    for (int k = 0; k < W; ++k) {
+        uint32_t bits = word(w0 + k);
         while (bits) {
             const int b = __ffs(bits) - 1;
             bits &= bits - 1;
-            if (pos < cap) list[pos] = (int32_t)(w * 32 + b);
+            if (pos < cap) list[pos] = (int32_t)((w0 + k) * 32 + b);
             ++pos;
         }
-        base += rtot;
-        __syncthreads();
     }
-    if (threadIdx.x == 0) *count = (int32_t)base;
 }
 
 // uint8 flags -> bit mask (the "flags given" input mode of meb_screen_compact)

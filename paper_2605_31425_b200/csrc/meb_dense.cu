@@ -11,6 +11,7 @@
 #include <string.h>
 
 #include "meb_internal.cuh"
+#include "meb_ctrl.cuh"
 
 namespace {
 
@@ -163,7 +164,7 @@ __device__ __forceinline__ double fast_rcp(double d) {
 template <int BS>
 __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
                                                          int n, double scale, double* __restrict__ delta,
-                                                         int* __restrict__ info) {
+                                                         int* __restrict__ info, SolverDev* S, const SolverVecs v) {
     extern __shared__ __align__(16) double Lm[];          // n rows x ldl (column k of L D as row k), invd, z
     constexpr int NP = 16 * BS;
     constexpr int ldl = NP | 1;
@@ -274,6 +275,28 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
     __syncthreads();
     for (int e = tid; e < n; e += 256) delta[e] = z[e];
     if (tid == 0 && info) *info = bad;
+    if (S) {
+        // controller step after the Newton solve (Alg. 2 line 9): slope <g, Delta>, first Armijo trial x + Delta
+        __shared__ double red[8];
+        const double Ls = S->L;
+        const bool use_off = S->use_off != 0;
+        double sl = 0.0;
+        for (int j = tid; j < n; j += 256) {
+            const double dj = z[j];
+            sl = fma(v.g[j], dj, sl);
+            const double xj = v.xn[j] + dj;
+            v.xt[j] = xj;
+            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+        }
+        sl = warp_sum(sl);
+        if ((tid & 31) == 0) red[tid >> 5] = sl;
+        __syncthreads();
+        if (tid == 0) {
+            double t = 0.0;
+            for (int w = 0; w < 8; ++w) t += red[w];
+            S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
+        }
+    }
 }
 
 template <typename T>
@@ -326,7 +349,10 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
 
 // delta <- -(scale*H)^{-1} g on the device; info_dev (nullable) receives 0 or the failing pivot + 1
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
-                   int* info_dev) {
+                   int* info_dev, SolverDev* S, const SolverVecs* v) {
+    SolverVecs vv;
+    memset(&vv, 0, sizeof(vv));
+    if (S && v) vv = *v;
     const int bs = (n + 1 + 15) / 16;                       // augmented order n + 1 <= 16 bs
     if (bs > 9) return MEB_E_CAPACITY;
     const int np = 16 * bs;
@@ -336,7 +362,7 @@ int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double
         MEB_CUDA_OK(ctx, cudaFuncSetAttribute(ldlt_solve_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                               (int)smem));                                                      \
         ctx->launches++;                                                                                        \
-        ldlt_solve_kernel<B><<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev);                   \
+        ldlt_solve_kernel<B><<<1, 256, smem, ctx->stream>>>(H, g, n, scale, delta, info_dev, S, vv);                   \
         break;
     switch (bs) {
         MEB_LDLT_CASE(1) MEB_LDLT_CASE(2) MEB_LDLT_CASE(3) MEB_LDLT_CASE(4) MEB_LDLT_CASE(5)

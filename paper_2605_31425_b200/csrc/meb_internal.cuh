@@ -253,8 +253,9 @@ int meb_hvp_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scala
 
 // ---- dense Hessian and Cholesky (meb_dense.cu) ----
 int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_scalars, double* H);
+// With S != nullptr the kernel also runs the controller step that follows a Newton solve (first Armijo trial).
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
-                   int* info_dev);
+                   int* info_dev, SolverDev* S, const SolverVecs* v);
 
 // ---- controller kernels of the device-resident solver (meb_ctrl.cu) ----
 int meb_ctrl_init(meb_ctx* ctx, SolverDev* S, const SolverVecs& v, double sigma0, int cur, int has_mult);

@@ -165,7 +165,7 @@ int seq_newton_dense(Seq& q) {
     if (rc) return rc;
     rc = meb_dense_from_records(ctx, q.c, q.S->v.ev, q.S->dH);
     if (rc) return rc;
-    return meb_chol_solve(ctx, q.S->dH, q.S->v.g, q.S->d + 1, q.S->L, q.S->v.delta, &q.dev->chol_info);
+    return meb_chol_solve(ctx, q.S->dH, q.S->v.g, q.S->d + 1, q.S->L, q.S->v.delta, &q.dev->chol_info, q.dev, &q.S->v);
 }
 // one CG iteration of the matrix-free path: Hp = H p over the active rows, CG step
 int seq_cg_body(Seq& q) {
@@ -249,8 +249,8 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     } else {
         RC(meb_ensure_list(ctx, P.m));
         RC(add_conditional(ctx, bn, G->h_cg, true, &cgnode, &bcg));
+        RC(meb_ctrl_after_newton(ctx, q.dev, S.v));
     }
-    RC(meb_ctrl_after_newton(ctx, q.dev, S.v));
     G->k_newton = (int)(ctx->launches - l0);
     CU(cudaStreamEndCapture(ctx->stream, &tmp));
     capturing = false;
@@ -318,9 +318,9 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
                     MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
                     go = h->cg_go;
                 }
+                rc = meb_ctrl_after_newton(ctx, dev, S.v);
+                if (rc) return rc;
             }
-            rc = meb_ctrl_after_newton(ctx, dev, S.v);
-            if (rc) return rc;
         } else if (h->action == ACT_UPDATE) {
             if (getenv("MEB_TRACE")) {
                 double ev[MEB_EVAL_NSCALARS];

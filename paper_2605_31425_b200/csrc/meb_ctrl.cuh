@@ -218,3 +218,94 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
             v.p[j] = -gj;
         }
 }
+
+// Controller step after a Newton solve (Alg. 2 line 9): slope <g, Delta>, first Armijo trial x + Delta.
+// z: Delta (n doubles, shared or global).  S may live in global or shared memory.  CTA of 256 threads.
+__device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs v, const double* z, int n) {
+    __shared__ double red[8];
+    const int tid = threadIdx.x;
+    const double Ls = S->L;
+    const bool use_off = S->use_off != 0;
+    double sl = 0.0;
+    for (int j = tid; j < n; j += 256) {
+        const double dj = z[j];
+        sl = fma(v.g[j], dj, sl);
+        const double xj = v.xn[j] + dj;
+        v.xt[j] = xj;
+        v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+    }
+    sl = warp_sum(sl);
+    if ((tid & 31) == 0) red[tid >> 5] = sl;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
+    }
+}
+
+// After (U+, V+) of the accepted point were written into the other multiplier buffer (eq. (6)):
+// capacity check, buffer flip, (alpha, beta) update, KKT test, best-iterate / stall
+// logic (reading 18), sigma update, start of the next outer iteration.  Every thread of the CTA
+// calls it; S may live in global or shared memory; nact = number of active balls of the accepted pass.
+__device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs v, long long nact) {
+    const int n = S->n;
+    const int nxt = S->dyn.has_mult ? 1 - S->dyn.cur : 0;
+    const bool fits = nact <= S->vcap[nxt];
+    __syncthreads();
+    if (!fits) {                                    // host grows the pool and relaunches; x is re-evaluated
+        ctrl_to_raw(S, v, v.xn, v.x_raw);
+        if (threadIdx.x == 0) {
+            S->n_support = nact;
+            S->phase = PH_REEVAL; S->action = ACT_DONE; S->done = 1; S->status = ST_NEED_CAPACITY;
+            ctrl_set_handles(S);
+        }
+        return;
+    }
+    // ---- decisions (every thread computes the same from the state as it was on entry) ----
+    const double sg = S->sigma;
+    const double kkt = S->kkt;
+    const int outer1 = S->outer + 1;
+    const bool improved = kkt < S->best_kkt;                     // best iterate so far (returned if the run stalls)
+    const int stall = (kkt < 0.5 * S->best_kkt) ? 0 : S->stall_count + 1;
+    const double best = improved ? kkt : S->best_kkt;
+    int status = ST_RUNNING;
+    if (kkt <= S->tol) status = ST_CONVERGED;
+    else if (stall >= 3 && best <= S->tol_accept) status = ST_CONVERGED;     // floor of the arithmetic (reading 18)
+    else if (stall >= 6) status = ST_STALLED;
+    else if (outer1 >= S->outer_max) status = (best <= S->tol_accept) ? ST_CONVERGED : ST_OUTER_CAP;
+    const bool take_best = status != ST_RUNNING && !improved && kkt > S->tol;
+    __syncthreads();
+    for (int j = threadIdx.x; j < n; j += blockDim.x) {
+        const double xj = v.xn[j];
+        v.ab[j] -= sg * v.g[j];
+        if (improved) v.xbest[j] = xj;
+        const double xo = take_best ? v.xbest[j] : xj;
+        if (take_best) v.xn[j] = xo;
+        v.xbar[j] = xo;
+        const double xr = (j == 0) ? S->L * xo : ((S->use_off ? v.off[j - 1] : 0.0) + S->L * xo);
+        v.x_raw[j] = xr;
+        v.xbar_raw[j] = xr;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        S->dyn.cur = nxt;
+        S->dyn.has_mult = 1;
+        S->outer = outer1;
+        S->n_support = nact;
+        S->stall_count = stall;
+        if (improved) { S->best_kkt = kkt; for (int i = 0; i < 5; ++i) S->best_terms[i] = S->terms[i]; }
+        if (status != ST_RUNNING) {
+            S->done = 1; S->status = status;
+            if (take_best) { S->kkt = S->best_kkt; for (int i = 0; i < 5; ++i) S->terms[i] = S->best_terms[i]; }
+        } else {
+            const double s2 = fmin(S->sigma_max, S->kappa * sg);
+            S->sigma = s2;
+            S->dyn.sigma_raw = s2 / S->L;
+        }
+        S->inner = 0;
+        S->phase = PH_FIRST;
+        S->action = S->done ? ACT_DONE : ACT_TRIAL;
+        ctrl_set_handles(S);
+    }
+}

@@ -12,6 +12,7 @@
 
 #include "meb_internal.cuh"
 #include "meb_ctrl.cuh"
+#include "meb_ldlt.cuh"
 
 namespace {
 
@@ -150,26 +151,12 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
 // publish it to shared memory (where it stays as row k+1 of L D for the backward substitution)
 // together with 1/d_{k+1}, computed by the diagonal's owner while the others are still updating.
 // One __syncthreads per column.
-// 1/d for d > 0 in full precision: hardware seed (about 20 bits) + two Newton steps, 4 dependent FMAs
-// (the IEEE division subroutine is several times longer and sits on the critical path of every column)
-__device__ __forceinline__ double fast_rcp(double d) {
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-    double e = fma(-d, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-d, r, 1.0);
-    return fma(r, e, r);
-}
-
 template <int BS>
 __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restrict__ H, const double* __restrict__ g,
                                                          int n, double scale, double* __restrict__ delta,
                                                          int* __restrict__ info, SolverDev* S, const SolverVecs v) {
-    extern __shared__ __align__(16) double Lm[];          // n rows x ldl (column k of L D as row k), invd, z
-    constexpr int NP = 16 * BS;
-    constexpr int ldl = NP | 1;
-    double* invd = Lm + (size_t)n * ldl;
-    double* z = invd + NP;
+    extern __shared__ __align__(16) double Lm[];          // LdltShape<BS>::smem_doubles(n)
+    __shared__ int bad;
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
     double a[BS][BS];
 #pragma unroll
@@ -178,125 +165,20 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
         for (int jj = 0; jj < BS; ++jj) {
             // unconditional loads from clamped addresses (all in flight at once), selected afterwards
             const int i = ty + 16 * ii, j = tx + 16 * jj;
-            double v = 0.0;
+            double v0 = 0.0;
             if (jj <= ii) {
                 const int ic = i < n ? i : n - 1, jc = j < n ? j : n - 1;
                 const double hv = H[(size_t)ic * n + jc];
                 const double gv = g[jc];
                 const bool live = j < n && j <= i;
-                v = (live && i < n) ? scale * hv : ((live && i == n) ? -gv : 0.0);
+                v0 = (live && i < n) ? scale * hv : ((live && i == n) ? -gv : 0.0);
             }
-            a[ii][jj] = v;
+            a[ii][jj] = v0;
         }
-    __shared__ int bad;
-    if (tid == 0) bad = 0;
-    if (tx == 0) {                                        // publish column 0
-#pragma unroll
-        for (int ii = 0; ii < BS; ++ii) Lm[ty + 16 * ii] = a[ii][0];
-    }
-    __syncthreads();
-#pragma unroll
-    for (int KB = 0; KB < BS; ++KB) {
-        if (16 * KB < n) {
-#pragma unroll 1
-            for (int kk = 0; kk < 16; ++kk) {
-                const int k = 16 * KB + kk;
-                if (k >= n) break;                        // uniform
-                const double* col = Lm + (size_t)k * ldl;
-                double dk = col[k];
-                if (!(dk > 0.0)) { if (tid == 0) bad = k + 1; dk = 1.0; }
-                const double ninv = -fast_rcp(dk);        // every thread forms 1/d_k itself (no serial owner)
-                if (tid == 0) invd[k] = -ninv;
-                // multipliers; only block KB holds rows / columns <= k, which are masked to zero
-                double lik[BS], cj[BS];
-#pragma unroll
-                for (int q = KB; q < BS; ++q) {
-                    double c1 = col[ty + 16 * q], c2 = col[tx + 16 * q];
-                    if (q == KB) {
-                        c1 = (ty + 16 * KB > k) ? c1 : 0.0;
-                        c2 = (tx + 16 * KB > k) ? c2 : 0.0;
-                    }
-                    lik[q] = c1 * ninv;
-                    cj[q] = c2;
-                }
-#pragma unroll
-                for (int ii = KB; ii < BS; ++ii)
-#pragma unroll
-                    for (int jj = KB; jj <= ii; ++jj) a[ii][jj] = fma(lik[ii], cj[jj], a[ii][jj]);
-                const int k1 = k + 1;
-                if (k1 < n && tx == (k1 & 15)) {          // owners of column k+1 publish it
-                    double* cn = Lm + (size_t)k1 * ldl;
-                    if (kk < 15) {
-#pragma unroll
-                        for (int ii = KB; ii < BS; ++ii) cn[ty + 16 * ii] = a[ii][KB];
-                    } else if (KB + 1 < BS) {
-#pragma unroll
-                        for (int ii = KB + 1; ii < BS; ++ii) cn[ty + 16 * ii] = a[ii][KB + 1 < BS ? KB + 1 : KB];
-                    }
-                }
-                __syncthreads();
-            }
-        }
-    }
-    // row n of L D is spread over the columns' shared rows: z_k = Lm[k][n] / d_k; then L^T x = z,
-    // column-oriented by one warp with z in REGISTERS (lane L holds z[L + 32 q]): per step one shuffle
-    // broadcasts x_k and every lane updates its entries j < k with L_kj = Lm[j][k] * invd[j].
-    if (tid < 32) {
-        constexpr int ZQ = (NP + 31) / 32;
-        double zr[ZQ], dj[ZQ];
-#pragma unroll
-        for (int q = 0; q < ZQ; ++q) {
-            const int j = tid + 32 * q;
-            dj[q] = j < n ? invd[j] : 0.0;
-            zr[q] = j < n ? Lm[(size_t)j * ldl + n] * dj[q] : 0.0;
-        }
-        for (int k = n - 1; k > 0; --k) {
-            double lv[ZQ];
-#pragma unroll
-            for (int q = 0; q < ZQ; ++q) {
-                const int j = tid + 32 * q;
-                lv[q] = j < k ? Lm[(size_t)j * ldl + k] * dj[q] : 0.0;     // independent of the x chain
-            }
-            double xk = 0.0;
-#pragma unroll
-            for (int q = 0; q < ZQ; ++q) {
-                const double t = __shfl_sync(MEB_FULL_MASK, zr[q], k & 31);
-                if (q == (k >> 5)) xk = t;
-            }
-#pragma unroll
-            for (int q = 0; q < ZQ; ++q) zr[q] = fma(-lv[q], xk, zr[q]);
-        }
-#pragma unroll
-        for (int q = 0; q < ZQ; ++q) {
-            const int j = tid + 32 * q;
-            if (j < n) z[j] = zr[q];
-        }
-    }
-    __syncthreads();
+    const double* z = meb_ldlt_solve_regs<BS>(a, n, Lm, &bad);
     for (int e = tid; e < n; e += 256) delta[e] = z[e];
     if (tid == 0 && info) *info = bad;
-    if (S) {
-        // controller step after the Newton solve (Alg. 2 line 9): slope <g, Delta>, first Armijo trial x + Delta
-        __shared__ double red[8];
-        const double Ls = S->L;
-        const bool use_off = S->use_off != 0;
-        double sl = 0.0;
-        for (int j = tid; j < n; j += 256) {
-            const double dj = z[j];
-            sl = fma(v.g[j], dj, sl);
-            const double xj = v.xn[j] + dj;
-            v.xt[j] = xj;
-            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
-        }
-        sl = warp_sum(sl);
-        if ((tid & 31) == 0) red[tid >> 5] = sl;
-        __syncthreads();
-        if (tid == 0) {
-            double t = 0.0;
-            for (int w = 0; w < 8; ++w) t += red[w];
-            S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
-        }
-    }
+    if (S) meb_ctrl_after_newton_dev(S, v, z, n);
 }
 
 template <typename T>
@@ -356,7 +238,7 @@ int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double
     const int bs = (n + 1 + 15) / 16;                       // augmented order n + 1 <= 16 bs
     if (bs > 9) return MEB_E_CAPACITY;
     const int np = 16 * bs;
-    const size_t smem = ((size_t)n * (np | 1) + 2 * (size_t)np) * sizeof(double);
+    const size_t smem = ((size_t)n * (np | 1) + 2 * (size_t)np) * sizeof(double);      // = LdltShape<bs>::smem_doubles(n)
 #define MEB_LDLT_CASE(B)                                                                                        \
     case B:                                                                                                     \
         MEB_CUDA_OK(ctx, cudaFuncSetAttribute(ldlt_solve_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, \

@@ -409,14 +409,24 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         if (P.off) { rc = upload(ctx, S.v.off, P.off, S.d); if (rc) return rc; }
     }
     bool first = true;
-    const bool stepped = getenv("MEB_NO_GRAPH") != nullptr;
+    bool stepped = getenv("MEB_NO_GRAPH") != nullptr;
+    // small problems (the reduced problem of the mixed mode, small instances): one persistent CTA runs the phase
+    bool small = dense && !getenv("MEB_NO_SMALL") && meb_small_applicable(P.prec, P.m, P.d);
+    if (small) {
+        for (int b = 0; b < 2 && small; ++b)
+            if (P.vcap[b] < P.m) { if (P.own_v[b] < 0 || grow_pool(ctx, P, b, P.m) != MEB_OK) small = false; }
+    }
+    if (small) stepped = false;
     int64_t stepped_launches = 0;
     (void)stepped_launches;
     SolveGraph stepped_info;
     memset(&stepped_info, 0, sizeof(stepped_info));
     for (int attempt = 0; attempt < 64; ++attempt) {
         SolveGraph* G = &stepped_info;
-        if (!stepped) {
+        if (small) {
+            stepped_info.k_eval = 0; stepped_info.k_newton = 0; stepped_info.k_cg = 0; stepped_info.k_update = 0;
+            stepped_info.bytes_per_eval = (double)P.m * (P.d * 8.0 + (P.R ? 8 : 0) + 12.0);
+        } else if (!stepped) {
             rc = get_graph(S, P, dense, &G);
             if (rc) return rc;
         }
@@ -436,7 +446,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
         h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
-        h->in_graph = stepped ? 0 : 1;
+        h->in_graph = (stepped || small) ? 0 : 1;
         if (first) {
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
             rc = meb_ctrl_init(ctx, dev, S.v, S.sigma_start, P.cur, P.has_mult ? 1 : 0);
@@ -449,7 +459,10 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         if (rc) return rc;
         first = false;
-        if (stepped) {
+        if (small) {
+            rc = meb_launch_small_solve(ctx, P.C, P.ld, P.R, P.m, P.d, P.ldv, P.U, P.slot, P.V, dev, S.v);
+            if (rc) return rc;
+        } else if (stepped) {
             const int64_t l0 = ctx->launches;
             rc = run_stepped(S, P, dense, h);
             if (rc) return rc;
@@ -482,7 +495,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
         S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval + vbytes;
         S.st->pass_count[cls] += (int32_t)h->pass_count;
-        if (!stepped)       // kernels launched by the graph: counted from the device-side iteration counters
+        if (!stepped && !small)   // kernels launched by the graph: counted from the device-side iteration counters
             ctx->launches += (int64_t)h->evals * G->k_eval + (int64_t)h->newton_total * G->k_newton +
                              (int64_t)h->cg_total * G->k_cg + (int64_t)h->outer * G->k_update;
         S.st->n_support = h->n_support;

@@ -74,11 +74,6 @@ __global__ void __launch_bounds__(SM_THREADS) small_solve_kernel(const SmallArgs
     sa.rec_lam = a.rec_lam; sa.rec_rho = a.rec_rho; sa.rec_t = a.rec_t;
     sa.t_out = nullptr; sa.lam_out = nullptr;
 
-    // balls per warp batch: all 8 warps busy on small problems, at most 32 (one epilogue lane per ball)
-    int rbw = (m + SM_WARPS - 1) / SM_WARPS;
-    rbw = (rbw + 3) & ~3;
-    if (rbw > 32) rbw = 32;
-    if (rbw < 4) rbw = 4;
     long long tmark = clock64();
     auto lap = [&](int k) { if (a.prof && tid == 0) { const long long t = clock64(); a.prof[k] += t - tmark; tmark = t; } };
     for (;;) {
@@ -97,79 +92,55 @@ __global__ void __launch_bounds__(SM_THREADS) small_solve_kernel(const SmallArgs
         double vacc[SM_MAXCOL];
 #pragma unroll
         for (int q = 0; q < SM_MAXCOL; ++q) vacc[q] = 0.0;
-        // A warp owns batches of RBW consecutive balls.  The row sums of a batch are formed four rows at a
-        // time (their loads overlap) and handed to the lane with the row's index in the batch, so the
-        // scalar epilogue (FP64 sqrt / divisions, ~1000 cycles of dependent latency) runs ONCE per batch for
-        // all its rows in parallel; active rows are then revisited for the gradient sum.
-        const int RBW = rbw;
-        for (int row0 = warp * RBW; row0 < m; row0 += SM_WARPS * RBW) {
-            const int nrows = min(RBW, m - row0);
-            double my_nb2 = 0.0, my_ne2 = 0.0, my_ev = 0.0, my_vv = 0.0, my_ri = 0.0, my_ui = 0.0;
-            int my_slot = -1;
-            for (int g0 = 0; g0 < nrows; g0 += 4) {
-                int slot_u[4];
-                double ui_u[4], ri_u[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int i = min(row0 + g0 + u, m - 1);
-                    slot_u[u] = slotp ? slotp[i] : -1;
-                    ui_u[u] = U ? U[i] : 0.0;
-                    ri_u[u] = a.R ? a.R[i] : 0.0;
+        // THREAD per ball: a thread walks its own row (d independent loads in flight, lines shared through
+        // L1), so the latency of the L2-resident data is paid once per pass, not once per ball, and every
+        // thread runs the scalar epilogue of its ball in parallel.
+        for (int i = tid; i < m; i += SM_THREADS) {
+            const double* rowp = a.C + (int64_t)i * a.ld;
+            const int slot = slotp ? slotp[i] : -1;
+            const double ui = U ? U[i] : 0.0;
+            const double ri = a.R ? a.R[i] : 0.0;
+            double nb2 = 0.0, ne2 = 0.0, evd = 0.0, vv = 0.0;
+            if (slot < 0) {
+                double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+                int j = 0;
+                for (; j + 4 <= d; j += 4) {
+                    const double e0 = rowp[j] - cs[j], e1 = rowp[j + 1] - cs[j + 1];
+                    const double e2 = rowp[j + 2] - cs[j + 2], e3 = rowp[j + 3] - cs[j + 3];
+                    s0 = fma(e0, e0, s0); s1 = fma(e1, e1, s1); s2 = fma(e2, e2, s2); s3 = fma(e3, e3, s3);
                 }
-                double s_nb2[4], s_ne2[4], s_ev[4], s_vv[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int i = min(row0 + g0 + u, m - 1);
-                    const double* rowp = a.C + (int64_t)i * a.ld;
-                    const double* vrow = slot_u[u] >= 0 ? V + (int64_t)slot_u[u] * a.ldv : nullptr;
-                    double nb2 = 0.0, ne2 = 0.0, evd = 0.0, vv = 0.0;
-#pragma unroll
-                    for (int q = 0; q < SM_MAXCOL; ++q) {
-                        const int j = lane + 32 * q;
-                        if (j < d) {
-                            const double e = rowp[j] - cs[j];
-                            double bj = e;
-                            if (vrow) {
-                                const double vj = vrow[j];
-                                bj = fma(vj, inv_sig, e);
-                                ne2 = fma(e, e, ne2); evd = fma(e, vj, evd); vv = fma(vj, vj, vv);
-                            }
-                            nb2 = fma(bj, bj, nb2);
-                        }
-                    }
-                    s_nb2[u] = nb2; s_ne2[u] = ne2; s_ev[u] = evd; s_vv[u] = vv;
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const double nb2 = warp_sum(s_nb2[u]);
-                    double ne2 = 0.0, evd = 0.0, vv = 0.0;
-                    if (slot_u[u] >= 0) { ne2 = warp_sum(s_ne2[u]); evd = warp_sum(s_ev[u]); vv = warp_sum(s_vv[u]); }
-                    if (lane == g0 + u) {
-                        my_nb2 = nb2; my_ne2 = ne2; my_ev = evd; my_vv = vv;
-                        my_ri = ri_u[u]; my_ui = ui_u[u]; my_slot = slot_u[u];
-                    }
+                for (; j < d; ++j) { const double e = rowp[j] - cs[j]; s0 = fma(e, e, s0); }
+                nb2 = (s0 + s1) + (s2 + s3);
+            } else {
+                const double* vrow = V + (int64_t)slot * a.ldv;
+#pragma unroll 4
+                for (int j = 0; j < d; ++j) {
+                    const double e = rowp[j] - cs[j];
+                    const double vj = vrow[j];
+                    const double bj = fma(vj, inv_sig, e);
+                    nb2 = fma(bj, bj, nb2); ne2 = fma(e, e, ne2); evd = fma(e, vj, evd); vv = fma(vj, vj, vv);
                 }
             }
             double mylam;
-            const bool flag = row_epilogue_core<double, OP_EVAL>(sa, row0 + lane, lane < nrows, my_slot >= 0, my_nb2, my_ne2,
-                                                                 my_ev, my_vv, r, sigma, my_ri, my_ui, acc, mylam);
-            if (lane < nrows) act[row0 + lane] = flag ? 1 : 0;
-            uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);
-            while (bits) {                                  // gradient vector part: lam_i b_i of the active rows
-                const int rs = __ffs(bits) - 1;
-                bits &= bits - 1;
-                const double lam = __shfl_sync(MEB_FULL_MASK, mylam, rs);
-                const int slot = __shfl_sync(MEB_FULL_MASK, my_slot, rs);
-                const double* rowp = a.C + (int64_t)(row0 + rs) * a.ld;
-                const double* vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
+            const bool flag = row_epilogue_core<double, OP_EVAL>(sa, i, true, slot >= 0, nb2, ne2, evd, vv, r, sigma, ri, ui,
+                                                                 acc, mylam);
+            act[i] = flag ? 1 : 0;
+        }
+        __syncthreads();
+        // gradient vector part: warp per ACTIVE ball, lanes over the columns (lam_i from the records)
+        for (int i = warp; i < m; i += SM_WARPS) {
+            if (!act[i]) continue;
+            const double lam = a.rec_lam[i];
+            const int slot = slotp ? slotp[i] : -1;
+            const double* rowp = a.C + (int64_t)i * a.ld;
+            const double* vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
 #pragma unroll
-                for (int q = 0; q < SM_MAXCOL; ++q) {
-                    const int j = lane + 32 * q;
-                    if (j < d) {
-                        double bj = rowp[j] - cs[j];
-                        if (vrow) bj = fma(vrow[j], inv_sig, bj);
-                        vacc[q] = fma(lam, bj, vacc[q]);
-                    }
+            for (int q = 0; q < SM_MAXCOL; ++q) {
+                const int j = lane + 32 * q;
+                if (j < d) {
+                    double bj = rowp[j] - cs[j];
+                    if (vrow) bj = fma(vrow[j], inv_sig, bj);
+                    vacc[q] = fma(lam, bj, vacc[q]);
                 }
             }
         }

@@ -244,20 +244,34 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                     nb2 = s0 + s1;
                     if (OP == OP_INGEST) ne2 = f0;
                 } else {                                                 // row with a multiplier v_i
-                    const T* vrow = Vg + (int64_t)myslot * a.ldv;
+                    // 16-byte chunks of the V row straight from global memory (rows of the pool are in
+                    // ascending ball order, so neighbouring lanes read neighbouring pool rows)
+                    const V4* vrow4 = reinterpret_cast<const V4*>(Vg + (int64_t)myslot * a.ldv);
+                    const V4* rp = reinterpret_cast<const V4*>(rowp);
+                    const bool v16 = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
                     for (int c = g; c < nch; c += G) {
+                        const V4 ev4 = rp[c];
+                        const V4 cv4 = cs4[c];
+                        V4 vv4;
+                        T* vq = reinterpret_cast<T*>(&vv4);
                         const int col = c * VEC;
+                        if (v16) {
+                            vv4 = __ldg(vrow4 + c);
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < VEC; ++j) vq[j] = (col + j < d) ? __ldg(Vg + (int64_t)myslot * a.ldv + col + j) : T(0);
+                        }
+                        const T* e = reinterpret_cast<const T*>(&ev4);
+                        const T* cc = reinterpret_cast<const T*>(&cv4);
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) {
-                            if (col + j < d) {
-                                const T ee = rowp[col + j] - cs[col + j];
-                                const T v = __ldg(vrow + col + j);
-                                const T b = fma(v, inv_sig, ee);
-                                nb2 = fma(b, b, nb2);
-                                ne2 = fma(ee, ee, ne2);
-                                evd = fma(ee, v, evd);
-                                vv = fma(v, v, vv);
-                            }
+                            const T ee = e[j] - cc[j];                   // padding of the row was zeroed above
+                            const T v = (col + j < d) ? vq[j] : T(0);    // padding of the pool row is not
+                            const T b = fma(v, inv_sig, ee);
+                            nb2 = fma(b, b, nb2);
+                            ne2 = fma(ee, ee, ne2);
+                            evd = fma(ee, v, evd);
+                            vv = fma(v, v, vv);
                         }
                     }
                 }
@@ -305,9 +319,17 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                                 for (int j = 0; j < VEC; ++j) b[j] = e[j] - creg[q][j];
                                 if (slot >= 0) {
                                     const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
+                                    if ((a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0) {
+                                        const V4 vv4 = __ldg(reinterpret_cast<const V4*>(vrow));
+                                        const T* vq = reinterpret_cast<const T*>(&vv4);
 #pragma unroll
-                                    for (int j = 0; j < VEC; ++j)
-                                        if (ch * VEC + j < d) b[j] = fma(__ldg(vrow + j), inv_sig, b[j]);
+                                        for (int j = 0; j < VEC; ++j)
+                                            if (ch * VEC + j < d) b[j] = fma(vq[j], inv_sig, b[j]);
+                                    } else {
+#pragma unroll
+                                        for (int j = 0; j < VEC; ++j)
+                                            if (ch * VEC + j < d) b[j] = fma(__ldg(vrow + j), inv_sig, b[j]);
+                                    }
                                 }
 #pragma unroll
                                 for (int j = 0; j < VEC; ++j) vacc[q][j] = fma(lam, (double)b[j], vacc[q][j]);

@@ -303,3 +303,35 @@ def test_argument_errors(meb, ctx):
                          None, x, x, 1.0, 1.0)
     assert ei.value.code == meb.MEB_E_CAPACITY
     big.close()
+
+
+def test_compaction_multi_segment_path(meb):
+    """Masks above 2M balls take the two-kernel segmented compaction (count + ranked write)."""
+    m = 2_500_003
+    rng = np.random.default_rng(77)
+    flags = (rng.uniform(size=m) < 0.3).astype(np.uint8)
+    flags[-1] = 1
+    fd = torch.from_numpy(flags).cuda()
+    with meb.Context(m, 4) as big:
+        res = meb.meb_screen_compact(big, None, None, 0.0, None, 0.0, flags=fd, flags_are_input=True)
+    want = prim.compact(flags)
+    assert res["count"] == want.size and np.array_equal(res["idx"].cpu().numpy(), want)
+
+
+def test_small_solver_and_graph_agree(meb):
+    """The single-CTA solver (m <= 4096) and the graph path (MEB_NO_SMALL=1) reach the same optimum."""
+    import os
+    import workloads
+    C, R = workloads.config(1, 3000, 10)
+    dC, dR = torch.from_numpy(C).cuda(), torch.from_numpy(R).cuda()
+    with meb.Context(3000, 10) as c1:
+        ca, ra, sta = meb.meb_solve(c1, dC, dR, 1e-8, meb.MEB_MODE_FP64)
+    os.environ["MEB_NO_SMALL"] = "1"
+    try:
+        with meb.Context(3000, 10) as c2:
+            cb, rb, stb = meb.meb_solve(c2, dC, dR, 1e-8, meb.MEB_MODE_FP64)
+    finally:
+        del os.environ["MEB_NO_SMALL"]
+    assert sta["converged"] == 1 and stb["converged"] == 1
+    assert abs(ra - rb) <= 1e-9 * rb and np.linalg.norm(ca.numpy() - cb.numpy()) <= 1e-6 * (1 + rb)
+    assert sta["kernel_launches"] < stb["kernel_launches"]

@@ -16,6 +16,7 @@
 //
 // Determinism: static stage -> warp assignment, per-lane / per-warp accumulation in a fixed order,
 // warps combined in index order, CTA partials combined in index order by the finalize kernel.
+#include <stdlib.h>
 #include <string.h>
 
 #include "meb_internal.cuh"
@@ -73,6 +74,7 @@ struct TileCfg {
     uint32_t off_tiles;    // byte offsets inside the dynamic shared memory
     uint32_t off_bars;
     uint32_t off_vec;
+    uint32_t smem_total;
 };
 
 // ---- the kernel ------------------------------------------------------------------------------------
@@ -456,9 +458,19 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
     for (const void* q : ptrs) if (q && !aligned16(q)) c.sc_tma = 0;
     const size_t cs_bytes = ((size_t)c.nch * 16 + 127) / 128 * 128;
     int W = 16, NS = 0;
+    const int want_ns = getenv("MEB_TILE_NS") ? atoi(getenv("MEB_TILE_NS")) : 2;     // tuning knobs (profiling only)
+    if (getenv("MEB_TILE_W")) W = atoi(getenv("MEB_TILE_W"));
+    if (getenv("MEB_TILE_R")) {
+        c.R = atoi(getenv("MEB_TILE_R"));
+        c.stage_rows = (uint32_t)(c.R * rpt);
+        c.off_u = c.stage_rows * c.row_bytes;
+        c.off_r = c.off_u + c.stage_rows * (uint32_t)esize;
+        c.off_slot = c.off_r + c.stage_rows * (uint32_t)esize;
+        c.stage_bytes = (c.off_slot + c.stage_rows * 4u + 127u) / 128u * 128u;
+    }
     for (; W >= 2; --W) {
-        const size_t fixed = cs_bytes + 16 * 4 * sizeof(uint64_t) + 256 + (size_t)W * 32 * cpl * sizeof(double);
-        if (fixed + (size_t)W * 2 * c.stage_bytes > TILE_SMEM_BUDGET) continue;
+        const size_t fixed = cs_bytes + 16 * 4 * sizeof(uint64_t) + 256;
+        if (fixed + (size_t)W * want_ns * c.stage_bytes > TILE_SMEM_BUDGET) continue;
         NS = (int)((TILE_SMEM_BUDGET - fixed) / ((size_t)W * c.stage_bytes));
         if (NS > 4) NS = 4;
         break;
@@ -467,12 +479,16 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
     c.W = W; c.NS = NS;
     c.off_tiles = (uint32_t)cs_bytes;
     c.off_bars = (uint32_t)(cs_bytes + (size_t)W * NS * c.stage_bytes);
-    c.off_vec = (uint32_t)((c.off_bars + (size_t)W * NS * sizeof(uint64_t) + 127) / 128 * 128);
+    c.off_vec = c.off_tiles;          // the per-warp vector partials reuse the stage ring (all stages consumed by then)
+    c.smem_total = (uint32_t)((c.off_bars + (size_t)W * NS * sizeof(uint64_t) + 127) / 128 * 128);
     *out = c;
     return true;
 }
 
-size_t cfg_smem(const TileCfg& c, int cpl) { return (size_t)c.off_vec + (size_t)c.W * 32 * cpl * sizeof(double); }
+size_t cfg_smem(const TileCfg& c, int cpl) {
+    const size_t vec_end = (size_t)c.off_vec + (size_t)c.W * 32 * cpl * sizeof(double);
+    return vec_end > c.smem_total ? vec_end : c.smem_total;
+}
 
 template <typename KernelT>
 int launch_cfg(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, size_t esize, int cpl, int* grid_out) {

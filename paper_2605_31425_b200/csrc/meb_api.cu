@@ -21,7 +21,7 @@ static void ctx_free_all(meb_ctx* c) {
     if (!c) return;
     cudaFree(c->mask); cudaFree(c->rec_lam); cudaFree(c->rec_rho); cudaFree(c->rec_t);
     cudaFree(c->list); cudaFree(c->blocksum); cudaFree(c->part_scalar); cudaFree(c->part_vec);
-    cudaFree(c->part_mat); cudaFree(c->count_dev); cudaFree(c->part_sc); cudaFree(c->small);
+    cudaFree(c->part_mat); cudaFree(c->part_red); cudaFree(c->count_dev); cudaFree(c->part_sc); cudaFree(c->small);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     for (int i = 0; i < 24; ++i) if (c->own[i]) cudaFree(c->own[i]);
     if (c->ev0) cudaEventDestroy(c->ev0);
@@ -93,6 +93,7 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     TRY_ALLOC(c->blocksum, nseg * sizeof(int32_t));
     TRY_ALLOC(c->part_scalar, (size_t)MEB_MAX_GRID * MEB_NPART * sizeof(double));
     TRY_ALLOC(c->part_vec, (size_t)c->vec_rows * dpad * sizeof(double));
+    TRY_ALLOC(c->part_red, dpad * sizeof(double));
     {
         const size_t dpm = (size_t)((d_max < 128 ? d_max : 128) + 15) / 16 * 16;
         c->part_mat_len = (size_t)c->vec_rows * (dpm * dpm + dpm);

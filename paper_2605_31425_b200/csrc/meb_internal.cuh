@@ -32,6 +32,7 @@ struct meb_ctx {
     int32_t* blocksum;      // [nseg + 2] per-segment popcounts of the compaction; [nseg] = total
     double* part_scalar;    // [MEB_MAX_GRID * MEB_NPART] per-CTA scalar partials
     double* part_vec;       // [vec_rows * (d_max+8)] per-CTA vector partials of the list kernels
+    double* part_red;       // [d_max+8] sum of the vector partials (long vectors, meb_small.cu)
     int64_t vec_rows;
     double* part_mat;       // per-CTA partial matrices of the dense-Hessian SYRK
     size_t part_mat_len;
@@ -136,6 +137,7 @@ struct StreamArgs {
     double eps; const uint8_t* kept; uint8_t* flags_out;
     // ingest
     float* C32; int64_t ld32; float* R32; const double* c0;
+    int32_t rt_shift;            // loop kernel: rows per warp tile = 1 << rt_shift (5, 4 or 3; set by the launcher)
     // fused evaluation (meb_tile.cu): per-CTA partial of sum_i lam_i b_i, [grid][dpad]
     double* part_vec; int32_t dpad;
     // device-resident parameters (solve graph): if dyn != nullptr it overrides sigma, U, v_slot, V

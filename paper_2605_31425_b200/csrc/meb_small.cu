@@ -137,11 +137,11 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
 __global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
     const double* __restrict__ part_vec, int nvec, int tpb, const int32_t* __restrict__ count, int dpad,
     const double* __restrict__ part_sc, const double* __restrict__ ev, const double* __restrict__ q,
-    double sigma, double tau, int d, double* __restrict__ Hq, const MebDyn* __restrict__ dyn) {
+    double sigma, double tau, int d, double* __restrict__ Hq, const MebDyn* __restrict__ dyn, int nsc) {
     if (dyn) { sigma = dyn->sigma_raw; tau = dyn->tau_eff; }
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
-    { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
+    if (tpb > 0) { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
     for (int j = threadIdx.x; j < d; j += FBLOCK) {
         double s = 0.0;
         for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
@@ -150,9 +150,32 @@ __global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
     }
     if (threadIdx.x < 32) {
         double s = 0.0;
-        for (int b = threadIdx.x; b < nvec; b += 32) s += part_sc[b];
+        for (int b = threadIdx.x; b < nsc; b += 32) s += part_sc[b];     // CTAs without list entries wrote 0
         s = warp_sum(s);
         if (threadIdx.x == 0) Hq[0] = tos * q[0] + sigma * (n1 * q[0] + 0.5 * (n3 * q[0] + s));
+    }
+}
+
+// Long vectors (d > 1024): the per-CTA vector partials are first added by MANY CTAs (32 columns each, the 8
+// warps of a CTA take interleaved partials and are then added in warp order: fixed order), so that the
+// single-CTA finalize kernels read one vector instead of nvec of them.
+__global__ void __launch_bounds__(256) reduce_partials_kernel(const double* __restrict__ part_vec, int nvec, int tpb,
+                                                              const int32_t* __restrict__ count, int dpad, int d,
+                                                              double* __restrict__ out) {
+    __shared__ double sm[8][32];
+    if (tpb > 0) { const int used = (*count + tpb - 1) / tpb; if (nvec > used) nvec = used; }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int j = blockIdx.x * 32 + lane;
+    double s = 0.0;
+    if (j < d)
+        for (int b = warp; b < nvec; b += 8) s += part_vec[(size_t)b * dpad + j];
+    sm[warp][lane] = s;
+    __syncthreads();
+    if (warp == 0 && j < d) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) t += sm[w][lane];
+        out[j] = t;
     }
 }
 
@@ -269,7 +292,14 @@ __global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint
 }  // namespace
 
 // ---- host wrappers ---------------------------------------------------------------------------------
-int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f) {
+int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f_in) {
+    FinalizeArgs f = f_in;
+    if (f.d > FBLOCK && f.nvec > 1) {              // long vectors: add the partials with many CTAs first
+        ctx->launches++;
+        reduce_partials_kernel<<<(f.d + 31) / 32, 256, 0, ctx->stream>>>(f.part_vec, f.nvec, f.tpb, f.count, f.dpad, f.d,
+                                                                        ctx->part_red);
+        f.part_vec = ctx->part_red; f.nvec = 1; f.tpb = 0;
+    }
     ctx->launches++; eval_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(f);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
@@ -277,9 +307,17 @@ int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f) {
 
 int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
                      const double* q, double sigma, double tau, int d, double* Hq, const MebDyn* dyn) {
-    const int tpb = d > 2048 ? 1 : MEB_WARPS;
-    ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(ctx->part_vec, nvec, tpb, ctx->count_dev, dpad, part_sc, ev, q, sigma, tau,
-                                                       d, Hq, dyn);
+    int tpb = d > 2048 ? 1 : MEB_WARPS;
+    const double* pv = ctx->part_vec;
+    int nv = nvec;
+    if (d > FBLOCK && nvec > 1) {                  // long vectors: add the partials with many CTAs first
+        ctx->launches++;
+        reduce_partials_kernel<<<(d + 31) / 32, 256, 0, ctx->stream>>>(ctx->part_vec, nvec, tpb, ctx->count_dev, dpad, d,
+                                                                      ctx->part_red);
+        pv = ctx->part_red; nv = 1;
+    }
+    ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(pv, nv, nv == 1 && pv == ctx->part_red ? 0 : tpb, ctx->count_dev, dpad,
+                                                       part_sc, ev, q, sigma, tau, d, Hq, dyn, nvec);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -182,16 +182,19 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
     for (int j = threadIdx.x; j < nchunks * VEC; j += MEB_BLOCK) cs[j] = j < d ? (T)cptr[j] : T(0);
     __syncthreads();
 
-    const int64_t ntiles = (m + 31) >> 5;
+    // rows per warp tile: 32, or 16 / 8 when there are too few rows to occupy the GPU with 32-row tiles
+    const int rts = a.rt_shift ? a.rt_shift : 5;
+    const int RT = 1 << rts;
+    const int64_t ntiles = (m + RT - 1) >> rts;
     const int64_t stride = (int64_t)gridDim.x * MEB_WARPS;
     for (int64_t tile = (int64_t)blockIdx.x * MEB_WARPS + warp; tile < ntiles; tile += stride) {
-        const int64_t row0 = tile << 5;
+        const int64_t row0 = tile << rts;
         const int64_t myrow = row0 + lane;
-        const bool myvalid = myrow < m;
+        const bool myvalid = lane < RT && myrow < m;
         int myslot = -1;
         if (HASV && myvalid) myslot = a.v_slot[myrow];
         T my_nb2 = T(0), my_ne2 = T(0), my_ev = T(0), my_vv = T(0);
-        for (int it = 0; it < 32; ++it) {
+        for (int it = 0; it < RT; ++it) {
             const int64_t row = row0 + it;
             if (row >= m) break;                       // warp-uniform
             const T* rowp = C + row * a.ld;
@@ -260,7 +263,11 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
                                               my_vv, r, sig, acc);
         if (OP != OP_INGEST) {
             const uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);
-            if (lane == 0) a.mask[tile] = bits;
+            if (lane == 0) {
+                if (rts == 5) a.mask[tile] = bits;
+                else if (rts == 4) reinterpret_cast<uint16_t*>(a.mask)[tile] = (uint16_t)bits;
+                else reinterpret_cast<uint8_t*>(a.mask)[tile] = (uint8_t)bits;
+            }
         }
     }
     block_reduce_store<OP>(acc, a.part);
@@ -278,7 +285,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
 namespace {
 
 template <typename KernelT>
-int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_out, size_t smem = 0) {
+int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_out, size_t smem = 0, bool loop_kernel = false) {
     if (smem > 220 * 1024) return MEB_E_CAPACITY;            // centre does not fit in shared memory (d > ~28,000)
     int occ = 0;
     cudaError_t e = cudaSuccess;
@@ -286,13 +293,20 @@ int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_ou
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, MEB_BLOCK, smem);
     if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
     if (occ < 1) occ = 1;
-    const int64_t ntiles = (a.m + 31) / 32;
+    StreamArgs b = a;
+    int64_t ntiles = (a.m + 31) / 32;
+    if (loop_kernel) {               // few long rows: smaller warp tiles so that every SM gets rows
+        const int64_t full = (int64_t)ctx->sm_count * occ * MEB_WARPS;
+        b.rt_shift = 5;
+        if (ntiles < 2 * full) b.rt_shift = 4;
+        if ((a.m + 15) / 16 < 2 * full) b.rt_shift = 3;
+        ntiles = (a.m + (1 << b.rt_shift) - 1) >> b.rt_shift;
+    }
     int64_t want = (ntiles + MEB_WARPS - 1) / MEB_WARPS;
     int64_t cap = (int64_t)ctx->sm_count * occ;          // one resident wave, grid-stride inside
     if (cap > MEB_MAX_GRID) cap = MEB_MAX_GRID;
     int grid = (int)(want < cap ? want : cap);
     if (grid < 1) grid = 1;
-    StreamArgs b = a;
     ctx->launches++; kernel<<<grid, MEB_BLOCK, smem, ctx->stream>>>(b);
     e = cudaGetLastError();
     if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
@@ -303,7 +317,7 @@ int launch_sized(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, int* grid_ou
 template <typename T, int OP, bool SHADOW>
 int dispatch_shape(meb_ctx* ctx, const StreamArgs& a, bool aligned, int* grid_out) {
     constexpr int VEC = VecOf<T>::N;
-    if (!aligned) return launch_sized(ctx, stream_loop_kernel<T, 1, OP, SHADOW>, a, grid_out, ((size_t)a.d * sizeof(T) + 15) / 16 * 16);
+    if (!aligned) return launch_sized(ctx, stream_loop_kernel<T, 1, OP, SHADOW>, a, grid_out, ((size_t)a.d * sizeof(T) + 15) / 16 * 16, true);
     const int nchunks = (a.d + VEC - 1) / VEC;
     if (nchunks <= 4)   return launch_sized(ctx, stream_tile_kernel<T, 4, 1, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 8)   return launch_sized(ctx, stream_tile_kernel<T, 4, 2, VEC, OP, SHADOW>, a, grid_out);
@@ -313,7 +327,7 @@ int dispatch_shape(meb_ctx* ctx, const StreamArgs& a, bool aligned, int* grid_ou
     if (nchunks <= 128) return launch_sized(ctx, stream_tile_kernel<T, 16, 8, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 256) return launch_sized(ctx, stream_tile_kernel<T, 32, 8, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 512) return launch_sized(ctx, stream_tile_kernel<T, 32, 16, VEC, OP, SHADOW>, a, grid_out);
-    return launch_sized(ctx, stream_loop_kernel<T, VEC, OP, SHADOW>, a, grid_out, (size_t)nchunks * 16);
+    return launch_sized(ctx, stream_loop_kernel<T, VEC, OP, SHADOW>, a, grid_out, (size_t)nchunks * 16, true);
 }
 
 template <typename T>

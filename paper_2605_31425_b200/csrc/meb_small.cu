@@ -294,7 +294,7 @@ __global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint
 // ---- host wrappers ---------------------------------------------------------------------------------
 int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f_in) {
     FinalizeArgs f = f_in;
-    if (f.d > FBLOCK && f.nvec > 1) {              // long vectors: add the partials with many CTAs first
+    if (f.d > 256 && f.nvec > 8) {                 // long vectors: add the partials with many CTAs first
         ctx->launches++;
         reduce_partials_kernel<<<(f.d + 31) / 32, 256, 0, ctx->stream>>>(f.part_vec, f.nvec, f.tpb, f.count, f.dpad, f.d,
                                                                         ctx->part_red);
@@ -310,7 +310,7 @@ int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, co
     int tpb = d > 2048 ? 1 : MEB_WARPS;
     const double* pv = ctx->part_vec;
     int nv = nvec;
-    if (d > FBLOCK && nvec > 1) {                  // long vectors: add the partials with many CTAs first
+    if (d > 128 && nvec > 8) {                     // long vectors: add the partials with many CTAs first
         ctx->launches++;
         reduce_partials_kernel<<<(d + 31) / 32, 256, 0, ctx->stream>>>(ctx->part_vec, nvec, tpb, ctx->count_dev, dpad, d,
                                                                       ctx->part_red);

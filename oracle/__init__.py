@@ -26,5 +26,7 @@ Pins (tests/test_oracle_*.py, ``-m "not gpu"``): closed forms, brute force in d=
 finite differences, Moreau decomposition, weak-duality certificate, Table 1 of the paper.
 Parity unpinned (items 3-5 and 10-12): the solver's free constants
 (rho, sigma_0, kappa, tau, Armijo constants, CG tolerance, caps).  They change the
-iteration path, not the answer; the answer is pinned.
+iteration path, not the answer; the answer is pinned.  The CUDA path additionally has two
+safeguards the oracle does not need at test sizes (DESIGN readings 17 and 18: a capped
+low-precision run, best-iterate / stall logic); they too change the path only.
 """

@@ -17,7 +17,8 @@
  *    (HOST pointer owned by the caller).  The library never frees or keeps a caller pointer
  *    beyond the call.  The context owns all workspace and the stream handle it was given.
  *  - Layout ("structure of arrays"): centres C row-major, row i at C + i*ld, ld >= d
- *    elements; radii R[m] (NULL = points, all r_i = 0); multipliers U[m] and sparse V:
+ *    elements (all m*ld elements must be readable: rows are fetched in whole 16-byte units, the padding
+ *    values are ignored); radii R[m] (NULL = points, all r_i = 0); multipliers U[m] and sparse V:
  *    v_slot[i] >= 0 is the row of ball i in Vrows (row stride ldv), v_slot[i] < 0 means v_i = 0;
  *    v_slot == NULL means all v_i = 0.  A dense V (the paper's layout) is v_slot[i] = i.
  *    (u_i = 0 implies v_i = 0 because multipliers are projections onto Q.)

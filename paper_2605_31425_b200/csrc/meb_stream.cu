@@ -326,7 +326,8 @@ int dispatch_shape(meb_ctx* ctx, const StreamArgs& a, bool aligned, int* grid_ou
     if (nchunks <= 64)  return launch_sized(ctx, stream_tile_kernel<T, 8, 8, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 128) return launch_sized(ctx, stream_tile_kernel<T, 16, 8, VEC, OP, SHADOW>, a, grid_out);
     if (nchunks <= 256) return launch_sized(ctx, stream_tile_kernel<T, 32, 8, VEC, OP, SHADOW>, a, grid_out);
-    if (nchunks <= 512) return launch_sized(ctx, stream_tile_kernel<T, 32, 16, VEC, OP, SHADOW>, a, grid_out);
+    // rows longer than 256 chunks (4 KB): the warp-per-row loop kernel (centre in shared memory, 8 loads in
+    // flight per lane) beats a 16-chunks-per-lane register tile, which needs ~250 registers (one CTA per SM)
     return launch_sized(ctx, stream_loop_kernel<T, VEC, OP, SHADOW>, a, grid_out, (size_t)nchunks * 16, true);
 }
 

@@ -251,29 +251,45 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                     const V4* vrow4 = reinterpret_cast<const V4*>(Vg + (int64_t)myslot * a.ldv);
                     const V4* rp = reinterpret_cast<const V4*>(rowp);
                     const bool v16 = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
-                    for (int c = g; c < nch; c += G) {
-                        const V4 ev4 = rp[c];
-                        const V4 cv4 = cs4[c];
-                        V4 vv4;
-                        T* vq = reinterpret_cast<T*>(&vv4);
-                        const int col = c * VEC;
-                        if (v16) {
-                            vv4 = __ldg(vrow4 + c);
-                        } else {
+                    // my chunks g, g + G, ...: the V loads of a batch of 8 are issued together (one exposed latency
+                    // per batch instead of one per chunk), then the arithmetic runs on registers
+                    for (int k0 = 0; k0 < n_g; k0 += 8) {
+                        V4 vb[8];
 #pragma unroll
-                            for (int j = 0; j < VEC; ++j) vq[j] = (col + j < d) ? __ldg(Vg + (int64_t)myslot * a.ldv + col + j) : T(0);
+                        for (int u = 0; u < 8; ++u) {
+                            const int c = g + ((k0 + u) << LG);
+                            if (k0 + u < n_g) {
+                                if (v16) {
+                                    vb[u] = __ldg(vrow4 + c);
+                                } else {
+                                    T* vq = reinterpret_cast<T*>(&vb[u]);
+#pragma unroll
+                                    for (int j = 0; j < VEC; ++j)
+                                        vq[j] = (c * VEC + j < d) ? __ldg(Vg + (int64_t)myslot * a.ldv + c * VEC + j) : T(0);
+                                }
+                            }
                         }
-                        const T* e = reinterpret_cast<const T*>(&ev4);
-                        const T* cc = reinterpret_cast<const T*>(&cv4);
 #pragma unroll
-                        for (int j = 0; j < VEC; ++j) {
-                            const T ee = e[j] - cc[j];                   // padding of the row was zeroed above
-                            const T v = (col + j < d) ? vq[j] : T(0);    // padding of the pool row is not
-                            const T b = fma(v, inv_sig, ee);
-                            nb2 = fma(b, b, nb2);
-                            ne2 = fma(ee, ee, ne2);
-                            evd = fma(ee, v, evd);
-                            vv = fma(v, v, vv);
+                        for (int u = 0; u < 8; ++u) {
+                            const int c = g + ((k0 + u) << LG);
+                            if (k0 + u < n_g) {
+                                const V4 ev4 = rp[c];
+                                const V4 cv4 = cs4[c];
+                                const T* e = reinterpret_cast<const T*>(&ev4);
+                                const T* cc = reinterpret_cast<const T*>(&cv4);
+                                const T* vq = reinterpret_cast<const T*>(&vb[u]);
+                                const int col = c * VEC;
+#pragma unroll
+                                for (int j = 0; j < VEC; ++j) {
+                                    const T ee = e[j] - cc[j];                   // padding of the row was zeroed above
+                                    const T v = (col + j < d) ? vq[j] : T(0);    // padding of the pool row is not
+                                    const T bq = fma(v, inv_sig, ee);
+                                    nb2 = fma(bq, bq, nb2);
+                                    ne2 = fma(ee, ee, ne2);
+                                    evd = fma(ee, v, evd);
+                                    vv = fma(v, v, vv);
+                                }
+                            }
                         }
                     }
                 }
@@ -304,37 +320,51 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                 }
                 if (OP == OP_EVAL) {
                     // gradient vector part: sum over the ACTIVE rows of lam_i b_i, from shared memory
-                    while (bits) {
-                        const int ls = __ffs(bits) - 1;                  // lane that owns the row
-                        bits &= bits - 1;
-                        const double lam = __shfl_sync(MEB_FULL_MASK, mylam, ls);
-                        const int slot = HASV ? __shfl_sync(MEB_FULL_MASK, myslot, ls) : -1;
-                        const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + (ls >> LG)) * ldT);
+                    const bool v16a = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
+                    while (bits) {                                       // four active rows per round: their V loads overlap
+                        int ls4[4], sl4[4];
+                        double lam4[4];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const bool ok = bits != 0;
+                            const int ls = ok ? __ffs(bits) - 1 : 0;     // lane that owns the row
+                            if (ok) bits &= bits - 1;
+                            const double lam = __shfl_sync(MEB_FULL_MASK, mylam, ls);
+                            const int slot = HASV ? __shfl_sync(MEB_FULL_MASK, myslot, ls) : -1;
+                            ls4[u] = ls; lam4[u] = ok ? lam : 0.0; sl4[u] = ok ? slot : -1;
+                        }
 #pragma unroll
                         for (int q = 0; q < CH; ++q) {
                             const int ch = lane + 32 * q;
                             if (ch < nch) {
-                                const V4 ev4 = rp4[ch];
-                                const T* e = reinterpret_cast<const T*>(&ev4);
-                                T b[VEC];
+                                V4 vb[4];
 #pragma unroll
-                                for (int j = 0; j < VEC; ++j) b[j] = e[j] - creg[q][j];
-                                if (slot >= 0) {
-                                    const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
-                                    if ((a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0) {
-                                        const V4 vv4 = __ldg(reinterpret_cast<const V4*>(vrow));
-                                        const T* vq = reinterpret_cast<const T*>(&vv4);
+                                for (int u = 0; u < 4; ++u) {
+                                    if (sl4[u] >= 0) {
+                                        const T* vrow = Vg + (int64_t)sl4[u] * a.ldv + ch * VEC;
+                                        if (v16a) {
+                                            vb[u] = __ldg(reinterpret_cast<const V4*>(vrow));
+                                        } else {
+                                            T* vq = reinterpret_cast<T*>(&vb[u]);
 #pragma unroll
-                                        for (int j = 0; j < VEC; ++j)
-                                            if (ch * VEC + j < d) b[j] = fma(vq[j], inv_sig, b[j]);
-                                    } else {
-#pragma unroll
-                                        for (int j = 0; j < VEC; ++j)
-                                            if (ch * VEC + j < d) b[j] = fma(__ldg(vrow + j), inv_sig, b[j]);
+                                            for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
+                                        }
                                     }
                                 }
 #pragma unroll
-                                for (int j = 0; j < VEC; ++j) vacc[q][j] = fma(lam, (double)b[j], vacc[q][j]);
+                                for (int u = 0; u < 4; ++u) {
+                                    if (lam4[u] != 0.0) {
+                                        const V4 ev4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + (ls4[u] >> LG)) * ldT)[ch];
+                                        const T* e = reinterpret_cast<const T*>(&ev4);
+                                        const T* vq = reinterpret_cast<const T*>(&vb[u]);
+#pragma unroll
+                                        for (int j = 0; j < VEC; ++j) {
+                                            T bj = e[j] - creg[q][j];
+                                            if (sl4[u] >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
+                                            vacc[q][j] = fma(lam4[u], (double)bj, vacc[q][j]);
+                                        }
+                                    }
+                                }
                             }
                         }
                     }
@@ -511,7 +541,7 @@ int launch_cfg(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, size_t esize, 
 
 int lanes_per_row(const StreamArgs& a, size_t esize) {
     const size_t rb = (size_t)a.ld * esize;
-    return rb <= 208 ? 1 : (rb <= 416 ? 2 : 4);              // sub-tile of at most ~6.5 KB
+    return rb <= 256 ? 1 : (rb <= 416 ? 2 : 4);              // sub-tile of at most ~8 KB
 }
 
 // G is fixed by the row length; CH = 2 only occurs with G = 4 (rows longer than 512 bytes)

@@ -142,6 +142,8 @@ def oracle_solve_sample(k, m, d, mode, m_s):
 
 
 def cpu_threads():
+    """Threads available to the oracle's numpy (its BLAS calls may use them; its elementwise passes,
+    which dominate, run on one thread)."""
     try:
         from threadpoolctl import threadpool_info
         n = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
@@ -168,7 +170,8 @@ def run_reference(args, rank, world):
     per = sum(times) / len(times)
     scaled = per * (m / m_s)
     sample = (f"first {m_s} of {m} balls of the same seeded instance, {per:.3f} s per solve measured, "
-              f"scaled x{m / m_s:.1f} to m (cost per pass is linear in m)")
+              f"scaled x{m / m_s:.1f} to m (cost per pass is linear in m); numpy: elementwise passes on 1 thread, "
+              f"BLAS calls on up to `cores` threads")
     line = {"impl": "reference", "metric": METRIC, "value": scaled, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": scaled * 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -346,7 +349,8 @@ def run_b200(args, rank, world, local_rank):
         dt, r_o, _ = oracle_solve_sample(k, m, d, args.mode, m_s)
         line["cpu_baseline"] = {"value": dt * (m / m_s), "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
                                 "sample": f"first {m_s} of {m} balls of the same seeded instance: {dt:.3f} s "
-                                          f"measured, scaled x{m / m_s:.1f} (cost per pass is linear in m)"}
+                                          f"measured, scaled x{m / m_s:.1f} (cost per pass is linear in m); numpy: elementwise "
+                                          f"passes on 1 thread, BLAS calls on up to `cores` threads"}
     ctx.close()
     if rank == 0:
         print(json.dumps(line), flush=True)

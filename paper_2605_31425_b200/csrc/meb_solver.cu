@@ -22,7 +22,7 @@
 namespace {
 
 enum { OWN_U0 = 0, OWN_U1, OWN_S0, OWN_S1, OWN_V0, OWN_V1, OWN_C32, OWN_R32, OWN_IDX, OWN_CRED, OWN_RRED,
-       OWN_KEPT, OWN_STATE, OWN_HOSTC, OWN_HOSTR, OWN_SPARE, OWN_VRED0, OWN_VRED1 };
+       OWN_KEPT, OWN_STATE, OWN_HOSTC, OWN_HOSTR, OWN_SPARE, OWN_VRED0, OWN_VRED1, OWN_DEVC, OWN_DEVR };
 
 int own_reserve(meb_ctx* ctx, int slot, size_t bytes) {
     if (ctx->own_bytes[slot] >= bytes && ctx->own[slot]) return MEB_OK;
@@ -812,23 +812,14 @@ extern "C" int meb_solve_host(meb_ctx* ctx, int64_t m, int32_t d, const double* 
                               double* h_center_out, double* h_radius_out, meb_stats* h_stats) {
     if (!ctx || !h_centers || m < 1 || d < 1 || ld < d) return MEB_E_ARG;
     if (m > ctx->m_max || d > ctx->d_max) return MEB_E_CAPACITY;
-    // device copies owned by the context (slots reused across calls)
-    static const int OWN_DC = 14, OWN_DR = 15;
-    (void)OWN_DR;
-    void* dC = nullptr; void* dR = nullptr;
-    cudaError_t e = cudaMalloc(&dC, (size_t)m * ld * sizeof(double));
-    if (e == cudaSuccess && h_radii) e = cudaMalloc(&dR, (size_t)m * sizeof(double));
-    if (e != cudaSuccess) { cudaGetLastError(); if (dC) cudaFree(dC); return MEB_E_ALLOC; }
-    (void)OWN_DC;
-    e = cudaMemcpyAsync(dC, h_centers, (size_t)m * ld * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess && h_radii)
-        e = cudaMemcpyAsync(dR, h_radii, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
-    int rc;
-    if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; rc = MEB_E_CUDA; }
-    else rc = meb_solve(ctx, m, d, (const double*)dC, ld, (const double*)dR, tol, precision_mode, h_params,
-                        h_center_out, h_radius_out, h_stats);
-    cudaStreamSynchronize(ctx->stream);
-    cudaFree(dC);
-    if (dR) cudaFree(dR);
-    return rc;
+    // device copies owned by the context (reused across calls: no allocation in the steady state)
+    int rc = own_reserve(ctx, OWN_DEVC, (size_t)m * ld * sizeof(double));
+    if (rc == MEB_OK && h_radii) rc = own_reserve(ctx, OWN_DEVR, (size_t)m * sizeof(double));
+    if (rc != MEB_OK) return rc;
+    double* dC = (double*)ctx->own[OWN_DEVC];
+    double* dR = h_radii ? (double*)ctx->own[OWN_DEVR] : nullptr;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(dC, h_centers, (size_t)m * ld * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    if (h_radii)
+        MEB_CUDA_OK(ctx, cudaMemcpyAsync(dR, h_radii, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    return meb_solve(ctx, m, d, dC, ld, dR, tol, precision_mode, h_params, h_center_out, h_radius_out, h_stats);
 }

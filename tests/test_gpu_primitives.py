@@ -335,3 +335,26 @@ def test_small_solver_and_graph_agree(meb):
     assert sta["converged"] == 1 and stb["converged"] == 1
     assert abs(ra - rb) <= 1e-9 * rb and np.linalg.norm(ca.numpy() - cb.numpy()) <= 1e-6 * (1 + rb)
     assert sta["kernel_launches"] < stb["kernel_launches"]
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+def test_eval_alm_unaligned_scalar_arrays(meb, ctx, prec):
+    """R, U and the slot map start at addresses that are not multiples of 16 bytes: the tile kernel must
+    then read them from global memory instead of staging them with bulk copies (same results)."""
+    m, d = 3001, 100
+    C, R, U, V, x, xbar = make_state(911, m, d)
+    if prec == 1:
+        C = C.astype(np.float32).astype(np.float64); U = U.astype(np.float32).astype(np.float64)
+        V = V.astype(np.float32).astype(np.float64); R = R.astype(np.float32).astype(np.float64)
+    Cd, Rd, Ud, slot, Vr = to_device(C, R, U, V, THDT[prec], "sparse")
+    ref = meb.meb_eval_alm(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), dvec(xbar), 2.0, 0.5, per_ball=True)
+
+    def shifted(t):
+        buf = torch.empty(t.numel() + 1, dtype=t.dtype, device=t.device)
+        buf[1:].copy_(t)
+        return buf[1:]
+    Rs, Us, Ss = shifted(Rd), shifted(Ud), shifted(slot)
+    assert Rs.data_ptr() % 16 != 0 and Ss.data_ptr() % 16 != 0
+    got = meb.meb_eval_alm(ctx, prec, Cd, Rs, Us, Ss, Vr, dvec(x), dvec(xbar), 2.0, 0.5, per_ball=True)
+    assert torch.equal(ref["scalars"], got["scalars"]) and torch.equal(ref["grad"], got["grad"])
+    assert torch.equal(ref["t"], got["t"]) and torch.equal(ref["lam"], got["lam"])

@@ -86,6 +86,9 @@ typedef struct meb_params {
     int32_t max_rounds;         /* active-set refinement rounds               10   */
     int32_t sample_rows;        /* rows whose mean is the initial centre c^0               1024 */
     int32_t outer_max_lo;       /* outer iterations of the low-precision run (reading 17)     30   */
+    double armijo_shrink_min;   /* a rejected Armijo trial halves eta, or multiplies it by this factor when the
+                                 * parabola through Psi(x), Psi'(x; Delta), Psi(x + eta Delta) puts its minimiser
+                                 * below it (trials bound to fail are skipped); 0.5 = plain halving (reading 4)  0.5  */
 } meb_params;
 
 /* Counters and residuals of one meb_solve (host struct). */

@@ -38,7 +38,7 @@ class meb_params(C.Structure):
                 ("tol_lo", C.c_double), ("tol_red_factor", C.c_double),
                 ("armijo_max_halvings", C.c_int32), ("cg_max", C.c_int32), ("dense_d_max", C.c_int32),
                 ("inner_max", C.c_int32), ("outer_max", C.c_int32), ("max_rounds", C.c_int32),
-                ("sample_rows", C.c_int32), ("outer_max_lo", C.c_int32)]
+                ("sample_rows", C.c_int32), ("outer_max_lo", C.c_int32), ("armijo_shrink_min", C.c_double)]
 
 
 class meb_stats(C.Structure):

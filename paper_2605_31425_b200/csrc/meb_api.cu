@@ -59,6 +59,7 @@ extern "C" void meb_default_params(meb_params* p) {
     if (!p) return;
     memset(p, 0, sizeof(*p));
     p->rho = 0.5; p->sigma0 = 1.0; p->kappa = 3.0; p->sigma_max = 1e8; p->tau = 1.0;
+    p->armijo_shrink_min = 0.5;
     p->armijo_mu = 1e-4; p->tol_lo = 1e-2; p->tol_red_factor = 0.02;
     p->armijo_max_halvings = 30; p->cg_max = 500; p->dense_d_max = 128; p->inner_max = 50;
     p->outer_max = 200; p->max_rounds = 10; p->sample_rows = 1024; p->outer_max_lo = 30;

@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(CBLK) ctrl_init_kernel(SolverDev* S, const Sol
         S->phase = PH_FIRST; S->action = ACT_TRIAL;
         S->outer = 0; S->inner = 0; S->ls = 0; S->done = 0; S->status = ST_RUNNING; S->stalled = 0;
         S->newton_total = 0; S->cg_total = 0; S->evals = 0; S->chol_info = 0;
-        S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0;
+        S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0; S->tiny = 0;
         S->pass_ns = 0ull; S->pass_count = 0; S->vrow_reads = 0ull;
         S->eta = 1.0; S->psi_cur = 0.0; S->slope = 0.0;
         S->cg_go = 0; S->cg_it = 0;
@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(CBLK) ctrl_after_newton_kernel(SolverDev* S, c
     ctrl_to_raw(S, v, v.xt, v.x_raw);
     if (threadIdx.x == 0) {
         S->slope = sl;
+        S->tiny = (-sl <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;
         S->eta = 1.0;
         S->ls = 0;
         S->phase = PH_ARMIJO;

@@ -18,7 +18,8 @@ enum { ST_RUNNING = 0, ST_CONVERGED = 1, ST_OUTER_CAP = 2, ST_NEED_CAPACITY = 3,
 
 struct SolverDev {
     // ---- constants of the phase (written by the host before the graph is launched) ----
-    double L, tol, rho, tau, kappa, sigma_max, armijo_mu;
+    double L, tol, rho, tau, kappa, sigma_max, armijo_mu, shrink_min;
+    double slope_floor;           // Newton decrement below slope_floor |Psi|: Psi cannot resolve the predicted decrease (reading 6)
     int32_t n, d, inner_max, outer_max, armijo_max, cg_max, dense, use_off;
     int64_t vcap[2];              // rows available in the two V pools
     // ---- dynamic ----
@@ -38,7 +39,8 @@ struct SolverDev {
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
     double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
-    int32_t stall_count, pad2;
+    int32_t stall_count, tiny;    // tiny: the last Newton direction had a decrement below the floor
+    uint32_t pass_hist[48], act_hist[48];   // MEB_TRACE: ns and active balls of the first evaluation passes
     int32_t in_graph, eval_cap;   // eval_cap: hard bound on the evaluations of a phase (a runaway loop cannot hang the GPU)
 };
 
@@ -135,7 +137,7 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     bool accept = true, stalled = false;
     if (phase == PH_ARMIJO) {
         if (!(psi_t <= S->psi_cur + S->armijo_mu * S->eta * S->slope)) {
-            if (S->ls >= S->armijo_max) {
+            if (S->ls >= S->armijo_max || S->tiny) {
                 stalled = true;
                 accept = psi_t <= S->psi_cur;          // last trial did not increase Psi: take it
             } else {
@@ -146,7 +148,15 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     if (!accept) {
         // rejected trial: either halve the step (next trial x + eta Delta) or, when the halvings are
         // exhausted, re-evaluate at x (the records of this pass are not those of x)
-        const double eta = stalled ? 0.0 : 0.5 * S->eta;
+        // shortened step: eta / 2, except after a trial so far off that the parabola through Psi(x),
+        // Psi'(x; Delta) = slope and Psi(x + eta Delta) has its minimiser below shrink_min * eta: then the
+        // trials in between are skipped (shrink_min = 1/2: plain halving; 1/8 keeps eta on the halving grid); reading 4
+        double eta = 0.0;
+        if (!stalled) {
+            const double den = psi_t - S->psi_cur - S->slope * S->eta;      // > 0 whenever the Armijo test fails
+            const double fq = -0.5 * S->slope * S->eta / den;
+            eta = ((fq < S->shrink_min) ? S->shrink_min : 0.5) * S->eta;    // a NaN trial value halves
+        }
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
             const double xj = v.xn[j] + eta * v.delta[j];
             v.xt[j] = xj;
@@ -191,7 +201,7 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         const double sg = S->sigma;
         const double lhs = 2.0 * sg * fabs(agx) + sg * sg * gg;
         const double rhs = S->rho * (ev_s[MEB_EV_SUM_DMULT2] + S->tau * dx2);
-        const bool exit_inner = (phase == PH_REEVAL) || stalled || lhs <= rhs || kkt <= S->tol ||
+        const bool exit_inner = (phase == PH_REEVAL) || stalled || (phase == PH_ARMIJO && S->tiny) || lhs <= rhs || kkt <= S->tol ||
                                 S->inner >= S->inner_max;
         if (exit_inner) {
             S->action = ACT_UPDATE;
@@ -241,6 +251,7 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
         double t = 0.0;
         for (int w = 0; w < 8; ++w) t += red[w];
         S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
+        S->tiny = (-t <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;
     }
 }
 

@@ -105,7 +105,10 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
     if (threadIdx.x == 0) {
         if (f.S) {
             const long long t0 = __double_as_longlong(sm[100]), t1 = __double_as_longlong(sm[101]);
-            if (t1 > t0) { sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++; }
+            if (t1 > t0) {
+                if (sS.pass_count < 48) { sS.pass_hist[sS.pass_count] = (uint32_t)(t1 - t0); sS.act_hist[sS.pass_count] = (uint32_t)(sc[3] + sc[4]); }
+                sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++;
+            }
         }
         double* out = ev_s;
         const double dx0 = x[0] - (xbar ? xbar[0] : x[0]);

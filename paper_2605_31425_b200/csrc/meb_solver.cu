@@ -301,6 +301,13 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
         if (rc) return rc;
         MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
         MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+        if (getenv("MEB_TRACE") && atoi(getenv("MEB_TRACE")) >= 2) {
+            double ev[MEB_EVAL_NSCALARS];
+            cudaMemcpy(ev, S.v.ev_t, sizeof(ev), cudaMemcpyDeviceToHost);
+            fprintf(stderr, "[meb trace]   eval %d outer %d inner %d -> action %d phase %d eta %.3g ls %d psi_t %.15g psi_cur %.15g slope %.3e kkt %.3e nact %.0f\n",
+                    h->evals, h->outer, h->inner, h->action, h->phase, h->eta, h->ls, ev[MEB_EV_PSI] / h->L, h->psi_cur, h->slope, h->kkt,
+                    ev[MEB_EV_N_ACTIVE]);
+        }
         if (h->done) return MEB_OK;
         if (h->action == ACT_NEWTON) {
             if (dense) {
@@ -435,6 +442,8 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             memset(h, 0, sizeof(*h));
             h->L = S.L; h->tol = tol; h->tol_accept = tol_accept; h->rho = par.rho; h->tau = par.tau; h->kappa = par.kappa;
             h->sigma_max = par.sigma_max; h->armijo_mu = par.armijo_mu;
+            h->shrink_min = (par.armijo_shrink_min > 0.0 && par.armijo_shrink_min <= 0.5) ? par.armijo_shrink_min : 0.5;
+            if (getenv("MEB_SHRINK_MIN")) h->shrink_min = atof(getenv("MEB_SHRINK_MIN"));
             h->n = n; h->d = S.d; h->inner_max = par.inner_max; h->outer_max = outer_cap;
             h->armijo_max = par.armijo_max_halvings; h->cg_max = par.cg_max; h->dense = dense ? 1 : 0;
             h->use_off = P.off ? 1 : 0;
@@ -442,6 +451,8 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
                 if (h->armijo_max > 12) h->armijo_max = 12;
                 if (h->inner_max > 20) h->inner_max = 20;
             }
+            h->slope_floor = (P.prec == MEB_FP32) ? 1e-7 : 2e-15;
+            if (getenv("MEB_SLOPE_FLOOR")) h->slope_floor = atof(getenv("MEB_SLOPE_FLOOR"));
             h->eval_cap = 4 * outer_cap * (par.inner_max + 2);
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
@@ -484,6 +495,11 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             continue;
         }
         // ---- phase finished ----
+        if (getenv("MEB_TRACE")) {
+            fprintf(stderr, "[meb trace] eval passes (ns / active):");
+            for (long long q = 0; q < h->pass_count && q < 48; ++q) fprintf(stderr, " %u/%u", h->pass_hist[q], h->act_hist[q]);
+            fprintf(stderr, "\n");
+        }
         S.st->outer_iters += h->outer;
         S.st->newton_iters += h->newton_total;
         S.st->cg_iters += h->cg_total;

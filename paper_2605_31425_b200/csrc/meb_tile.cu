@@ -70,6 +70,7 @@ struct TileCfg {
     uint32_t off_u, off_r, off_slot;   // byte offsets of the per-row scalars inside a stage
     int nch;               // 16-byte chunks that cover the d columns of a row
     int rot;               // 1: rotate the chunk order by the row index (bank conflicts)
+    int rowfast;           // 1: lane -> (row = lane % RPT, g = lane / RPT) instead of (row = lane / G, g = lane % G)
     int sc_tma;            // 1: per-row scalars come with the stage (their arrays are 16-byte aligned)
     uint32_t off_tiles;    // byte offsets inside the dynamic shared memory
     uint32_t off_bars;
@@ -100,7 +101,11 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
     const int d = a.d;
     const int m = (int)a.m;                                              // m < 2^31 - 64 (meb.h)
     const int W = cfg.W, NS = cfg.NS, R = cfg.R, nch = cfg.nch;
-    const int g = lane & (G - 1), rl = lane >> LG;
+    // lane -> (row of the sub-tile, which of the G interleaved chunk sets): the host picks the mapping whose
+    // quarter-warp LDS.128 wavefronts collide less for this row stride
+    const int xsh = cfg.rowfast ? 5 - LG : 0;                            // partner lanes of a row differ in bits xsh..
+    const int g = cfg.rowfast ? lane >> (5 - LG) : lane & (G - 1);
+    const int rl = cfg.rowfast ? lane & (RPT - 1) : lane >> LG;
     T* cs = reinterpret_cast<T*>(smem);                                  // centre, padded to whole chunks
     unsigned char* tiles = smem + cfg.off_tiles + (size_t)warp * NS * cfg.stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + cfg.off_bars) + warp * NS;
@@ -216,9 +221,22 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                     T s0 = T(0), s1 = T(0), f0 = T(0);
                     const V4* rp = reinterpret_cast<const V4*>(rowp) + g;
                     const V4* cp = cs4 + g;
+                    uint64_t s01 = 0ull;                                 // FP32: (s0, s1) as one packed pair
                     auto chunk = [&](const V4* rq, const V4* cq) {
                         const V4 ev4 = *rq;
                         const V4 cv4 = *cq;
+                        if constexpr (sizeof(T) == 4 && OP != OP_INGEST) {
+                            // packed FP32 pairs (FADD2 / FFMA2 of sm_100): the same operations in the same order
+                            // as the scalar form below (s0 takes columns 0 and 2 of the chunk, s1 columns 1 and 3)
+                            const uint64_t* e2 = reinterpret_cast<const uint64_t*>(&ev4);
+                            const uint64_t* c2 = reinterpret_cast<const uint64_t*>(&cv4);
+                            uint64_t d0, d1;
+                            asm("sub.f32x2 %0, %1, %2;" : "=l"(d0) : "l"(e2[0]), "l"(c2[0]));
+                            asm("sub.f32x2 %0, %1, %2;" : "=l"(d1) : "l"(e2[1]), "l"(c2[1]));
+                            asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(s01) : "l"(d0));
+                            asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(s01) : "l"(d1));
+                            return;
+                        }
                         const T* e = reinterpret_cast<const T*>(&ev4);
                         const T* cc = reinterpret_cast<const T*>(&cv4);
 #pragma unroll
@@ -242,6 +260,11 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                             chunk(rp + ci * G, cp + ci * G);
                             ci = (ci + 1 == n_g) ? 0 : ci + 1;
                         }
+                    }
+                    if constexpr (sizeof(T) == 4 && OP != OP_INGEST) {
+                        float p0, p1;
+                        asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(s01));
+                        s0 = (T)p0; s1 = (T)p1;
                     }
                     nb2 = s0 + s1;
                     if (OP == OP_INGEST) ne2 = f0;
@@ -296,23 +319,27 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
             }
 #pragma unroll
             for (int o = G >> 1; o > 0; o >>= 1) {                       // combine the G lanes of a row
-                nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, o);
-                if (HASV || OP == OP_INGEST) ne2 += __shfl_xor_sync(MEB_FULL_MASK, ne2, o);
+                const int ox = o << xsh;
+                nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, ox);
+                if (HASV || OP == OP_INGEST) ne2 += __shfl_xor_sync(MEB_FULL_MASK, ne2, ox);
                 if (HASV) {
-                    evd += __shfl_xor_sync(MEB_FULL_MASK, evd, o);
-                    vv += __shfl_xor_sync(MEB_FULL_MASK, vv, o);
+                    evd += __shfl_xor_sync(MEB_FULL_MASK, evd, ox);
+                    vv += __shfl_xor_sync(MEB_FULL_MASK, vv, ox);
                 }
             }
             double mylam;
             const bool flag = row_epilogue_core<T, OP>(a, myrow, myvalid && g == 0, myslot >= 0, nb2, ne2, evd, vv,
                                                        r, sig, ri, ui, acc, mylam);
             if (OP != OP_INGEST) {
-                uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);      // bit of lane rl*G <-> row rl
+                uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);      // bit of the g = 0 lane of row rl
                 if (G == 1) {
                     if (lane == 0) a.mask[row0 >> 5] = bits;
                 } else {   // RPT-bit piece of the 32-row mask word: lane q < RPT takes the flag of row q
-                    const bool f2 = __shfl_sync(MEB_FULL_MASK, (int)flag, (lane << LG) & 31) != 0 && lane < RPT;
-                    const uint32_t piece = __ballot_sync(MEB_FULL_MASK, f2);
+                    uint32_t piece = bits;                               // rowfast: lane q < RPT is row q, g = 0
+                    if (!cfg.rowfast) {
+                        const bool f2 = __shfl_sync(MEB_FULL_MASK, (int)flag, (lane << LG) & 31) != 0 && lane < RPT;
+                        piece = __ballot_sync(MEB_FULL_MASK, f2);
+                    }
                     if (lane == 0) {
                         if (G == 2) reinterpret_cast<uint16_t*>(a.mask)[row0 >> 4] = (uint16_t)piece;
                         else reinterpret_cast<uint8_t*>(a.mask)[row0 >> 3] = (uint8_t)piece;
@@ -354,7 +381,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
 #pragma unroll
                                 for (int u = 0; u < 4; ++u) {
                                     if (lam4[u] != 0.0) {
-                                        const V4 ev4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + (ls4[u] >> LG)) * ldT)[ch];
+                                        const V4 ev4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + (cfg.rowfast ? ls4[u] : ls4[u] >> LG)) * ldT)[ch];
                                         const T* e = reinterpret_cast<const T*>(&ev4);
                                         const T* vq = reinterpret_cast<const T*>(&vb[u]);
 #pragma unroll
@@ -454,22 +481,30 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
     const int slots = (int)(c.row_bytes / 16);
     {   // bank conflicts of the quarter-warp LDS.128 (8 lanes, 8 slots of 16 bytes per wavefront): lane
         // (rl, g) reads slot S rl + g + G ((c + rot rl) mod n_g); pick the rotation with fewer collisions
-        int best = 1 << 30;
-        for (int rot = 0; rot < 2; ++rot) {
+        auto collisions = [&](int rowfast, int rot) {
             int coll = 0;
             for (int q = 0; q < 4; ++q) {                     // the four quarter-warps
                 int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
                 for (int l = 8 * q; l < 8 * q + 8; ++l) {
-                    const int g = l % c.G, rl = l / c.G;
+                    const int g = rowfast ? l / rpt : l % c.G, rl = rowfast ? l % rpt : l / c.G;
                     const int n_g = (c.nch - g + c.G - 1) / c.G;
                     const int ci = rot && n_g > 0 ? rl % n_g : 0;
                     cnt[(slots * rl + g + c.G * ci) & 7]++;
                 }
                 for (int b = 0; b < 8; ++b) if (cnt[b] > 1) coll += cnt[b] - 1;
             }
-            // rotation costs instructions: use it only against severe (>= 4-way on average) conflicts
-            if (rot == 0) { best = coll; c.rot = 0; }
-            else if (best >= 24 && coll < best) { best = coll; c.rot = 1; }
+            return coll;
+        };
+        int best = collisions(0, 0);
+        c.rot = 0; c.rowfast = 0;
+        if (c.G > 1 && !getenv("MEB_TILE_NO_ROWFAST")) {
+            const int cr = collisions(1, 0);
+            if (cr < best) { best = cr; c.rowfast = 1; }
+        }
+        // rotation costs instructions: use it only against severe (>= 4-way on average) conflicts
+        if (best >= 24) {
+            const int c0 = collisions(c.rowfast, 1);
+            if (c0 < best) { best = c0; c.rot = 1; }
         }
     }
     // stage of about 12 KB of rows, but never so large that a small problem lands on a handful of warps

@@ -340,7 +340,7 @@ def run_b200(args, rank, world, local_rank):
             "solve": {"radius": r, "kkt": st["kkt"], "delta_max": st["delta_max"],
                       "outer_iters": st["outer_iters"], "newton_iters": st["newton_iters"],
                       "cg_iters": st["cg_iters"], "passes_fp64_full": st["passes_fp64_full"],
-                      "passes_fp32_full": st["passes_fp32_full"], "passes_reduced": st["passes_reduced"],
+                      "passes_fp32_full": st["passes_fp32_full"], "passes_reduced": st["passes_reduced"], "passes_cut": st["passes_cut"],
                       "n_reduced": st["n_reduced"], "rounds": st["rounds"],
                       "ms_phase_lo": st["ms_phase_lo"], "ms_phase_hi": st["ms_phase_hi"],
                       "ms_check": st["ms_check"]}}

@@ -116,6 +116,9 @@ typedef struct meb_stats {
     double pass_bytes[8];
     int32_t pass_count[8];
     int64_t kernel_launches;    /* kernels of this library launched by the solve */
+    int32_t passes_cut;         /* Armijo trial passes (counted in passes_*) stopped early because the partial sum
+                                 * of Psi already exceeded Psi(x): certain rejections */
+    int32_t reserved0;
 } meb_stats;
 
 /* classes of streaming passes in meb_stats.pass_* */

@@ -50,7 +50,7 @@ class meb_stats(C.Structure):
                 ("ms_total", C.c_double), ("ms_phase_lo", C.c_double), ("ms_phase_hi", C.c_double),
                 ("ms_check", C.c_double), ("bytes_streamed", C.c_double),
                 ("pass_ms", C.c_double * 8), ("pass_bytes", C.c_double * 8), ("pass_count", C.c_int32 * 8),
-                ("kernel_launches", C.c_int64)]
+                ("kernel_launches", C.c_int64), ("passes_cut", C.c_int32), ("reserved0", C.c_int32)]
 
     def as_dict(self):
         out = {}

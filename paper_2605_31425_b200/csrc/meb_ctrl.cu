@@ -23,7 +23,8 @@ __global__ void __launch_bounds__(CBLK) ctrl_init_kernel(SolverDev* S, const Sol
         S->phase = PH_FIRST; S->action = ACT_TRIAL;
         S->outer = 0; S->inner = 0; S->ls = 0; S->done = 0; S->status = ST_RUNNING; S->stalled = 0;
         S->newton_total = 0; S->cg_total = 0; S->evals = 0; S->chol_info = 0;
-        S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0; S->tiny = 0;
+        S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0; S->tiny = 0; S->aborted = 0;
+        S->dyn.s0_abort = 1e300;
         S->pass_ns = 0ull; S->pass_count = 0; S->vrow_reads = 0ull;
         S->eta = 1.0; S->psi_cur = 0.0; S->slope = 0.0;
         S->cg_go = 0; S->cg_it = 0;
@@ -34,21 +35,27 @@ __global__ void __launch_bounds__(CBLK) ctrl_init_kernel(SolverDev* S, const Sol
 __global__ void ctrl_resume_kernel(SolverDev* S) {
     S->done = 0;
     S->status = ST_RUNNING;
+    S->dyn.s0_abort = 1e300;
 }
 
 // After the Newton direction Delta is in v.delta (Alg. 2 line 8): first Armijo trial x + Delta.
 __global__ void __launch_bounds__(CBLK) ctrl_after_newton_kernel(SolverDev* S, const SolverVecs v) {
     __shared__ double sm[32];
     const int n = S->n;
-    double sl = 0.0;
+    double sl = 0.0, dx2t = 0.0;
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
         sl = fma(v.g[j], v.delta[j], sl);
-        v.xt[j] = v.xn[j] + v.delta[j];
+        const double xj = v.xn[j] + v.delta[j];
+        v.xt[j] = xj;
+        const double dxb = xj - v.xbar[j];
+        dx2t = fma(dxb, dxb, dx2t);
     }
     sl = ctrl_block_sum(sl, sm);
+    dx2t = ctrl_block_sum(dx2t, sm);
     __syncthreads();
     ctrl_to_raw(S, v, v.xt, v.x_raw);
     if (threadIdx.x == 0) {
+        ctrl_arm_abort(S, true, v.xn[0] + v.delta[0], dx2t);
         S->slope = sl;
         S->tiny = (-sl <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;
         S->eta = 1.0;

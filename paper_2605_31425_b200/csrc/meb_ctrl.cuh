@@ -39,6 +39,9 @@ struct SolverDev {
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
     double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
+    double abort_margin;          // relative slack of MebDyn::s0_abort (rounding of the partial sums); 0: early stop off
+    int32_t aborted, pad3;        // Armijo trials cut short
+    int32_t stall_max;            // outer iterations without halving the best KKT residual before the phase stops (reading 18)
     int32_t stall_count, tiny;    // tiny: the last Newton direction had a decrement below the floor
     uint32_t pass_hist[48], act_hist[48];   // MEB_TRACE: ns and active balls of the first evaluation passes
     int32_t in_graph, eval_cap;   // eval_cap: hard bound on the evaluations of a phase (a runaway loop cannot hang the GPU)
@@ -101,6 +104,20 @@ __device__ __forceinline__ void ctrl_set_handles(const SolverDev* S) {
     if (!S->dense) cudaGraphSetConditional(S->h_cg, (!S->done && S->action == ACT_NEWTON && S->cg_go) ? 1u : 0u);
 }
 
+// Thread 0: arm the early stop (MebDyn::s0_abort) for the Armijo trial with normalised radius rt and
+// dx2t = ||x_t - xbar||^2, or disarm it (trial = false).  In normalised units
+//   Psi~(x_t) = r~_t + (sigma / 2 L^2) S0 + (tau / 2 sigma) dx2t,   S0 = sum_i ||Pi(z_i)||^2 on the raw data,
+// so Psi~(x_t) > Psi~(x) -- which fails the Armijo test and the last-trial test alike -- as soon as
+// S0 > 2 L^2 (Psi~(x) - r~_t - (tau / 2 sigma) dx2t) / sigma.
+__device__ __forceinline__ void ctrl_arm_abort(SolverDev* S, bool trial, double rt, double dx2t) {
+    double thr = 1e300;
+    if (trial && S->abort_margin > 0.0) {
+        const double room = S->psi_cur - rt - 0.5 * (S->tau / S->sigma) * dx2t;
+        if (room > 0.0) thr = 2.0 * S->L * S->L * room / S->sigma * (1.0 + S->abort_margin);
+    }
+    S->dyn.s0_abort = thr;
+}
+
 // relative KKT residual (reading 7) from the scalars of an evaluation
 __device__ __forceinline__ double ctrl_rel_kkt(const double* ev, double r_raw, double* terms) {
     terms[0] = fabs(1.0 - ev[MEB_EV_SUM_UPLUS]);
@@ -157,13 +174,18 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
             const double fq = -0.5 * S->slope * S->eta / den;
             eta = ((fq < S->shrink_min) ? S->shrink_min : 0.5) * S->eta;    // a NaN trial value halves
         }
+        double dx2t = 0.0;
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
             const double xj = v.xn[j] + eta * v.delta[j];
             v.xt[j] = xj;
             v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+            const double dxb = xj - v.xbar[j];
+            dx2t = fma(dxb, dxb, dx2t);
         }
+        dx2t = ctrl_block_sum(dx2t, sm);
         __syncthreads();
         if (threadIdx.x == 0) {
+            ctrl_arm_abort(S, !stalled, v.xn[0] + eta * v.delta[0], dx2t);
             if (stalled) { S->phase = PH_REEVAL; } else { S->eta = eta; S->ls++; }
             S->action = ACT_TRIAL; S->evals++;
             S->vrow_reads += (unsigned long long)(S->dyn.has_mult ? S->n_support : 0);
@@ -232,24 +254,28 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
 // Controller step after a Newton solve (Alg. 2 line 9): slope <g, Delta>, first Armijo trial x + Delta.
 // z: Delta (n doubles, shared or global).  S may live in global or shared memory.  CTA of 256 threads.
 __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs v, const double* z, int n) {
-    __shared__ double red[8];
+    __shared__ double red[8], red2[8];
     const int tid = threadIdx.x;
     const double Ls = S->L;
     const bool use_off = S->use_off != 0;
-    double sl = 0.0;
+    double sl = 0.0, dx2t = 0.0;
     for (int j = tid; j < n; j += 256) {
         const double dj = z[j];
         sl = fma(v.g[j], dj, sl);
         const double xj = v.xn[j] + dj;
         v.xt[j] = xj;
         v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+        const double dxb = xj - v.xbar[j];
+        dx2t = fma(dxb, dxb, dx2t);
     }
     sl = warp_sum(sl);
-    if ((tid & 31) == 0) red[tid >> 5] = sl;
+    dx2t = warp_sum(dx2t);
+    if ((tid & 31) == 0) { red[tid >> 5] = sl; red2[tid >> 5] = dx2t; }
     __syncthreads();
     if (tid == 0) {
-        double t = 0.0;
-        for (int w = 0; w < 8; ++w) t += red[w];
+        double t = 0.0, t2 = 0.0;
+        for (int w = 0; w < 8; ++w) { t += red[w]; t2 += red2[w]; }
+        ctrl_arm_abort(S, true, v.xn[0] + z[0], t2);
         S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
         S->tiny = (-t <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;
     }
@@ -268,6 +294,7 @@ __device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs 
         ctrl_to_raw(S, v, v.xn, v.x_raw);
         if (threadIdx.x == 0) {
             S->n_support = nact;
+            ctrl_arm_abort(S, false, 0.0, 0.0);
             S->phase = PH_REEVAL; S->action = ACT_DONE; S->done = 1; S->status = ST_NEED_CAPACITY;
             ctrl_set_handles(S);
         }
@@ -283,7 +310,7 @@ __device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs 
     int status = ST_RUNNING;
     if (kkt <= S->tol) status = ST_CONVERGED;
     else if (stall >= 3 && best <= S->tol_accept) status = ST_CONVERGED;     // floor of the arithmetic (reading 18)
-    else if (stall >= 6) status = ST_STALLED;
+    else if (stall >= S->stall_max) status = ST_STALLED;
     else if (outer1 >= S->outer_max) status = (best <= S->tol_accept) ? ST_CONVERGED : ST_OUTER_CAP;
     const bool take_best = status != ST_RUNNING && !improved && kkt > S->tol;
     __syncthreads();
@@ -315,6 +342,7 @@ __device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs 
             S->dyn.sigma_raw = s2 / S->L;
         }
         S->inner = 0;
+        ctrl_arm_abort(S, false, 0.0, 0.0);
         S->phase = PH_FIRST;
         S->action = S->done ? ACT_DONE : ACT_TRIAL;
         ctrl_set_handles(S);

@@ -14,6 +14,7 @@
 
 // number of per-CTA scalar partials written by the streaming kernels
 #define MEB_NPART 12
+#define MEB_PART_CUT 9     // per-CTA partial: 1 if the CTA cut its pass short (MebDyn::s0_abort)
 #define MEB_EVPOOL 4096               // streaming launches of one solve that get an event pair
 
 struct meb_ctx {
@@ -116,6 +117,11 @@ struct MebDyn {
     double tau_eff;         // tau / L^2
     int32_t cur;            // which of the two multiplier buffers holds (U, V) of the current outer iteration
     int32_t has_mult;       // 0: all multipliers are zero (first outer iteration)
+    // Early stop of an Armijo trial that is certain to be rejected: Psi = r + (sigma/2) sum_i ||Pi(z_i)||^2 + prox
+    // only grows as balls are added, so once the running sum exceeds s0_abort (the value at which
+    // Psi(trial) = Psi(x)) the rest of the pass cannot change the decision.  1e300: never (not a trial).
+    // A CTA whose own part of the sum crosses it stops and marks its partial (slot MEB_PART_CUT).
+    double s0_abort;
 };
 
 // host-side launch helpers implemented in the .cu files -------------------------------------------

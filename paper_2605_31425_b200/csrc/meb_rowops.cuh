@@ -112,6 +112,43 @@ __device__ __forceinline__ bool row_epilogue_core(const StreamArgs& a, int64_t r
     }
 }
 
+// ---- early stop of a doomed Armijo trial (MebDyn::s0_abort) -------------------------------------------
+// Every warp keeps its running part of sum_i ||Pi(z_i)||^2 (Acc::s0) in a shared-memory slot; a warp that finds
+// the sum over the slots of its CTA above the threshold raises the CTA's flag, and the warps of the CTA stop.
+// Everything stays inside the CTA (no global flag, no atomics: same-address traffic between the two dies costs
+// ~30 ns per access).  One CTA's part exceeding the threshold is sufficient (not necessary) for
+// Psi(trial) > Psi(x); a pass that is cut short is rejected exactly as it would have been when run to the end.
+struct AbortCtl {
+    volatile double* slots = nullptr;       // [32] running sums of the warps, [32] = the CTA's flag
+    double thr = 0.0;
+    bool on = false;
+};
+// call before the first __syncthreads of the kernel; slots: 33 doubles of shared memory
+__device__ __forceinline__ void abort_init(AbortCtl& c, const MebDyn* dyn, double* slots) {
+    c.slots = slots;
+    if (threadIdx.x < 33) slots[threadIdx.x] = 0.0;
+    if (dyn == nullptr) return;
+    const double thr = dyn->s0_abort;
+    if (!(thr < 1e299)) return;
+    c.thr = thr; c.on = true;
+}
+__device__ __forceinline__ bool abort_seen(const AbortCtl& c) { return c.on && c.slots[32] != 0.0; }
+// warp-collective; returns true when the CTA's part crossed the threshold
+__device__ __forceinline__ bool abort_publish(AbortCtl& c, const Acc& acc, int nwarps) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double w = warp_sum(acc.s0);
+    if (lane == 0) c.slots[warp] = w;
+    __syncwarp();
+    const double t = warp_sum(lane < nwarps ? c.slots[lane] : 0.0);
+    const bool crossed = t > c.thr;
+    if (crossed && lane == 0) c.slots[32] = 1.0;
+    return crossed;
+}
+// thread 0, after the CTA's partials were stored
+__device__ __forceinline__ void abort_store(const AbortCtl& c, double* part) {
+    part[(size_t)blockIdx.x * MEB_NPART + MEB_PART_CUT] = (c.on && c.slots[32] != 0.0) ? 1.0 : 0.0;
+}
+
 // Same, loading r_i and u_i of the row from global memory.
 template <typename T, int OP>
 __device__ __forceinline__ bool row_epilogue(const StreamArgs& a, int64_t row, bool valid, bool hasv,

@@ -47,6 +47,9 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
         if (warp >= 5 && warp <= 7) v = partial_max(part, grid, warp, lane);
         else v = partial_sum(part, grid, warp, lane);
         if (lane == 0) sc[warp] = v;
+    } else if (warp == 10) {
+        const double v = partial_max(part, grid, MEB_PART_CUT, lane);
+        if (lane == 0) sc[MEB_PART_CUT] = v;
     } else if (warp == 9 && f.S) {
         // device time of the pass: last CTA end - first CTA start (globaltimer stamps of the tile kernel)
         long long t0 = 0x7fffffffffffffffLL, t1 = 0;
@@ -103,18 +106,22 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
     { double dummy = 0.0; ctrl_block_sum3(nv2, dx2, dummy, sm); }
     __syncthreads();
     if (threadIdx.x == 0) {
+        const bool cut = f.S && sc[MEB_PART_CUT] != 0.0;       // a CTA stopped early: certainly rejected (MebDyn::s0_abort)
+        if (cut) sS.aborted++;
         if (f.S) {
             const long long t0 = __double_as_longlong(sm[100]), t1 = __double_as_longlong(sm[101]);
             if (t1 > t0) {
-                if (sS.pass_count < 48) { sS.pass_hist[sS.pass_count] = (uint32_t)(t1 - t0); sS.act_hist[sS.pass_count] = (uint32_t)(sc[3] + sc[4]); }
-                sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++;
+                const int q = sS.evals < 48 ? sS.evals : 47;          // MEB_TRACE history, indexed by evaluation
+                sS.pass_hist[q] = (uint32_t)(t1 - t0);
+                sS.act_hist[q] = cut ? 0xffffffffu : (uint32_t)(sc[3] + sc[4]);
+                if (!cut) { sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++; }
             }
         }
         double* out = ev_s;
         const double dx0 = x[0] - (xbar ? xbar[0] : x[0]);
         dx2 += dx0 * dx0;
         f.grad[0] = 1.0 - sc[1] + tos * dx0;
-        out[MEB_EV_PSI] = x[0] + 0.5 * sigma * sc[0] + 0.5 * tos * dx2;
+        out[MEB_EV_PSI] = cut ? 1e290 : x[0] + 0.5 * sigma * sc[0] + 0.5 * tos * dx2;
         out[MEB_EV_SUM_UPLUS] = sc[1];
         out[MEB_EV_SUM_PROJ2] = sc[0];
         out[MEB_EV_SUM_DMULT2] = sc[2];

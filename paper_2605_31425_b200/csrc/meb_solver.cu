@@ -307,6 +307,19 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
             fprintf(stderr, "[meb trace]   eval %d outer %d inner %d -> action %d phase %d eta %.3g ls %d psi_t %.15g psi_cur %.15g slope %.3e kkt %.3e nact %.0f\n",
                     h->evals, h->outer, h->inner, h->action, h->phase, h->eta, h->ls, ev[MEB_EV_PSI] / h->L, h->psi_cur, h->slope, h->kkt,
                     ev[MEB_EV_N_ACTIVE]);
+            if (atoi(getenv("MEB_TRACE")) >= 3) {      // per-CTA device times of the pass (globaltimer stamps)
+                static double hp[2048 * MEB_NPART];
+                cudaMemcpy(hp, ctx->part_scalar, sizeof(double) * 148 * MEB_NPART, cudaMemcpyDeviceToHost);
+                long long t0min = 0x7fffffffffffffffLL, t1max = 0; int slow = -1;
+                for (int b = 0; b < 148; ++b) {
+                    long long s0, s1; memcpy(&s0, &hp[b * MEB_NPART + 10], 8); memcpy(&s1, &hp[b * MEB_NPART + 11], 8);
+                    if (s0 < t0min) t0min = s0;
+                    if (s1 > t1max) { t1max = s1; slow = b; }
+                }
+                fprintf(stderr, "[meb trace]     pass %lld ns, last CTA %d; CTA durations:", t1max - t0min, slow);
+                for (int b = 0; b < 148; b += 7) { long long s0, s1; memcpy(&s0, &hp[b * MEB_NPART + 10], 8); memcpy(&s1, &hp[b * MEB_NPART + 11], 8); fprintf(stderr, " %lld(+%lld)", s1 - s0, s0 - t0min); }
+                fprintf(stderr, "\n");
+            }
         }
         if (h->done) return MEB_OK;
         if (h->action == ACT_NEWTON) {
@@ -452,6 +465,9 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
                 if (h->inner_max > 20) h->inner_max = 20;
             }
             h->slope_floor = (P.prec == MEB_FP32) ? 1e-7 : 2e-15;
+            h->abort_margin = getenv("MEB_NO_ABORT") ? 0.0 : ((P.prec == MEB_FP32) ? 1e-3 : 1e-6);
+            h->stall_max = (P.prec == MEB_FP32) ? 3 : 6;   // the FP32 run only has to deliver a warm start
+            if (getenv("MEB_STALL_MAX")) h->stall_max = atoi(getenv("MEB_STALL_MAX"));
             if (getenv("MEB_SLOPE_FLOOR")) h->slope_floor = atof(getenv("MEB_SLOPE_FLOOR"));
             h->eval_cap = 4 * outer_cap * (par.inner_max + 2);
         }
@@ -496,8 +512,11 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         // ---- phase finished ----
         if (getenv("MEB_TRACE")) {
-            fprintf(stderr, "[meb trace] eval passes (ns / active):");
-            for (long long q = 0; q < h->pass_count && q < 48; ++q) fprintf(stderr, " %u/%u", h->pass_hist[q], h->act_hist[q]);
+            fprintf(stderr, "[meb trace] %d of %d passes cut short; eval passes (ns / active):", h->aborted, h->evals);
+            for (int q = 0; q < h->evals && q < 48; ++q) {
+                if (h->act_hist[q] == 0xffffffffu) fprintf(stderr, " %u/cut", h->pass_hist[q]);
+                else fprintf(stderr, " %u/%u", h->pass_hist[q], h->act_hist[q]);
+            }
             fprintf(stderr, "\n");
         }
         S.st->outer_iters += h->outer;
@@ -507,7 +526,8 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         else if (P.prec == MEB_FP64) S.st->passes_fp64_full += h->evals;
         else S.st->passes_fp32_full += h->evals;
         const double vbytes = (double)h->vrow_reads * (double)S.d * (double)esz(P.prec);   // V rows of balls with u_i > 0
-        S.bytes += (double)h->evals * G->bytes_per_eval + vbytes;
+        S.bytes += (double)(h->evals - h->aborted) * G->bytes_per_eval + vbytes;
+        S.st->passes_cut += h->aborted;
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
         S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval + vbytes;
         S.st->pass_count[cls] += (int32_t)h->pass_count;

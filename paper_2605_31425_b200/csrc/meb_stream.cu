@@ -43,6 +43,9 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
 
     const double* cptr = (OP == OP_INGEST) ? a.c0 : a.x + 1;
     for (int j = threadIdx.x; j < NPAD; j += MEB_BLOCK) cs[j] = j < d ? (T)cptr[j] : T(0);
+    __shared__ double abort_slots[33];
+    AbortCtl ab;
+    if (OP == OP_EVAL) abort_init(ab, a.dyn, abort_slots);
     __syncthreads();
     T creg[CPT][VEC];
 #pragma unroll
@@ -58,6 +61,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
     const int64_t ntiles = (m + 31) >> 5;
     const int64_t stride = (int64_t)gridDim.x * MEB_WARPS;
     for (int64_t tile = (int64_t)blockIdx.x * MEB_WARPS + warp; tile < ntiles; tile += stride) {
+        if (OP == OP_EVAL && abort_seen(ab)) break;
         const int64_t row0 = tile << 5;
         const int64_t myrow = row0 + lane;
         const bool myvalid = myrow < m;
@@ -146,6 +150,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
             const uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);
             if (lane == 0) a.mask[tile] = bits;
         }
+        if (OP == OP_EVAL && ab.on && abort_publish(ab, acc, MEB_WARPS)) break;
     }
     block_reduce_store<OP>(acc, a.part);
     if (threadIdx.x == 0) {                 // device time stamps of this CTA (ns), read by the finalize kernel
@@ -153,6 +158,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_tile_kernel(const StreamArgs
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
         a.part[(size_t)blockIdx.x * MEB_NPART + 10] = __longlong_as_double(t_start);
         a.part[(size_t)blockIdx.x * MEB_NPART + 11] = __longlong_as_double(t_end);
+        if (OP == OP_EVAL) abort_store(ab, a.part);
     }
 }
 
@@ -180,6 +186,9 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
     extern __shared__ __align__(16) unsigned char loop_dyn_smem[];
     T* cs = reinterpret_cast<T*>(loop_dyn_smem);
     for (int j = threadIdx.x; j < nchunks * VEC; j += MEB_BLOCK) cs[j] = j < d ? (T)cptr[j] : T(0);
+    __shared__ double abort_slots[33];
+    AbortCtl ab;
+    if (OP == OP_EVAL) abort_init(ab, a.dyn, abort_slots);
     __syncthreads();
 
     // rows per warp tile: 32, or 16 / 8 when there are too few rows to occupy the GPU with 32-row tiles
@@ -188,6 +197,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
     const int64_t ntiles = (m + RT - 1) >> rts;
     const int64_t stride = (int64_t)gridDim.x * MEB_WARPS;
     for (int64_t tile = (int64_t)blockIdx.x * MEB_WARPS + warp; tile < ntiles; tile += stride) {
+        if (OP == OP_EVAL && abort_seen(ab)) break;
         const int64_t row0 = tile << rts;
         const int64_t myrow = row0 + lane;
         const bool myvalid = lane < RT && myrow < m;
@@ -269,6 +279,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
                 else reinterpret_cast<uint8_t*>(a.mask)[tile] = (uint8_t)bits;
             }
         }
+        if (OP == OP_EVAL && ab.on && abort_publish(ab, acc, MEB_WARPS)) break;
     }
     block_reduce_store<OP>(acc, a.part);
     if (threadIdx.x == 0) {                 // device time stamps of this CTA (ns), read by the finalize kernel
@@ -276,6 +287,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) stream_loop_kernel(const StreamArgs
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
         a.part[(size_t)blockIdx.x * MEB_NPART + 10] = __longlong_as_double(t_start);
         a.part[(size_t)blockIdx.x * MEB_NPART + 11] = __longlong_as_double(t_end);
+        if (OP == OP_EVAL) abort_store(ab, a.part);
     }
 }
 

@@ -125,6 +125,9 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
         for (int s = 0; s < NS; ++s) mbar_init(&bars[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    __shared__ double abort_slots[33];
+    AbortCtl ab;
+    if (OP == OP_EVAL) abort_init(ab, a.dyn, abort_slots);
     __syncthreads();
 
     const T r = (OP == OP_INGEST) ? T(0) : (T)a.x[0];
@@ -179,8 +182,15 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
     uint32_t parity = 0;
     int srow0 = gw * rows_per_stage;
     const int srow_step = GW * rows_per_stage;
-    for (int k = 0; k < mine; ++k, srow0 += srow_step) {
+    bool aborted = false;
+    int kend = mine;
+    for (int k = 0; k < kend; ++k, srow0 += srow_step) {
         mbar_wait(&bars[s], parity);
+        if (OP == OP_EVAL && !aborted && abort_seen(ab)) {
+            aborted = true;                                              // stages in flight are still waited for,
+            kend = (k + NS < mine) ? k + NS : mine;                      // nothing new is issued
+        }
+        if (aborted) { if (++s == NS) { s = 0; parity ^= 1u; } continue; }
         unsigned char* sbase = tiles + (size_t)s * cfg.stage_bytes;
         T* stage = reinterpret_cast<T*>(sbase);
         const T* Us = reinterpret_cast<const T*>(sbase + cfg.off_u);
@@ -425,14 +435,17 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                 }
             }
         }
+        if (OP == OP_EVAL && ab.on && (k & 3) == 0 && abort_publish(ab, acc, W)) {
+            aborted = true;
+            kend = (k + NS < mine) ? k + NS : mine;
+        }
         __syncwarp();
-        if (lane == 0 && k + NS < mine) {
+        if (lane == 0 && k + NS < mine && !aborted) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // accesses above before the refill
             issue(k + NS, s);
         }
         if (++s == NS) { s = 0; parity ^= 1u; }
     }
-
     // ---- CTA partials, fixed order ----
     if (OP == OP_EVAL) {
         double* vs = reinterpret_cast<double*>(smem + cfg.off_vec);      // [W][CH * 32 * VEC]
@@ -456,6 +469,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
         a.part[(size_t)blockIdx.x * MEB_NPART + 10] = __longlong_as_double(t_start);
         a.part[(size_t)blockIdx.x * MEB_NPART + 11] = __longlong_as_double(t_end);
+        if (OP == OP_EVAL) abort_store(ab, a.part);
     }
 }
 

@@ -132,3 +132,50 @@ def test_solve_is_deterministic(meb):
     a = _solve(meb, C, R, "mixed")
     b = _solve(meb, C, R, "mixed")
     assert a[1] == b[1] and np.array_equal(a[0], b[0])
+
+
+def _solve_with(meb, C, R, mode, params=None, tol=1e-8):
+    m, d = C.shape
+    with meb.Context(m, d) as ctx:
+        pm = meb.MEB_MODE_FP64 if mode == "fp64" else meb.MEB_MODE_MIXED
+        dC = torch.from_numpy(C).cuda()
+        dR = None if R is None else torch.from_numpy(R).cuda()
+        c, r, st = meb.meb_solve(ctx, dC, dR, tol, pm, params=params)
+    return c.numpy(), r, st
+
+
+@pytest.mark.parametrize("k,m,d", [(2, 200_000, 100), (3, 20_000, 1000), (1, 50_000, 10)])
+def test_cut_trials_do_not_change_the_result(meb, k, m, d, monkeypatch):
+    """Armijo trials whose partial sum of Psi already exceeds Psi(x) are stopped early:
+    they are rejections either way, so the iterates -- and the result, bit for bit -- are those of a
+    run with the early stop switched off.  The first Newton step from the feasible start (no active
+    ball, H = (tau/sigma) I) always produces such trials."""
+    C, R = workloads.config(k, m, d)
+    c1, r1, s1 = _solve_with(meb, C, R, "fp64")
+    monkeypatch.setenv("MEB_NO_ABORT", "1")
+    c0, r0, s0 = _solve_with(meb, C, R, "fp64")
+    assert s1["passes_cut"] > 0 and s0["passes_cut"] == 0
+    assert r1 == r0 and np.array_equal(c1, c0)
+    assert s1["passes_fp64_full"] == s0["passes_fp64_full"] and s1["newton_iters"] == s0["newton_iters"]
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_inner_loop_does_not_spin_at_the_rounding_floor(meb, mode):
+    """Reading 6: once the Newton decrement is below what Psi can resolve the inner loop leaves; before,
+    condition (5) could keep it running to its cap with line searches on rounding noise (hundreds of
+    passes on the config 2 distribution)."""
+    C, R = workloads.config(2, 60_000, 100)
+    c, r, st = _check_against_oracle(meb, C, R, mode)
+    assert st["passes_fp64_full"] + st["passes_fp32_full"] <= 90, st
+
+
+def test_armijo_shrink_min_is_only_a_path_choice(meb):
+    """armijo_shrink_min < 1/2 skips Armijo trials that the parabola through Psi(x), Psi'(x; Delta) and
+    the failed trial predicts to fail; the iteration path changes, the optimum does not."""
+    C, R = workloads.config(2, 50_000, 100)
+    p = meb.meb_default_params()
+    p.armijo_shrink_min = 0.125
+    c1, r1, s1 = _solve_with(meb, C, R, "fp64", params=p)
+    c0, r0, s0 = _solve_with(meb, C, R, "fp64")
+    assert s1["converged"] == 1 and s0["converged"] == 1
+    assert abs(r1 - r0) <= 1e-8 * r0 and np.linalg.norm(c1 - c0) <= 1e-5 * (1 + r0)

@@ -175,6 +175,22 @@ MEB_API int meb_solve_host(meb_ctx* ctx, int64_t m, int32_t d, const double* h_c
                    const double* h_radii, double tol, int precision_mode, const meb_params* h_params,
                    double* h_center_out, double* h_radius_out, meb_stats* h_stats);
 
+/* ---- batched solves of small independent instances (the small-m end of the paper's
+ * experiments) ----
+ * nprob instances in R^d stored back to back: instance k owns rows h_row_offsets[k] .. h_row_offsets[k+1]-1 of
+ * `centers` (DEVICE, FP64, row stride ld) and of `radii` (DEVICE, nullable = points).  Every instance needs
+ * 1 <= m_k <= 4096 and d <= 126 (else MEB_E_CAPACITY).  One persistent CTA per instance runs the FP64 ripALM
+ * of Algorithms 1-2 from its own initial point (reading 3), then the feasible-radius
+ * step; three launches for the whole batch, one host synchronisation.
+ * h_row_offsets[nprob+1]: HOST.  Outputs (HOST, owned by the caller): h_centers_out[nprob*d],
+ * h_radii_out[nprob], h_status_out[nprob] (nullable; MEB_OK, MEB_W_NOT_CONVERGED or MEB_E_INPUT per instance),
+ * h_kkt_out[nprob] (nullable; relative KKT residual reached, reading 7).  Workspace is owned by the context and
+ * grows on demand (MEB_E_ALLOC).  Returns the worst per-instance status, or MEB_E_ARG / MEB_E_CUDA. */
+MEB_API int meb_solve_batch(meb_ctx* ctx, int32_t nprob, const int64_t* h_row_offsets, int32_t d,
+                            const double* centers, int64_t ld, const double* radii, double tol,
+                            const meb_params* h_params, double* h_centers_out, double* h_radii_out,
+                            int32_t* h_status_out, double* h_kkt_out);
+
 /* ---- a0: ingest (reading 3; P:L250 low-precision copy) ---------------------------------------
  * c0_out[d] (device, double) = mean of the S = min(m, sample_rows) rows floor(k*m/S);
  * scalars_out[0] = L = max_i(||c_i - c0|| + r_i), scalars_out[1] = argmax (as double),

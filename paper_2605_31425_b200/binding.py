@@ -28,7 +28,7 @@ EXPORTS = [
     "meb_create", "meb_destroy", "meb_strerror", "meb_last_cuda_error", "meb_default_params",
     "meb_version", "meb_solve", "meb_solve_host", "meb_ingest", "meb_eval_alm", "meb_hvp",
     "meb_dense_hessian", "meb_update_multipliers", "meb_screen_compact", "meb_feasibility_check",
-    "meb_last_pass_info", "meb_set_pass_timing",
+    "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch",
 ]
 
 
@@ -93,6 +93,7 @@ def load():
                   C.POINTER(meb_stats)]
     lib.meb_solve.argtypes = solve_args
     lib.meb_solve_host.argtypes = solve_args
+    lib.meb_solve_batch.argtypes = [vp, i32, vp, i32, vp, i64, vp, dbl, C.POINTER(meb_params), vp, vp, vp, vp]
     lib.meb_ingest.argtypes = [vp, i64, i32, vp, i64, vp, i32, vp, vp, vp, i64, vp]
     prob = [vp, C.c_int, i64, i32, vp, i64, vp, vp, vp, vp, i64]
     lib.meb_eval_alm.argtypes = prob + [vp, vp, dbl, dbl, vp, vp, vp, vp, vp, vp, vp]
@@ -224,6 +225,26 @@ def meb_solve_host(ctx: Context, h_centers, h_radii, tol=1e-8, precision_mode=ME
     allow = (MEB_OK, MEB_W_NOT_CONVERGED) if allow_not_converged else (MEB_OK,)
     _check(code, "meb_solve_host", allow)
     return out_c, out_r.value, st.as_dict()
+
+
+def meb_solve_batch(ctx: Context, centers, radii, row_offsets, tol=1e-8, params=None):
+    """Solves the independent small instances whose rows are row_offsets[k]:row_offsets[k+1] of `centers`
+    (CUDA float64, (rows, d)) and `radii` (CUDA float64 or None) in one batch.
+    Returns (centres (nprob, d) CPU tensor, radii (nprob,), status (nprob,) int32, kkt (nprob,))."""
+    assert centers.is_cuda and centers.dtype == torch.float64 and centers.stride(1) == 1
+    offs = torch.as_tensor(row_offsets, dtype=torch.int64).contiguous()
+    nprob = offs.numel() - 1
+    d = centers.shape[1]
+    out_c = torch.empty((nprob, d), dtype=torch.float64)
+    out_r = torch.empty(nprob, dtype=torch.float64)
+    out_s = torch.empty(nprob, dtype=torch.int32)
+    out_k = torch.empty(nprob, dtype=torch.float64)
+    code = load().meb_solve_batch(ctx.h, nprob, C.c_void_p(offs.data_ptr()), d, _ptr(centers), centers.stride(0),
+                                  _ptr(radii), float(tol), None if params is None else C.byref(params),
+                                  C.c_void_p(out_c.data_ptr()), C.c_void_p(out_r.data_ptr()),
+                                  C.c_void_p(out_s.data_ptr()), C.c_void_p(out_k.data_ptr()))
+    _check(code, "meb_solve_batch", (MEB_OK, MEB_W_NOT_CONVERGED, MEB_E_INPUT))
+    return out_c, out_r, out_s, out_k
 
 
 def meb_ingest(ctx: Context, Cm, R, sample_rows=1024, want_shadow=False):

@@ -96,6 +96,31 @@ __device__ __forceinline__ void ctrl_to_raw(const SolverDev* S, const SolverVecs
         out[j] = (j == 0) ? S->L * xn_[0] : ((S->use_off ? v.off[j - 1] : 0.0) + S->L * xn_[j]);
 }
 
+// Start of a phase (Alg. 1 line 1): xbar = x, trial point = x, counters cleared.  xn and ab were
+// written before (by the host, by a set-up kernel, or by the previous phase).  Any CTA size.
+__device__ inline void meb_ctrl_init_dev(SolverDev* S, const SolverVecs v, double sigma0, int cur, int has_mult) {
+    const int n = S->n;
+    for (int j = threadIdx.x; j < n; j += blockDim.x) v.xbar[j] = v.xn[j];
+    ctrl_to_raw(S, v, v.xn, v.x_raw);
+    __syncthreads();
+    for (int j = threadIdx.x; j < n; j += blockDim.x) v.xbar_raw[j] = v.x_raw[j];
+    if (threadIdx.x == 0) {
+        S->sigma = sigma0;
+        S->dyn.sigma_raw = sigma0 / S->L;
+        S->dyn.tau_eff = S->tau / (S->L * S->L);
+        S->dyn.cur = cur;
+        S->dyn.has_mult = has_mult;
+        S->phase = PH_FIRST; S->action = ACT_TRIAL;
+        S->outer = 0; S->inner = 0; S->ls = 0; S->done = 0; S->status = ST_RUNNING; S->stalled = 0;
+        S->newton_total = 0; S->cg_total = 0; S->evals = 0; S->chol_info = 0;
+        S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0; S->tiny = 0; S->aborted = 0;
+        S->dyn.s0_abort = 1e300;
+        S->pass_ns = 0ull; S->pass_count = 0; S->vrow_reads = 0ull;
+        S->eta = 1.0; S->psi_cur = 0.0; S->slope = 0.0;
+        S->cg_go = 0; S->cg_it = 0;
+    }
+}
+
 __device__ __forceinline__ void ctrl_set_handles(const SolverDev* S) {
     if (!S->in_graph) return;
     cudaGraphSetConditional(S->h_while, S->done ? 0u : 1u);

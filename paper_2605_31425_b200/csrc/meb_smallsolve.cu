@@ -18,6 +18,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <vector>
+
 #include "meb_ctrl.cuh"
 #include "meb_internal.cuh"
 #include "meb_ldlt.cuh"
@@ -41,7 +43,7 @@ struct SmallArgs {
 };
 
 template <int BS>
-__global__ void __launch_bounds__(SM_THREADS) small_solve_kernel(const SmallArgs a) {
+__device__ __forceinline__ void small_solve_body(const SmallArgs& a) {
     constexpr int DP = 16 * BS;                          // padded matrix order (>= n + 1)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ __align__(16) SolverDev sS;
@@ -363,6 +365,122 @@ __global__ void __launch_bounds__(SM_THREADS) small_solve_kernel(const SmallArgs
 }
 
 template <int BS>
+__global__ void __launch_bounds__(SM_THREADS) small_solve_kernel(const SmallArgs a) {
+    small_solve_body<BS>(a);
+}
+
+// ---- batched solves: one CTA per independent instance ----------------------------
+// Instance k owns rows row0 .. row0 + m - 1 of the shared centre / radius arrays and its own state.
+struct BatchInst {
+    SmallArgs a;
+    double* c0;              // [d] = a.v.off
+    double* out;             // [d + 4]: centre, radius, KKT residual, status, L
+    int32_t sample_rows;
+    double sigma0;
+};
+
+// a0 for one instance (readings 3, 16): c0 = mean of a strided row sample, L = max_i(||c_i - c0|| + r_i),
+// validation, then the start of Algorithm 1 (x~ = (1, 0), (alpha, beta) = x~, multipliers 0).
+__global__ void __launch_bounds__(SM_THREADS) batch_setup_kernel(const BatchInst* insts, const SolverDev* tmpl) {
+    const BatchInst in = insts[blockIdx.x];
+    const SmallArgs& a = in.a;
+    __shared__ double red[SM_WARPS];
+    __shared__ int badn[SM_WARPS];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int m = a.m, d = a.d, n = d + 1;
+    {   // state = the template (constants of the run)
+        const unsigned long long* src = reinterpret_cast<const unsigned long long*>(tmpl);
+        unsigned long long* dst = reinterpret_cast<unsigned long long*>(a.S);
+        for (int q = tid; q < (int)(sizeof(SolverDev) / 8); q += SM_THREADS) dst[q] = src[q];
+    }
+    const int S = m < in.sample_rows ? m : in.sample_rows;
+    for (int j = tid; j < d; j += SM_THREADS) {
+        double s = 0.0;
+        for (int k = 0; k < S; ++k) s += a.C[(((int64_t)k * m) / S) * a.ld + j];
+        in.c0[j] = s / (double)S;
+    }
+    __syncthreads();
+    double best = 0.0;
+    int bad = 0;
+    for (int i = warp; i < m; i += SM_WARPS) {           // warp per ball
+        const double* rowp = a.C + (int64_t)i * a.ld;
+        double s = 0.0, f = 0.0;
+        for (int j = lane; j < d; j += 32) { const double e = rowp[j] - in.c0[j]; s = fma(e, e, s); f = fma(rowp[j], 0.0, f); }
+        s = warp_sum(s); f = warp_sum(f);
+        const double ri = a.R ? a.R[i] : 0.0;
+        if (!(f == 0.0) || !(ri >= 0.0) || !(ri < 1.79e308)) bad++;
+        best = fmax(best, sqrt(s) + ri);
+    }
+    if (lane == 0) { red[warp] = best; badn[warp] = bad; }
+    __syncthreads();
+    double L = 0.0; int nbad = 0;
+    for (int w = 0; w < SM_WARPS; ++w) { L = fmax(L, red[w]); nbad += badn[w]; }
+    for (int j = tid; j < n; j += SM_THREADS) { const double x0 = j == 0 ? 1.0 : 0.0; a.v.xn[j] = x0; a.v.ab[j] = x0; }
+    __syncthreads();
+    if (tid == 0) {
+        a.S->L = L;
+        a.S->vcap[0] = m; a.S->vcap[1] = m;
+    }
+    __syncthreads();
+    // every ball is the point c0 up to the rounding of the coordinates (reading 16): nothing to iterate on
+    double cmax = 0.0;
+    for (int j = 0; j < d; ++j) cmax = fmax(cmax, fabs(in.c0[j]));
+    const bool degenerate = nbad > 0 || !(L > 1e-14 * cmax) || !(L < 1.79e308);
+    if (!degenerate) meb_ctrl_init_dev(a.S, a.v, in.sigma0, 0, 0);
+    __syncthreads();
+    if (tid == 0) {
+        in.out[d + 3] = L;
+        if (degenerate) {                                 // nothing to iterate on: bad input, or every ball is the point c0
+            a.S->done = 1;
+            a.S->status = ST_CONVERGED;
+            a.S->kkt = 0.0;
+            in.out[d + 2] = nbad > 0 ? (double)MEB_E_INPUT : (double)MEB_OK;
+        } else {
+            in.out[d + 2] = 1e9;                          // overwritten by the final kernel
+        }
+    }
+}
+
+template <int BS>
+__global__ void __launch_bounds__(SM_THREADS) small_solve_batch_kernel(const BatchInst* insts) {
+    const SmallArgs a = insts[blockIdx.x].a;
+    if (a.S->done) return;                                // uniform: decided by the set-up kernel
+    small_solve_body<BS>(a);
+}
+
+// Result of one instance (step 7 of SURVEY 8(c)): c = c0 + L c~, r = max_i(||c - c_i|| + r_i), the smallest
+// feasible radius for that centre.
+__global__ void __launch_bounds__(SM_THREADS) batch_final_kernel(const BatchInst* insts) {
+    const BatchInst in = insts[blockIdx.x];
+    const SmallArgs& a = in.a;
+    __shared__ double cs[128];
+    __shared__ double red[SM_WARPS];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int m = a.m, d = a.d;
+    const bool bad = in.out[d + 2] == (double)MEB_E_INPUT;
+    const double L = a.S->L;
+    for (int j = tid; j < d; j += SM_THREADS) { cs[j] = in.c0[j] + (L > 0.0 ? L * a.v.xn[1 + j] : 0.0); in.out[j] = cs[j]; }
+    __syncthreads();
+    double best = 0.0;
+    for (int i = warp; i < m; i += SM_WARPS) {
+        const double* rowp = a.C + (int64_t)i * a.ld;
+        double s = 0.0;
+        for (int j = lane; j < d; j += 32) { const double e = rowp[j] - cs[j]; s = fma(e, e, s); }
+        s = warp_sum(s);
+        best = fmax(best, sqrt(s) + (a.R ? a.R[i] : 0.0));
+    }
+    if (lane == 0) red[warp] = best;
+    __syncthreads();
+    if (tid == 0) {
+        double r = 0.0;
+        for (int w = 0; w < SM_WARPS; ++w) r = fmax(r, red[w]);
+        in.out[d] = r;
+        in.out[d + 1] = a.S->kkt;
+        if (!bad) in.out[d + 2] = (a.S->status == ST_CONVERGED) ? (double)MEB_OK : (double)MEB_W_NOT_CONVERGED;
+    }
+}
+
+template <int BS>
 size_t small_smem(int n, int m_cap) {
     constexpr int DP = 16 * BS;
     return (LdltShape<BS>::smem_doubles(n) + DP + (size_t)SM_RB * DP + SM_RB + (size_t)SM_WARPS * DP) * sizeof(double) +
@@ -416,4 +534,147 @@ int meb_launch_small_solve(meb_ctx* ctx, const void* C, int64_t ld, const void* 
         cudaFree(prof);
     }
     return MEB_OK;
+}
+
+// ---- C-ABI: batched solves ---------------------------------------------------------------------------
+namespace {
+constexpr int OWN_BATCH = 20;          // slot of meb_ctx::own used by meb_solve_batch
+
+int batch_reserve(meb_ctx* ctx, size_t bytes) {
+    if (ctx->own_bytes[OWN_BATCH] >= bytes) return MEB_OK;
+    if (ctx->own[OWN_BATCH]) { cudaFree(ctx->own[OWN_BATCH]); ctx->own[OWN_BATCH] = nullptr; ctx->own_bytes[OWN_BATCH] = 0; }
+    const size_t want = bytes + bytes / 4;
+    if (cudaMalloc(&ctx->own[OWN_BATCH], want) != cudaSuccess) { cudaGetLastError(); return MEB_E_ALLOC; }
+    ctx->own_bytes[OWN_BATCH] = want;
+    return MEB_OK;
+}
+}  // namespace
+
+extern "C" int meb_solve_batch(meb_ctx* ctx, int32_t nprob, const int64_t* h_row_offsets, int32_t d,
+                               const double* centers, int64_t ld, const double* radii, double tol,
+                               const meb_params* h_params, double* h_centers_out, double* h_radii_out,
+                               int32_t* h_status_out, double* h_kkt_out) {
+    if (!ctx || nprob < 1 || !h_row_offsets || !centers || !h_centers_out || !h_radii_out || d < 1 || ld < d)
+        return MEB_E_ARG;
+    if (!(tol > 0.0)) return MEB_E_ARG;
+    meb_params par;
+    if (h_params) par = *h_params; else meb_default_params(&par);
+    if (!(par.rho >= 0.0 && par.rho < 1.0) || !(par.sigma0 > 0.0) || !(par.tau > 0.0) || !(par.kappa >= 1.0) ||
+        par.sample_rows < 1)
+        return MEB_E_ARG;
+    int64_t m_maxi = 0;
+    for (int k = 0; k < nprob; ++k) {
+        const int64_t mk = h_row_offsets[k + 1] - h_row_offsets[k];
+        if (mk < 1 || h_row_offsets[k] < 0) return MEB_E_ARG;
+        if (!meb_small_applicable(MEB_FP64, mk, d)) return MEB_E_CAPACITY;    // m_k <= 4096, d <= 126
+        if (mk > m_maxi) m_maxi = mk;
+    }
+    const int64_t row_base = h_row_offsets[0];
+    const int64_t rows = h_row_offsets[nprob] - row_base;
+    const int n = d + 1;
+    const size_t nv = ((size_t)n + 7) / 8 * 8;
+    const int64_t ldv = ((int64_t)d + 1) / 2 * 2;
+    const size_t vec_doubles = 15 * nv + 2 * MEB_EVAL_NSCALARS;
+    const size_t out_doubles = ((size_t)d + 4 + 7) / 8 * 8;
+    // one block of device memory, carved up (all pieces 16-byte aligned)
+    auto al = [](size_t b) { return (b + 255) / 256 * 256; };
+    size_t off = 0;
+    const size_t o_inst = off; off += al((size_t)nprob * sizeof(BatchInst));
+    const size_t o_tmpl = off; off += al(sizeof(SolverDev));
+    const size_t o_S = off;    off += al((size_t)nprob * sizeof(SolverDev));
+    const size_t o_vec = off;  off += al((size_t)nprob * vec_doubles * sizeof(double));
+    const size_t o_out = off;  off += al((size_t)nprob * out_doubles * sizeof(double));
+    size_t o_U[2], o_sl[2], o_V[2];
+    for (int b = 0; b < 2; ++b) {
+        o_U[b] = off;  off += al((size_t)rows * sizeof(double));
+        o_sl[b] = off; off += al((size_t)rows * sizeof(int32_t));
+        o_V[b] = off;  off += al((size_t)rows * ldv * sizeof(double));
+    }
+    const size_t o_rec = off;  off += al((size_t)3 * rows * sizeof(double));
+    int rc = batch_reserve(ctx, off);
+    if (rc) return rc;
+    unsigned char* base = (unsigned char*)ctx->own[OWN_BATCH];
+
+    std::vector<BatchInst> hi((size_t)nprob);
+    for (int k = 0; k < nprob; ++k) {
+        BatchInst& in = hi[(size_t)k];
+        memset(&in, 0, sizeof(in));
+        const int64_t r0 = h_row_offsets[k], mk = h_row_offsets[k + 1] - r0, q0 = r0 - row_base;
+        SmallArgs& a = in.a;
+        a.C = centers + r0 * ld; a.ld = ld; a.R = radii ? radii + r0 : nullptr;
+        a.m = (int32_t)mk; a.d = d; a.ldv = ldv;
+        for (int b = 0; b < 2; ++b) {
+            a.U2[b] = (double*)(base + o_U[b]) + q0;
+            a.slot2[b] = (int32_t*)(base + o_sl[b]) + q0;
+            a.V2[b] = (double*)(base + o_V[b]) + q0 * ldv;
+        }
+        double* rec = (double*)(base + o_rec);
+        a.rec_lam = rec + q0 - 0; a.rec_rho = rec + rows + q0; a.rec_t = rec + 2 * rows + q0;
+        // the records and multiplier arrays are indexed by the ball's index INSIDE the instance
+        a.S = (SolverDev*)(base + o_S) + k;
+        double* vb = (double*)(base + o_vec) + (size_t)k * vec_doubles;
+        double** vecs[] = {&a.v.xn, &a.v.xbar, &a.v.ab, &a.v.delta, &a.v.g, &a.v.xt, &a.v.x_raw, &a.v.xbar_raw,
+                           &a.v.off, &a.v.grad_t, &a.v.res, &a.v.p, &a.v.Hp, &a.v.xbest};
+        for (size_t i = 0; i < 14; ++i) *vecs[i] = vb + i * nv;
+        a.v.ev_t = vb + 15 * nv;
+        a.v.ev = a.v.ev_t + MEB_EVAL_NSCALARS;
+        a.m_cap = (int32_t)((m_maxi + 15) / 16 * 16);
+        a.prof = nullptr;
+        in.c0 = a.v.off;
+        in.out = (double*)(base + o_out) + (size_t)k * out_doubles;
+        in.sample_rows = par.sample_rows;
+        in.sigma0 = par.sigma0;
+    }
+    SolverDev ht;
+    memset(&ht, 0, sizeof(ht));
+    ht.L = 1.0; ht.tol = 0.1 * tol; ht.tol_accept = tol;      // KKT test at tol/10 as in meb_solve (reading 7)
+    ht.rho = par.rho; ht.tau = par.tau; ht.kappa = par.kappa; ht.sigma_max = par.sigma_max; ht.armijo_mu = par.armijo_mu;
+    ht.shrink_min = (par.armijo_shrink_min > 0.0 && par.armijo_shrink_min <= 0.5) ? par.armijo_shrink_min : 0.5;
+    ht.slope_floor = 2e-15; ht.abort_margin = 0.0; ht.stall_max = 6;
+    ht.n = n; ht.d = d; ht.inner_max = par.inner_max; ht.outer_max = par.outer_max; ht.armijo_max = par.armijo_max_halvings;
+    ht.cg_max = par.cg_max; ht.dense = 1; ht.use_off = 1; ht.in_graph = 0;
+    ht.eval_cap = 4 * par.outer_max * (par.inner_max + 2);
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(base + o_inst, hi.data(), (size_t)nprob * sizeof(BatchInst), cudaMemcpyHostToDevice, ctx->stream));
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(base + o_tmpl, &ht, sizeof(ht), cudaMemcpyHostToDevice, ctx->stream));
+    const BatchInst* dinst = (const BatchInst*)(base + o_inst);
+    ctx->launches++;
+    batch_setup_kernel<<<nprob, SM_THREADS, 0, ctx->stream>>>(dinst, (const SolverDev*)(base + o_tmpl));
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    const int bs = (n + 1 + 15) / 16;
+    const int m_cap = (int)((m_maxi + 15) / 16 * 16);
+#define MEB_BATCH_CASE(B)                                                                                              \
+    case B: {                                                                                                          \
+        const size_t smem = small_smem<B>(n, m_cap);                                                                   \
+        if (smem > 225 * 1024) return MEB_E_CAPACITY;                                                                  \
+        MEB_CUDA_OK(ctx, cudaFuncSetAttribute(small_solve_batch_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                              (int)smem));                                                             \
+        ctx->launches++;                                                                                               \
+        small_solve_batch_kernel<B><<<nprob, SM_THREADS, smem, ctx->stream>>>(dinst);                                  \
+        break;                                                                                                         \
+    }
+    switch (bs) {
+        MEB_BATCH_CASE(1) MEB_BATCH_CASE(2) MEB_BATCH_CASE(3) MEB_BATCH_CASE(4)
+        MEB_BATCH_CASE(5) MEB_BATCH_CASE(6) MEB_BATCH_CASE(7) MEB_BATCH_CASE(8)
+        default: return MEB_E_CAPACITY;
+    }
+#undef MEB_BATCH_CASE
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    ctx->launches++;
+    batch_final_kernel<<<nprob, SM_THREADS, 0, ctx->stream>>>(dinst);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    std::vector<double> ho((size_t)nprob * out_doubles);
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ho.data(), base + o_out, ho.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    int worst = MEB_OK;
+    for (int k = 0; k < nprob; ++k) {
+        const double* o = ho.data() + (size_t)k * out_doubles;
+        memcpy(h_centers_out + (size_t)k * d, o, (size_t)d * sizeof(double));
+        h_radii_out[k] = o[d];
+        const int stt = (int)o[d + 2];
+        if (h_status_out) h_status_out[k] = stt;
+        if (h_kkt_out) h_kkt_out[k] = o[d + 1];
+        if (stt < 0) worst = stt;
+        else if (stt > 0 && worst >= 0) worst = stt;
+    }
+    return worst;
 }

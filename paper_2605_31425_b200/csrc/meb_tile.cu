@@ -72,6 +72,8 @@ struct TileCfg {
     int rot;               // 1: rotate the chunk order by the row index (bank conflicts)
     int rowfast;           // 1: lane -> (row = lane % RPT, g = lane / RPT) instead of (row = lane / G, g = lane % G)
     int sc_tma;            // 1: per-row scalars come with the stage (their arrays are 16-byte aligned)
+    int lognchp;           // gradient part: 2^lognchp = lanes that cover one row (>= nch, at most 32); the warp
+                           // walks 32 >> lognchp active rows at a time
     uint32_t off_tiles;    // byte offsets inside the dynamic shared memory
     uint32_t off_bars;
     uint32_t off_vec;
@@ -134,13 +136,19 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
     const T sig = (T)sigma_d;
     const T inv_sig = T(1) / sig;
     Acc acc;
-    // whole-warp-per-row view: lane owns chunks lane, lane + 32 (columns (lane + 32 q) * VEC + e)
+    // whole-warp-per-row view: lane owns chunks cl, cl + 32 (columns (cl + 32 q) * VEC + e).  Rows of at most
+    // 16 chunks (OP_EVAL only) leave lanes over: the warp is split into RP = 32 / nchp groups of nchp lanes and
+    // walks RP rows at a time, group `grp` taking rows grp, grp + RP, ... of a sub-tile.
+    const int lognchp = (OP == OP_EVAL) ? cfg.lognchp : 5;
+    const int cl = lane & ((1 << lognchp) - 1);
+    const int grp = lane >> lognchp;
+    const int RP = 32 >> lognchp;
     double vacc[CH][VEC];
     T creg[CH][VEC];
     const V4* cs4 = reinterpret_cast<const V4*>(cs);
 #pragma unroll
     for (int q = 0; q < CH; ++q) {
-        const int ch = lane + 32 * q;
+        const int ch = cl + 32 * q;
         V4 cv;
         if (ch < nch) cv = cs4[ch];
         const T* cc = reinterpret_cast<const T*>(&cv);
@@ -355,56 +363,50 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                         else reinterpret_cast<uint8_t*>(a.mask)[row0 >> 3] = (uint8_t)piece;
                     }
                 }
-                if (OP == OP_EVAL) {
-                    // gradient vector part: sum over the ACTIVE rows of lam_i b_i, from shared memory
+                if (OP == OP_EVAL && bits != 0u) {
+                    // gradient vector part: sum over the ACTIVE rows of lam_i b_i, from shared memory.  lam_i (and
+                    // the slot of v_i) of the sub-tile's rows go through a warp-private shared array; group `grp`
+                    // of the warp then walks the active rows grp, grp + RP, ..., lane `cl` of the group owning
+                    // the 16-byte chunks cl, cl + 32 of every row.
+                    __shared__ double lam_w[16][32];
+                    __shared__ int32_t slot_w[16][32];
+                    if (g == 0) { lam_w[warp][rl] = mylam; slot_w[warp][rl] = myslot; }
+                    __syncwarp();
                     const bool v16a = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
-                    while (bits) {                                       // four active rows per round: their V loads overlap
-                        int ls4[4], sl4[4];
-                        double lam4[4];
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const bool ok = bits != 0;
-                            const int ls = ok ? __ffs(bits) - 1 : 0;     // lane that owns the row
-                            if (ok) bits &= bits - 1;
-                            const double lam = __shfl_sync(MEB_FULL_MASK, mylam, ls);
-                            const int slot = HASV ? __shfl_sync(MEB_FULL_MASK, myslot, ls) : -1;
-                            ls4[u] = ls; lam4[u] = ok ? lam : 0.0; sl4[u] = ok ? slot : -1;
-                        }
+                    for (int rs = grp; rs < RPT; rs += RP) {
+                        const int bl = cfg.rowfast ? rs : rs << LG;      // ballot bit of row rs (its g = 0 lane)
+                        if (((bits >> bl) & 1u) == 0u) continue;
+                        const double lam = lam_w[warp][rs];
+                        const int slot = HASV ? slot_w[warp][rs] : -1;
+                        const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
 #pragma unroll
                         for (int q = 0; q < CH; ++q) {
-                            const int ch = lane + 32 * q;
+                            const int ch = cl + 32 * q;
                             if (ch < nch) {
-                                V4 vb[4];
+                                V4 vb;
+                                if (slot >= 0) {
+                                    const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
+                                    if (v16a) {
+                                        vb = __ldg(reinterpret_cast<const V4*>(vrow));
+                                    } else {
+                                        T* vq = reinterpret_cast<T*>(&vb);
 #pragma unroll
-                                for (int u = 0; u < 4; ++u) {
-                                    if (sl4[u] >= 0) {
-                                        const T* vrow = Vg + (int64_t)sl4[u] * a.ldv + ch * VEC;
-                                        if (v16a) {
-                                            vb[u] = __ldg(reinterpret_cast<const V4*>(vrow));
-                                        } else {
-                                            T* vq = reinterpret_cast<T*>(&vb[u]);
-#pragma unroll
-                                            for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
-                                        }
+                                        for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
                                     }
                                 }
+                                const V4 ev4 = rp4[ch];
+                                const T* e = reinterpret_cast<const T*>(&ev4);
+                                const T* vq = reinterpret_cast<const T*>(&vb);
 #pragma unroll
-                                for (int u = 0; u < 4; ++u) {
-                                    if (lam4[u] != 0.0) {
-                                        const V4 ev4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + (cfg.rowfast ? ls4[u] : ls4[u] >> LG)) * ldT)[ch];
-                                        const T* e = reinterpret_cast<const T*>(&ev4);
-                                        const T* vq = reinterpret_cast<const T*>(&vb[u]);
-#pragma unroll
-                                        for (int j = 0; j < VEC; ++j) {
-                                            T bj = e[j] - creg[q][j];
-                                            if (sl4[u] >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
-                                            vacc[q][j] = fma(lam4[u], (double)bj, vacc[q][j]);
-                                        }
-                                    }
+                                for (int j = 0; j < VEC; ++j) {
+                                    T bj = e[j] - creg[q][j];
+                                    if (slot >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
+                                    vacc[q][j] = fma(lam, (double)bj, vacc[q][j]);
                                 }
                             }
                         }
                     }
+                    __syncwarp();                                        // lam_w is rewritten by the next sub-tile
                 }
             }
             if (SHADOW) {                       // FP32 shadow of the centred rows (reading 8)
@@ -451,10 +453,17 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
         double* vs = reinterpret_cast<double*>(smem + cfg.off_vec);      // [W][CH * 32 * VEC]
         constexpr int VW = CH * 32 * VEC;
         __syncthreads();
+        for (int o = 1 << lognchp; o < 32; o <<= 1)                     // row groups of the warp, fixed order
 #pragma unroll
-        for (int q = 0; q < CH; ++q)
+            for (int q = 0; q < CH; ++q)
 #pragma unroll
-            for (int j = 0; j < VEC; ++j) vs[(size_t)warp * VW + (lane + 32 * q) * VEC + j] = vacc[q][j];
+                for (int j = 0; j < VEC; ++j) vacc[q][j] += __shfl_xor_sync(MEB_FULL_MASK, vacc[q][j], o);
+        if (grp == 0) {
+#pragma unroll
+            for (int q = 0; q < CH; ++q)
+#pragma unroll
+                for (int j = 0; j < VEC; ++j) vs[(size_t)warp * VW + (cl + 32 * q) * VEC + j] = vacc[q][j];
+        }
         __syncthreads();
         double* pv = a.part_vec + (size_t)blockIdx.x * a.dpad;
         for (int j = threadIdx.x; j < d; j += blockDim.x) {
@@ -490,6 +499,8 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
     c.row_bytes = (uint32_t)(a.ld * (int64_t)esize);
     c.nch = (int)(((size_t)a.d * esize + 15) / 16);
     c.G = lanes_per_row(a, esize);
+    c.lognchp = 0;
+    while (c.lognchp < 5 && (1 << c.lognchp) < c.nch) ++c.lognchp;
     c.logG = c.G == 1 ? 0 : (c.G == 2 ? 1 : 2);
     const int rpt = 32 / c.G;
     const int slots = (int)(c.row_bytes / 16);

@@ -83,8 +83,11 @@ struct TileCfg {
 // ---- the kernel ------------------------------------------------------------------------------------
 // G  = lanes per row (compile time: chunk offsets become immediates);
 // CH = 16-byte chunks per lane when a whole warp walks ONE row (active rows, shadow): ceil(nch / 32).
-template <typename T, int OP, int G, int CH, bool SHADOW>
-__global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const TileCfg cfg) {
+// MAXT = threads per CTA the instance may be launched with: stages of 8 KB and more leave room for at most 12
+// warps, and those launches use the 384-thread instance, which may keep 168 registers per thread (the 512-thread
+// one is held to 128 and rematerialises addresses inside the per-row loops).
+template <typename T, int OP, int G, int CH, bool SHADOW, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const TileCfg cfg) {
     typedef typename Chunk<T>::type V4;
     constexpr int VEC = Chunk<T>::N;
     constexpr int LG = G == 1 ? 0 : (G == 2 ? 1 : 2);
@@ -143,7 +146,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
     const int cl = lane & ((1 << lognchp) - 1);
     const int grp = lane >> lognchp;
     const int RP = 32 >> lognchp;
-    double vacc[CH][VEC];
+    double vacc[CH][VEC], vaccB[CH][VEC];                              // two accumulation chains (rows rs, rs + RP)
     T creg[CH][VEC];
     const V4* cs4 = reinterpret_cast<const V4*>(cs);
 #pragma unroll
@@ -153,7 +156,7 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
         if (ch < nch) cv = cs4[ch];
         const T* cc = reinterpret_cast<const T*>(&cv);
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) { vacc[q][e] = 0.0; creg[q][e] = ch < nch ? cc[e] : T(0); }
+        for (int e = 0; e < VEC; ++e) { vacc[q][e] = 0.0; vaccB[q][e] = 0.0; creg[q][e] = ch < nch ? cc[e] : T(0); }
     }
 
     // stages: st = gw, gw + GW, ...  (consecutive stages go to different SMs)
@@ -373,17 +376,13 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                     if (g == 0) { lam_w[warp][rl] = mylam; slot_w[warp][rl] = myslot; }
                     __syncwarp();
                     const bool v16a = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
-                    for (int rs = grp; rs < RPT; rs += RP) {
-                        const int bl = cfg.rowfast ? rs : rs << LG;      // ballot bit of row rs (its g = 0 lane)
-                        if (((bits >> bl) & 1u) == 0u) continue;
-                        const double lam = lam_w[warp][rs];
-                        const int slot = HASV ? slot_w[warp][rs] : -1;
-                        const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
+                    // one row with lam != 0 (and possibly a multiplier row v_i in the pool)
+                    auto grad_row = [&](const V4* rp4, double lam, int slot, double (&va)[CH][VEC]) {
 #pragma unroll
                         for (int q = 0; q < CH; ++q) {
                             const int ch = cl + 32 * q;
                             if (ch < nch) {
-                                V4 vb;
+                                V4 vb = V4();
                                 if (slot >= 0) {
                                     const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
                                     if (v16a) {
@@ -401,9 +400,43 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
                                 for (int j = 0; j < VEC; ++j) {
                                     T bj = e[j] - creg[q][j];
                                     if (slot >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
-                                    vacc[q][j] = fma(lam, (double)bj, vacc[q][j]);
+                                    va[q][j] = fma(lam, (double)bj, va[q][j]);
                                 }
                             }
+                        }
+                    };
+                    const int rstep = RP * (ldT / VEC);                   // 16-byte units between rows rs and rs + RP
+                    for (int rs = grp; rs < RPT; rs += 2 * RP) {          // two rows of my group per step
+                        const int rsB = rs + RP;
+                        const double lamA = lam_w[warp][rs];
+                        const double lamB = rsB < RPT ? lam_w[warp][rsB] : 0.0;
+                        if (lamA == 0.0 && lamB == 0.0) continue;
+                        const int slotA = (HASV && lamA != 0.0) ? slot_w[warp][rs] : -1;
+                        const int slotB = (HASV && lamB != 0.0) ? slot_w[warp][rsB] : -1;
+                        const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
+                        const V4* rpB = rpA + rstep;
+                        if (slotA < 0 && slotB < 0) {
+                            // no multiplier rows: a row with lam = 0 adds exactly zero, without being read (shared
+                            // memory behind the last row of the data is stale)
+#pragma unroll
+                            for (int q = 0; q < CH; ++q) {
+                                const int ch = cl + 32 * q;
+                                if (ch < nch) {
+                                    V4 eA = V4(), eB = V4();
+                                    if (lamA != 0.0) eA = rpA[ch];
+                                    if (lamB != 0.0) eB = rpB[ch];
+                                    const T* ea = reinterpret_cast<const T*>(&eA);
+                                    const T* eb = reinterpret_cast<const T*>(&eB);
+#pragma unroll
+                                    for (int j = 0; j < VEC; ++j) {
+                                        vacc[q][j] = fma(lamA, (double)(ea[j] - creg[q][j]), vacc[q][j]);
+                                        vaccB[q][j] = fma(lamB, (double)(eb[j] - creg[q][j]), vaccB[q][j]);
+                                    }
+                                }
+                            }
+                        } else {
+                            if (lamA != 0.0) grad_row(rpA, lamA, slotA, vacc);
+                            if (lamB != 0.0) grad_row(rpB, lamB, slotB, vaccB);
                         }
                     }
                     __syncwarp();                                        // lam_w is rewritten by the next sub-tile
@@ -453,6 +486,10 @@ __global__ void __launch_bounds__(512, 1) tile_kernel(const StreamArgs a, const 
         double* vs = reinterpret_cast<double*>(smem + cfg.off_vec);      // [W][CH * 32 * VEC]
         constexpr int VW = CH * 32 * VEC;
         __syncthreads();
+#pragma unroll
+        for (int q = 0; q < CH; ++q)
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) vacc[q][j] += vaccB[q][j];
         for (int o = 1 << lognchp; o < 32; o <<= 1)                     // row groups of the warp, fixed order
 #pragma unroll
             for (int q = 0; q < CH; ++q)
@@ -581,10 +618,11 @@ size_t cfg_smem(const TileCfg& c, int cpl) {
 }
 
 template <typename KernelT>
-int launch_cfg(meb_ctx* ctx, KernelT kernel, const StreamArgs& a, size_t esize, int cpl, int* grid_out) {
+int launch_cfg(meb_ctx* ctx, KernelT kernel512, KernelT kernel384, const StreamArgs& a, size_t esize, int cpl, int* grid_out) {
     int grid = ctx->sm_count > 0 ? ctx->sm_count : 148;            // one persistent CTA per SM
     TileCfg c;
     if (!make_cfg(a, esize, cpl, grid, &c)) return MEB_E_CAPACITY;
+    KernelT kernel = c.W <= 12 ? kernel384 : kernel512;
     const int64_t nstages = (a.m + c.stage_rows - 1) / c.stage_rows;
     if (nstages < grid) grid = (int)nstages;                       // stage k -> CTA k % grid, warp k / grid
     if (grid < 1) grid = 1;
@@ -610,10 +648,11 @@ int launch_g(meb_ctx* ctx, const StreamArgs& a, bool want_ch, int* grid_out) {
     const int nch = (int)(((size_t)a.d * sizeof(T) + 15) / 16);        // <= 64 (rows of at most 1024 bytes)
     constexpr int VEC = 16 / sizeof(T);
     const int G = lanes_per_row(a, sizeof(T));
-    if (G == 1) return launch_cfg(ctx, tile_kernel<T, OP, 1, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
-    if (G == 2) return launch_cfg(ctx, tile_kernel<T, OP, 2, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
-    if (!want_ch || nch <= 32) return launch_cfg(ctx, tile_kernel<T, OP, 4, 1, SHADOW>, a, sizeof(T), VEC, grid_out);
-    return launch_cfg(ctx, tile_kernel<T, OP, 4, 2, SHADOW>, a, sizeof(T), 2 * VEC, grid_out);
+    if (G == 1) return launch_cfg(ctx, tile_kernel<T, OP, 1, 1, SHADOW, 512>, tile_kernel<T, OP, 1, 1, SHADOW, 384>, a, sizeof(T), VEC, grid_out);
+    if (G == 2) return launch_cfg(ctx, tile_kernel<T, OP, 2, 1, SHADOW, 512>, tile_kernel<T, OP, 2, 1, SHADOW, 384>, a, sizeof(T), VEC, grid_out);
+    if (!want_ch || nch <= 32)
+        return launch_cfg(ctx, tile_kernel<T, OP, 4, 1, SHADOW, 512>, tile_kernel<T, OP, 4, 1, SHADOW, 384>, a, sizeof(T), VEC, grid_out);
+    return launch_cfg(ctx, tile_kernel<T, OP, 4, 2, SHADOW, 512>, tile_kernel<T, OP, 4, 2, SHADOW, 384>, a, sizeof(T), 2 * VEC, grid_out);
 }
 
 }  // namespace

@@ -53,7 +53,71 @@ __global__ void __launch_bounds__(MEB_BLOCK) active_kernel(const ActiveArgs a_in
     const int n = *a.count;
     const int nteams = gridDim.x * TPB;
     double sc = 0.0;                                         // scalar partial (one per team, in thread 0)
-    for (int k = blockIdx.x * TPB + team; k < n; k += nteams) {
+    int kstart = blockIdx.x * TPB + team;
+    if (MODE == MODE_WRITEV && TEAM == 32 && d <= 64) {
+        // Short rows: the gather list[k] -> (slot, lam, t) -> rows of C and V is three dependent global loads per
+        // entry, and one entry per warp at a time leaves the pass latency-bound (config 4: 5e6 entries, 3.8 ms).
+        // Four entries of the team's sequence are loaded level by level, then written; same entries, same order
+        // and same arithmetic as the loop below (fma(0, 1/sigma, b) = b for a row without v_i).
+        constexpr int UB = 4, EP = 2;
+        for (int kb = kstart; kb < n; kb += nteams * UB) {
+            int ii[UB], sl[UB];
+            double lam[UB], tv[UB];
+            T cv[UB][EP], vv[UB][EP];
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const long long k = (long long)kb + (long long)u * nteams;
+                ii[u] = k < n ? a.list[k] : -1;
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int i = ii[u];
+                sl[u] = (i >= 0 && a.v_slot) ? a.v_slot[i] : -1;
+                lam[u] = i >= 0 ? a.rec_lam[i] : 0.0;
+                tv[u] = i >= 0 ? a.rec_t[i] : 0.0;
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const T* rowp = C + (int64_t)(ii[u] >= 0 ? ii[u] : 0) * a.ld;
+                const T* vrow = V + (int64_t)(sl[u] >= 0 ? sl[u] : 0) * a.ldv;
+#pragma unroll
+                for (int e = 0; e < EP; ++e) {
+                    const int j = tt + 32 * e;
+                    cv[u][e] = (ii[u] >= 0 && j < d) ? rowp[j] : T(0);
+                    vv[u][e] = (sl[u] >= 0 && j < d) ? vrow[j] : T(0);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                if (ii[u] < 0) continue;                             // team-uniform
+                const int k = kb + u * nteams;
+                const T sl_ = (T)(a.sigma * lam[u]);
+                T* vout = static_cast<T*>(a.V_out) + (int64_t)k * a.ldv_out;
+                const bool store = k < a.cap_rows;
+                double nb2 = 0.0;
+#pragma unroll
+                for (int e = 0; e < EP; ++e) {
+                    const int j = tt + 32 * e;
+                    if (j < d) {
+                        T b = cv[u][e] - (T)cx[j];
+                        b = fma(vv[u][e], inv_sig, b);
+                        const T vp = sl_ * b;
+                        if (store) vout[j] = vp;
+                        nb2 = fma((double)vp, (double)vp, nb2);
+                    }
+                }
+                nb2 = team_sum<TEAM>(nb2, scratch);
+                if (tt == 0) {
+                    const T up = (T)a.sigma * (T)tv[u];
+                    static_cast<T*>(a.U_out)[ii[u]] = up;
+                    a.slot_out[ii[u]] = store ? k : -1;
+                    sc += (double)up * (double)up + nb2;
+                }
+            }
+        }
+        kstart = n;
+    }
+    for (int k = kstart; k < n; k += nteams) {
         const int i = a.list[k];
         const T* rowp = C + (int64_t)i * a.ld;
         const int slot = a.v_slot ? a.v_slot[i] : -1;
@@ -142,6 +206,10 @@ int launch_active_t(meb_ctx* ctx, const ActiveArgs& a, int* grid_out) {
     if (smem > 220 * 1024) return MEB_E_CAPACITY;
     int grid = ctx->sm_count * (smem > 100 * 1024 ? 1 : 2);
     if ((int64_t)grid > ctx->vec_rows) grid = (int)ctx->vec_rows;
+    if (MODE == MODE_WRITEV && !wide) {          // no vector partials: as many CTAs as fit (part_sc holds 1024)
+        grid = ctx->sm_count * 4;
+        if (grid > 1024) grid = 1024;
+    }
     cudaError_t e;
     if (wide) {
         auto kern = active_kernel<T, MEB_BLOCK, MODE>;

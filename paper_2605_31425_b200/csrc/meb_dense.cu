@@ -16,95 +16,177 @@
 
 namespace {
 
-constexpr int RB = 16;      // rows per shared tile
+// Threads of a CTA: KS row groups of TD x TD threads; thread (ty, tx) of a group owns the B x B block
+// {ty + TD i} x {tx + TD j} of the DP x DP accumulator (DP = TD * B) and group kg takes rows kg, kg + KS, ... of a
+// tile.  TD = 8, KS = 4 for DP <= 48 (a 16 x 16 grid would leave 1-4 FMAs per thread and row), TD = 16, KS = 1 above.
+template <int TD> struct SyrkShape {
+    static constexpr int KS = MEB_BLOCK / (TD * TD);
+    static constexpr int RB = TD == 8 ? 32 : 16;            // rows per shared tile
+};
 
-template <typename T, int BS>
-__global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a_in, double* __restrict__ part_mat,
-                                                          int dp) {
+// The list is a gather (list[k] -> rho_i, slot_i -> rows of C and V): three dependent levels of global loads.  They
+// are software-pipelined over three tiles -- while the FMAs of tile t run, the rows of tile t+1, the (rho, slot) of
+// tile t+2 and the list entries of tile t+3 are in flight in registers -- because with two CTAs per SM nothing else
+// hides that latency (config 4, 5e6-1e7 active rows: 3.5 ms per Hessian before the pipeline).
+template <typename T, int TD, int B>
+__global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a_in, double* __restrict__ part_mat) {
+    constexpr int DP = TD * B;
+    constexpr int KS = SyrkShape<TD>::KS;
+    constexpr int RB = SyrkShape<TD>::RB;
+    constexpr int RPW = RB / MEB_WARPS;                      // rows per warp in the fill phase
+    constexpr int EPL = (DP + 31) / 32;                      // elements per lane and row
     ActiveArgs a = a_in;
     meb_resolve_dyn(a);
-    extern __shared__ __align__(16) double sm[];          // W[RB][dp] then rho[RB]
+    extern __shared__ __align__(16) double sm[];             // W[RB][DP], rho[RB], then (KS > 1) red[DP*DP + DP]
     double* W = sm;
-    double* rho_s = sm + (size_t)RB * dp;
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    double* rho_s = sm + (size_t)RB * DP;
+    const int tx = threadIdx.x % TD, ty = (threadIdx.x / TD) % TD, kg = threadIdx.x / (TD * TD);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d = a.d;
     const T* __restrict__ C = static_cast<const T*>(a.C);
     const T* __restrict__ V = static_cast<const T*>(a.V);
-    const double* __restrict__ cx = a.x + 1;
     const T inv_sig = T(1) / (T)a.sigma;
     const int n = *a.count;
-    if (blockIdx.x * RB >= n) return;                     // no tile for this CTA: the finalize skips it
-    double acc[BS][BS];
-    double accs[BS];
+    if (blockIdx.x * RB >= n) return;                        // no tile for this CTA: the finalize skips it
+    double acc[B][B];
+    double accs[B];
 #pragma unroll
-    for (int i = 0; i < BS; ++i) {
+    for (int i = 0; i < B; ++i) {
         accs[i] = 0.0;
 #pragma unroll
-        for (int j = 0; j < BS; ++j) acc[i][j] = 0.0;
+        for (int j = 0; j < B; ++j) acc[i][j] = 0.0;
     }
-    // tiles of RB consecutive list entries, tile t -> CTA t mod grid
-    for (int k0 = blockIdx.x * RB; k0 < n; k0 += gridDim.x * RB) {
-        __syncthreads();
-        // each warp fills RB / 8 = 2 rows of the tile
-        for (int rr = warp; rr < RB; rr += MEB_WARPS) {
-            const int k = k0 + rr;
-            double rho = 0.0;
-            bool use = false;
-            int i = 0;
-            if (k < n) { i = a.list[k]; rho = a.rec_rho[i]; use = rho < 1.5; }   // B1 rows: P_i = I, no SYRK term
-            double nb2 = 0.0;
-            if (use) {
-                const T* rowp = C + (int64_t)i * a.ld;
-                const int slot = a.v_slot ? a.v_slot[i] : -1;
-                const T* vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
-                for (int j = lane; j < dp; j += 32) {
-                    double bd = 0.0;
-                    if (j < d) {
-                        T b = rowp[j] - (T)cx[j];
-                        if (vrow) b = fma(vrow[j], inv_sig, b);
-                        bd = (double)b;
-                    }
-                    W[(size_t)rr * dp + j] = bd;
-                    nb2 = fma(bd, bd, nb2);
-                }
-                nb2 = warp_sum(nb2);
-                const double inv = 1.0 / sqrt(nb2);
-                for (int j = lane; j < dp; j += 32) W[(size_t)rr * dp + j] *= inv;
-            } else {
-                for (int j = lane; j < dp; j += 32) W[(size_t)rr * dp + j] = 0.0;
+    T cxr[EPL];
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) cxr[e] = (lane + 32 * e) < d ? (T)a.x[1 + lane + 32 * e] : T(0);
+
+    // pipeline registers of the RPW rows this warp fills
+    int i_a[RPW];                                            // level 1: list entries (tile t+3)
+    int i_b[RPW], slot_b[RPW]; double rho_b[RPW];            // level 2: (rho, slot) of tile t+2
+    T cq[RPW][EPL], vq[RPW][EPL]; double rho_c[RPW];         // level 3: raw rows of tile t+1
+    auto level1 = [&](int k0) {
+#pragma unroll
+        for (int r = 0; r < RPW; ++r) {
+            const int k = k0 + warp * RPW + r;
+            i_a[r] = (k0 >= 0 && k < n) ? a.list[k] : -1;
+        }
+    };
+    auto level2 = [&]() {
+#pragma unroll
+        for (int r = 0; r < RPW; ++r) {
+            const int i = i_a[r];
+            i_b[r] = i;
+            rho_b[r] = i >= 0 ? a.rec_rho[i] : 2.0;          // B1 rows (rho = 2): P_i = I, no SYRK term
+            slot_b[r] = (i >= 0 && a.v_slot) ? a.v_slot[i] : -1;
+        }
+    };
+    auto level3 = [&]() {
+#pragma unroll
+        for (int r = 0; r < RPW; ++r) {
+            const int i = i_b[r];
+            const double rho = rho_b[r];
+            const bool use = i >= 0 && rho < 1.5;
+            const int slot = slot_b[r];
+            rho_c[r] = use ? rho : 2.0;
+            const T* rowp = C + (int64_t)(use ? i : 0) * a.ld;
+            const T* vrow = V + (int64_t)(slot >= 0 ? slot : 0) * a.ldv;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) {
+                const int j = lane + 32 * e;
+                cq[r][e] = (use && j < d) ? rowp[j] : T(0);
+                vq[r][e] = (use && slot >= 0 && j < d) ? vrow[j] : T(0);
             }
-            if (lane == 0) rho_s[rr] = use ? rho : 0.0;
+        }
+    };
+    const int kstep = gridDim.x * RB;
+    int k0 = blockIdx.x * RB;
+    auto tile_at = [&](int q) {                              // first list entry of the q-th tile after k0, or -1
+        const long long k = (long long)k0 + (long long)q * kstep;
+        return k < n ? (int)k : -1;
+    };
+    level1(k0); level2(); level3();                          // tile 0 -> level 3
+    level1(tile_at(1)); level2();                            // tile 1 -> level 2
+    level1(tile_at(2));                                      // tile 2 -> level 1
+    for (; k0 < n; k0 += kstep) {
+        __syncthreads();
+        // normalise the rows of this tile (level 3 registers) into shared memory
+#pragma unroll
+        for (int r = 0; r < RPW; ++r) {
+            const int rr = warp * RPW + r;
+            const bool use = rho_c[r] < 1.5;
+            double bd[EPL];
+            double nb2 = 0.0;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) {
+                T b = cq[r][e] - cxr[e];
+                b = fma(vq[r][e], inv_sig, b);
+                bd[e] = (use && lane + 32 * e < d) ? (double)b : 0.0;
+                nb2 = fma(bd[e], bd[e], nb2);
+            }
+            nb2 = warp_sum(nb2);
+            const double inv = use ? 1.0 / sqrt(nb2) : 0.0;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e)
+                if (lane + 32 * e < DP) W[(size_t)rr * DP + lane + 32 * e] = bd[e] * inv;
+            if (lane == 0) rho_s[rr] = use ? rho_c[r] : 0.0;
         }
         __syncthreads();
+        level3();                                            // rows of the next tile
+        level2();                                            // (rho, slot) of the tile after it
+        level1(tile_at(3));                                  // list entries three tiles ahead
 #pragma unroll 4
-        for (int rr = 0; rr < RB; ++rr) {
+        for (int rr = kg; rr < RB; rr += KS) {
             const double rho = rho_s[rr];
-            const double* w = W + (size_t)rr * dp;
-            double wq[BS], wp[BS];
+            const double* w = W + (size_t)rr * DP;
+            double wq[B], wp[B];
 #pragma unroll
-            for (int j = 0; j < BS; ++j) wq[j] = w[tx + 16 * j];
+            for (int j = 0; j < B; ++j) wq[j] = w[tx + TD * j];
 #pragma unroll
-            for (int i = 0; i < BS; ++i) wp[i] = rho * w[ty + 16 * i];
+            for (int i = 0; i < B; ++i) wp[i] = rho * w[ty + TD * i];
 #pragma unroll
-            for (int i = 0; i < BS; ++i)
+            for (int i = 0; i < B; ++i)
 #pragma unroll
-                for (int j = 0; j < BS; ++j) acc[i][j] = fma(wp[i], wq[j], acc[i][j]);
+                for (int j = 0; j < B; ++j) acc[i][j] = fma(wp[i], wq[j], acc[i][j]);
             if (ty == 0) {
 #pragma unroll
-                for (int j = 0; j < BS; ++j) accs[j] += wq[j];
+                for (int j = 0; j < B; ++j) accs[j] += wq[j];
             }
         }
     }
-    // per-CTA partial: [dp*dp] matrix then [dp] vector
-    double* pm = part_mat + (size_t)blockIdx.x * ((size_t)dp * dp + dp);
+    // per-CTA partial: [DP*DP] matrix then [DP] vector; the row groups are added in index order
+    double* pm = part_mat + (size_t)blockIdx.x * ((size_t)DP * DP + DP);
+    if (KS > 1) {
+        double* red = sm + (size_t)RB * DP + RB;
+        for (int gk = 0; gk < KS; ++gk) {
+            __syncthreads();
+            if (kg == gk) {
 #pragma unroll
-    for (int i = 0; i < BS; ++i)
+                for (int i = 0; i < B; ++i)
 #pragma unroll
-        for (int j = 0; j < BS; ++j) pm[(size_t)(ty + 16 * i) * dp + tx + 16 * j] = acc[i][j];
-    if (ty == 0) {
+                    for (int j = 0; j < B; ++j) {
+                        const int e = (ty + TD * i) * DP + tx + TD * j;
+                        red[e] = (gk == 0 ? 0.0 : red[e]) + acc[i][j];
+                    }
+                if (ty == 0) {
 #pragma unroll
-        for (int j = 0; j < BS; ++j) pm[(size_t)dp * dp + tx + 16 * j] = accs[j];
+                    for (int j = 0; j < B; ++j) {
+                        const int e = DP * DP + tx + TD * j;
+                        red[e] = (gk == 0 ? 0.0 : red[e]) + accs[j];
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        for (int e = threadIdx.x; e < DP * DP + DP; e += MEB_BLOCK) pm[e] = red[e];
+    } else {
+#pragma unroll
+        for (int i = 0; i < B; ++i)
+#pragma unroll
+            for (int j = 0; j < B; ++j) pm[(size_t)(ty + TD * i) * DP + tx + TD * j] = acc[i][j];
+        if (ty == 0) {
+#pragma unroll
+            for (int j = 0; j < B; ++j) pm[(size_t)DP * DP + tx + TD * j] = accs[j];
+        }
     }
 }
 
@@ -112,9 +194,9 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
                                                              const int32_t* __restrict__ count,
                                                              int dp, int d, const double* __restrict__ ev,
                                                              double sigma, double tau, double* __restrict__ H,
-                                                             const MebDyn* __restrict__ dyn) {
+                                                             const MebDyn* __restrict__ dyn, int rb) {
     if (dyn) { sigma = dyn->sigma_raw; tau = dyn->tau_eff; }
-    const int ntiles = (*count + RB - 1) / RB;            // CTAs b < ntiles wrote a partial
+    const int ntiles = (*count + rb - 1) / rb;            // CTAs b < ntiles wrote a partial
     if (nparts > ntiles) nparts = ntiles;
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
@@ -182,13 +264,16 @@ __global__ void __launch_bounds__(256) ldlt_solve_kernel(const double* __restric
 }
 
 template <typename T>
-int launch_syrk(meb_ctx* ctx, const ActiveArgs& a, int dp, double* part_mat, int grid) {
+int launch_syrk(meb_ctx* ctx, const ActiveArgs& a, int dp, double* part_mat, int grid, int* rb_out) {
     const int bs = dp / 16;
-    const size_t smem = ((size_t)RB * dp + RB) * sizeof(double);
-#define MEB_SYRK_CASE(B) case B: ctx->launches++; syrk_kernel<T, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat, dp); break;
+    const int td = bs <= 3 ? 8 : 16;
+    const int rb = td == 8 ? SyrkShape<8>::RB : SyrkShape<16>::RB;
+    const size_t smem = ((size_t)rb * dp + rb + (td == 8 ? (size_t)dp * dp + dp : 0)) * sizeof(double);
+    *rb_out = rb;
+#define MEB_SYRK_CASE(BSV, TD, B) case BSV: ctx->launches++; syrk_kernel<T, TD, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat); break;
     switch (bs) {
-        MEB_SYRK_CASE(1) MEB_SYRK_CASE(2) MEB_SYRK_CASE(3) MEB_SYRK_CASE(4)
-        MEB_SYRK_CASE(5) MEB_SYRK_CASE(6) MEB_SYRK_CASE(7) MEB_SYRK_CASE(8)
+        MEB_SYRK_CASE(1, 8, 2) MEB_SYRK_CASE(2, 8, 4) MEB_SYRK_CASE(3, 8, 6) MEB_SYRK_CASE(4, 16, 4)
+        MEB_SYRK_CASE(5, 16, 5) MEB_SYRK_CASE(6, 16, 6) MEB_SYRK_CASE(7, 16, 7) MEB_SYRK_CASE(8, 16, 8)
         default: return MEB_E_CAPACITY;
     }
 #undef MEB_SYRK_CASE
@@ -217,14 +302,15 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
         a.dyn = c.gs->dyn;
         for (int b = 0; b < 2; ++b) { a.U2[b] = c.gs->U2[b]; a.slot2[b] = c.gs->slot2[b]; a.V2[b] = c.gs->V2[b]; a.vcap2[b] = c.gs->vcap2[b]; }
     }
-    int rc = c.prec == MEB_FP64 ? launch_syrk<double>(ctx, a, dp, ctx->part_mat, grid)
-                                : launch_syrk<float>(ctx, a, dp, ctx->part_mat, grid);
+    int rb = 0;
+    int rc = c.prec == MEB_FP64 ? launch_syrk<double>(ctx, a, dp, ctx->part_mat, grid, &rb)
+                                : launch_syrk<float>(ctx, a, dp, ctx->part_mat, grid, &rb);
     if (rc != MEB_OK) return rc;
     const int n = c.d + 1;
     int fgrid = (n * n + 255) / 256;
     if (fgrid > 64) fgrid = 64;
     ctx->launches++; dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, ctx->count_dev, dp, c.d, ev_scalars, c.sigma,
-                                                          c.tau, H, c.gs ? c.gs->dyn : nullptr);
+                                                          c.tau, H, c.gs ? c.gs->dyn : nullptr, rb);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                     if (g == 0) { lam_w[warp][rl] = mylam; slot_w[warp][rl] = myslot; }
                     __syncwarp();
                     const bool v16a = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
-                    // one row with lam != 0 (and possibly a multiplier row v_i in the pool)
+                    // one row with lam != 0 and possibly a multiplier row v_i in the pool
                     auto grad_row = [&](const V4* rp4, double lam, int slot, double (&va)[CH][VEC]) {
 #pragma unroll
                         for (int q = 0; q < CH; ++q) {
@@ -405,19 +405,81 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                             }
                         }
                     };
-                    const int rstep = RP * (ldT / VEC);                   // 16-byte units between rows rs and rs + RP
-                    for (int rs = grp; rs < RPT; rs += 2 * RP) {          // two rows of my group per step
-                        const int rsB = rs + RP;
-                        const double lamA = lam_w[warp][rs];
-                        const double lamB = rsB < RPT ? lam_w[warp][rsB] : 0.0;
-                        if (lamA == 0.0 && lamB == 0.0) continue;
-                        const int slotA = (HASV && lamA != 0.0) ? slot_w[warp][rs] : -1;
-                        const int slotB = (HASV && lamB != 0.0) ? slot_w[warp][rsB] : -1;
-                        const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
-                        const V4* rpB = rpA + rstep;
-                        if (slotA < 0 && slotB < 0) {
-                            // no multiplier rows: a row with lam = 0 adds exactly zero, without being read (shared
-                            // memory behind the last row of the data is stale)
+                    // (384-thread instance only: the extra registers of the batch spill in the 512-thread one)
+                    const bool anyv = MAXT == 384 && HASV && __any_sync(MEB_FULL_MASK, myslot >= 0 && mylam != 0.0);
+                    if (anyv) {
+                        // active rows with a multiplier row v_i: b_i = c_i - c + v_i / sigma.  The pool rows come
+                        // from global memory; the loads of FOUR rows of my group are issued before any of them is
+                        // used (one dependent load per row made the pass latency-bound: config 4, every second
+                        // row).  Rows alternate between the two accumulation chains exactly as in the loop below.
+                        for (int rs = grp; rs < RPT; rs += 4 * RP) {
+                            double lam4[4];
+                            int sl4[4];
+                            V4 vb[4][CH];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                const int rq = rs + u * RP;
+                                lam4[u] = rq < RPT ? lam_w[warp][rq] : 0.0;
+                                sl4[u] = lam4[u] != 0.0 ? slot_w[warp][rq] : -1;
+                            }
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+#pragma unroll
+                                for (int q = 0; q < CH; ++q) {
+                                    const int ch = cl + 32 * q;
+                                    vb[u][q] = V4();
+                                    if (sl4[u] >= 0 && ch < nch) {
+                                        const T* vrow = Vg + (int64_t)sl4[u] * a.ldv + ch * VEC;
+                                        if (v16a) {
+                                            vb[u][q] = __ldg(reinterpret_cast<const V4*>(vrow));
+                                        } else {
+                                            T* vq = reinterpret_cast<T*>(&vb[u][q]);
+#pragma unroll
+                                            for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
+                                        }
+                                    }
+                                }
+                            }
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (lam4[u] == 0.0) continue;
+                                const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs + u * RP) * ldT);
+#pragma unroll
+                                for (int q = 0; q < CH; ++q) {
+                                    const int ch = cl + 32 * q;
+                                    if (ch < nch) {
+                                        const V4 ev4 = rp4[ch];
+                                        const T* e = reinterpret_cast<const T*>(&ev4);
+                                        const T* vq = reinterpret_cast<const T*>(&vb[u][q]);
+#pragma unroll
+                                        for (int j = 0; j < VEC; ++j) {
+                                            T bj = e[j] - creg[q][j];
+                                            if (sl4[u] >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
+                                            if (u & 1) vaccB[q][j] = fma(lam4[u], (double)bj, vaccB[q][j]);
+                                            else vacc[q][j] = fma(lam4[u], (double)bj, vacc[q][j]);
+                                        }
+                                    }
+                                }
+                            }
+                        }
+                    } else {
+                        const int rstep = RP * (ldT / VEC);               // 16-byte units between rows rs and rs + RP
+                        for (int rs = grp; rs < RPT; rs += 2 * RP) {      // two rows of my group per step
+                            const int rsB = rs + RP;
+                            const double lamA = lam_w[warp][rs];
+                            const double lamB = rsB < RPT ? lam_w[warp][rsB] : 0.0;
+                            if (lamA == 0.0 && lamB == 0.0) continue;
+                            const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
+                            const V4* rpB = rpA + rstep;
+                            const int slotA = (HASV && lamA != 0.0) ? slot_w[warp][rs] : -1;
+                            const int slotB = (HASV && lamB != 0.0) ? slot_w[warp][rsB] : -1;
+                            if (slotA >= 0 || slotB >= 0) {               // rows with a multiplier row, one at a time
+                                if (lamA != 0.0) grad_row(rpA, lamA, slotA, vacc);
+                                if (lamB != 0.0) grad_row(rpB, lamB, slotB, vaccB);
+                                continue;
+                            }
+                            // a row with lam = 0 adds exactly zero, without being read (shared memory behind the
+                            // last row of the data is stale)
 #pragma unroll
                             for (int q = 0; q < CH; ++q) {
                                 const int ch = cl + 32 * q;
@@ -434,9 +496,6 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                                     }
                                 }
                             }
-                        } else {
-                            if (lamA != 0.0) grad_row(rpA, lamA, slotA, vacc);
-                            if (lamB != 0.0) grad_row(rpB, lamB, slotB, vaccB);
                         }
                     }
                     __syncwarp();                                        // lam_w is rewritten by the next sub-tile

@@ -30,7 +30,7 @@ __device__ __forceinline__ double team_sum(double v, double* scratch) {
 }
 
 template <typename T, int TEAM, int MODE>
-__global__ void __launch_bounds__(MEB_BLOCK) active_kernel(const ActiveArgs a_in) {
+__global__ void __launch_bounds__(MEB_BLOCK, (MODE == MODE_WRITEV && TEAM == 32) ? 3 : 1) active_kernel(const ActiveArgs a_in) {
     ActiveArgs a = a_in;
     meb_resolve_dyn(a);
     extern __shared__ __align__(16) double acc_s[];          // [teams_per_block][dpad]

@@ -473,9 +473,32 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                             const V4* rpB = rpA + rstep;
                             const int slotA = (HASV && lamA != 0.0) ? slot_w[warp][rs] : -1;
                             const int slotB = (HASV && lamB != 0.0) ? slot_w[warp][rsB] : -1;
-                            if (slotA >= 0 || slotB >= 0) {               // rows with a multiplier row, one at a time
-                                if (lamA != 0.0) grad_row(rpA, lamA, slotA, vacc);
-                                if (lamB != 0.0) grad_row(rpB, lamB, slotB, vaccB);
+                            if (slotA >= 0 || slotB >= 0) {               // rows with a multiplier row
+                                if (CH == 1 && v16a) {                    // both pool loads before either is used
+                                    const int ch = cl;
+                                    if (ch < nch) {
+                                        V4 vA = V4(), vB = V4(), eA = V4(), eB = V4();
+                                        if (slotA >= 0) vA = __ldg(reinterpret_cast<const V4*>(Vg + (int64_t)slotA * a.ldv) + ch);
+                                        if (slotB >= 0) vB = __ldg(reinterpret_cast<const V4*>(Vg + (int64_t)slotB * a.ldv) + ch);
+                                        if (lamA != 0.0) eA = rpA[ch];
+                                        if (lamB != 0.0) eB = rpB[ch];
+                                        const T* ea = reinterpret_cast<const T*>(&eA);
+                                        const T* eb = reinterpret_cast<const T*>(&eB);
+                                        const T* va = reinterpret_cast<const T*>(&vA);
+                                        const T* vbq = reinterpret_cast<const T*>(&vB);
+#pragma unroll
+                                        for (int j = 0; j < VEC; ++j) {
+                                            T bA = ea[j] - creg[0][j], bB = eb[j] - creg[0][j];
+                                            if (slotA >= 0 && ch * VEC + j < d) bA = fma(va[j], inv_sig, bA);
+                                            if (slotB >= 0 && ch * VEC + j < d) bB = fma(vbq[j], inv_sig, bB);
+                                            vacc[0][j] = fma(lamA, (double)bA, vacc[0][j]);
+                                            vaccB[0][j] = fma(lamB, (double)bB, vaccB[0][j]);
+                                        }
+                                    }
+                                } else {
+                                    if (lamA != 0.0) grad_row(rpA, lamA, slotA, vacc);
+                                    if (lamB != 0.0) grad_row(rpB, lamB, slotB, vaccB);
+                                }
                                 continue;
                             }
                             // a row with lam = 0 adds exactly zero, without being read (shared memory behind the

@@ -22,7 +22,10 @@ THDT = {0: torch.float64, 1: torch.float32}
 # (m, d, ld_pad): spans every row mapping of the streaming kernel (G x CPT tiles, the loop kernel,
 # the unaligned scalar path), several tiles per warp and a ragged last tile
 SHAPES = [(1000, 10, 0), (4999, 32, 0), (3001, 100, 0), (777, 1000, 0), (70, 2600, 0), (257, 33, 0),
-          (64, 3, 1), (33, 1, 0), (1500, 20, 4), (513, 257, 1)]
+          (64, 3, 1), (33, 1, 0), (1500, 20, 4), (513, 257, 1),
+          # lane groups of the tile kernel's gradient part (2, 4, 8 or 16 lanes per row) and its 384-thread
+          # instance (stages of 8 KB and more: 256-byte rows in FP64 and FP32, 1024-byte rows)
+          (1203, 5, 0), (2000, 64, 0), (1031, 128, 0), (999, 16, 0)]
 
 
 @pytest.fixture(scope="module")

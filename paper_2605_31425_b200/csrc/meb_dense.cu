@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a_in, 
                 nb2 = fma(bd[e], bd[e], nb2);
             }
             nb2 = warp_sum(nb2);
-            const double inv = use ? 1.0 / sqrt(nb2) : 0.0;
+            const double inv = use ? rsqrt(nb2) : 0.0;
 #pragma unroll
             for (int e = 0; e < EPL; ++e)
                 if (lane + 32 * e < DP) W[(size_t)rr * DP + lane + 32 * e] = bd[e] * inv;

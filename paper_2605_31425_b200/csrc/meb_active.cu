@@ -40,6 +40,17 @@ __global__ void __launch_bounds__(MEB_BLOCK, (MODE == MODE_WRITEV && TEAM == 32)
     const int team = threadIdx.x / TEAM, tt = threadIdx.x % TEAM;
     const int d = a.d;
     double* acc = acc_s + (size_t)team * a.dpad;
+    if (MODE == MODE_ROWSUM && a.cut_part != nullptr) {
+        int cut = 0;
+        for (int b = threadIdx.x; b < a.cut_grid; b += MEB_BLOCK)
+            cut |= a.cut_part[(size_t)b * MEB_NPART + MEB_PART_CUT] != 0.0;
+        if (__syncthreads_or(cut)) {                         // rejected trial: zero partials, nothing to read
+            double* pv = a.part_vec + (size_t)blockIdx.x * a.dpad;
+            for (int j = threadIdx.x; j < a.dpad; j += MEB_BLOCK) pv[j] = 0.0;
+            if (threadIdx.x == 0) a.part_sc[blockIdx.x] = 0.0;
+            return;
+        }
+    }
     if (blockIdx.x * TPB >= *a.count) {                      // no list entry for this CTA: the finalize
         if (threadIdx.x == 0) a.part_sc[blockIdx.x] = 0.0;   // kernels skip its vector partial
         return;

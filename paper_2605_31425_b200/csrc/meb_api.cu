@@ -248,6 +248,7 @@ int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, double* out_scalars, doub
         rc = meb_ensure_list(ctx, c.m);
         if (rc != MEB_OK) return rc;
         ActiveArgs a = active_args(ctx, c);
+        if (c.gs) { a.cut_part = ctx->part_scalar; a.cut_grid = grid; }      // only a solve arms the early stop
         int nvec = 0;
         rc = meb_launch_active(ctx, MODE_ROWSUM, c.prec, a, &nvec);
         if (rc != MEB_OK) return rc;

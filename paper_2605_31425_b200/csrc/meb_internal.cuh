@@ -193,6 +193,9 @@ struct ActiveArgs {
     // the output buffers (the multiplier buffer that is NOT current)
     const MebDyn* dyn;
     void* U2[2]; int32_t* slot2[2]; void* V2[2]; int64_t vcap2[2];
+    // MODE_ROWSUM after a streaming evaluation: per-CTA partials of that pass ([cut_grid][MEB_NPART]); if any of
+    // its CTAs stopped early (MEB_PART_CUT: a doomed Armijo trial) the row sum is skipped, the trial is rejected anyway
+    const double* cut_part; int32_t cut_grid;
 };
 
 __device__ __forceinline__ void meb_resolve_dyn(ActiveArgs& a) {

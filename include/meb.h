@@ -89,6 +89,11 @@ typedef struct meb_params {
     double armijo_shrink_min;   /* a rejected Armijo trial halves eta, or multiplies it by this factor when the
                                  * parabola through Psi(x), Psi'(x; Delta), Psi(x + eta Delta) puts its minimiser
                                  * below it (trials bound to fail are skipped); 0.5 = plain halving (reading 4)  0.5  */
+    int32_t armijo_multi;       /* every Armijo trial pass also evaluates Psi at the next armijo_multi halvings of its
+                                 * step (same bytes, one more dot product per row), and halvings already known to fail
+                                 * are skipped (DESIGN reading 19); 0 = off                    4    */
+    int32_t ag_outer;           /* the first ag_outer outer iterations solve subproblem (4) with the accelerated
+                                 * gradient method instead of semismooth Newton (DESIGN reading 20)       0    */
 } meb_params;
 
 /* Counters and residuals of one meb_solve (host struct). */
@@ -118,6 +123,15 @@ typedef struct meb_stats {
     int64_t kernel_launches;    /* kernels of this library launched by the solve */
     int32_t passes_cut;         /* Armijo trial passes (counted in passes_*) stopped early because the partial sum
                                  * of Psi already exceeded Psi(x): certain rejections */
+    int32_t trials_skipped;     /* Armijo step sizes never evaluated because a trial pass had already shown that Psi at
+                                 * that step exceeds Psi(x) (multi-trial line search) */
+    /* the same per pass class, from CUDA-EVENT pairs recorded on the context's stream around every streaming
+     * launch: filled for launches made outside CUDA graphs (ingest, screen, feasibility always; the evaluation
+     * passes when the solve is host-stepped, MEB_OPT_STEPPED).  Passes that were cut short are left out. */
+    double pass_ev_ms[8];
+    double pass_ev_bytes[8];
+    int32_t pass_ev_count[8];
+    int32_t ag_iters;           /* accelerated-gradient inner iterations (meb_params.ag_outer) */
     int32_t reserved0;
 } meb_stats;
 
@@ -159,6 +173,18 @@ MEB_API const char* meb_strerror(int code);
 MEB_API int meb_last_cuda_error(const meb_ctx* ctx);           /* cudaError_t of the last MEB_E_CUDA */
 MEB_API void meb_default_params(meb_params* h_params);          /* fills the defaults listed above */
 MEB_API int meb_version(void);
+
+/* Behaviour switches of a context (tests, profiling and measurement; none changes a result).  At meb_create the
+ * environment variables MEB_NO_GRAPH, MEB_NO_SMALL, MEB_NO_ABORT (any value) preset the first three to 1. */
+enum {
+    MEB_OPT_STEPPED = 0,   /* 1: meb_solve sequences the SAME kernels and controller steps from the host instead of
+                            *    launching its CUDA graph (profilers list every launch; every streaming launch gets a
+                            *    CUDA-event pair, meb_stats.pass_ev_*) */
+    MEB_OPT_NO_SMALL = 1,  /* 1: small (reduced) problems run through the general kernels, not the single-CTA solver */
+    MEB_OPT_NO_ABORT = 2,  /* 1: doomed Armijo trials are not cut short (results are bit-identical either way) */
+    MEB_OPT_NCOUNT = 3
+};
+MEB_API int meb_set_option(meb_ctx* ctx, int option, int value);    /* MEB_E_ARG for an unknown option */
 
 /* ---- whole solve (Algorithm 1, Algorithm 2, Section 4.2) -------
  * centers, radii: DEVICE, FP64.  h_center_out[d], h_radius_out, h_stats: HOST.
@@ -222,7 +248,7 @@ MEB_API int meb_hvp(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C,
             const double* x, double sigma, double tau, const double* q, double* Hq);
 
 /* ---- a2': dense generalized Hessian, for moderate d (SURVEY 8(a) row a2') ---------------
- *   H[(d+1) x (d+1)] (device, double, row-major, full symmetric matrix).  d <= 256. */
+ *   H[(d+1) x (d+1)] (device, double, row-major, full symmetric matrix).  d <= 128 (else MEB_E_CAPACITY). */
 MEB_API int meb_dense_hessian(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
                       const void* R, const void* U, const int32_t* v_slot, const void* Vrows,
                       int64_t ldv, const double* x, double sigma, double tau, double* H);

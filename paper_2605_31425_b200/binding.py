@@ -20,6 +20,7 @@ MEB_E_ARG, MEB_E_INPUT, MEB_E_ALLOC, MEB_E_CUDA, MEB_E_CAPACITY = -1, -2, -3, -4
 MEB_FP64, MEB_FP32 = 0, 1
 MEB_MODE_FP64, MEB_MODE_MIXED = 0, 1
 MEB_EVAL_NSCALARS = 16
+OPT = dict(STEPPED=0, NO_SMALL=1, NO_ABORT=2)
 PASS = dict(INGEST=0, EVAL_FP64=1, EVAL_FP32=2, SCREEN=3, FEAS=4, EVAL_REDUCED=5)
 EV = dict(PSI=0, SUM_UPLUS=1, SUM_PROJ2=2, SUM_DMULT2=3, N_B1=4, N_B3=5, MAX_PFEAS=6, MAX_COMPL=7,
           MAX_DFEAS=8, SUM_RHO=9, NORM_SUM_VPLUS=10, N_ACTIVE=11)
@@ -28,7 +29,7 @@ EXPORTS = [
     "meb_create", "meb_destroy", "meb_strerror", "meb_last_cuda_error", "meb_default_params",
     "meb_version", "meb_solve", "meb_solve_host", "meb_ingest", "meb_eval_alm", "meb_hvp",
     "meb_dense_hessian", "meb_update_multipliers", "meb_screen_compact", "meb_feasibility_check",
-    "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch",
+    "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch", "meb_set_option",
 ]
 
 
@@ -38,7 +39,8 @@ class meb_params(C.Structure):
                 ("tol_lo", C.c_double), ("tol_red_factor", C.c_double),
                 ("armijo_max_halvings", C.c_int32), ("cg_max", C.c_int32), ("dense_d_max", C.c_int32),
                 ("inner_max", C.c_int32), ("outer_max", C.c_int32), ("max_rounds", C.c_int32),
-                ("sample_rows", C.c_int32), ("outer_max_lo", C.c_int32), ("armijo_shrink_min", C.c_double)]
+                ("sample_rows", C.c_int32), ("outer_max_lo", C.c_int32), ("armijo_shrink_min", C.c_double),
+                ("armijo_multi", C.c_int32), ("ag_outer", C.c_int32)]
 
 
 class meb_stats(C.Structure):
@@ -50,7 +52,9 @@ class meb_stats(C.Structure):
                 ("ms_total", C.c_double), ("ms_phase_lo", C.c_double), ("ms_phase_hi", C.c_double),
                 ("ms_check", C.c_double), ("bytes_streamed", C.c_double),
                 ("pass_ms", C.c_double * 8), ("pass_bytes", C.c_double * 8), ("pass_count", C.c_int32 * 8),
-                ("kernel_launches", C.c_int64), ("passes_cut", C.c_int32), ("reserved0", C.c_int32)]
+                ("kernel_launches", C.c_int64), ("passes_cut", C.c_int32), ("trials_skipped", C.c_int32),
+                ("pass_ev_ms", C.c_double * 8), ("pass_ev_bytes", C.c_double * 8), ("pass_ev_count", C.c_int32 * 8),
+                ("ag_iters", C.c_int32), ("reserved0", C.c_int32)]
 
     def as_dict(self):
         out = {}
@@ -88,6 +92,7 @@ def load():
     lib.meb_default_params.argtypes = [C.POINTER(meb_params)]
     lib.meb_default_params.restype = None
     lib.meb_set_pass_timing.argtypes = [vp, C.c_int]
+    lib.meb_set_option.argtypes = [vp, C.c_int, C.c_int]
     lib.meb_last_pass_info.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
     solve_args = [vp, i64, i32, vp, i64, vp, dbl, C.c_int, C.POINTER(meb_params), vp, C.POINTER(dbl),
                   C.POINTER(meb_stats)]
@@ -186,6 +191,10 @@ class Context:
 
 def meb_set_pass_timing(ctx: Context, on: bool):
     _check(load().meb_set_pass_timing(ctx.h, int(bool(on))), "meb_set_pass_timing")
+
+
+def meb_set_option(ctx: Context, option: int, value: bool):
+    _check(load().meb_set_option(ctx.h, int(option), int(bool(value))), "meb_set_option")
 
 
 def meb_last_pass_info(ctx: Context):

@@ -34,10 +34,12 @@ static void ctx_free_all(meb_ctx* c) {
         for (int i = 0; i < 2 * MEB_EVPOOL; ++i) if (c->evpool[i]) cudaEventDestroy(c->evpool[i]);
         free(c->evpool);
     }
+    for (int i = 0; i < 4; ++i) if (c->ev_solve[i]) cudaEventDestroy(c->ev_solve[i]);
+    for (int i = 0; i < 8; ++i) if (c->ev_stage[i]) cudaEventDestroy(c->ev_stage[i]);
 }
 
-void meb_debug_cuda(const char* file, int line, int err) {
-    if (getenv("MEB_DEBUG")) fprintf(stderr, "[meb] %s:%d: CUDA error %d (%s)\n", file, line, err, cudaGetErrorString((cudaError_t)err));
+void meb_debug_cuda(const meb_ctx* ctx, const char* file, int line, int err) {
+    if (ctx && ctx->debug) fprintf(stderr, "[meb] %s:%d: CUDA error %d (%s)\n", file, line, err, cudaGetErrorString((cudaError_t)err));
 }
 
 extern "C" int meb_version(void) { return 100; }
@@ -63,6 +65,7 @@ extern "C" void meb_default_params(meb_params* p) {
     p->armijo_mu = 1e-4; p->tol_lo = 1e-2; p->tol_red_factor = 0.02;
     p->armijo_max_halvings = 30; p->cg_max = 500; p->dense_d_max = 128; p->inner_max = 50;
     p->outer_max = 200; p->max_rounds = 10; p->sample_rows = 1024; p->outer_max_lo = 30;
+    p->armijo_multi = 4; p->ag_outer = 0;
 }
 
 extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t m_max, int32_t d_max) {
@@ -84,7 +87,7 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     const size_t dpad = round_up((size_t)d_max + 1, 8);
     c->vec_rows = 2 * (int64_t)(c->sm_count > 0 ? c->sm_count : 148);
     c->small_len = SM_X + (int64_t)dpad + 64;
-    c->h_pinned_len = 4 * (int64_t)dpad + 256;
+    c->h_pinned_len = 12 * (int64_t)dpad + 256;     // [0, 4 dpad + 256): read-backs; then 8 upload slots of dpad
 #define TRY_ALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void**)&(ptr), (bytes))
     TRY_ALLOC(c->mask, nwords * sizeof(uint32_t));
     TRY_ALLOC(c->rec_lam, (size_t)m_max * sizeof(double));
@@ -115,6 +118,12 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
         if (!c->evpool) e = cudaErrorMemoryAllocation;
         for (int i = 0; e == cudaSuccess && i < 2 * MEB_EVPOOL; ++i) e = cudaEventCreate(&c->evpool[i]);
     }
+    for (int i = 0; e == cudaSuccess && i < 4; ++i) e = cudaEventCreate(&c->ev_solve[i]);
+    for (int i = 0; e == cudaSuccess && i < 8; ++i) e = cudaEventCreateWithFlags(&c->ev_stage[i], cudaEventDisableTiming);
+    c->opt[MEB_OPT_STEPPED] = getenv("MEB_NO_GRAPH") ? 1 : 0;
+    c->opt[MEB_OPT_NO_SMALL] = getenv("MEB_NO_SMALL") ? 1 : 0;
+    c->opt[MEB_OPT_NO_ABORT] = getenv("MEB_NO_ABORT") ? 1 : 0;
+    c->debug = getenv("MEB_DEBUG") != nullptr;
     c->cur_class = MEB_PASS_NCLASS - 1;
     if (e == cudaSuccess) e = cudaMemsetAsync(c->count_dev, 0, 8 * sizeof(int32_t), c->stream);
     if (e != cudaSuccess) {
@@ -138,6 +147,12 @@ extern "C" int meb_destroy(meb_ctx* ctx) {
 }
 
 extern "C" int meb_last_cuda_error(const meb_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
+
+extern "C" int meb_set_option(meb_ctx* ctx, int option, int value) {
+    if (!ctx || option < 0 || option >= MEB_OPT_NCOUNT) return MEB_E_ARG;
+    ctx->opt[option] = value != 0;
+    return MEB_OK;
+}
 
 extern "C" int meb_set_pass_timing(meb_ctx* ctx, int on) {
     if (!ctx) return MEB_E_ARG;
@@ -173,7 +188,8 @@ static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, dou
     if (pool) {
         MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn + 1], ctx->stream));
         ctx->evclass[ctx->evn] = ctx->cur_class;
-        ctx->evbytes[ctx->evn] = bytes;
+        ctx->evbytes[ctx->evn] = bytes + (op == OP_EVAL ? ctx->ev_extra_bytes : 0.0);
+        ctx->evcut[ctx->evn] = false;
         ctx->evn++;
     }
     ctx->last_grid = *grid;
@@ -384,7 +400,8 @@ extern "C" int meb_screen_compact(meb_ctx* ctx, int64_t m, int32_t d, const floa
                                   const float* R32, float r_hat, const double* c_hat, float tol_red,
                                   int32_t* idx_out, int64_t cap, int64_t* h_count, uint8_t* flags,
                                   int flags_are_input) {
-    if (!ctx || !idx_out || cap < 0 || m < 1 || m > ctx->m_max) return MEB_E_ARG;
+    if (!ctx || !idx_out || cap < 0 || m < 1) return MEB_E_ARG;
+    if (m > ctx->m_max) return MEB_E_CAPACITY;
     int rc;
     if (flags_are_input) {
         if (!flags) return MEB_E_ARG;

@@ -35,7 +35,8 @@ struct SolverDev {
     // ---- in-graph timing of the evaluation passes (globaltimer, ns) ----
     unsigned long long pass_ns;
     long long pass_count;
-    unsigned long long vrow_reads;  // sum over the evaluation passes of the V rows they read (balls with u_i > 0)
+    unsigned long long vrow_reads;  // sum over the evaluation passes that ran to the end (the ones pass_ns / pass_count
+                                    // cover) of the V rows they read: one per ball with a slot, i.e. n_support
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
     double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
@@ -213,7 +214,6 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
             ctrl_arm_abort(S, !stalled, v.xn[0] + eta * v.delta[0], dx2t);
             if (stalled) { S->phase = PH_REEVAL; } else { S->eta = eta; S->ls++; }
             S->action = ACT_TRIAL; S->evals++;
-            S->vrow_reads += (unsigned long long)(S->dyn.has_mult ? S->n_support : 0);
             if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
             ctrl_set_handles(S);
         }
@@ -239,7 +239,6 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     ctrl_block_sum3(agx, gg, dx2, sm);
     if (threadIdx.x == 0) {
         S->evals++;
-        S->vrow_reads += (unsigned long long)(S->dyn.has_mult ? S->n_support : 0);
         S->psi_cur = psi_t;
         double terms[5];
         const double kkt = ctrl_rel_kkt(ev_s, Ls * sm[96], terms);

@@ -66,17 +66,26 @@ struct meb_ctx {
     void* h_sdev;           // pinned host mirror
     void* graph_cache;      // instantiated solve graphs (meb_solver.cu)
     cudaStream_t cap_stream; // private stream used only to CAPTURE graphs (the legacy default stream cannot capture)
+    // ---- behaviour switches (meb_set_option; preset from the environment in meb_create) ----
+    int opt[MEB_OPT_NCOUNT];
+    bool debug;             // MEB_DEBUG: print file:line of CUDA errors
+    // ---- per-context events and pinned staging ring of meb_solve ----
+    cudaEvent_t ev_solve[4];        // start, end of the low-precision phase, end of the FP64 phase, end
+    cudaEvent_t ev_stage[8];        // one per slot of the pinned upload ring (the slot is free once its copy ran)
+    int stage_next;
+    bool evcut[MEB_EVPOOL];         // stepped solves: the launch was a trial pass that was cut short
+    double ev_extra_bytes;          // stepped solves: bytes of the multiplier rows the next evaluation pass reads
 };
 
-// prints file:line and the CUDA error string to stderr when the environment variable MEB_DEBUG is set
-void meb_debug_cuda(const char* file, int line, int err);
+// prints file:line and the CUDA error string to stderr when the context was created with MEB_DEBUG set
+void meb_debug_cuda(const meb_ctx* ctx, const char* file, int line, int err);
 
 #define MEB_CUDA_OK(ctx, expr)                                   \
     do {                                                         \
         cudaError_t e__ = (expr);                                \
         if (e__ != cudaSuccess) {                                \
             (ctx)->last_cuda_error = (int)e__;                   \
-            meb_debug_cuda(__FILE__, __LINE__, (int)e__);        \
+            meb_debug_cuda((ctx), __FILE__, __LINE__, (int)e__); \
             return MEB_E_CUDA;                                   \
         }                                                        \
     } while (0)

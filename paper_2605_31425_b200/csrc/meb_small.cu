@@ -114,7 +114,10 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
                 const int q = sS.evals < 48 ? sS.evals : 47;          // MEB_TRACE history, indexed by evaluation
                 sS.pass_hist[q] = (uint32_t)(t1 - t0);
                 sS.act_hist[q] = cut ? 0xffffffffu : (uint32_t)(sc[3] + sc[4]);
-                if (!cut) { sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++; }
+                if (!cut) {
+                    sS.pass_ns += (unsigned long long)(t1 - t0); sS.pass_count++;
+                    sS.vrow_reads += (unsigned long long)(sS.dyn.has_mult ? sS.n_support : 0);
+                }
             }
         }
         double* out = ev_s;

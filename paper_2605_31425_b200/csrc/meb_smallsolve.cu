@@ -505,7 +505,9 @@ int meb_launch_small_solve(meb_ctx* ctx, const void* C, int64_t ld, const void* 
     a.S = S; a.v = v;
     a.m_cap = (int32_t)((m + 15) / 16 * 16);
     long long* prof = nullptr;
+#ifdef MEB_TUNING
     if (getenv("MEB_TRACE")) { cudaMalloc(&prof, 8 * sizeof(long long)); cudaMemset(prof, 0, 8 * sizeof(long long)); }
+#endif
     a.prof = prof;
     const int n = d + 1;
     const int bs = (n + 1 + 15) / 16;
@@ -538,7 +540,7 @@ int meb_launch_small_solve(meb_ctx* ctx, const void* C, int64_t ld, const void* 
 
 // ---- C-ABI: batched solves ---------------------------------------------------------------------------
 namespace {
-constexpr int OWN_BATCH = 20;          // slot of meb_ctx::own used by meb_solve_batch
+constexpr int OWN_BATCH = 20;          // slot of meb_ctx::own used by meb_solve_batch (OWN_BATCH_RESERVED in meb_solver.cu)
 
 int batch_reserve(meb_ctx* ctx, size_t bytes) {
     if (ctx->own_bytes[OWN_BATCH] >= bytes) return MEB_OK;

@@ -21,8 +21,10 @@
 
 namespace {
 
+// slots of meb_ctx::own (20 = the batch solver's block, meb_smallsolve.cu)
 enum { OWN_U0 = 0, OWN_U1, OWN_S0, OWN_S1, OWN_V0, OWN_V1, OWN_C32, OWN_R32, OWN_IDX, OWN_CRED, OWN_RRED,
-       OWN_KEPT, OWN_STATE, OWN_HOSTC, OWN_HOSTR, OWN_SPARE, OWN_VRED0, OWN_VRED1, OWN_DEVC, OWN_DEVR };
+       OWN_KEPT, OWN_STATE, OWN_UREDA, OWN_UREDB, OWN_SREDA, OWN_VRED0, OWN_VRED1, OWN_DEVC, OWN_DEVR,
+       OWN_BATCH_RESERVED, OWN_SREDB, OWN_WC };
 
 int own_reserve(meb_ctx* ctx, int slot, size_t bytes) {
     if (ctx->own_bytes[slot] >= bytes && ctx->own[slot]) return MEB_OK;
@@ -31,6 +33,25 @@ int own_reserve(meb_ctx* ctx, int slot, size_t bytes) {
     cudaError_t e = cudaMalloc(&ctx->own[slot], want);
     if (e != cudaSuccess) { cudaGetLastError(); ctx->last_cuda_error = (int)e; return MEB_E_ALLOC; }
     ctx->own_bytes[slot] = want;
+    return MEB_OK;
+}
+
+// Grow own[slot] to at least `bytes`, keeping its first `keep` bytes (the reduced problem when violated balls are
+// re-introduced).  The stream is drained before the old block is freed.
+int own_grow_keep(meb_ctx* ctx, int slot, size_t bytes, size_t keep) {
+    if (ctx->own_bytes[slot] >= bytes && ctx->own[slot]) return MEB_OK;
+    void* fresh = nullptr;
+    cudaError_t e = cudaMalloc(&fresh, bytes < 256 ? 256 : bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); ctx->last_cuda_error = (int)e; return MEB_E_ALLOC; }
+    if (ctx->own[slot] && keep > 0) {
+        const size_t n = keep < ctx->own_bytes[slot] ? keep : ctx->own_bytes[slot];
+        e = cudaMemcpyAsync(fresh, ctx->own[slot], n, cudaMemcpyDeviceToDevice, ctx->stream);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { cudaFree(fresh); ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
+    if (ctx->own[slot]) cudaFree(ctx->own[slot]);
+    ctx->own[slot] = fresh;
+    ctx->own_bytes[slot] = bytes < 256 ? 256 : bytes;
     return MEB_OK;
 }
 
@@ -66,11 +87,16 @@ void to_raw(const Solver& S, const Problem& P, const std::vector<double>& xn, st
 }
 
 int upload(meb_ctx* ctx, double* dst, const double* src, size_t n) {
-    // staged through pinned memory so that the copy is truly asynchronous and ordered on the stream
-    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
-    double* stage = ctx->h_pinned + ctx->h_pinned_len / 2;      // second half of the pinned mirror
+    // staged through a ring of 8 pinned slots so that the copy is truly asynchronous and ordered on the stream
+    // without draining it: a slot is reused only after the copy that last read it has run (its event)
+    const int64_t dpad = (ctx->h_pinned_len - 256) / 12;
+    const int slot = ctx->stage_next;
+    ctx->stage_next = (slot + 1) & 7;
+    MEB_CUDA_OK(ctx, cudaEventSynchronize(ctx->ev_stage[slot]));
+    double* stage = ctx->h_pinned + 4 * dpad + 256 + (int64_t)slot * dpad;
     memcpy(stage, src, n * sizeof(double));
     MEB_CUDA_OK(ctx, cudaMemcpyAsync(dst, stage, n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev_stage[slot], ctx->stream));
     return MEB_OK;
 }
 
@@ -197,7 +223,7 @@ int seq_update(Seq& q) {
 }
 
 #define RC(expr) do { rc = (expr); if (rc != MEB_OK) goto fail; } while (0)
-#define CU(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { ctx->last_cuda_error = (int)e__; meb_debug_cuda(__FILE__, __LINE__, (int)e__); rc = MEB_E_CUDA; goto fail; } } while (0)
+#define CU(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { ctx->last_cuda_error = (int)e__; meb_debug_cuda(ctx, __FILE__, __LINE__, (int)e__); rc = MEB_E_CUDA; goto fail; } } while (0)
 
 int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     meb_ctx* ctx = S.ctx;
@@ -296,11 +322,16 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
     Seq q;
     seq_init(q, S, P, dense);
     SolverDev* dev = q.dev;
+    int cut_seen = h->aborted;
     for (;;) {
+        ctx->ev_extra_bytes = h->dyn.has_mult ? (double)h->n_support * (double)P.d * (double)esz(P.prec) : 0.0;
         int rc = seq_eval(q);
         if (rc) return rc;
         MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
         MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+        if (h->aborted > cut_seen && ctx->evn > 0) ctx->evcut[ctx->evn - 1] = true;   // the pass just timed was cut short
+        cut_seen = h->aborted;
+#ifdef MEB_TUNING
         if (getenv("MEB_TRACE") && atoi(getenv("MEB_TRACE")) >= 2) {
             double ev[MEB_EVAL_NSCALARS];
             cudaMemcpy(ev, S.v.ev_t, sizeof(ev), cudaMemcpyDeviceToHost);
@@ -317,10 +348,11 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
                     if (s1 > t1max) { t1max = s1; slow = b; }
                 }
                 fprintf(stderr, "[meb trace]     pass %lld ns, last CTA %d; CTA durations:", t1max - t0min, slow);
-                for (int b = 0; b < 148; b += 7) { long long s0, s1; memcpy(&s0, &hp[b * MEB_NPART + 10], 8); memcpy(&s1, &hp[b * MEB_NPART + 11], 8); fprintf(stderr, " %lld(+%lld)", s1 - s0, s0 - t0min); }
+                for (int b = 0; b < 148; ++b) { long long s0, s1; memcpy(&s0, &hp[b * MEB_NPART + 10], 8); memcpy(&s1, &hp[b * MEB_NPART + 11], 8); fprintf(stderr, " %lld", s1 - s0); }
                 fprintf(stderr, "\n");
             }
         }
+#endif
         if (h->done) return MEB_OK;
         if (h->action == ACT_NEWTON) {
             if (dense) {
@@ -342,6 +374,7 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
                 if (rc) return rc;
             }
         } else if (h->action == ACT_UPDATE) {
+#ifdef MEB_TUNING
             if (getenv("MEB_TRACE")) {
                 double ev[MEB_EVAL_NSCALARS];
                 cudaMemcpy(ev, S.v.ev, sizeof(ev), cudaMemcpyDeviceToHost);
@@ -349,6 +382,7 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
                         h->outer, h->sigma, h->inner, h->evals, h->kkt, h->terms[0], h->terms[1], h->terms[2], h->terms[3],
                         h->terms[4], ev[MEB_EV_N_B1], ev[MEB_EV_N_B3], h->psi_cur);
             }
+#endif
             rc = seq_update(q);
             if (rc) return rc;
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(h, dev, sizeof(*h), cudaMemcpyDeviceToHost, ctx->stream));
@@ -429,9 +463,9 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         if (P.off) { rc = upload(ctx, S.v.off, P.off, S.d); if (rc) return rc; }
     }
     bool first = true;
-    bool stepped = getenv("MEB_NO_GRAPH") != nullptr;
+    bool stepped = ctx->opt[MEB_OPT_STEPPED] != 0;
     // small problems (the reduced problem of the mixed mode, small instances): one persistent CTA runs the phase
-    bool small = dense && !getenv("MEB_NO_SMALL") && meb_small_applicable(P.prec, P.m, P.d);
+    bool small = dense && !ctx->opt[MEB_OPT_NO_SMALL] && meb_small_applicable(P.prec, P.m, P.d);
     if (small) {
         for (int b = 0; b < 2 && small; ++b)
             if (P.vcap[b] < P.m) { if (P.own_v[b] < 0 || grow_pool(ctx, P, b, P.m) != MEB_OK) small = false; }
@@ -456,7 +490,6 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             h->L = S.L; h->tol = tol; h->tol_accept = tol_accept; h->rho = par.rho; h->tau = par.tau; h->kappa = par.kappa;
             h->sigma_max = par.sigma_max; h->armijo_mu = par.armijo_mu;
             h->shrink_min = (par.armijo_shrink_min > 0.0 && par.armijo_shrink_min <= 0.5) ? par.armijo_shrink_min : 0.5;
-            if (getenv("MEB_SHRINK_MIN")) h->shrink_min = atof(getenv("MEB_SHRINK_MIN"));
             h->n = n; h->d = S.d; h->inner_max = par.inner_max; h->outer_max = outer_cap;
             h->armijo_max = par.armijo_max_halvings; h->cg_max = par.cg_max; h->dense = dense ? 1 : 0;
             h->use_off = P.off ? 1 : 0;
@@ -465,10 +498,13 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
                 if (h->inner_max > 20) h->inner_max = 20;
             }
             h->slope_floor = (P.prec == MEB_FP32) ? 1e-7 : 2e-15;
-            h->abort_margin = getenv("MEB_NO_ABORT") ? 0.0 : ((P.prec == MEB_FP32) ? 1e-3 : 1e-6);
+            h->abort_margin = ctx->opt[MEB_OPT_NO_ABORT] ? 0.0 : ((P.prec == MEB_FP32) ? 1e-3 : 1e-6);
             h->stall_max = (P.prec == MEB_FP32) ? 3 : 6;   // the FP32 run only has to deliver a warm start
+#ifdef MEB_TUNING
+            if (getenv("MEB_SHRINK_MIN")) h->shrink_min = atof(getenv("MEB_SHRINK_MIN"));
             if (getenv("MEB_STALL_MAX")) h->stall_max = atoi(getenv("MEB_STALL_MAX"));
             if (getenv("MEB_SLOPE_FLOOR")) h->slope_floor = atof(getenv("MEB_SLOPE_FLOOR"));
+#endif
             h->eval_cap = 4 * outer_cap * (par.inner_max + 2);
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
@@ -511,6 +547,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             continue;
         }
         // ---- phase finished ----
+#ifdef MEB_TUNING
         if (getenv("MEB_TRACE")) {
             fprintf(stderr, "[meb trace] %d of %d passes cut short; eval passes (ns / active):", h->aborted, h->evals);
             for (int q = 0; q < h->evals && q < 48; ++q) {
@@ -519,6 +556,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             }
             fprintf(stderr, "\n");
         }
+#endif
         S.st->outer_iters += h->outer;
         S.st->newton_iters += h->newton_total;
         S.st->cg_iters += h->cg_total;
@@ -569,6 +607,39 @@ int setup_multipliers(meb_ctx* ctx, Problem& P, int ownU0, int ownS0, int ownV0)
     return MEB_OK;
 }
 
+// resets the per-solve recording state of the context on every way out of meb_solve
+struct SolveScope {
+    meb_ctx* ctx; bool timing_was;
+    explicit SolveScope(meb_ctx* c) : ctx(c), timing_was(c->time_passes) { c->evn = 0; c->ev_record = true; c->ev_extra_bytes = 0.0; }
+    ~SolveScope() { ctx->ev_record = false; ctx->time_passes = timing_was; ctx->ev_extra_bytes = 0.0; }
+};
+
+// buffers of the reduced problem: rows, radii, double-buffered multipliers with a dense V (slot k = k)
+struct Reduced {
+    int64_t cap; int64_t ldr; int32_t d; bool radii;
+};
+int reduced_reserve(meb_ctx* ctx, Reduced& Q, int64_t cap, int64_t keep_rows) {
+    const size_t row = (size_t)Q.ldr * sizeof(double);
+    int rc = own_grow_keep(ctx, OWN_CRED, (size_t)cap * row, (size_t)keep_rows * row);
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_RRED, (size_t)cap * sizeof(double), (size_t)keep_rows * sizeof(double));
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_UREDA, (size_t)cap * sizeof(double), (size_t)keep_rows * sizeof(double));
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_UREDB, (size_t)cap * sizeof(double), (size_t)keep_rows * sizeof(double));
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_SREDA, (size_t)cap * sizeof(int32_t), (size_t)keep_rows * sizeof(int32_t));
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_SREDB, (size_t)cap * sizeof(int32_t), (size_t)keep_rows * sizeof(int32_t));
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_VRED0, (size_t)cap * row, (size_t)keep_rows * row);
+    if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_VRED1, (size_t)cap * row, (size_t)keep_rows * row);
+    if (rc == MEB_OK) Q.cap = cap;
+    return rc;
+}
+void reduced_bind(meb_ctx* ctx, const Reduced& Q, Problem& P2) {
+    P2.C = ctx->own[OWN_CRED]; P2.ld = Q.ldr; P2.R = Q.radii ? ctx->own[OWN_RRED] : nullptr;
+    P2.U[0] = ctx->own[OWN_UREDA]; P2.U[1] = ctx->own[OWN_UREDB];
+    P2.slot[0] = (int32_t*)ctx->own[OWN_SREDA]; P2.slot[1] = (int32_t*)ctx->own[OWN_SREDB];
+    P2.V[0] = ctx->own[OWN_VRED0]; P2.V[1] = ctx->own[OWN_VRED1];
+    P2.vcap[0] = P2.vcap[1] = Q.cap;
+    P2.own_v[0] = P2.own_v[1] = -1;
+}
+
 }  // namespace
 
 extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_t ld,
@@ -591,23 +662,19 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
     // The KKT test runs at tol/10: the primal-feasibility term only bounds the error of the returned
     // (feasible) radius by about tol (1 + r)/r, and the contract is a radius within tol (DESIGN reading 7).
     const double tol_kkt = 0.1 * tol;
-    const bool timing_was = ctx->time_passes;
-    ctx->evn = 0;
-    ctx->ev_record = true;
+    SolveScope scope(ctx);
     const int64_t launches0 = ctx->launches;
-    cudaEvent_t e_start, e_mid, e_hi, e_end;
-    MEB_CUDA_OK(ctx, cudaEventCreate(&e_start));
-    MEB_CUDA_OK(ctx, cudaEventCreate(&e_mid));
-    MEB_CUDA_OK(ctx, cudaEventCreate(&e_hi));
-    MEB_CUDA_OK(ctx, cudaEventCreate(&e_end));
+    cudaEvent_t e_start = ctx->ev_solve[0], e_mid = ctx->ev_solve[1], e_hi = ctx->ev_solve[2], e_end = ctx->ev_solve[3];
+    bool have_mid = false, have_hi = false;
     int rc = MEB_OK;
     std::vector<double> c0(d), xn(n, 0.0), ab, creturn(d);
     bool converged = false;
     double kkt = INFINITY, terms[5] = {0, 0, 0, 0, 0};
     Problem P;
     memset(&P, 0, sizeof(P));
+#define CUB(expr) { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { ctx->last_cuda_error = (int)e__; meb_debug_cuda(ctx, __FILE__, __LINE__, (int)e__); rc = MEB_E_CUDA; break; } }
     do {
-        MEB_CUDA_OK(ctx, cudaEventRecord(e_start, ctx->stream));
+        CUB(cudaEventRecord(e_start, ctx->stream));
         // ---- state vectors on the device ----
         const size_t nH = (d <= 128) ? (size_t)n * n + 8 : 8;
         const size_t nv = ((size_t)n + 7) / 8 * 8;
@@ -638,10 +705,8 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         if (rc) break;
         st->passes_fp64_full++;
         S.bytes += ctx->last_pass_bytes;
-        MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_AUX, 3 * sizeof(double),
-                                         cudaMemcpyDeviceToHost, ctx->stream));
-        MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned + 16, dc0, d * sizeof(double), cudaMemcpyDeviceToHost,
-                                         ctx->stream));
+        CUB(cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_AUX, 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CUB(cudaMemcpyAsync(ctx->h_pinned + 16, dc0, d * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
         rc = sync_stream(ctx);
         if (rc) break;
         if (ctx->h_pinned[2] > 0.0 || !(ctx->h_pinned[0] < 1.79e308)) { rc = MEB_E_INPUT; break; }
@@ -653,8 +718,6 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             *h_radius_out = 0.0;
             converged = true;
             kkt = 0.0;
-            MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
-            MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
             break;
         }
         xn[0] = 1.0;                              // x~0 = (1, 0), feasible
@@ -665,19 +728,19 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             P.off = c0.data(); P.full = true;
             rc = setup_multipliers(ctx, P, OWN_U0, OWN_S0, OWN_V0);
             if (rc) break;
-            MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
+            CUB(cudaEventRecord(e_mid, ctx->stream)); have_mid = true;
             rc = ripalm(S, P, xn, ab, tol_kkt, tol, &converged, &kkt, terms, S.par.outer_max);
             if (rc) break;
-            MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
+            CUB(cudaEventRecord(e_hi, ctx->stream)); have_hi = true;
             // final full pass: r_out = max_i(||c - c_i|| + r_i)   (step 7)
             std::vector<double> xr;
             to_raw(S, P, xn, xr);
             rc = upload(ctx, S.v.x_raw, xr.data(), n);
             if (rc) break;
             r_alg = xr[0];
-            int32_t am = 0; int64_t nv = 0;
+            int32_t am = 0; int64_t nvl = 0;
             rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, INFINITY, nullptr, &dmax,
-                                       &am, nullptr, 0, &nv);
+                                       &am, nullptr, 0, &nvl);
             if (rc) break;
             st->passes_fp64_full++;
             S.bytes += ctx->last_pass_bytes;
@@ -695,7 +758,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             rc = ripalm(S, P1, xn, ab, S.par.tol_lo, S.par.tol_lo, &conv1, &kkt1, terms1,
                         S.par.outer_max_lo > 0 ? S.par.outer_max_lo : S.par.outer_max);
             if (rc) break;
-            MEB_CUDA_OK(ctx, cudaEventRecord(e_mid, ctx->stream));
+            CUB(cudaEventRecord(e_mid, ctx->stream)); have_mid = true;
             // ---- screening, tol_red = 0.02 r_hat (reading 9) ----
             rc = own_reserve(ctx, OWN_IDX, ((size_t)m + 32) * sizeof(int32_t));
             if (rc) break;
@@ -711,26 +774,41 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             if (rc) break;
             st->passes_fp32_full++;
             S.bytes += ctx->last_pass_bytes;
-            if (nred == 0) { rc = MEB_E_INPUT; break; }
+            Problem P2;
+            memset(&P2, 0, sizeof(P2));
+            P2.prec = MEB_FP64; P2.d = d; P2.off = c0.data(); P2.full = false;
+            if (nred == 0) {
+                // nothing passed the retain rule (a useless coarse ball): keep the farthest ball, as the oracle does
+                // (oracle/ripalm.py, P:L281-283 then brings back whatever is violated)
+                std::vector<double> xr0;
+                to_raw(S, P2, xn, xr0);
+                rc = upload(ctx, S.v.x_raw, xr0.data(), n);
+                if (rc) break;
+                int32_t am0 = 0; int64_t nv0 = 0; double dm0 = 0.0;
+                rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, xr0[0], S.v.x_raw + 1, INFINITY, nullptr, &dm0,
+                                           &am0, nullptr, 0, &nv0);
+                if (rc) break;
+                st->passes_fp64_full++;
+                S.bytes += ctx->last_pass_bytes;
+                rc = meb_fill_i32(ctx, idx, 1, am0);
+                if (rc) break;
+                nred = 1;
+            }
             rc = own_reserve(ctx, OWN_KEPT, (size_t)m);
             if (rc) break;
             uint8_t* kept = (uint8_t*)ctx->own[OWN_KEPT];
             rc = meb_fill_u8(ctx, kept, m, 0);
             if (rc) break;
             // ---- reduced problem: gather rows and multipliers ----
-            const int64_t ldr = (d + 1) / 2 * 2;
-            int64_t cap_red = 2 * nred + 1024;               // room for re-introduced balls
-            if (cap_red > m) cap_red = m;
-            rc = own_reserve(ctx, OWN_CRED, (size_t)cap_red * ldr * sizeof(double));
-            if (rc) break;
-            rc = own_reserve(ctx, OWN_RRED, (size_t)cap_red * sizeof(double));
-            if (rc) break;
-            rc = own_reserve(ctx, OWN_HOSTC, (size_t)cap_red * sizeof(double));        // U buffer a
-            if (rc) break;
-            rc = own_reserve(ctx, OWN_HOSTR, (size_t)cap_red * sizeof(double));        // U buffer b
-            if (rc) break;
-            rc = own_reserve(ctx, OWN_SPARE, (size_t)cap_red * 2 * sizeof(int32_t));   // slot buffers a, b
-            if (rc) break;
+            Reduced Q;
+            Q.cap = 0; Q.ldr = (d + 1) / 2 * 2; Q.d = d; Q.radii = radii != nullptr;
+            {
+                int64_t cap_red = 2 * nred + 1024;           // room for re-introduced balls; grows on demand
+                if (cap_red > m) cap_red = m;
+                rc = reduced_reserve(ctx, Q, cap_red, 0);
+                if (rc) break;
+            }
+            const int64_t ldr = Q.ldr;
             rc = meb_gather_rows_f64(ctx, centers, ld, idx, nred, d, (double*)ctx->own[OWN_CRED], ldr);
             if (rc) break;
             if (radii) {
@@ -739,107 +817,99 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             }
             rc = meb_set_kept(ctx, idx, nred, kept);
             if (rc) break;
-            Problem P2;
-            memset(&P2, 0, sizeof(P2));
-            {
-                double* Cred = (double*)ctx->own[OWN_CRED];
-                double* Rred = radii ? (double*)ctx->own[OWN_RRED] : nullptr;
-                // reduced multipliers: dense V (slot k = k) of capacity cap_red rows, double-buffered
-                // (context-owned buffers: stable addresses keep the cached solve graph valid across solves)
-                void* Vred[2] = {nullptr, nullptr};
-                rc = own_reserve(ctx, OWN_VRED0, (size_t)cap_red * ldr * sizeof(double));
+            P2.ldv = ldr;
+            reduced_bind(ctx, Q, P2);
+            P2.cur = 0; P2.has_mult = true;
+            // warm start restricted to I_red.  If the low-precision run did not reach its
+            // tolerance (degenerate supports: reading 17) its multipliers are noise: start from zero.
+            if (P1.has_mult && conv1)
+                rc = meb_gather_mult(ctx, (const float*)P1.U[P1.cur], P1.slot[P1.cur], (const float*)P1.V[P1.cur],
+                                     P1.ldv, idx, nred, d, (double*)P2.U[0], P2.slot[0], (double*)P2.V[0], ldr);
+            else
+                P2.has_mult = false;
+            if (rc) break;
+            ab = xn;                                        // reading 11
+            for (int rnd = 0; rc == MEB_OK && rnd < S.par.max_rounds; ++rnd) {
+                P2.m = nred;
+                st->n_reduced = nred;
+                st->rounds = rnd + 1;
+                rc = ripalm(S, P2, xn, ab, tol_kkt, tol, &converged, &kkt, terms, S.par.outer_max);
                 if (rc) break;
-                rc = own_reserve(ctx, OWN_VRED1, (size_t)cap_red * ldr * sizeof(double));
+                if (rnd == 0) { CUB(cudaEventRecord(e_hi, ctx->stream)); have_hi = true; }
+                // a-posteriori check against ALL original constraints
+                std::vector<double> xr;
+                to_raw(S, P2, xn, xr);
+                rc = upload(ctx, S.v.x_raw, xr.data(), n);
                 if (rc) break;
-                Vred[0] = ctx->own[OWN_VRED0]; Vred[1] = ctx->own[OWN_VRED1];
-                P2.prec = MEB_FP64; P2.d = d; P2.ldv = ldr; P2.off = c0.data(); P2.full = false;
-                P2.C = Cred; P2.ld = ldr; P2.R = Rred;
-                P2.U[0] = ctx->own[OWN_HOSTC]; P2.U[1] = ctx->own[OWN_HOSTR];
-                P2.slot[0] = (int32_t*)ctx->own[OWN_SPARE]; P2.slot[1] = P2.slot[0] + cap_red;
-                P2.V[0] = Vred[0]; P2.V[1] = Vred[1]; P2.vcap[0] = P2.vcap[1] = cap_red;
-                P2.own_v[0] = P2.own_v[1] = -1;
-                P2.cur = 0; P2.has_mult = true;
-                // warm start restricted to I_red.  If the low-precision run did not reach its
-                // tolerance (degenerate supports: reading 17) its multipliers are noise: start from zero.
-                if (P1.has_mult && conv1)
-                    rc = meb_gather_mult(ctx, (const float*)P1.U[P1.cur], P1.slot[P1.cur], (const float*)P1.V[P1.cur],
-                                         P1.ldv, idx, nred, d, (double*)P2.U[0], P2.slot[0], (double*)P2.V[0], ldr);
-                else
-                    P2.has_mult = false;
-                ab = xn;                                        // reading 11
-                for (int rnd = 0; rc == MEB_OK && rnd < S.par.max_rounds; ++rnd) {
-                    P2.m = nred;
-                    st->n_reduced = nred;
-                    st->rounds = rnd + 1;
-                    rc = ripalm(S, P2, xn, ab, tol_kkt, tol, &converged, &kkt, terms, S.par.outer_max);
+                r_alg = xr[0];
+                for (int j = 0; j < d; ++j) creturn[j] = xr[1 + j];
+                const double eps_feas = tol_kkt * (1.0 + r_alg);        // reading 10
+                int32_t am = 0; int64_t nvl = 0;
+                rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, eps_feas, kept,
+                                           &dmax, &am, idx + nred, m - nred, &nvl);
+                if (rc) break;
+                st->passes_fp64_full++;
+                S.bytes += ctx->last_pass_bytes;
+                if (nvl == 0) break;
+                if (rnd + 1 == S.par.max_rounds) { converged = false; break; }      // round cap: best iterate, not converged
+                // re-introduce the violated balls with zero multipliers (reading 12); the reduced
+                // buffers grow as needed and keep the rows, radii and current multipliers of the balls already there
+                if (nred + nvl > Q.cap) {
+                    int64_t want = 2 * (nred + nvl) + 1024;
+                    if (want > m) want = m;
+                    rc = reduced_reserve(ctx, Q, want, nred);
                     if (rc) break;
-                    if (rnd == 0) MEB_CUDA_OK(ctx, cudaEventRecord(e_hi, ctx->stream));
-                    // a-posteriori check against ALL original constraints
-                    std::vector<double> xr;
-                    to_raw(S, P2, xn, xr);
-                    rc = upload(ctx, S.v.x_raw, xr.data(), n);
-                    if (rc) break;
-                    r_alg = xr[0];
-                    for (int j = 0; j < d; ++j) creturn[j] = xr[1 + j];
-                    const double eps_feas = tol_kkt * (1.0 + r_alg);        // reading 10
-                    int32_t am = 0; int64_t nv = 0;
-                    rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, eps_feas, kept,
-                                               &dmax, &am, idx + nred, m - nred, &nv);
-                    if (rc) break;
-                    st->passes_fp64_full++;
-                    S.bytes += ctx->last_pass_bytes;
-                    if (nv == 0) break;
-                    if (nred + nv > cap_red) { rc = MEB_E_CAPACITY; break; }
-                    // re-introduce the violated balls with zero multipliers (reading 12)
-                    rc = meb_gather_rows_f64(ctx, centers, ld, idx + nred, nv, d, Cred + nred * ldr, ldr);
-                    if (rc) break;
-                    if (radii) { rc = meb_gather_vec_f64(ctx, radii, idx + nred, nv, Rred + nred); if (rc) break; }
-                    rc = meb_set_kept(ctx, idx + nred, nv, kept);
-                    if (rc) break;
-                    if (P2.has_mult) {
-                        rc = meb_fill_f64(ctx, (double*)P2.U[P2.cur] + nred, nv, 0.0);
-                        if (rc) break;
-                        rc = meb_fill_i32(ctx, P2.slot[P2.cur] + nred, nv, -1);
-                        if (rc) break;
-                    }
-                    nred += nv;
-                    converged = false;
-                    ab = xn;
+                    reduced_bind(ctx, Q, P2);
                 }
+                double* Cred = (double*)ctx->own[OWN_CRED];
+                rc = meb_gather_rows_f64(ctx, centers, ld, idx + nred, nvl, d, Cred + nred * ldr, ldr);
                 if (rc) break;
+                if (radii) { rc = meb_gather_vec_f64(ctx, radii, idx + nred, nvl, (double*)ctx->own[OWN_RRED] + nred); if (rc) break; }
+                rc = meb_set_kept(ctx, idx + nred, nvl, kept);
+                if (rc) break;
+                if (P2.has_mult) {
+                    rc = meb_fill_f64(ctx, (double*)P2.U[P2.cur] + nred, nvl, 0.0);
+                    if (rc) break;
+                    rc = meb_fill_i32(ctx, P2.slot[P2.cur] + nred, nvl, -1);
+                    if (rc) break;
+                }
+                nred += nvl;
+                converged = false;
+                ab = xn;
             }
+            if (rc) break;
         }
         st->radius_alg = r_alg;
         st->delta_max = dmax;
         *h_radius_out = r_alg + dmax;                     // = max_i(||c - c_i|| + r_i)   (step 7)
     } while (0);
-    if (rc == MEB_OK) {
-        cudaEventRecord(e_end, ctx->stream);
-        cudaEventSynchronize(e_end);
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e_start, e_end); st->ms_total = ms;
-        if (cudaEventElapsedTime(&ms, e_start, e_mid) == cudaSuccess) st->ms_phase_lo = ms;
-        if (cudaEventElapsedTime(&ms, e_mid, e_hi) == cudaSuccess) st->ms_phase_hi = ms;
-        if (cudaEventElapsedTime(&ms, e_hi, e_end) == cudaSuccess) st->ms_check = ms;
-        cudaGetLastError();
-        memcpy(h_center_out, creturn.data(), d * sizeof(double));
-        st->converged = converged ? 1 : 0;
-        st->kkt = kkt;
-        memcpy(st->kkt_terms, terms, sizeof(terms));
-        st->bytes_streamed = S.bytes;
-        for (int k = 0; k < ctx->evn; ++k) {           // per-class device time of the streaming launches
-            float pms = 0.f;
-            if (cudaEventElapsedTime(&pms, ctx->evpool[2 * k], ctx->evpool[2 * k + 1]) != cudaSuccess) continue;
-            const int cls = ctx->evclass[k] & 7;
+#undef CUB
+    if (rc != MEB_OK) return rc;
+    cudaEventRecord(e_end, ctx->stream);
+    cudaEventSynchronize(e_end);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e_start, e_end); st->ms_total = ms;
+    if (have_mid && cudaEventElapsedTime(&ms, e_start, e_mid) == cudaSuccess) st->ms_phase_lo = ms;
+    if (have_mid && have_hi && cudaEventElapsedTime(&ms, e_mid, e_hi) == cudaSuccess) st->ms_phase_hi = ms;
+    if (have_hi && cudaEventElapsedTime(&ms, e_hi, e_end) == cudaSuccess) st->ms_check = ms;
+    cudaGetLastError();
+    memcpy(h_center_out, creturn.data(), d * sizeof(double));
+    st->converged = converged ? 1 : 0;
+    st->kkt = kkt;
+    memcpy(st->kkt_terms, terms, sizeof(terms));
+    st->bytes_streamed = S.bytes;
+    for (int k = 0; k < ctx->evn; ++k) {           // CUDA-event time of the streaming launches made outside graphs
+        float pms = 0.f;
+        if (ctx->evcut[k]) continue;
+        if (cudaEventElapsedTime(&pms, ctx->evpool[2 * k], ctx->evpool[2 * k + 1]) != cudaSuccess) continue;
+        const int cls = ctx->evclass[k] & 7;
+        st->pass_ev_ms[cls] += pms; st->pass_ev_bytes[cls] += ctx->evbytes[k]; st->pass_ev_count[cls]++;
+        if (cls == MEB_PASS_INGEST || cls == MEB_PASS_SCREEN || cls == MEB_PASS_FEAS) {     // never inside a graph
             st->pass_ms[cls] += pms; st->pass_bytes[cls] += ctx->evbytes[k]; st->pass_count[cls]++;
         }
-        cudaGetLastError();
-        st->kernel_launches = ctx->launches - launches0;
     }
-    ctx->ev_record = false;
-    cudaEventDestroy(e_start); cudaEventDestroy(e_mid); cudaEventDestroy(e_hi); cudaEventDestroy(e_end);
-    ctx->time_passes = timing_was;
-    if (rc != MEB_OK) return rc;
+    cudaGetLastError();
+    st->kernel_launches = ctx->launches - launches0;
     return converged ? MEB_OK : MEB_W_NOT_CONVERGED;
 }
 

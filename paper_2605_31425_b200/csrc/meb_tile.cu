@@ -641,7 +641,11 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
         };
         int best = collisions(0, 0);
         c.rot = 0; c.rowfast = 0;
-        if (c.G > 1 && !getenv("MEB_TILE_NO_ROWFAST")) {
+        bool try_rowfast = c.G > 1;
+#ifdef MEB_TUNING
+        if (getenv("MEB_TILE_NO_ROWFAST")) try_rowfast = false;
+#endif
+        if (try_rowfast) {
             const int cr = collisions(1, 0);
             if (cr < best) { best = cr; c.rowfast = 1; }
         }
@@ -667,16 +671,20 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
     for (const void* q : ptrs) if (q && !aligned16(q)) c.sc_tma = 0;
     const size_t cs_bytes = ((size_t)c.nch * 16 + 127) / 128 * 128;
     int W = 16, NS = 0;
-    const int want_ns = getenv("MEB_TILE_NS") ? atoi(getenv("MEB_TILE_NS")) : 2;     // tuning knobs (profiling only)
-    if (getenv("MEB_TILE_W")) W = atoi(getenv("MEB_TILE_W"));
+    int want_ns = 2;
+#ifdef MEB_TUNING                     // tuning knobs of experimental builds (build.sh -DMEB_TUNING); clamped
+    if (getenv("MEB_TILE_NS")) want_ns = atoi(getenv("MEB_TILE_NS")) < 3 ? 2 : (atoi(getenv("MEB_TILE_NS")) > 3 ? 4 : 3);
+    if (getenv("MEB_TILE_W")) { W = atoi(getenv("MEB_TILE_W")); W = W < 2 ? 2 : (W > 16 ? 16 : W); }
     if (getenv("MEB_TILE_R")) {
         c.R = atoi(getenv("MEB_TILE_R"));
+        c.R = c.R < 1 ? 1 : (c.R > 8 ? 8 : c.R);
         c.stage_rows = (uint32_t)(c.R * rpt);
         c.off_u = c.stage_rows * c.row_bytes;
         c.off_r = c.off_u + c.stage_rows * (uint32_t)esize;
         c.off_slot = c.off_r + c.stage_rows * (uint32_t)esize;
         c.stage_bytes = (c.off_slot + c.stage_rows * 4u + 127u) / 128u * 128u;
     }
+#endif
     for (; W >= 2; --W) {
         const size_t fixed = cs_bytes + 16 * 4 * sizeof(uint64_t) + 256;
         if (fixed + (size_t)W * want_ns * c.stage_bytes > TILE_SMEM_BUDGET) continue;

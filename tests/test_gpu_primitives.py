@@ -5,6 +5,16 @@ within 1e-5 of the oracle, relative to the sum of |terms| of the reduction; per-
 the same tolerance of sigma-free magnitudes |a_i| + nb_i; integer work (compaction, argmax, index
 sets given flags) bit-exact.  Counts and flags may differ only on balls within the tolerance of a
 branch / threshold boundary; the tests evaluate at generic points and list those balls.
+
+Balls near a branch boundary (SURVEY.md section 8(c) "Parity metrics": "balls within
+10 tol_p of a branch or threshold boundary may land on the other side"): the evaluation point of
+`make_state` is moved off the data by a factor 1.0001 and such balls are MASKED out of the per-ball,
+count and list comparisons -- the two sides evaluate ||b_i|| with different summation orders, so which
+side of `nb <= a` a ball within rounding of the boundary lands on is not defined by the paper.  The
+REDUCTIONS get no allowance for them: Pi_Q is continuous, so a ball that flips branch changes its own
+terms of psi, the gradient and the multiplier sums only in second order (t -> 0 at the B2/B3 boundary,
+lam -> 1 at the B1/B3 boundary).  Only P_i (hvp, dense H) jumps across a boundary; there the allowance
+is the listed balls' own bound sigma ||P_i||_F.
 """
 import numpy as np
 import pytest
@@ -84,8 +94,10 @@ def _check_eval(meb, ctx, prec, C, R, U, V, x, xbar, sigma, tau, layout, ld_pad)
         assert int(s[E["N_ACTIVE"]]) == act_o.size
         lam_list = res["active_lam"].cpu().numpy()
         assert np.all(np.abs(lam_list - ev["lam"][act_o]) <= 4 * tol)
-    slack = near.sum() * 4.0 * float(np.max(mag)) ** 2 * sigma      # contribution of boundary balls
-    # reductions, relative to the sum of |terms|
+    # reductions, relative to the sum of |terms|.  No allowance for the `near` balls: every summand is a
+    # continuous function of (a_i, nb_i) across the branch boundaries (see the module docstring)
+    assert near.sum() <= (2 if prec == 0 else 12), int(near.sum())
+    slack = 0.0
     assert abs(s[E["SUM_PROJ2"]] - ev["sum_proj2"]) <= tol * ev["scale_proj2"] + slack
     assert abs(s[E["SUM_UPLUS"]] - ev["sum_uplus"]) <= tol * ev["scale_uplus"] + slack
     assert abs(s[E["SUM_DMULT2"]] - ev["sum_dmult2"]) <= 4 * tol * ev["scale_dmult2"] + slack
@@ -190,7 +202,7 @@ def test_update_multipliers(meb, ctx, prec, m, d):
     both = both[ok[both]]
     assert np.all(np.abs(Vg[sl[both]] - Vp[both]) <= TOL[prec] * mag[both][:, None])
     assert np.all(Ug[sl < 0] == 0)
-    assert abs(res["sum_mult2"] - m2) <= 4 * TOL[prec] * m2 + near.sum() * 4.0 * float(np.max(mag)) ** 2
+    assert abs(res["sum_mult2"] - m2) <= 4 * TOL[prec] * m2          # continuous across the branch boundaries
     act = act_g
     # capacity error: too few rows for the active balls
     res2 = meb.meb_update_multipliers(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), 1.7, cap_rows=act.size - 1)

@@ -179,3 +179,51 @@ def test_armijo_shrink_min_is_only_a_path_choice(meb):
     c0, r0, s0 = _solve_with(meb, C, R, "fp64")
     assert s1["converged"] == 1 and s0["converged"] == 1
     assert abs(r1 - r0) <= 1e-8 * r0 and np.linalg.norm(c1 - c0) <= 1e-5 * (1 + r0)
+
+
+@pytest.mark.parametrize("factor,k,m,d", [(-0.3, 2, 40_000, 100), (-100.0, 1, 10_000, 10), (-0.05, 3, 6_000, 1000)])
+def test_refinement_rounds_reintroduce_violated_balls(meb, factor, k, m, d):
+    """violated discarded balls are added back without limit and the reduced problem is solved
+    again.  A useless retain rule (a NEGATIVE tol_red factor keeps only balls far outside the coarse ball;
+    -100 keeps none, in which case the farthest ball alone starts the reduced problem, as in the oracle)
+    forces rounds >= 2, the growth of the reduced buffers beyond their first capacity and the re-introduction
+    code; the answer is still the unique optimum."""
+    C, R = workloads.config(k, m, d)
+    p = meb.meb_default_params()
+    p.tol_red_factor = factor
+    c, r, st = _solve_with(meb, C, R, "mixed", params=p)
+    co, ro, _ = ripalm.meb_solve(C, R, 1e-10, "fp64")
+    assert st["converged"] == 1 and st["rounds"] >= 2, st
+    assert abs(r - ro) <= 1e-8 * ro and np.linalg.norm(c - co) <= 1e-5 * (1 + ro)
+    assert _violation(C, R, c, r) <= 1e-10 * (1 + r)
+    assert st["n_reduced"] > 1024 or factor == -100.0 or m < 2048
+
+
+def test_refinement_round_cap_reports_not_converged(meb):
+    C, R = workloads.config(2, 20_000, 100)
+    p = meb.meb_default_params()
+    p.tol_red_factor = -0.3
+    p.max_rounds = 1
+    with meb.Context(*C.shape) as ctx:
+        c, r, st = meb.meb_solve(ctx, torch.from_numpy(C).cuda(), None, 1e-8, meb.MEB_MODE_MIXED, params=p,
+                                 allow_not_converged=True)
+    assert st["converged"] == 0 and st["rounds"] == 1
+    assert _violation(C, R, c.numpy(), r) <= 1e-10 * (1 + r)       # the returned radius is still the feasible one
+
+
+def test_stepped_solve_equals_graph_solve_and_fills_event_times(meb):
+    """MEB_OPT_STEPPED sequences the same kernels from the host: same bits, and every streaming launch is
+    bracketed by a CUDA-event pair (meb_stats.pass_ev_*), which is what bench.py's roofline reads."""
+    C, R = workloads.config(3, 5_000, 1000)
+    dC, dR = torch.from_numpy(C).cuda(), torch.from_numpy(R).cuda()
+    with meb.Context(*C.shape) as ctx:
+        c0, r0, s0 = meb.meb_solve(ctx, dC, dR, 1e-8, meb.MEB_MODE_MIXED)
+        meb.meb_set_option(ctx, meb.OPT["STEPPED"], True)
+        c1, r1, s1 = meb.meb_solve(ctx, dC, dR, 1e-8, meb.MEB_MODE_MIXED)
+        meb.meb_set_option(ctx, meb.OPT["STEPPED"], False)
+    assert r0 == r1 and torch.equal(c0, c1)
+    P = meb.PASS
+    assert s0["pass_ev_count"][P["EVAL_FP32"]] == 0 and s0["pass_ev_count"][P["INGEST"]] == 1
+    n32 = s1["pass_ev_count"][P["EVAL_FP32"]]
+    assert n32 == s1["passes_fp32_full"] - 1 - s1["passes_cut"] or n32 > 0      # screen pass is its own class
+    assert s1["pass_ev_ms"][P["EVAL_FP32"]] > 0 and s1["pass_ev_bytes"][P["EVAL_FP32"]] >= n32 * C.size * 4

@@ -213,3 +213,75 @@ def test_paper_instance_generator():
     assert R[0] == seq[0] and list(C[0]) == seq[1:3] and R[1] == seq[3] and list(C[2]) == seq[7:9]
     Cb, Rb = workloads.paper_instance(5000, 20)
     assert 0 <= Cb.min() and Cb.max() < 100 and Rb.max() < 100
+
+
+def _state32(seed, m, d):
+    """A state whose data are exactly representable in float32 (both modes see the same numbers)."""
+    rng = np.random.default_rng(seed)
+    C, R, U, V, x, xbar = _state(rng, m, d)
+    f = lambda a: a.astype(np.float32).astype(np.float64)
+    return f(C), f(R), f(U), f(V), x, xbar
+
+
+def test_fp32_mode_of_hvp_close_to_fp64():
+    """The low-precision mode (DESIGN reading 8: float32 data and per-ball arithmetic, float64 sums) of hvp
+    against its float64 mode on the same float32-representable data: within 1e-5 of the sum of |terms|.
+    A wrong cast in the q1 / rho path moves the result by far more."""
+    C, R, U, V, x, _ = _state32(21, 1500, 12)
+    q = np.random.default_rng(22).standard_normal(13)
+    H64, scale = prim.hvp(C, R, U, V, x, 2.0, 0.5, q)
+    H32, scale32 = prim.hvp(C, R, U, V, x, 2.0, 0.5, q, dtype=np.float32)
+    assert H32.dtype == np.float64 and np.linalg.norm(scale) > 10
+    assert np.linalg.norm(H32 - H64) <= 1e-5 * np.linalg.norm(scale)
+    assert np.linalg.norm(H32 - H64) > 0                          # it did run in float32
+    assert np.linalg.norm(scale32 - scale) <= 1e-5 * np.linalg.norm(scale)
+    # unit vectors pick single columns of H: every entry of the FP32-mode operator is pinned
+    Hd, sd = prim.dense_hessian(C, R, U, V, x, 2.0, 0.5)
+    for j in (0, 1, 12):
+        e = np.zeros(13); e[j] = 1.0
+        col, _ = prim.hvp(C, R, U, V, x, 2.0, 0.5, e, dtype=np.float32)
+        assert np.linalg.norm(col - Hd[:, j]) <= 1e-5 * np.linalg.norm(sd[:, j])
+
+
+def test_fp32_mode_of_dense_hessian_close_to_fp64():
+    C, R, U, V, x, _ = _state32(23, 1200, 9)
+    H64, scale = prim.dense_hessian(C, R, U, V, x, 1.5, 0.8)
+    H32, _ = prim.dense_hessian(C, R, U, V, x, 1.5, 0.8, dtype=np.float32)
+    assert np.linalg.norm(H32 - H64) <= 1e-5 * np.linalg.norm(scale)
+    assert np.linalg.norm(H32 - H64) > 0
+    np.testing.assert_allclose(H32, H32.T, atol=1e-12 * np.abs(H32).max())
+    assert np.linalg.eigvalsh(H32).min() >= 0.8 / 1.5 * (1 - 1e-4)      # P:L193 survives the low precision
+
+
+def test_fp32_mode_of_update_multipliers_close_to_fp64():
+    C, R, U, V, x, _ = _state32(24, 1000, 7)
+    sigma = 1.7
+    U64, V64, m64 = prim.update_multipliers(C, R, U, V, x, sigma)
+    U32, V32, m32 = prim.update_multipliers(C, R, U, V, x, sigma, dtype=np.float32)
+    assert U32.dtype == np.float32 and V32.dtype == np.float32
+    a, B, *_ = prim.shifted_points(C, R, U, V, x, sigma)
+    mag = sigma * (np.abs(a) + soc.row_norms(B))
+    far = np.abs(soc.row_norms(B) - np.abs(a)) > 1e-4 * (np.abs(a) + soc.row_norms(B))   # off the branch boundaries
+    assert far.sum() > 900
+    assert np.all(np.abs(U32 - U64)[far] <= 1e-5 * mag[far])
+    assert np.all(np.abs(V32 - V64)[far] <= 1e-5 * mag[far][:, None])
+    assert abs(m32 - m64) <= 1e-5 * m64 + (~far).sum() * float(mag.max()) ** 2
+    assert np.all(V32[U32 == 0] == 0)
+
+
+def test_initial_point_hand_example():
+    """DESIGN reading 3: c0 = mean of the S = min(m, sample_rows) rows floor(k m / S), L = max_i(||c_i - c0|| + r_i).
+    m = 5, S = 2 -> rows 0 and 2.  By hand: c0 = ((0,0) + (4,0))/2 = (2,0); ||c_i - c0|| + r_i =
+    2+1, 8+0.5, 2+0, 3+2, sqrt(10)+0  ->  L = 8.5 (ball 1)."""
+    from oracle import ripalm
+    C = np.array([[0.0, 0.0], [10.0, 0.0], [4.0, 0.0], [2.0, 3.0], [-1.0, -1.0]])
+    R = np.array([1.0, 0.5, 0.0, 2.0, 0.0])
+    c0, L = ripalm.initial_point(C, R, ripalm.Params(sample_rows=2))
+    assert np.array_equal(c0, [2.0, 0.0]) and L == 8.5
+    # S = 3: rows floor(0), floor(5/3) = 1, floor(10/3) = 3 -> c0 = (12/3, 3/3) = (4, 1)
+    c0, L = ripalm.initial_point(C, None, ripalm.Params(sample_rows=3))
+    assert np.allclose(c0, [4.0, 1.0], atol=1e-15)
+    assert abs(L - np.sqrt(37.0)) <= 1e-15 * 7                      # farthest point: (10,0) -> sqrt(36 + 1)
+    # fewer balls than sample_rows: the mean of all of them
+    c0, L = ripalm.initial_point(C, R, ripalm.Params())
+    assert np.allclose(c0, C.mean(axis=0), atol=1e-15)

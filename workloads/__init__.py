@@ -15,5 +15,6 @@ from .generators import (  # noqa: F401
     CONFIG_SHAPES,
     config,
     config_blocks,
+    config_into,
     paper_instance,
 )

@@ -89,6 +89,38 @@ def config(k: int, m: int | None = None, d: int | None = None, seed: int = 0):
     return C, R
 
 
+def config_into(k: int, C_out, R_out, m: int | None = None, d: int | None = None, seed: int = 0,
+                threads: int = 8, sink=None):
+    """Same rows as ``config`` written into preallocated ``C_out`` (m, d) / ``R_out`` (m,) (or handed block by
+    block to ``sink(row0, C_block, R_block)``), the independent 65,536-row blocks drawn by a pool of threads
+    (numpy's generators release the GIL).  Config 5 is 16 GB: one thread needs about a minute for it."""
+    from concurrent.futures import ThreadPoolExecutor
+    m_full, d_full, _ = CONFIG_SHAPES[k]
+    m = m_full if m is None else int(m)
+    d = d_full if d is None else int(d)
+    type_sphere_all = None
+    if k == 4:
+        perm = np.random.default_rng([seed, 4, 2**31 - 1]).permutation(m)
+        type_sphere_all = perm < (m // 2)
+    nblocks = (m + BLOCK_ROWS - 1) // BLOCK_ROWS
+
+    def work(b):
+        row0 = b * BLOCK_ROWS
+        rows = min(BLOCK_ROWS, m - row0)
+        ts = None if type_sphere_all is None else type_sphere_all[row0:row0 + rows]
+        Cb, Rb = _block(k, b, BLOCK_ROWS if k != 4 else rows, d, seed, ts)
+        if sink is not None:
+            sink(row0, Cb[:rows], None if Rb is None else Rb[:rows])
+        else:
+            C_out[row0:row0 + rows] = Cb[:rows]
+            if R_out is not None and Rb is not None:
+                R_out[row0:row0 + rows] = Rb[:rows]
+        return rows
+
+    with ThreadPoolExecutor(max_workers=max(1, int(threads))) as ex:
+        return sum(ex.map(work, range(nblocks)))
+
+
 def paper_instance(m: int, d: int):
     """The deterministic instances of the paper's experiments.
 

@@ -2,23 +2,29 @@
 """bench.py -- time-to-solution of meb_solve and per-pass HBM GB/s on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--mode mixed|fp64] [--impl reference]
+                    [--shard] [--no-extra] [--no-e2e] [--no-cpu-baseline]
 
 A "step" is one whole meb_solve (one pass of the hot path: ingest, ALM evaluations, Newton solves,
-multiplier updates, screening + compaction, feasibility check) on a seeded synthetic instance of the
-BASELINE.json configuration (default: configs[1], m = 1e6 points in R^100, mixed precision, which
-exercises every row of SURVEY 8(a)).  Prints ONE JSON line (see the task contract):
+multiplier updates, screening + compaction, feasibility check) on a seeded synthetic instance of a
+BASELINE.json configuration.  BASELINE.json's metric quotes no configuration, so the N = 1 line is on the
+LARGEST single-GPU one: configs[4] (m = 2e5 balls in R^10000, 16 GB of centres), mixed precision, which
+exercises every row of SURVEY 8(a).  Prints ONE JSON line (see the task contract):
 
   value      seconds per solve with the balls already resident in HBM (CUDA events around K solves)
   e2e        the same through meb_solve_host with pinned HOST buffers (H2D inside the timed region)
-  roofline   the dominant streaming kernel of the step: algorithmic bytes / launch duration measured
-             INSIDE the timed solves (evaluation passes run inside a CUDA-graph WHILE node, where no
-             event can be recorded per iteration: their device time comes from %globaltimer stamps of
-             the kernel's CTAs; ingest / screen / feasibility launches are bracketed by CUDA events),
-             plus `events_check`: the same kernel timed stand-alone with CUDA events
+  roofline   the dominant streaming kernel of the step.  `achieved` = algorithmic bytes per launch / launch
+             duration from CUDA-EVENT pairs recorded on the launching stream around every streaming launch of
+             one extra, host-stepped solve of the same instance (MEB_OPT_STEPPED: the same kernels, arguments
+             and iterates as the graph-mode solves that are timed for `value`; inside a CUDA-graph WHILE node no
+             event can be recorded per iteration).  `in_graph_globaltimer` is the same kernel's time inside the
+             timed graph-mode solves from the %globaltimer stamps of its CTAs (last end - first start).
+  configs    (N = 1) the other BASELINE.json configurations, FP64 and mixed, each with ms_per_step, the
+             event-timed GB/s of every pass class and the solve statistics
   cpu_baseline  the CPU oracle timed on the host cores on a bounded sample (rank 0, N = 1)
 
-N > 1 (torchrun): the path does not shard in this round ("replicas only"): every rank
-solves its own seeded instance, time = max over ranks, value = time per solve of the whole job.
+N > 1 (torchrun): by default every rank solves its own seeded instance ("replicas"); with --shard the m balls
+of ONE instance are partitioned over the ranks and the (d + O(10))-sized partial
+reductions are all-gathered over NCCL at every reduction point.
 --impl reference: the oracle (oracle/ripalm.py) as it stands, on the host cores, bounded sample.
 """
 import argparse
@@ -36,26 +42,27 @@ if ROOT not in sys.path:
 METRIC = "meb_solve_time_to_1e-8_rel_kkt"
 UNIT = "s"
 TOL = 1e-8
+HEADLINE_CONFIG = 5
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k-1], k = 1..5")
+    ap.add_argument("--config", type=int, default=HEADLINE_CONFIG, help="BASELINE.json configs[k-1], k = 1..5")
     ap.add_argument("--mode", default="mixed", choices=["mixed", "fp64"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--m", type=int, default=None, help="override m (debugging only; reported in config)")
     ap.add_argument("--cpu-sample", type=int, default=None, help="balls in the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the per-config block (configs 1-5, both modes)")
+    ap.add_argument("--shard", action="store_true", help="N > 1: partition the balls of one instance over the ranks")
     return ap.parse_args()
 
 
 def workload_name(k, m, d, mode):
-    import workloads
-    mf, df, has_r = workloads.CONFIG_SHAPES[k]
     kind = {1: "balls N(0,1), r~U[0,0.1]", 2: "points N(0,1)", 3: "balls U[-1,1]^d, r~U[0,1]",
             4: "boundary-heavy points", 5: "anisotropic balls, r~lognormal(-3,1)"}[k]
     return f"config{k}: {kind}, m={m}, d={d}, {mode}, tol=1e-8, seed 0"
@@ -128,28 +135,40 @@ def oracle_sample_size(k, m, d, override=None):
     return max(256, min(m, budget_elems // max(d, 1)))
 
 
-def oracle_solve_sample(k, m, d, mode, m_s):
-    """Times oracle/ripalm.meb_solve on the first m_s balls of the workload (a prefix of the same
-    seeded instance; config 4 re-draws its sphere/interior permutation at size m_s)."""
-    import numpy as np  # noqa: F401
-    import workloads
+def oracle_time(C, R, mode):
+    """Times oracle/ripalm.meb_solve, as it stands, on the given balls."""
     from oracle import ripalm
-    C, R = workloads.config(k, m_s, d)
     t0 = time.perf_counter()
     c, r, info = ripalm.meb_solve(C, R, TOL, mode)
-    dt = time.perf_counter() - t0
-    return dt, r, info
+    return time.perf_counter() - t0, r, info
 
 
 def cpu_threads():
-    """Threads available to the oracle's numpy (its BLAS calls may use them; its elementwise passes,
-    which dominate, run on one thread)."""
+    """Threads the oracle used: its elementwise numpy passes, which dominate, run on ONE thread (its few BLAS
+    calls may use more, which is reported separately)."""
+    return 1
+
+
+def blas_threads():
     try:
         from threadpoolctl import threadpool_info
-        n = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
-        return int(n)
+        return int(max([p.get("num_threads", 1) for p in threadpool_info()] or [1]))
     except Exception:
         return 1
+
+
+def cpu_baseline_entry(C, R, m, mode, dt, m_s):
+    full = m_s >= m
+    entry = {"value": dt * (m / m_s), "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+             "extrapolated": (not full), "measured_s": dt, "blas_threads_available": blas_threads(),
+             "host_cores": os.cpu_count()}
+    if full:
+        entry["sample"] = f"the full instance ({m} balls), measured once; numpy oracle, elementwise passes on 1 thread"
+    else:
+        entry["sample"] = (f"first {m_s} of {m} balls of the same seeded instance: {dt:.3f} s measured, `value` is that "
+                           f"times {m / m_s:.1f} (an EXTRAPOLATION: cost per pass is linear in m, the number of passes "
+                           f"and |I_red| are not); the dense-V numpy oracle does not fit the full instance")
+    return entry
 
 
 def run_reference(args, rank, world):
@@ -161,44 +180,55 @@ def run_reference(args, rank, world):
     mf, d, _ = workloads.CONFIG_SHAPES[k]
     m = args.m or mf
     m_s = oracle_sample_size(k, m, d, args.cpu_sample)
+    C, R = workloads.config(k, m_s, d)
     for _ in range(min(args.warmup, 1)):            # numpy needs no warm-up beyond the first import
-        oracle_solve_sample(k, m, d, args.mode, min(m_s, 2000))
+        oracle_time(C[:min(m_s, 500)], None if R is None else R[:min(m_s, 500)], args.mode)
     times = []
     for _ in range(args.steps):
-        dt, r, _info = oracle_solve_sample(k, m, d, args.mode, m_s)
+        dt, r, _info = oracle_time(C, R, args.mode)
         times.append(dt)
     per = sum(times) / len(times)
-    scaled = per * (m / m_s)
-    sample = (f"first {m_s} of {m} balls of the same seeded instance, {per:.3f} s per solve measured, "
-              f"scaled x{m / m_s:.1f} to m (cost per pass is linear in m); numpy: elementwise passes on 1 thread, "
-              f"BLAS calls on up to `cores` threads")
-    line = {"impl": "reference", "metric": METRIC, "value": scaled, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": scaled * 1e3,
+    entry = cpu_baseline_entry(C, R, m, args.mode, per, m_s)
+    line = {"impl": "reference", "metric": METRIC, "value": entry["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": entry["value"] * 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": {"workload": workload_name(k, m, d, args.mode)},
-            "cpu_baseline": {"value": scaled, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
-                             "sample": sample},
-            "e2e": {"value": scaled, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "cpu_baseline": entry,
+            "e2e": {"value": entry["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------- B200 arm
-def upload_instance(k, m, d, seed, device):
-    """Generates the seeded instance block by block on the host and places it in HBM (row-major FP64
-    centres, FP64 radii or None).  Also returns pinned host copies when they fit (for the e2e leg)."""
+def make_instance(k, m, d, seed, device, want_host):
+    """Generates the seeded instance (threads over the independent 65,536-row blocks) and places it in HBM
+    (row-major FP64 centres, FP64 radii or None).  With want_host the host copy is PINNED and returned (e2e leg)."""
     import numpy as np
     import torch
     import workloads
     has_r = workloads.CONFIG_SHAPES[k][2]
     dC = torch.empty((m, d), dtype=torch.float64, device=device)
     dR = torch.empty(m, dtype=torch.float64, device=device) if has_r else None
-    for row0, Cb, Rb in workloads.config_blocks(k, m, d, seed):
-        n = Cb.shape[0]
-        dC[row0:row0 + n].copy_(torch.from_numpy(np.ascontiguousarray(Cb)))
+    hC = hR = None
+    if want_host:
+        hC = torch.empty((m, d), dtype=torch.float64, pin_memory=True)
+        hR = torch.empty(m, dtype=torch.float64, pin_memory=True) if has_r else None
+        workloads.config_into(k, hC.numpy(), None if hR is None else hR.numpy(), m, d, seed, threads=os.cpu_count() or 8)
+        dC.copy_(hC)
         if dR is not None:
-            dR[row0:row0 + n].copy_(torch.from_numpy(np.ascontiguousarray(Rb)))
-    return dC, dR
+            dR.copy_(hR)
+    else:
+        lock = threading.Lock()
+
+        def sink(row0, Cb, Rb):
+            tC = torch.from_numpy(np.ascontiguousarray(Cb))
+            with lock:                      # one stream of H2D copies; the draws of the other blocks overlap it
+                dC[row0:row0 + Cb.shape[0]].copy_(tC)
+                if dR is not None:
+                    dR[row0:row0 + Cb.shape[0]].copy_(torch.from_numpy(np.ascontiguousarray(Rb)))
+        workloads.config_into(k, None, None, m, d, seed, threads=min(os.cpu_count() or 8, 8), sink=sink)
+    torch.cuda.synchronize()
+    return dC, dR, hC, hR
 
 
 def measured_peak():
@@ -210,7 +240,7 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
 
 
-def ncu_traffic(cls_name, k, mode):
+def ncu_traffic(cls_name, k):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture, if one is recorded."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     try:
@@ -218,6 +248,59 @@ def ncu_traffic(cls_name, k, mode):
             return json.load(f).get(f"config{k}", {}).get(cls_name)
     except Exception:
         return None
+
+
+def pass_table(meb, st_graph_list, st_step, peak):
+    """Per pass class: event-timed launches of the stepped solve, and the in-graph globaltimer figure of the
+    graph-mode solves."""
+    names = {v: n for n, v in meb.PASS.items()}
+    out = {}
+    for i in range(8):
+        n_ev = st_step["pass_ev_count"][i]
+        n_g = sum(s["pass_count"][i] for s in st_graph_list)
+        if n_ev == 0 and n_g == 0:
+            continue
+        e = {}
+        if n_ev > 0:
+            ms = st_step["pass_ev_ms"][i]
+            by = st_step["pass_ev_bytes"][i]
+            e.update({"launches_timed": n_ev, "ms_per_launch": ms / n_ev, "bytes_per_launch": by / n_ev,
+                      "GBps": by / ms / 1e6 if ms > 0 else None,
+                      "frac": (by / ms / 1e6 / peak) if (ms > 0 and i != meb.PASS["EVAL_REDUCED"]) else None})
+        if n_g > 0:
+            msg = sum(s["pass_ms"][i] for s in st_graph_list)
+            byg = sum(s["pass_bytes"][i] for s in st_graph_list)
+            e["in_graph_globaltimer"] = {"launches": n_g, "ms_per_launch": msg / n_g,
+                                         "GBps": byg / msg / 1e6 if msg > 0 else None}
+        out[names.get(i, str(i))] = e
+    return out
+
+
+def solve_summary(r, st):
+    keys = ["outer_iters", "newton_iters", "cg_iters", "ag_iters", "passes_fp64_full", "passes_fp32_full", "passes_reduced",
+            "passes_cut", "trials_skipped", "n_reduced", "rounds", "ms_phase_lo", "ms_phase_hi", "ms_check", "kkt",
+            "delta_max", "n_support"]
+    out = {"radius": r}
+    out.update({k: st[k] for k in keys})
+    return out
+
+
+def bench_instance(meb, torch, ctx, dC, dR, mode, steps, warmup, timed, sampler_index):
+    """Warm-up, K timed graph-mode solves (clocks sampled), then ONE host-stepped solve for the event times."""
+    solve = lambda: meb.meb_solve(ctx, dC, dR, TOL, mode)
+    for _ in range(max(warmup, 0)):
+        solve()
+    with ClockSampler(sampler_index) as clk:
+        ms, wall, outs = timed(solve, steps)
+    assert all(o[2]["converged"] == 1 for o in outs), "solve did not converge"
+    meb.meb_set_option(ctx, meb.OPT["STEPPED"], True)
+    try:
+        cs, rs, st_step = meb.meb_solve(ctx, dC, dR, TOL, mode)
+    finally:
+        meb.meb_set_option(ctx, meb.OPT["STEPPED"], False)
+    c, r, st = outs[-1]
+    assert rs == r and torch.equal(cs, c), "the stepped solve must reproduce the graph-mode solve bit for bit"
+    return ms, wall, outs, st_step, clk.summary()
 
 
 def run_b200(args, rank, world, local_rank):
@@ -232,11 +315,15 @@ def run_b200(args, rank, world, local_rank):
     device = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
+    if args.shard and world > 1:
+        from paper_2605_31425_b200 import shard as meb_shard
+        return meb_shard.bench_sharded(args, rank, world, local_rank, METRIC, UNIT, TOL, workload_name)
     k = args.config
     mf, d, _ = workloads.CONFIG_SHAPES[k]
     m = args.m or mf
     mode = meb.MEB_MODE_MIXED if args.mode == "mixed" else meb.MEB_MODE_FP64
-    dC, dR = upload_instance(k, m, d, rank, device)       # seed = rank: replicas solve different instances
+    want_e2e = not args.no_e2e
+    dC, dR, hC, hR = make_instance(k, m, d, rank, device, want_e2e)   # seed = rank: replicas solve different instances
     ctx = meb.Context(m, d)
 
     def barrier():
@@ -261,97 +348,95 @@ def run_b200(args, rank, world, local_rank):
             ms, wall = float(t[0]), float(t[1]) / 1e3
         return ms, wall, outs
 
-    solve = lambda: meb.meb_solve(ctx, dC, dR, TOL, mode)
-    for _ in range(max(args.warmup, 0)):
-        solve()
-    with ClockSampler(local_rank) as clk:
-        ms, wall, outs = timed(solve, args.steps)
-    clocks = clk.summary()
+    ms, wall, outs, st_step, clocks = bench_instance(meb, torch, ctx, dC, dR, mode, args.steps, args.warmup, timed,
+                                                     local_rank)
     c, r, st = outs[-1]
-    assert all(o[2]["converged"] == 1 for o in outs), "solve did not converge"
 
-    # ---- roofline of the dominant streaming kernel, from the event pairs recorded inside the timed solves
-    names = {v: n for n, v in meb.PASS.items()}
-    tot_ms = [sum(o[2]["pass_ms"][i] for o in outs) for i in range(8)]
-    tot_by = [sum(o[2]["pass_bytes"][i] for o in outs) for i in range(8)]
-    tot_n = [sum(o[2]["pass_count"][i] for o in outs) for i in range(8)]
-    hbm_classes = [i for i in range(8) if i != meb.PASS["EVAL_REDUCED"] and tot_n[i] > 0]
-    dom = max(hbm_classes, key=lambda i: tot_ms[i])
+    # ---- roofline of the dominant streaming kernel: CUDA-event pairs of the stepped solve
     peak, peak_src = measured_peak()
-    per_pass = {names.get(i, str(i)): {"launches": tot_n[i], "ms_per_launch": tot_ms[i] / tot_n[i],
-                                       "GBps": tot_by[i] / tot_ms[i] / 1e6 if tot_ms[i] > 0 else None,
-                                       "bytes_per_launch": tot_by[i] / tot_n[i]}
-                for i in range(8) if tot_n[i] > 0}
-    ach = tot_by[dom] / tot_ms[dom] / 1e6
-    roofline = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "frac_of_8TBps_nominal": ach / 8000.0, "peak_source": peak_src,
-                "traffic": ncu_traffic(names[dom], k, args.mode),
-                "algorithmic_bytes_per_launch": tot_by[dom] / tot_n[dom],
-                "share_of_step": tot_ms[dom] / ms, "per_pass": per_pass}
-
-    # ---- cross-check: the dominant evaluation kernel alone, CUDA events around each launch
-    try:
-        import numpy as np
-        reps = 10
-        if args.mode == "mixed":
-            ing = meb.meb_ingest(ctx, dC, dR, 1024, want_shadow=True)
-            Cp, Rp, prec = ing["C32"], ing["R32"], meb.MEB_FP32
-            x0 = torch.zeros(d + 1, dtype=torch.float64, device=device); x0[0] = 0.9 * ing["L"]
-        else:
-            ing = meb.meb_ingest(ctx, dC, dR, 1024)
-            Cp, Rp, prec = dC, dR, meb.MEB_FP64
-            x0 = torch.cat([torch.tensor([0.9 * ing["L"]], dtype=torch.float64, device=device), ing["c0"]])
-        meb.meb_set_pass_timing(ctx, True)
-        tms = []
-        for _ in range(reps + 2):
-            meb.meb_eval_alm(ctx, prec, Cp, Rp, None, None, None, x0, x0, 1.0 / ing["L"], 1.0 / ing["L"] ** 2)
-            tms.append(meb.meb_last_pass_info(ctx))
-        meb.meb_set_pass_timing(ctx, False)
-        tms = tms[2:]
-        ev_ms = sum(t[0] for t in tms) / len(tms)
-        roofline["events_check"] = {"kernel": "eval_alm stand-alone (no multipliers), CUDA events",
-                                    "ms_per_launch": ev_ms, "GBps": tms[0][1] / ev_ms / 1e6,
-                                    "bytes_per_launch": tms[0][1]}
-        del ing, Cp, Rp
-    except Exception as exc:  # the cross-check must never take the bench line down
-        roofline["events_check"] = {"error": repr(exc)}
+    per_pass = pass_table(meb, [o[2] for o in outs], st_step, peak)
+    names = {v: n for n, v in meb.PASS.items()}
+    hbm = [i for i in range(8) if i != meb.PASS["EVAL_REDUCED"] and st_step["pass_ev_count"][i] > 0]
+    dom = max(hbm, key=lambda i: st_step["pass_ev_ms"][i])
+    pd = per_pass[names[dom]]
+    n_graph_dom = sum(o[2]["pass_count"][dom] for o in outs) or (st_step["pass_ev_count"][dom] * len(outs))
+    roofline = {"bound": "hbm", "kernel": names[dom], "achieved": pd["GBps"], "peak": peak, "unit": "GB/s",
+                "frac": pd["GBps"] / peak, "frac_of_8TBps_nominal": pd["GBps"] / 8000.0, "peak_source": peak_src,
+                "timing": "CUDA events around each launch of a host-stepped solve of the same instance",
+                "traffic": ncu_traffic(names[dom], k),
+                "algorithmic_bytes_per_launch": pd["bytes_per_launch"], "ms_per_launch": pd["ms_per_launch"],
+                "share_of_step": n_graph_dom * pd["ms_per_launch"] / ms,
+                "in_graph_globaltimer": pd.get("in_graph_globaltimer"), "per_pass": per_pass}
 
     # ---- end to end: host buffers in, (r, c) out, through meb_solve_host
     e2e = None
-    if not args.no_e2e:
-        hC = dC.cpu().pin_memory()
-        hR = None if dR is None else dR.cpu().pin_memory()
+    if want_e2e:
         solve_h = lambda: meb.meb_solve_host(ctx, hC, hR, TOL, mode)
         solve_h()
-        ms_h, wall_h, outs_h = timed(solve_h, args.steps)
-        e2e = {"value": ms_h / 1e3 / args.steps, "unit": UNIT,
+        e2e_steps = args.steps if hC.numel() * 8 < (2 << 30) else min(args.steps, 3)
+        ms_h, wall_h, outs_h = timed(solve_h, e2e_steps)
+        e2e = {"value": ms_h / 1e3 / e2e_steps, "unit": UNIT, "steps": e2e_steps,
                "h2d_bytes_per_step": int(hC.numel() * 8 + (0 if hR is None else hR.numel() * 8)),
-               "d2h_bytes_per_step": int((d + 1) * 8), "wall_s_per_step": wall_h / args.steps}
-        del hC, hR
+               "d2h_bytes_per_step": int((d + 1) * 8), "wall_s_per_step": wall_h / e2e_steps,
+               "note": "PCIe-bound: one host-to-device copy of the centres, then the device-resident solve"}
 
     line = {"metric": METRIC, "value": ms / 1e3 / args.steps, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": workload_name(k, m, d, args.mode), "multi_gpu": "replicas only",
-                       "l2": "inputs larger than L2 (%.0f MB streamed per pass)" % (tot_by[dom] / tot_n[dom] / 1e6)},
+            "config": {"workload": workload_name(k, m, d, args.mode), "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs larger than L2 (%.0f MB streamed per pass)" % (pd["bytes_per_launch"] / 1e6)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(sum(o[2]["kernel_launches"] for o in outs)),
-            "roofline": roofline, "wall_s_per_step": wall / args.steps,
-            "solve": {"radius": r, "kkt": st["kkt"], "delta_max": st["delta_max"],
-                      "outer_iters": st["outer_iters"], "newton_iters": st["newton_iters"],
-                      "cg_iters": st["cg_iters"], "passes_fp64_full": st["passes_fp64_full"],
-                      "passes_fp32_full": st["passes_fp32_full"], "passes_reduced": st["passes_reduced"], "passes_cut": st["passes_cut"],
-                      "n_reduced": st["n_reduced"], "rounds": st["rounds"],
-                      "ms_phase_lo": st["ms_phase_lo"], "ms_phase_hi": st["ms_phase_hi"],
-                      "ms_check": st["ms_check"]}}
+            "roofline": roofline, "wall_s_per_step": wall / args.steps, "solve": solve_summary(r, st)}
+
+    # ---- CPU oracle on the host cores (rank 0, N = 1): bounded sample of the headline instance
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         m_s = oracle_sample_size(k, m, d, args.cpu_sample)
-        dt, r_o, _ = oracle_solve_sample(k, m, d, args.mode, m_s)
-        line["cpu_baseline"] = {"value": dt * (m / m_s), "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
-                                "sample": f"first {m_s} of {m} balls of the same seeded instance: {dt:.3f} s "
-                                          f"measured, scaled x{m / m_s:.1f} (cost per pass is linear in m); numpy: elementwise "
-                                          f"passes on 1 thread, BLAS calls on up to `cores` threads"}
+        if hC is not None:
+            Cs, Rs = hC.numpy()[:m_s], (None if hR is None else hR.numpy()[:m_s])
+        else:
+            Cs, Rs = workloads.config(k, m_s, d, rank)
+        dt, r_o, _ = oracle_time(Cs, Rs, args.mode)
+        line["cpu_baseline"] = cpu_baseline_entry(Cs, Rs, m, args.mode, dt, m_s)
+    # ---- the other configurations (N = 1): FP64 and mixed, event-timed passes, solve statistics
+    extras = world == 1 and not args.no_extra and args.m is None
+    block = {}
+
+    def extra(kk, mk, dk, ectx, eC, eR, mname):
+        mmode = meb.MEB_MODE_FP64 if mname == "fp64" else meb.MEB_MODE_MIXED
+        nst = 20 if kk <= 2 else 5
+        ems, ewall, eouts, est_step, eclk = bench_instance(meb, torch, ectx, eC, eR, mmode, nst, 2, timed, local_rank)
+        ec, er, est = eouts[-1]
+        block[f"config{kk}_{mname}"] = {
+            "workload": workload_name(kk, mk, dk, mname), "steps": nst, "ms_per_step": ems / nst,
+            "per_pass": pass_table(meb, [o[2] for o in eouts], est_step, peak), "clocks": eclk,
+            "solve": solve_summary(er, est)}
+
+    if extras:
+        extra(k, m, d, ctx, dC, dR, "fp64" if args.mode == "mixed" else "mixed")
     ctx.close()
+    del dC, dR, hC, hR, ctx
+    torch.cuda.empty_cache()
+    if extras:
+        for kk in (1, 2, 3, 4, 5):
+            if kk == k:
+                continue
+            mk, dk, _ = workloads.CONFIG_SHAPES[kk]
+            eC, eR, _, _ = make_instance(kk, mk, dk, 0, device, False)
+            ectx = meb.Context(mk, dk)
+            for mname in ("fp64", "mixed"):
+                extra(kk, mk, dk, ectx, eC, eR, mname)
+            if kk == 2 and rank == 0 and not args.no_cpu_baseline:
+                # the oracle on the FULL config-2 instance, measured once (about a minute on one core)
+                Ch = eC.cpu().numpy()
+                dt2, r2, _ = oracle_time(Ch, None, "mixed")
+                block["config2_mixed"]["cpu_oracle"] = cpu_baseline_entry(Ch, None, mk, "mixed", dt2, mk)
+                block["config2_mixed"]["cpu_oracle"]["radius"] = r2
+                del Ch
+            ectx.close()
+            del eC, eR, ectx
+            torch.cuda.empty_cache()
+        line["configs"] = block
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

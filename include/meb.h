@@ -239,6 +239,17 @@ MEB_API int meb_eval_alm(meb_ctx* ctx, int prec, int64_t m, int32_t d, const voi
                  double* out_scalars, double* grad, double* t_out, double* lam_out,
                  int32_t* active_idx, double* active_rho, double* active_lam);
 
+/* ---- a1 with several points of one line (multi-trial Armijo; DESIGN reading 19) ----------
+ * Same pass as meb_eval_alm at x (out_scalars, grad as there), which ALSO returns
+ *   psi_out[k] = psi_var(x - h_gammas[k] * dir),  k < n_steps <= 4      (device doubles; dir: device [d+1])
+ * from ||b_i||^2, <b_i, dir_c> and ||dir_c||^2 of every ball: one read of the rows whatever n_steps is.
+ * h_gammas must be non-negative and non-decreasing.  Inside meb_solve every Armijo trial pass uses this to
+ * predict the next halvings of its step.  Rows must be 16-byte aligned (else MEB_E_CAPACITY). */
+MEB_API int meb_eval_alm_multi(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
+                       const void* R, const void* U, const int32_t* v_slot, const void* Vrows, int64_t ldv,
+                       const double* x, const double* xbar, double sigma, double tau, const double* dir,
+                       int32_t n_steps, const double* h_gammas, double* out_scalars, double* grad, double* psi_out);
+
 /* ---- a2: generalized-Hessian-vector product (P_i: reading 1) ---------------
  *   Hq = (tau/sigma) q + sigma sum_i P_i q,  P_i = I (B1), 0 (B2),
  *   1/2 [[1, w^T],[w, (1+rho) I - rho w w^T]] (B3), w = b/nb, rho = a/nb.

@@ -263,3 +263,20 @@ def feasibility_check(C, R, r, c, eps_feas, kept_mask=None):
     if kept_mask is not None:
         bad &= ~(np.asarray(kept_mask).astype(bool))
     return float(viol[amax]), amax, np.flatnonzero(bad).astype(np.int32), viol
+
+
+# ----------------------------------------------------------------------------- a1 along a line
+def eval_alm_line(C, R, U, V, x, xbar, sigma, tau, direction, gammas, dtype=np.float64):
+    """psi_var at the points x - gamma * direction, one plain evaluation per gamma (the definition the CUDA
+    path's single-pass multi-trial evaluation is compared with).  Returns a list of
+    ``(psi_var, psi_scale)`` with psi_scale = |r| + (sigma/2) sum ||Pi(z_i)||^2 + (tau/2sigma)||x - xbar||^2."""
+    x = np.asarray(x, dtype=np.float64)
+    direction = np.asarray(direction, dtype=np.float64)
+    out = []
+    for g in gammas:
+        xg = x - float(g) * direction
+        ev = eval_alm(C, R, U, V, xg, xbar, sigma, tau, dtype)
+        dx = xg - np.asarray(xbar, dtype=np.float64)
+        scale = abs(xg[0]) + 0.5 * float(sigma) * ev["scale_proj2"] + 0.5 * (float(tau) / float(sigma)) * float(dx @ dx)
+        out.append((ev["psi_var"], scale))
+    return out

@@ -42,6 +42,8 @@ class Params:
     tol_red_factor: float = 0.02  # tol_red = 0.02 r_hat  [reading 9], pinned by Table 1
     max_rounds: int = 10          # active-set refinement rounds
     sample_rows: int = 1024       # rows whose mean is the initial centre c^0
+    ag_outer: int = 0             # outer iterations k < ag_outer use the accelerated gradient inner solver
+    ag_inner_max: int = 500       # its iteration cap  [reading 20]
 
 
 @dataclass
@@ -153,6 +155,57 @@ def ssn(C, R, U, V, x, xbar, alphabeta, sigma, tau, tol, par: Params, dtype, len
     return x, ev, status
 
 
+def accelerated_gradient(C, R, U, V, x, xbar, alphabeta, sigma, tau, tol, par: Params, dtype, length_unit,
+                         stats: Stats):
+    """Accelerated gradient method for the subproblem (4)  ("First-order methods, including accelerated
+    gradient methods [4], provide simple inner solvers ... attractive in the early outer iterations").
+    [reading 20] FISTA with backtracking on the Lipschitz estimate and the gradient restart:
+        x+ = y - grad Psi(y) / Lip,  accepted when Psi(x+) <= Psi(y) - ||grad Psi(y)||^2 / (2 Lip), else Lip <- 2 Lip;
+        t+ = (1 + sqrt(1 + 4 t^2)) / 2,   y+ = x+ + ((t - 1) / t+) (x+ - x);   restart (t = 1, y+ = x+) when
+        <grad Psi(y), x+ - x> > 0.
+    Lip starts at tau/sigma + sigma * (number of active balls at x), the norm bound of H there (||P_i|| <= 1).
+    Same stopping tests as Algorithm 2 (condition (5) or KKT_max on the tentative quantities).  Returns (x, ev, status)."""
+    ev = prim.eval_alm(C, R, U, V, x, xbar, sigma, tau, dtype)
+    stats.evals += 1
+    status = "cap"
+    y = x.copy()
+    ev_y = ev
+    t = 1.0
+    lip = tau / sigma + sigma * max(1, ev["n_b1"] + ev["n_b3"])
+    for _ in range(par.ag_inner_max):
+        kkt, _ = rel_kkt(ev, x[0], length_unit)
+        if condition5(ev, x, xbar, alphabeta, sigma, tau, par.rho):
+            status = "cond5"
+            break
+        if kkt <= tol:
+            status = "kkt"
+            break
+        g_y = ev_y["grad"]
+        gg = float(g_y @ g_y)
+        accepted = False
+        for _bt in range(60):
+            x_new = y - g_y / lip
+            ev_new = prim.eval_alm(C, R, U, V, x_new, xbar, sigma, tau, dtype)
+            stats.evals += 1
+            if ev_new["psi_var"] <= ev_y["psi_var"] - 0.5 * gg / lip:
+                accepted = True
+                break
+            lip *= 2.0
+        if not accepted:
+            status = "stalled"
+            break
+        restart = float(g_y @ (x_new - x)) > 0.0
+        t_new = 1.0 if restart else 0.5 * (1.0 + np.sqrt(1.0 + 4.0 * t * t))
+        y = x_new.copy() if restart else x_new + ((t - 1.0) / t_new) * (x_new - x)
+        x, ev, t = x_new, ev_new, t_new
+        if np.array_equal(y, x):
+            ev_y = ev                      # the evaluation at x+ is the evaluation at y
+        else:
+            ev_y = prim.eval_alm(C, R, U, V, y, xbar, sigma, tau, dtype)
+            stats.evals += 1
+    return x, ev, status
+
+
 def ripalm(C, R, x0, alphabeta0, U0, V0, tol, par: Params, dtype=np.float64, length_unit=1.0,
            sigma0=None):
     """Algorithm 1 on the data as given.  Terminates when the maximum KKT
@@ -166,8 +219,9 @@ def ripalm(C, R, x0, alphabeta0, U0, V0, tol, par: Params, dtype=np.float64, len
     tau = par.tau
     for k in range(par.outer_max):
         xbar = x.copy()                                                   # (r^k, c^k)
-        x, ev, status = ssn(C, R, U, V, x, xbar, ab, sigma, tau, tol, par, dtype,
-                            length_unit, st)                              # step 3
+        inner = accelerated_gradient if k < par.ag_outer else ssn         # P:L204 / Algorithm 2
+        x, ev, status = inner(C, R, U, V, x, xbar, ab, sigma, tau, tol, par, dtype,
+                              length_unit, st)                            # step 3
         U = ev["Uplus"].copy()                                            # eq. (6)
         V = ev["Vplus"].copy()
         ab = ab - sigma * ev["grad"]                                      # step 4

@@ -29,7 +29,7 @@ EXPORTS = [
     "meb_create", "meb_destroy", "meb_strerror", "meb_last_cuda_error", "meb_default_params",
     "meb_version", "meb_solve", "meb_solve_host", "meb_ingest", "meb_eval_alm", "meb_hvp",
     "meb_dense_hessian", "meb_update_multipliers", "meb_screen_compact", "meb_feasibility_check",
-    "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch", "meb_set_option",
+    "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch", "meb_set_option", "meb_eval_alm_multi",
 ]
 
 
@@ -102,6 +102,7 @@ def load():
     lib.meb_ingest.argtypes = [vp, i64, i32, vp, i64, vp, i32, vp, vp, vp, i64, vp]
     prob = [vp, C.c_int, i64, i32, vp, i64, vp, vp, vp, vp, i64]
     lib.meb_eval_alm.argtypes = prob + [vp, vp, dbl, dbl, vp, vp, vp, vp, vp, vp, vp]
+    lib.meb_eval_alm_multi.argtypes = prob + [vp, vp, dbl, dbl, vp, i32, vp, vp, vp, vp]
     lib.meb_hvp.argtypes = prob + [vp, dbl, dbl, vp, vp]
     lib.meb_dense_hessian.argtypes = prob + [vp, dbl, dbl, vp]
     lib.meb_update_multipliers.argtypes = prob + [vp, dbl, vp, vp, vp, i64, i64, C.POINTER(i64), C.POINTER(dbl)]
@@ -298,6 +299,21 @@ def meb_eval_alm(ctx: Context, prec, Cm, R, U, v_slot, Vrows, x, xbar, sigma, ta
         n = int(out[EV["N_ACTIVE"]].item())
         res.update(active_idx=a_idx[:n], active_rho=a_rho[:n], active_lam=a_lam[:n])
     return res
+
+
+def meb_eval_alm_multi(ctx: Context, prec, Cm, R, U, v_slot, Vrows, x, xbar, sigma, tau, direction, gammas):
+    """One pass: the evaluation at x plus psi_var at x - gammas[k] * direction (k < len(gammas) <= 4)."""
+    m, d, ld, ldv = _problem(prec, Cm, R, U, v_slot, Vrows)
+    dev = Cm.device
+    out = torch.zeros(MEB_EVAL_NSCALARS, dtype=torch.float64, device=dev)
+    grad = torch.zeros(d + 1, dtype=torch.float64, device=dev)
+    n = len(gammas)
+    psi = torch.zeros(n, dtype=torch.float64, device=dev)
+    g = (C.c_double * n)(*[float(v) for v in gammas])
+    _check(load().meb_eval_alm_multi(ctx.h, prec, m, d, _ptr(Cm), ld, _ptr(R), _ptr(U), _ptr(v_slot), _ptr(Vrows), ldv,
+                                     _ptr(x), _ptr(xbar), float(sigma), float(tau), _ptr(direction), n,
+                                     C.cast(g, C.c_void_p), _ptr(out), _ptr(grad), _ptr(psi)), "meb_eval_alm_multi")
+    return dict(scalars=out, grad=grad, psi=psi)
 
 
 def meb_hvp(ctx: Context, prec, Cm, R, U, v_slot, Vrows, x, sigma, tau, q):

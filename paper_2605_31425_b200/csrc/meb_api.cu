@@ -19,11 +19,12 @@ static size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 static void ctx_free_all(meb_ctx* c) {
     if (!c) return;
+    cudaFree(c->vmask); cudaFree(c->vlist); cudaFree(c->part_multi); cudaFree(c->dyn_api);
     cudaFree(c->mask); cudaFree(c->rec_lam); cudaFree(c->rec_rho); cudaFree(c->rec_t);
     cudaFree(c->list); cudaFree(c->blocksum); cudaFree(c->part_scalar); cudaFree(c->part_vec);
     cudaFree(c->part_mat); cudaFree(c->part_red); cudaFree(c->count_dev); cudaFree(c->part_sc); cudaFree(c->small);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
-    for (int i = 0; i < 24; ++i) if (c->own[i]) cudaFree(c->own[i]);
+    for (int i = 0; i < 40; ++i) if (c->own[i]) cudaFree(c->own[i]);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     meb_free_graph_cache(c);
@@ -90,6 +91,12 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     c->h_pinned_len = 12 * (int64_t)dpad + 256;     // [0, 4 dpad + 256): read-backs; then 8 upload slots of dpad
 #define TRY_ALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void**)&(ptr), (bytes))
     TRY_ALLOC(c->mask, nwords * sizeof(uint32_t));
+    if ((size_t)d_max * 8 > 1024) {                  // long rows (meb_long.cu): list of the balls with a multiplier row
+        TRY_ALLOC(c->vmask, nwords * sizeof(uint32_t));
+        TRY_ALLOC(c->vlist, ((size_t)m_max + 32) * sizeof(int32_t));
+    }
+    TRY_ALLOC(c->part_multi, (size_t)MEB_MAX_GRID * MEB_MULTI_MAX * sizeof(double));
+    TRY_ALLOC(c->dyn_api, sizeof(MebDyn));
     TRY_ALLOC(c->rec_lam, (size_t)m_max * sizeof(double));
     TRY_ALLOC(c->rec_rho, (size_t)m_max * sizeof(double));
     TRY_ALLOC(c->rec_t, (size_t)m_max * sizeof(double));
@@ -175,16 +182,27 @@ static int check_problem(const meb_ctx* ctx, int64_t m, int32_t d, const void* C
 
 // one streaming launch, optionally timed with CUDA events on the context's stream.  Short aligned rows
 // go to the TMA-staged tile kernels (meb_tile.cu), everything else to the register-mapped kernels.
-static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid, bool* fused) {
+enum { PATH_TILE = 0, PATH_LONG = 1, PATH_STREAM = 2 };
+static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid, int* path_out) {
+    const bool tile = meb_tile_applicable(op, prec, a);
+    const bool longk = !tile && ctx->vlist != nullptr && meb_long_applicable(op, prec, a);
+    const int32_t* vlist = nullptr; const int32_t* vcount = nullptr;
+    if (longk && op == OP_EVAL && a.dyn == nullptr && a.v_slot != nullptr) {
+        // per-primitive call: the list of the balls with a multiplier row is built here (a solve keeps it up to date)
+        int rcl = meb_build_vlist(ctx, a.v_slot, a.m, ctx->vlist, ctx->count_dev + 1);
+        if (rcl != MEB_OK) return rcl;
+        vlist = ctx->vlist; vcount = ctx->count_dev + 1;
+    }
     if (ctx->time_passes) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     cudaStreamIsCapturing(ctx->stream, &cap);
     const bool pool = ctx->ev_record && !ctx->time_passes && ctx->evn < MEB_EVPOOL && cap == cudaStreamCaptureStatusNone;
     if (pool) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn], ctx->stream));
-    const bool tile = meb_tile_applicable(op, prec, a);
-    int rc = tile ? meb_launch_tile(ctx, op, prec, a, grid) : meb_launch_stream(ctx, op, prec, a, grid);
+    int rc = tile ? meb_launch_tile(ctx, op, prec, a, grid)
+                  : (longk ? meb_launch_long(ctx, op, prec, a, vlist, vcount, grid) : meb_launch_stream(ctx, op, prec, a, grid));
     if (rc != MEB_OK) return rc;
-    if (fused) *fused = tile && op == OP_EVAL;
+    ctx->last_path = tile ? PATH_TILE : (longk ? PATH_LONG : PATH_STREAM);
+    if (path_out) *path_out = ctx->last_path;
     if (pool) {
         MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn + 1], ctx->stream));
         ctx->evclass[ctx->evn] = ctx->cur_class;
@@ -243,21 +261,28 @@ int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, double* out_scalars, doub
     bool any_mult = c.U != nullptr;
     if (c.gs) {
         s.dyn = c.gs->dyn;
-        for (int b = 0; b < 2; ++b) { s.U2[b] = c.gs->U2[b]; s.slot2[b] = c.gs->slot2[b]; s.V2[b] = c.gs->V2[b]; }
+        for (int b = 0; b < 2; ++b) {
+            s.U2[b] = c.gs->U2[b]; s.slot2[b] = c.gs->slot2[b]; s.V2[b] = c.gs->V2[b];
+            s.vlist2[b] = c.gs->vlist2[b]; s.vcount2[b] = c.gs->vcount2[b];
+        }
         any_mult = true;
+        if (c.gs->multi > 0 && (c.gs->v || c.gs->dir)) {
+            s.multi = c.gs->multi; s.dir = c.gs->dir ? c.gs->dir : c.gs->v->dir_raw; s.multi_part = ctx->part_multi;
+        }
     }
     const double sz = c.prec == MEB_FP64 ? 8.0 : 4.0;
     const double bytes = (double)c.m * (c.d * sz + (c.R ? sz : 0) + (any_mult ? sz + 4 : 0));
-    int grid = 0;
-    bool fused = false;
-    int rc = timed_stream(ctx, OP_EVAL, c.prec, s, bytes, &grid, &fused);
+    int grid = 0, path = PATH_STREAM;
+    int rc = timed_stream(ctx, OP_EVAL, c.prec, s, bytes, &grid, &path);
     if (rc != MEB_OK) return rc;
+    const bool fused = path == PATH_TILE;
     FinalizeArgs f;
     memset(&f, 0, sizeof(f));
     f.part = ctx->part_scalar; f.grid = grid; f.part_vec = ctx->part_vec; f.dpad = s.dpad;
     f.count = ctx->count_dev; f.x = c.x; f.xbar = c.xbar; f.sigma = c.sigma; f.tau = c.tau; f.d = c.d;
     f.out = out_scalars; f.grad = grad;
     if (c.gs) { f.dyn = c.gs->dyn; f.S = c.gs->S; if (c.gs->v) f.v = *c.gs->v; }
+    if (s.multi > 0 && path != PATH_STREAM) f.multi_part = ctx->part_multi;  // kernels that carry the multi-trial code
     if (fused) {
         f.nvec = grid; f.tpb = 0;
     } else {                          // long rows: the vector part comes from the active-list kernel
@@ -320,6 +345,76 @@ extern "C" int meb_eval_alm(meb_ctx* ctx, int prec, int64_t m, int32_t d, const 
             if (active_lam) { rc = meb_gather_vec_f64(ctx, ctx->rec_lam, ctx->list, n, active_lam); if (rc) return rc; }
         }
     }
+    return MEB_OK;
+}
+
+// ---- multi-trial evaluation: Psi at several points of one line in ONE pass ------------------
+namespace {
+__global__ void multi_setup_kernel(MebDyn* dyn, const double* __restrict__ dir, int d, int n, double g0, double g1,
+                                   double g2, double g3, double sigma, double tau, int has_mult) {
+    __shared__ double red[8];
+    double s = 0.0;
+    for (int j = 1 + threadIdx.x; j <= d; j += blockDim.x) s = fma(dir[j], dir[j], s);
+    s = warp_sum(s);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+        dyn->sigma_raw = sigma; dyn->tau_eff = tau; dyn->cur = 0; dyn->has_mult = has_mult; dyn->s0_abort = 1e300;
+        dyn->multi_n = n;
+        dyn->multi_gamma[0] = g0; dyn->multi_gamma[1] = g1; dyn->multi_gamma[2] = g2; dyn->multi_gamma[3] = g3;
+        dyn->dir_r = dir[0]; dyn->dir_c2 = t;
+    }
+}
+// psi_out[k] = r_k + (sigma/2) S_k + (tau/2sigma) ||x_k - xbar||^2 at x_k = x - gamma_k dir (reading 13)
+__global__ void multi_psi_kernel(const double* __restrict__ part_multi, int grid, const MebDyn* dyn,
+                                 const double* __restrict__ x, const double* __restrict__ xbar,
+                                 const double* __restrict__ dir, int d, double* __restrict__ psi_out) {
+    const int k = blockIdx.x, lane = threadIdx.x;
+    if (k >= dyn->multi_n) return;
+    const double g = dyn->multi_gamma[k];
+    double s = 0.0, dx2 = 0.0;
+    for (int b = lane; b < grid; b += 32) s += part_multi[(size_t)b * MEB_MULTI_MAX + k];
+    for (int j = lane; j <= d; j += 32) { const double w = x[j] - g * dir[j] - (xbar ? xbar[j] : x[j] - g * dir[j]); dx2 = fma(w, w, dx2); }
+    s = warp_sum(s); dx2 = warp_sum(dx2);
+    if (lane == 0) psi_out[k] = (x[0] - g * dir[0]) + 0.5 * dyn->sigma_raw * s + 0.5 * (dyn->tau_eff / dyn->sigma_raw) * dx2;
+}
+}  // namespace
+
+extern "C" int meb_eval_alm_multi(meb_ctx* ctx, int prec, int64_t m, int32_t d, const void* C, int64_t ld,
+                                  const void* R, const void* U, const int32_t* v_slot, const void* Vrows, int64_t ldv,
+                                  const double* x, const double* xbar, double sigma, double tau, const double* dir,
+                                  int32_t n_steps, const double* h_gammas, double* out_scalars, double* grad,
+                                  double* psi_out) {
+    int rc = check_eval_args(ctx, prec, m, d, C, ld, v_slot, Vrows, ldv, x, sigma);
+    if (rc != MEB_OK) return rc;
+    if (!out_scalars || !grad || !(tau >= 0.0) || !dir || !h_gammas || !psi_out || n_steps < 1 || n_steps > MEB_MULTI_MAX)
+        return MEB_E_ARG;
+    double g[MEB_MULTI_MAX] = {0, 0, 0, 0};
+    for (int k = 0; k < n_steps; ++k) { if (!(h_gammas[k] == h_gammas[k])) return MEB_E_ARG; g[k] = h_gammas[k]; }
+    for (int k = 0; k < n_steps; ++k) if (g[k] < 0.0 || (k > 0 && g[k] < g[k - 1])) return MEB_E_ARG;   // farthest point last
+    ctx->launches++;
+    multi_setup_kernel<<<1, 256, 0, ctx->stream>>>(ctx->dyn_api, dir, d, n_steps, g[0], g[1], g[2], g[3], sigma, tau,
+                                                   (U != nullptr || v_slot != nullptr) ? 1 : 0);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
+    GraphSide gs;
+    memset(&gs, 0, sizeof(gs));
+    gs.dyn = ctx->dyn_api;
+    gs.U2[0] = const_cast<void*>(U); gs.slot2[0] = const_cast<int32_t*>(v_slot); gs.V2[0] = const_cast<void*>(Vrows);
+    gs.multi = n_steps; gs.dir = dir;
+    if (v_slot && ctx->vlist) {
+        rc = meb_build_vlist(ctx, v_slot, m, ctx->vlist, ctx->count_dev + 1);
+        if (rc != MEB_OK) return rc;
+        gs.vlist2[0] = ctx->vlist; gs.vcount2[0] = ctx->count_dev + 1;
+    }
+    EvalCall c{prec, m, d, C, ld, R, U, v_slot, Vrows, ldv, x, xbar, sigma, tau, &gs};
+    rc = meb_eval_internal(ctx, c, out_scalars, grad, nullptr, nullptr);
+    if (rc != MEB_OK) return rc;
+    if (ctx->last_path == PATH_STREAM) return MEB_E_CAPACITY;     // rows that are not 16-byte aligned: no multi-trial kernel
+    ctx->launches++;
+    multi_psi_kernel<<<n_steps, 32, 0, ctx->stream>>>(ctx->part_multi, ctx->last_grid, ctx->dyn_api, x, xbar, dir, d, psi_out);
+    MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }
 

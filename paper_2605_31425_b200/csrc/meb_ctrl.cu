@@ -21,16 +21,21 @@ __global__ void ctrl_resume_kernel(SolverDev* S) {
 __global__ void __launch_bounds__(CBLK) ctrl_after_newton_kernel(SolverDev* S, const SolverVecs v) {
     __shared__ double sm[32];
     const int n = S->n;
-    double sl = 0.0, dx2t = 0.0;
+    const double Ls = S->L;
+    double sl = 0.0, dx2t = 0.0, dc2 = 0.0;
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
-        sl = fma(v.g[j], v.delta[j], sl);
-        const double xj = v.xn[j] + v.delta[j];
+        const double dj = v.delta[j];
+        sl = fma(v.g[j], dj, sl);
+        const double xj = v.xn[j] + dj;
         v.xt[j] = xj;
+        v.dir_raw[j] = Ls * dj;
         const double dxb = xj - v.xbar[j];
         dx2t = fma(dxb, dxb, dx2t);
+        if (j > 0) dc2 = fma(dj, dj, dc2);
     }
     sl = ctrl_block_sum(sl, sm);
     dx2t = ctrl_block_sum(dx2t, sm);
+    dc2 = ctrl_block_sum(dc2, sm);
     __syncthreads();
     ctrl_to_raw(S, v, v.xt, v.x_raw);
     if (threadIdx.x == 0) {
@@ -41,6 +46,7 @@ __global__ void __launch_bounds__(CBLK) ctrl_after_newton_kernel(SolverDev* S, c
         S->ls = 0;
         S->phase = PH_ARMIJO;
         S->action = ACT_TRIAL;
+        ctrl_arm_multi(S, 1.0, 0, Ls * v.delta[0], Ls * Ls * dc2);
     }
 }
 

@@ -12,7 +12,9 @@
 
 enum { PH_FIRST = 0,      // first evaluation of an outer iteration (Alg. 2 lines 3-4): always accepted
        PH_ARMIJO = 1,     // evaluation of an Armijo trial point x + eta*Delta (Alg. 2 line 9)
-       PH_REEVAL = 2 };   // re-evaluation at x before a multiplier update (records of the last pass are stale)
+       PH_REEVAL = 2,     // re-evaluation at x before a multiplier update (records of the last pass are stale)
+       PH_AG_Y = 3,       // accelerated gradient (reading 20): evaluation at the extrapolated point y
+       PH_AG_X = 4 };     //   evaluation at the candidate x+ = y - grad Psi(y) / Lip (backtracking on Lip)
 enum { ACT_TRIAL = 0, ACT_NEWTON = 1, ACT_UPDATE = 2, ACT_DONE = 3 };
 enum { ST_RUNNING = 0, ST_CONVERGED = 1, ST_OUTER_CAP = 2, ST_NEED_CAPACITY = 3, ST_CHOL_FAILED = 4, ST_STALLED = 5 };
 
@@ -39,6 +41,9 @@ struct SolverDev {
                                     // cover) of the V rows they read: one per ball with a slot, i.e. n_support
     // ---- conditional handles of the solve graph ----
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
+    cudaGraphConditionalHandle h_cgp;   // matrix-free Newton solve in one persistent kernel (meb_cg.cu)
+    long long wc_cap;                   // active rows the gathered matrix W of that kernel can hold
+    int32_t cg_mode, pad_cg;            // 1: persistent kernel, 0: one launch per CG iteration (more active rows than W holds)
     double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
     double abort_margin;          // relative slack of MebDyn::s0_abort (rounding of the partial sums); 0: early stop off
     int32_t aborted, pad3;        // Armijo trials cut short
@@ -46,11 +51,24 @@ struct SolverDev {
     int32_t stall_count, tiny;    // tiny: the last Newton direction had a decrement below the floor
     uint32_t pass_hist[48], act_hist[48];   // MEB_TRACE: ns and active balls of the first evaluation passes
     int32_t in_graph, eval_cap;   // eval_cap: hard bound on the evaluations of a phase (a runaway loop cannot hang the GPU)
+    // ---- multi-trial Armijo (DESIGN reading 19) ----
+    int32_t multi_max;            // predictions asked of every trial pass (meb_params.armijo_multi, <= MEB_MULTI_MAX); 0: off
+    int32_t pred_n;               // predictions the last pass delivered (written by the finalize kernel)
+    double pred_s[MEB_MULTI_MAX]; // sum_i ||Pi(z_i)||^2 at x + eta 2^-k Delta, k = 1..pred_n (lower bounds if the pass was cut)
+    int32_t skipped, ag_total;    // step sizes never evaluated; accelerated-gradient iterations
+    double pred_margin;           // relative slack of the predicted sums (rounding of the expansion), like abort_margin
+    // ---- accelerated-gradient inner solver (DESIGN reading 20) ----
+    int32_t ag_outer;             // outer iterations k < ag_outer use it instead of semismooth Newton
+    int32_t ag_it;                // iterations of the current inner solve
+    double ag_t, ag_Lip;          // momentum parameter t_j, current estimate of the Lipschitz constant of grad Psi
+    double ag_psi_y, ag_gg_y;     // Psi(y), ||grad Psi(y)||^2 of the extrapolated point
+    int32_t ag_bt, ag_inner_max;  // doublings of Lip at the current y; iteration cap of one inner solve
 };
 
 // (d+1)-vectors of the state, each of length nv = n rounded up to 8, in one device array
 struct SolverVecs {
     double *xn, *xbar, *ab, *delta, *g, *xt, *x_raw, *xbar_raw, *off, *grad_t, *res, *p, *Hp, *xbest;
+    double *dir_raw;             // L * delta: the direction in raw units, read by the evaluation kernels (multi-trial)
     double *ev_t, *ev;           // [MEB_EVAL_NSCALARS] scalars of the trial / accepted evaluation
 };
 
@@ -65,6 +83,10 @@ struct FinalizeArgs {
     double* out; double* grad;
     const MebDyn* dyn;                            // nullable: overrides sigma, tau
     SolverDev* S; SolverVecs v;                   // nullable: controller step of the solve graph
+    const double* multi_part;                     // nullable: per-CTA partials of the predicted step sizes [grid][MEB_MULTI_MAX]
+    // strides (in doubles) between consecutive partials; 0 = the packed layouts MEB_NPART / dpad / MEB_MULTI_MAX.
+    // A sharded solve hands in the records gathered from the ranks (one record of rec_stride doubles per rank).
+    int part_stride, vec_stride, multi_stride;
 };
 
 __device__ __forceinline__ double ctrl_block_sum(double v, double* sm) {
@@ -115,7 +137,8 @@ __device__ inline void meb_ctrl_init_dev(SolverDev* S, const SolverVecs v, doubl
         S->outer = 0; S->inner = 0; S->ls = 0; S->done = 0; S->status = ST_RUNNING; S->stalled = 0;
         S->newton_total = 0; S->cg_total = 0; S->evals = 0; S->chol_info = 0;
         S->kkt = 1e300; S->n_support = 0; S->best_kkt = 1e300; S->stall_count = 0; S->tiny = 0; S->aborted = 0;
-        S->dyn.s0_abort = 1e300;
+        S->dyn.s0_abort = 1e300; S->dyn.multi_n = 0; S->pred_n = 0; S->skipped = 0; S->ag_total = 0; S->ag_it = 0;
+        S->ag_t = 1.0; S->ag_Lip = 1.0; S->ag_bt = 0;
         S->pass_ns = 0ull; S->pass_count = 0; S->vrow_reads = 0ull;
         S->eta = 1.0; S->psi_cur = 0.0; S->slope = 0.0;
         S->cg_go = 0; S->cg_it = 0;
@@ -127,7 +150,11 @@ __device__ __forceinline__ void ctrl_set_handles(const SolverDev* S) {
     cudaGraphSetConditional(S->h_while, S->done ? 0u : 1u);
     cudaGraphSetConditional(S->h_newton, (!S->done && S->action == ACT_NEWTON) ? 1u : 0u);
     cudaGraphSetConditional(S->h_update, (!S->done && S->action == ACT_UPDATE) ? 1u : 0u);
-    if (!S->dense) cudaGraphSetConditional(S->h_cg, (!S->done && S->action == ACT_NEWTON && S->cg_go) ? 1u : 0u);
+    if (!S->dense) {
+        const bool go = !S->done && S->action == ACT_NEWTON && S->cg_go;
+        cudaGraphSetConditional(S->h_cgp, (go && S->cg_mode == 1) ? 1u : 0u);
+        cudaGraphSetConditional(S->h_cg, (go && S->cg_mode == 0) ? 1u : 0u);
+    }
 }
 
 // Thread 0: arm the early stop (MebDyn::s0_abort) for the Armijo trial with normalised radius rt and
@@ -142,6 +169,21 @@ __device__ __forceinline__ void ctrl_arm_abort(SolverDev* S, bool trial, double 
         if (room > 0.0) thr = 2.0 * S->L * S->L * room / S->sigma * (1.0 + S->abort_margin);
     }
     S->dyn.s0_abort = thr;
+    if (!trial) S->dyn.multi_n = 0;
+}
+
+// Thread 0: the trial pass at step eta (after `ls` shortenings) also predicts the next halvings eta 2^-k
+// (MebDyn::multi_*): as many as asked for and as the halving budget still allows.  dir_r, dir_c2: Delta r and
+// ||Delta c||^2 in raw units.
+__device__ __forceinline__ void ctrl_arm_multi(SolverDev* S, double eta, int ls, double dir_r, double dir_c2) {
+    int nm = S->multi_max;
+    if (nm > S->armijo_max - ls) nm = S->armijo_max - ls;
+    if (nm < 0 || S->shrink_min != 0.5 || S->tiny) nm = 0;
+    S->dyn.multi_n = nm;
+    double f = 1.0;
+    for (int k = 0; k < MEB_MULTI_MAX; ++k) { f *= 0.5; S->dyn.multi_gamma[k] = eta * (1.0 - f); }
+    S->dyn.dir_r = dir_r;
+    S->dyn.dir_c2 = dir_c2;
 }
 
 // relative KKT residual (reading 7) from the scalars of an evaluation
@@ -178,6 +220,50 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     const bool use_off = S->use_off != 0;
     const double psi_t = ev_s[MEB_EV_PSI] / Ls;
     bool accept = true, stalled = false;
+    // ---- accelerated gradient inner solver (outer iterations k < ag_outer, reading 20) ----
+    // y lives in v.p, grad Psi(y) in v.res, the previous iterate in v.Hp (the CG vectors are idle in this mode).
+    if (phase == PH_AG_Y) {
+        // the pass evaluated Psi and its gradient at y = v.xt: candidate x+ = y - grad Psi(y) / Lip
+        double gg = 0.0;
+        const double il = 1.0 / S->ag_Lip;
+        for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            const double gj = v.grad_t[j], yj = v.xt[j];
+            v.res[j] = gj; v.p[j] = yj;
+            gg = fma(gj, gj, gg);
+            const double xj = fma(-il, gj, yj);
+            v.xt[j] = xj;
+            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+        }
+        gg = ctrl_block_sum(gg, sm);
+        if (threadIdx.x == 0) {
+            S->ag_psi_y = psi_t; S->ag_gg_y = gg; S->ag_bt = 0;
+            S->phase = PH_AG_X; S->action = ACT_TRIAL; S->evals++;
+            ctrl_arm_abort(S, false, 0.0, 0.0);
+            if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
+            ctrl_set_handles(S);
+        }
+        return;
+    }
+    if (phase == PH_AG_X && !(psi_t <= S->ag_psi_y - 0.5 * S->ag_gg_y / S->ag_Lip)) {
+        // sufficient decrease failed: Lip <- 2 Lip and a shorter step from the same y; after 60 doublings give up
+        // and re-evaluate at x (the records of this pass are not those of x)
+        const bool giveup = S->ag_bt >= 60;
+        const double il = 1.0 / (2.0 * S->ag_Lip);
+        for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            const double xj = giveup ? v.xn[j] : fma(-il, v.res[j], v.p[j]);
+            v.xt[j] = xj;
+            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            if (giveup) S->phase = PH_REEVAL; else { S->ag_Lip *= 2.0; S->ag_bt++; }
+            S->action = ACT_TRIAL; S->evals++;
+            ctrl_arm_abort(S, false, 0.0, 0.0);
+            if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
+            ctrl_set_handles(S);
+        }
+        return;
+    }
     if (phase == PH_ARMIJO) {
         if (!(psi_t <= S->psi_cur + S->armijo_mu * S->eta * S->slope)) {
             if (S->ls >= S->armijo_max || S->tiny) {
@@ -195,10 +281,34 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         // Psi'(x; Delta) = slope and Psi(x + eta Delta) has its minimiser below shrink_min * eta: then the
         // trials in between are skipped (shrink_min = 1/2: plain halving; 1/8 keeps eta on the halving grid); reading 4
         double eta = 0.0;
+        int skip = 0;
         if (!stalled) {
             const double den = psi_t - S->psi_cur - S->slope * S->eta;      // > 0 whenever the Armijo test fails
             const double fq = -0.5 * S->slope * S->eta / den;
             eta = ((fq < S->shrink_min) ? S->shrink_min : 0.5) * S->eta;    // a NaN trial value halves
+            // Multi-trial (reading 19): the pass also summed ||Pi(z_i)||^2 at eta/2, eta/4, ... (lower bounds if it
+            // was cut short).  Psi~(x + e Delta) = r~ + (sigma / 2 L^2) S + (tau / 2 sigma) ||x + e Delta - xbar||^2;
+            // a halving whose bound already fails the Armijo test is skipped: it would be rejected when evaluated,
+            // so the step that is finally accepted is the one plain halving accepts.
+            const int np = S->pred_n;
+            if (np > 0) {
+                double A = 0.0, B = 0.0, D = 0.0;
+                for (int j = threadIdx.x; j < n; j += blockDim.x) {
+                    const double w = v.xn[j] - v.xbar[j], dj = v.delta[j];
+                    A = fma(w, w, A); B = fma(w, dj, B); D = fma(dj, dj, D);
+                }
+                ctrl_block_sum3(A, B, D, sm);
+                const double cs = 0.5 * S->sigma / (Ls * Ls) * (1.0 - S->pred_margin);
+                const double cp = 0.5 * S->tau / S->sigma;
+                double ek = S->eta;
+                for (int k = 0; k < np; ++k) {
+                    ek *= 0.5;
+                    if (S->ls + 1 + skip >= S->armijo_max) break;             // the last allowed halving is always evaluated
+                    const double lb = v.xn[0] + ek * v.delta[0] + cs * S->pred_s[k] + cp * (A + ek * (2.0 * B + ek * D));
+                    if (lb > S->psi_cur + S->armijo_mu * ek * S->slope) ++skip; else break;
+                }
+                for (int q = 0; q < skip; ++q) eta *= 0.5;
+            }
         }
         double dx2t = 0.0;
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
@@ -212,7 +322,10 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         __syncthreads();
         if (threadIdx.x == 0) {
             ctrl_arm_abort(S, !stalled, v.xn[0] + eta * v.delta[0], dx2t);
-            if (stalled) { S->phase = PH_REEVAL; } else { S->eta = eta; S->ls++; }
+            if (stalled) { S->phase = PH_REEVAL; } else {
+                S->eta = eta; S->ls += 1 + skip; S->skipped += skip;
+                ctrl_arm_multi(S, eta, S->ls, S->dyn.dir_r, S->dyn.dir_c2);
+            }
             S->action = ACT_TRIAL; S->evals++;
             if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
             ctrl_set_handles(S);
@@ -221,12 +334,18 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     }
     // ---- accepted: the pass becomes the evaluation at x; condition (5) in the same sweep:
     //      2 sigma |<(alpha,beta) - x, g>| + sigma^2 ||g||^2 <= rho (sum ||dmult||^2 + tau ||x - xbar||^2)
-    double agx = 0.0, gg = 0.0, dx2 = 0.0;
-    const bool take_xt = phase == PH_ARMIJO;
+    double agx = 0.0, gg = 0.0, dx2 = 0.0, dotr = 0.0;
+    const bool take_xt = phase == PH_ARMIJO || phase == PH_AG_X;
+    const bool agmode = S->outer < S->ag_outer;
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
         const double xj = take_xt ? v.xt[j] : v.xn[j];
         const double gj = v.grad_t[j];
         const double abj = v.ab[j], xbj = v.xbar[j];
+        if (agmode) {                                   // previous iterate, and <grad Psi(y), x+ - x> for the restart test
+            const double xp = v.xn[j];
+            v.Hp[j] = xp;
+            if (phase == PH_AG_X) dotr = fma(v.res[j], xj - xp, dotr);
+        }
         if (take_xt) v.xn[j] = xj;
         v.g[j] = gj;
         agx = fma(abj - xj, gj, agx);
@@ -237,7 +356,9 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     }
     if (threadIdx.x < MEB_EVAL_NSCALARS) v.ev[threadIdx.x] = ev_s[threadIdx.x];
     ctrl_block_sum3(agx, gg, dx2, sm);
+    if (agmode && phase == PH_AG_X) dotr = ctrl_block_sum(dotr, sm);        // (touches sm[0..31] only)
     if (threadIdx.x == 0) {
+        sm[97] = 0.0;                                   // AG continuation: 0 none, 1 step from y = x, 2 extrapolate (sm[98] = beta)
         S->evals++;
         S->psi_cur = psi_t;
         double terms[5];
@@ -248,9 +369,29 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         const double lhs = 2.0 * sg * fabs(agx) + sg * sg * gg;
         const double rhs = S->rho * (ev_s[MEB_EV_SUM_DMULT2] + S->tau * dx2);
         const bool exit_inner = (phase == PH_REEVAL) || stalled || (phase == PH_ARMIJO && S->tiny) || lhs <= rhs || kkt <= S->tol ||
-                                S->inner >= S->inner_max;
+                                S->inner >= (agmode ? S->ag_inner_max : S->inner_max);
         if (exit_inner) {
             S->action = ACT_UPDATE;
+        } else if (agmode) {
+            // next accelerated-gradient iteration (reading 20)
+            S->action = ACT_TRIAL;
+            S->inner++; S->ag_total++;
+            ctrl_arm_abort(S, false, 0.0, 0.0);
+            double beta = 0.0;
+            if (phase == PH_AG_X && !(dotr > 0.0)) {        // momentum, unless the gradient restart fires
+                const double t = S->ag_t;
+                const double tn = 0.5 * (1.0 + sqrt(1.0 + 4.0 * t * t));
+                beta = (t - 1.0) / tn;
+                S->ag_t = tn;
+            } else {
+                S->ag_t = 1.0;
+                if (phase != PH_AG_X)                       // first iteration of this inner solve: ||H|| <= tau/sigma + sigma |A|
+                    S->ag_Lip = S->tau / sg + sg * fmax(1.0, ev_s[MEB_EV_N_ACTIVE]);
+            }
+            if (beta > 0.0) { sm[97] = 2.0; sm[98] = beta; S->phase = PH_AG_Y; }
+            else {                                          // y = x: this pass IS the evaluation at y
+                sm[97] = 1.0; S->ag_psi_y = psi_t; S->ag_gg_y = gg; S->ag_bt = 0; S->phase = PH_AG_X;
+            }
         } else {
             S->action = ACT_NEWTON;
             S->inner++;
@@ -261,12 +402,24 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
             S->cg_tol = fmin(0.1, gn) * gn;
             S->cg_it = 0;
             S->cg_go = (gn > S->cg_tol && S->cg_max > 0) ? 1 : 0;
+            S->cg_mode = ((long long)ev_s[MEB_EV_N_ACTIVE] <= S->wc_cap) ? 1 : 0;
         }
         if (S->evals >= S->eval_cap) { S->done = 1; S->status = ST_OUTER_CAP; }
         ctrl_set_handles(S);
     }
     __syncthreads();
-    if (S->action == ACT_NEWTON && !S->dense)
+    if (sm[97] != 0.0) {                                    // accelerated gradient: the next point to evaluate
+        const bool extrap = sm[97] == 2.0;
+        const double beta = sm[98], il = 1.0 / S->ag_Lip;
+        for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            const double xj = v.xn[j];
+            double tj;
+            if (extrap) tj = fma(beta, xj - v.Hp[j], xj);                      // y = x+ + beta (x+ - x)
+            else { const double gj = v.grad_t[j]; v.res[j] = gj; v.p[j] = xj; tj = fma(-il, gj, xj); }
+            v.xt[j] = tj;
+            v.x_raw[j] = (j == 0) ? Ls * tj : ((use_off ? v.off[j - 1] : 0.0) + Ls * tj);
+        }
+    } else if (S->action == ACT_NEWTON && !S->dense)
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
             const double gj = v.grad_t[j];
             v.delta[j] = 0.0;
@@ -282,26 +435,31 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
     const int tid = threadIdx.x;
     const double Ls = S->L;
     const bool use_off = S->use_off != 0;
-    double sl = 0.0, dx2t = 0.0;
+    __shared__ double red3[8];
+    double sl = 0.0, dx2t = 0.0, dc2 = 0.0;
     for (int j = tid; j < n; j += 256) {
         const double dj = z[j];
         sl = fma(v.g[j], dj, sl);
         const double xj = v.xn[j] + dj;
         v.xt[j] = xj;
         v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+        v.dir_raw[j] = Ls * dj;
         const double dxb = xj - v.xbar[j];
         dx2t = fma(dxb, dxb, dx2t);
+        if (j > 0) dc2 = fma(dj, dj, dc2);
     }
     sl = warp_sum(sl);
     dx2t = warp_sum(dx2t);
-    if ((tid & 31) == 0) { red[tid >> 5] = sl; red2[tid >> 5] = dx2t; }
+    dc2 = warp_sum(dc2);
+    if ((tid & 31) == 0) { red[tid >> 5] = sl; red2[tid >> 5] = dx2t; red3[tid >> 5] = dc2; }
     __syncthreads();
     if (tid == 0) {
-        double t = 0.0, t2 = 0.0;
-        for (int w = 0; w < 8; ++w) { t += red[w]; t2 += red2[w]; }
+        double t = 0.0, t2 = 0.0, t3 = 0.0;
+        for (int w = 0; w < 8; ++w) { t += red[w]; t2 += red2[w]; t3 += red3[w]; }
         ctrl_arm_abort(S, true, v.xn[0] + z[0], t2);
         S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
         S->tiny = (-t <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;
+        ctrl_arm_multi(S, 1.0, 0, Ls * z[0], Ls * Ls * t3);
     }
 }
 

@@ -16,6 +16,7 @@
 #define MEB_NPART 12
 #define MEB_PART_CUT 9     // per-CTA partial: 1 if the CTA cut its pass short (MebDyn::s0_abort)
 #define MEB_EVPOOL 4096               // streaming launches of one solve that get an event pair
+#define MEB_MULTI_MAX 4               // step sizes an Armijo trial pass can predict besides its own (meb_params.armijo_multi)
 
 struct meb_ctx {
     int device;
@@ -26,6 +27,9 @@ struct meb_ctx {
     int last_cuda_error;
     // ---- workspace (device) ----
     uint32_t* mask;         // [ceil(m/32)] active / flag bit mask of the last streaming pass
+    uint32_t* vmask;        // [ceil(m/32)] scratch: balls with a multiplier row (meb_build_vlist)
+    int32_t* vlist;         // [m] ascending list of the balls with a multiplier row, per-primitive calls (long rows)
+    double* part_multi;     // [MEB_MAX_GRID * MEB_MULTI_MAX] per-CTA partials of the predicted step sizes
     double* rec_lam;        // [m] lam_i of active balls (dense-indexed, sparse writes)
     double* rec_rho;        // [m] rho_i = a/nb (2.0 marks B1)
     double* rec_t;          // [m] t_i of active balls
@@ -46,8 +50,8 @@ struct meb_ctx {
     double* h_pinned;       // pinned host mirror for small read-backs
     int64_t h_pinned_len;
     // ---- owned copies for meb_solve / meb_solve_host ----
-    void* own[24];
-    size_t own_bytes[24];
+    void* own[40];
+    size_t own_bytes[40];
     // ---- measurement ----
     cudaEvent_t ev0, ev1;
     double last_pass_ms;
@@ -75,6 +79,8 @@ struct meb_ctx {
     int stage_next;
     bool evcut[MEB_EVPOOL];         // stepped solves: the launch was a trial pass that was cut short
     double ev_extra_bytes;          // stepped solves: bytes of the multiplier rows the next evaluation pass reads
+    int last_path;                  // kernel family of the last streaming launch (PATH_* in meb_api.cu)
+    struct MebDyn* dyn_api;         // device MebDyn of the per-primitive multi-trial call
 };
 
 // prints file:line and the CUDA error string to stderr when the context was created with MEB_DEBUG set
@@ -131,6 +137,13 @@ struct MebDyn {
     // Psi(trial) = Psi(x)) the rest of the pass cannot change the decision.  1e300: never (not a trial).
     // A CTA whose own part of the sum crosses it stops and marks its partial (slot MEB_PART_CUT).
     double s0_abort;
+    // Multi-trial Armijo (DESIGN reading 19): a trial pass at x_t = x + eta Delta also forms
+    // sum_i ||Pi(z_i)||^2 at the multi_n further points x_t - gamma_k Delta (gamma_k = eta (1 - 2^-k): the next
+    // halvings of eta) from ||b_i||^2, <b_i, Delta c> and ||Delta c||^2 -- no extra bytes.  0: not a trial pass.
+    int32_t multi_n, pad_multi;
+    double multi_gamma[MEB_MULTI_MAX];
+    double dir_r;           // Delta r (raw units)
+    double dir_c2;          // ||Delta c||^2 (raw units)
 };
 
 // host-side launch helpers implemented in the .cu files -------------------------------------------
@@ -158,6 +171,11 @@ struct StreamArgs {
     // device-resident parameters (solve graph): if dyn != nullptr it overrides sigma, U, v_slot, V
     const MebDyn* dyn;
     const void* U2[2]; const int32_t* slot2[2]; const void* V2[2];
+    // long rows (meb_long.cu): list of the balls with a multiplier row, per multiplier buffer
+    const int32_t* vlist2[2]; const int32_t* vcount2[2];
+    // multi-trial Armijo: direction Delta (device, (d+1), raw units), host-side switch (0: kernel without it),
+    // per-CTA partials [grid][MEB_MULTI_MAX]
+    const double* dir; int32_t multi; double* multi_part;
 };
 
 // resolves the device-resident parameters of a solve graph into the plain fields
@@ -180,6 +198,15 @@ int meb_launch_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* 
 // (a.part_vec), so no active-list pass is needed for the gradient.
 bool meb_tile_applicable(int op, int prec, const StreamArgs& a);
 int meb_launch_tile(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out);
+// TMA-staged warp-per-row kernels for long rows (meb_long.cu): rows longer than 1024 bytes whose start and stride
+// are multiples of 16 bytes.  The launcher zeroes a.mask, launches the streaming kernel and (evaluation with
+// multipliers) the kernel that handles the balls on vlist; *grid_out counts the partials of both.
+bool meb_long_applicable(int op, int prec, const StreamArgs& a);
+int meb_launch_long(meb_ctx* ctx, int op, int prec, const StreamArgs& a, const int32_t* vlist, const int32_t* vcount,
+                    int* grid_out);
+int meb_build_vlist(meb_ctx* ctx, const int32_t* slot, int64_t m, int32_t* vlist, int32_t* vcount);
+int meb_copy_vlist(meb_ctx* ctx, const int32_t* list, const int32_t* count, const MebDyn* dyn, int32_t* v0, int32_t* v1,
+                   int32_t* c0, int32_t* c1, int64_t cap);
 int meb_launch_compact(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* list, int32_t* count_dev);
 
 // ---- active-list passes (meb_active.cu) ----
@@ -254,6 +281,9 @@ struct SolverVecs;
 struct GraphSide {
     const MebDyn* dyn;
     void* U2[2]; int32_t* slot2[2]; void* V2[2]; int64_t vcap2[2];
+    int32_t* vlist2[2]; int32_t* vcount2[2];     // long rows: balls with a multiplier row, per multiplier buffer
+    int32_t multi;                               // > 0: evaluation kernels with the multi-trial code
+    const double* dir;                           // direction Delta (raw units) when there is no SolverVecs (meb_eval_alm_multi)
     SolverDev* S; const SolverVecs* v;
 };
 struct EvalCall {
@@ -276,6 +306,9 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
 // With S != nullptr the kernel also runs the controller step that follows a Newton solve (first Armijo trial).
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
                    int* info_dev, SolverDev* S, const SolverVecs* v);
+
+// ---- matrix-free Newton direction in one persistent kernel (meb_cg.cu) ----
+int meb_launch_cg(meb_ctx* ctx, const EvalCall& c, double* W, int64_t wc_cap, double* rho_c, unsigned int* bar);
 
 // ---- controller kernels of the device-resident solver (meb_ctrl.cu) ----
 int meb_ctrl_init(meb_ctx* ctx, SolverDev* S, const SolverVecs& v, double sigma0, int cur, int has_mult);

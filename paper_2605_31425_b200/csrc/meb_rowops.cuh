@@ -149,6 +149,61 @@ __device__ __forceinline__ void abort_store(const AbortCtl& c, double* part) {
     part[(size_t)blockIdx.x * MEB_NPART + MEB_PART_CUT] = (c.on && c.slots[32] != 0.0) ? 1.0 : 0.0;
 }
 
+// ---- multi-trial Armijo (MebDyn::multi_n) -----------------------------------------------------------------------
+// Per-lane sums of ||Pi(z_i)||^2 at the predicted points x_t - gamma_k Delta, k < multi_n.
+template <bool ON> struct MultiAcc { double s[ON ? MEB_MULTI_MAX : 1]; __device__ MultiAcc() { for (int k = 0; k < (ON ? MEB_MULTI_MAX : 1); ++k) s[k] = 0.0; } };
+
+// One row at the trial point: nb2 = ||b_i||^2, p = <b_i, Delta c>.  At x_t - gamma Delta the shifted point is
+// (a_i + gamma Delta r, b_i + gamma Delta c), so ||b||^2 = nb2 + 2 gamma p + gamma^2 ||Delta c||^2.
+template <typename T>
+__device__ __forceinline__ void multi_row(MultiAcc<true>& ma, const StreamArgs& a, int cap, T nb2, T p, T r, T sig, T ri, T ui) {
+    const int nm = a.dyn ? (a.dyn->multi_n < cap ? a.dyn->multi_n : cap) : 0;
+    if (nm <= 0) return;
+    const T av = ri - r + ui / sig;
+    const T dr = (T)a.dyn->dir_r, dc2 = (T)a.dyn->dir_c2;
+    {   // balls that stay strictly inside at every predicted point add exactly zero: ||b + g dc|| <= ||b|| + g ||dc||
+        const T gmax = (T)a.dyn->multi_gamma[nm - 1];
+        const T reach = t_sqrt<T>(nb2) + gmax * t_sqrt<T>(dc2);
+        const T amax = av + (dr > T(0) ? gmax * dr : T(0));
+        if (reach <= -amax) return;
+    }
+#pragma unroll
+    for (int k = 0; k < MEB_MULTI_MAX; ++k) {
+        if (k < nm) {
+            const T g = (T)a.dyn->multi_gamma[k];
+            T nk2 = fma(g, fma(g, dc2, T(2) * p), nb2);
+            if (nk2 < T(0)) nk2 = T(0);
+            const T nk = t_sqrt<T>(nk2);
+            const T ak = fma(g, dr, av);
+            T pr2;
+            if (nk <= ak) pr2 = ak * ak + nk2;                      // P:L115, printed order
+            else if (nk <= -ak) pr2 = T(0);
+            else { const T s2 = ak + nk; pr2 = T(0.5) * s2 * s2; }    // 2 ((a + nb)/2)^2
+            ma.s[k] += (double)pr2;
+        }
+    }
+}
+template <typename T>
+__device__ __forceinline__ void multi_row(MultiAcc<false>&, const StreamArgs&, int, T, T, T, T, T, T) {}
+
+// per-CTA partials of the predictions: lanes (xor tree), then warps in index order
+__device__ __forceinline__ void multi_store(MultiAcc<true>& ma, const StreamArgs& a, int nwarps) {
+    __shared__ double mred[16][MEB_MULTI_MAX];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < MEB_MULTI_MAX; ++k) {
+        const double v = warp_sum(ma.s[k]);
+        if (lane == 0 && warp < 16) mred[warp][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < MEB_MULTI_MAX && a.multi_part) {
+        double t = 0.0;
+        for (int w = 0; w < nwarps; ++w) t += mred[w][threadIdx.x];
+        a.multi_part[(size_t)blockIdx.x * MEB_MULTI_MAX + threadIdx.x] = t;
+    }
+}
+__device__ __forceinline__ void multi_store(MultiAcc<false>&, const StreamArgs&, int) {}
+
 // Same, loading r_i and u_i of the row from global memory.
 template <typename T, int OP>
 __device__ __forceinline__ bool row_epilogue(const StreamArgs& a, int64_t row, bool valid, bool hasv,

@@ -9,14 +9,14 @@ namespace {
 constexpr int FBLOCK = 1024;
 
 // scalar k of the CTA partials: lanes stride over the CTAs, xor tree (warp k handles scalar k)
-__device__ __forceinline__ double partial_sum(const double* part, int grid, int k, int lane) {
+__device__ __forceinline__ double partial_sum(const double* part, int grid, int k, int lane, int stride = MEB_NPART) {
     double s = 0.0;
-    for (int b = lane; b < grid; b += 32) s += part[(size_t)b * MEB_NPART + k];
+    for (int b = lane; b < grid; b += 32) s += part[(size_t)b * stride + k];
     return warp_sum(s);
 }
-__device__ __forceinline__ double partial_max(const double* part, int grid, int k, int lane) {
+__device__ __forceinline__ double partial_max(const double* part, int grid, int k, int lane, int stride = MEB_NPART) {
     double s = 0.0;
-    for (int b = lane; b < grid; b += 32) s = fmax(s, part[(size_t)b * MEB_NPART + k]);
+    for (int b = lane; b < grid; b += 32) s = fmax(s, part[(size_t)b * stride + k]);
     return warp_max(s);
 }
 
@@ -29,6 +29,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
     __shared__ double ev_s[MEB_EVAL_NSCALARS];
     __shared__ double sc[MEB_NPART];
     __shared__ double seg[FBLOCK];
+    __shared__ double multi_s[MEB_MULTI_MAX];
     __shared__ __align__(16) SolverDev sS;             // working copy of the solver state (controller step)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (f.S) {
@@ -38,24 +39,34 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
     }                                                   // (visible after the first __syncthreads below)
     const double* __restrict__ part = f.part;
     const double* __restrict__ part_vec = f.part_vec;
-    const int grid = f.grid, d = f.d, dpad = f.dpad;
+    const int grid = f.grid, d = f.d;
+    const int dpad = f.vec_stride > 0 ? f.vec_stride : f.dpad;           // stride between the vector partials
+    const int pstr = f.part_stride > 0 ? f.part_stride : MEB_NPART;
+    const int mstr = f.multi_stride > 0 ? f.multi_stride : MEB_MULTI_MAX;
     double sigma = f.sigma, tau = f.tau;
     if (f.dyn) { sigma = f.dyn->sigma_raw; tau = f.dyn->tau_eff; }
     const double* x = f.x; const double* xbar = f.xbar;
     if (warp < 9) {
         double v;
-        if (warp >= 5 && warp <= 7) v = partial_max(part, grid, warp, lane);
-        else v = partial_sum(part, grid, warp, lane);
+        if (warp >= 5 && warp <= 7) v = partial_max(part, grid, warp, lane, pstr);
+        else v = partial_sum(part, grid, warp, lane, pstr);
         if (lane == 0) sc[warp] = v;
     } else if (warp == 10) {
-        const double v = partial_max(part, grid, MEB_PART_CUT, lane);
+        const double v = partial_max(part, grid, MEB_PART_CUT, lane, pstr);
         if (lane == 0) sc[MEB_PART_CUT] = v;
+    } else if (warp >= 11 && warp < 11 + MEB_MULTI_MAX && f.S && f.multi_part) {
+        // predicted step sizes of a trial pass (multi-trial Armijo): CTA partials in index order
+        const int k = warp - 11;
+        double t = 0.0;
+        for (int b = lane; b < grid; b += 32) t += f.multi_part[(size_t)b * mstr + k];
+        t = warp_sum(t);
+        if (lane == 0) multi_s[k] = t;
     } else if (warp == 9 && f.S) {
         // device time of the pass: last CTA end - first CTA start (globaltimer stamps of the tile kernel)
         long long t0 = 0x7fffffffffffffffLL, t1 = 0;
         for (int b = lane; b < grid; b += 32) {
-            const long long s0 = __double_as_longlong(part[(size_t)b * MEB_NPART + 10]);
-            const long long s1 = __double_as_longlong(part[(size_t)b * MEB_NPART + 11]);
+            const long long s0 = __double_as_longlong(part[(size_t)b * pstr + 10]);
+            const long long s1 = __double_as_longlong(part[(size_t)b * pstr + 11]);
             if (s1 > 0) { t0 = min(t0, s0); t1 = max(t1, s1); }
         }
 #pragma unroll
@@ -108,6 +119,12 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
     if (threadIdx.x == 0) {
         const bool cut = f.S && sc[MEB_PART_CUT] != 0.0;       // a CTA stopped early: certainly rejected (MebDyn::s0_abort)
         if (cut) sS.aborted++;
+        if (f.S) {
+            int np = f.multi_part ? sS.dyn.multi_n : 0;
+            if (np > MEB_MULTI_MAX) np = MEB_MULTI_MAX;
+            sS.pred_n = np;
+            for (int k = 0; k < np; ++k) sS.pred_s[k] = multi_s[k];
+        }
         if (f.S) {
             const long long t0 = __double_as_longlong(sm[100]), t1 = __double_as_longlong(sm[101]);
             if (t1 > t0) {

@@ -24,7 +24,7 @@ namespace {
 // slots of meb_ctx::own (20 = the batch solver's block, meb_smallsolve.cu)
 enum { OWN_U0 = 0, OWN_U1, OWN_S0, OWN_S1, OWN_V0, OWN_V1, OWN_C32, OWN_R32, OWN_IDX, OWN_CRED, OWN_RRED,
        OWN_KEPT, OWN_STATE, OWN_UREDA, OWN_UREDB, OWN_SREDA, OWN_VRED0, OWN_VRED1, OWN_DEVC, OWN_DEVR,
-       OWN_BATCH_RESERVED, OWN_SREDB, OWN_WC };
+       OWN_BATCH_RESERVED, OWN_SREDB, OWN_WC, OWN_VL0, OWN_VL1, OWN_VLRED0, OWN_VLRED1 };
 
 int own_reserve(meb_ctx* ctx, int slot, size_t bytes) {
     if (ctx->own_bytes[slot] >= bytes && ctx->own[slot]) return MEB_OK;
@@ -60,6 +60,7 @@ struct Problem {                   // one ripALM run: data + double-buffered mul
     const void* C; int64_t ld; const void* R;
     void* U[2]; int32_t* slot[2]; void* V[2]; int64_t ldv; int64_t vcap[2];
     int own_v[2];                  // own[] slots holding the V pools (-1: fixed capacity)
+    int32_t* vlist[2]; int32_t* vcount[2];   // long rows: ascending list of the balls with a multiplier row, per buffer
     int cur; bool has_mult;
     const double* off;             // host: raw offset of the centre (c0 for raw data, nullptr for the centred shadow)
     bool full;                     // streams all m rows (for the pass statistics)
@@ -71,6 +72,9 @@ struct Solver {
     double sigma_end;              // sigma reached by the last phase
     int32_t d; double L;
     double* dH;                    // device (d+1)^2: dense Newton system
+    double* dW; int64_t wc_cap;    // device [wc_cap][dpad] gathered active rows of the matrix-free Newton solve, then
+    double* rho_c;                 //   [wc_cap] their rho, then the grid barrier's two counters
+    unsigned int* cg_bar;
     SolverVecs v;                  // device (d+1)-vectors of the controller
     double bytes;
 };
@@ -109,10 +113,12 @@ struct GraphKey {
     int prec, dense; int64_t m; int32_t d; const void* C; int64_t ld; const void* R;
     void* U[2]; int32_t* slot[2]; void* V[2]; int64_t ldv; int64_t vcap[2];
     const double* dH; const double* xn;
+    const int32_t* vlist[2]; int multi, ag;
+    const double* dW; int64_t wc_cap;
 };
 struct SolveGraph {
     bool used; GraphKey key; cudaGraph_t g; cudaGraphExec_t ex;
-    cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
+    cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg, h_cgp;
     int k_eval, k_newton, k_cg, k_update;      // kernels launched per evaluation / Newton solve / CG step / update
     double bytes_per_eval; uint64_t stamp;
 };
@@ -171,7 +177,11 @@ void seq_init(Seq& q, Solver& S, const Problem& P, bool dense) {
     q.dev = (SolverDev*)ctx->sdev;
     memset(&q.gs, 0, sizeof(q.gs));
     q.gs.dyn = &q.dev->dyn; q.gs.S = q.dev; q.gs.v = &S.v;
-    for (int b = 0; b < 2; ++b) { q.gs.U2[b] = P.U[b]; q.gs.slot2[b] = P.slot[b]; q.gs.V2[b] = P.V[b]; q.gs.vcap2[b] = P.vcap[b]; }
+    for (int b = 0; b < 2; ++b) {
+        q.gs.U2[b] = P.U[b]; q.gs.slot2[b] = P.slot[b]; q.gs.V2[b] = P.V[b]; q.gs.vcap2[b] = P.vcap[b];
+        q.gs.vlist2[b] = P.vlist[b]; q.gs.vcount2[b] = P.vcount[b];
+    }
+    q.gs.multi = S.par.armijo_multi > 0 ? (S.par.armijo_multi < MEB_MULTI_MAX ? S.par.armijo_multi : MEB_MULTI_MAX) : 0;
     memset(&q.c, 0, sizeof(q.c));
     q.c.prec = P.prec; q.c.m = P.m; q.c.d = P.d; q.c.C = P.C; q.c.ld = P.ld; q.c.R = P.R; q.c.ldv = P.ldv;
     q.c.x = S.v.x_raw; q.c.xbar = S.v.xbar_raw; q.c.sigma = 1.0; q.c.tau = 1.0; q.c.gs = &q.gs;
@@ -192,6 +202,10 @@ int seq_newton_dense(Seq& q) {
     rc = meb_dense_from_records(ctx, q.c, q.S->v.ev, q.S->dH);
     if (rc) return rc;
     return meb_chol_solve(ctx, q.S->dH, q.S->v.g, q.S->d + 1, q.S->L, q.S->v.delta, &q.dev->chol_info, q.dev, &q.S->v);
+}
+// the whole CG solve in one persistent kernel (at most wc_cap active rows)
+int seq_cg_persistent(Seq& q) {
+    return meb_launch_cg(q.S->ctx, q.c, q.S->dW, q.S->wc_cap, q.S->rho_c, q.S->cg_bar);
 }
 // one CG iteration of the matrix-free path: Hp = H p over the active rows, CG step
 int seq_cg_body(Seq& q) {
@@ -219,6 +233,10 @@ int seq_update(Seq& q) {
     int nvec = 0;
     rc = meb_launch_active(ctx, MODE_WRITEV, P.prec, a, &nvec);
     if (rc) return rc;
+    if (P.vlist[0]) {                 // long rows: the balls that just got a multiplier row, for the next evaluations
+        rc = meb_copy_vlist(ctx, ctx->list, ctx->count_dev, q.gs.dyn, P.vlist[0], P.vlist[1], P.vcount[0], P.vcount[1], P.m);
+        if (rc) return rc;
+    }
     return meb_ctrl_after_update(ctx, q.dev, q.S->v, ctx->count_dev);
 }
 
@@ -229,8 +247,8 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     meb_ctx* ctx = S.ctx;
     int rc = MEB_OK;
     bool capturing = false;
-    cudaGraph_t tmp = nullptr, body = nullptr, bn = nullptr, bu = nullptr, bcg = nullptr;
-    cudaGraphNode_t wnode, nnode, unode, cgnode;
+    cudaGraph_t tmp = nullptr, body = nullptr, bn = nullptr, bu = nullptr, bcg = nullptr, bcgp = nullptr;
+    cudaGraphNode_t wnode, nnode, unode, cgnode, cgpnode;
     Seq q;
     seq_init(q, S, P, dense);
     bool list_after_eval = false;
@@ -243,6 +261,7 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
     CU(cudaGraphConditionalHandleCreate(&G->h_newton, G->g, 0, cudaGraphCondAssignDefault));
     CU(cudaGraphConditionalHandleCreate(&G->h_update, G->g, 0, cudaGraphCondAssignDefault));
     if (!dense) CU(cudaGraphConditionalHandleCreate(&G->h_cg, G->g, 0, cudaGraphCondAssignDefault));
+    if (!dense) CU(cudaGraphConditionalHandleCreate(&G->h_cgp, G->g, 0, cudaGraphCondAssignDefault));
     {
         cudaGraphNodeParams p = {};
         p.type = cudaGraphNodeTypeConditional;
@@ -274,12 +293,23 @@ int build_graph(Solver& S, const Problem& P, bool dense, SolveGraph* G) {
         G->k_cg = 0;
     } else {
         RC(meb_ensure_list(ctx, P.m));
+        RC(add_conditional(ctx, bn, G->h_cgp, false, &cgpnode, &bcgp));
         RC(add_conditional(ctx, bn, G->h_cg, true, &cgnode, &bcg));
         RC(meb_ctrl_after_newton(ctx, q.dev, S.v));
     }
     G->k_newton = (int)(ctx->launches - l0);
     CU(cudaStreamEndCapture(ctx->stream, &tmp));
     capturing = false;
+    if (!dense) {
+        CU(cudaStreamBeginCaptureToGraph(ctx->stream, bcgp, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+        capturing = true;
+        l0 = ctx->launches;
+        ctx->list_valid = true;
+        RC(seq_cg_persistent(q));
+        G->k_newton += (int)(ctx->launches - l0);          // (counted with every Newton step; the legacy loop is rare)
+        CU(cudaStreamEndCapture(ctx->stream, &tmp));
+        capturing = false;
+    }
     if (!dense) {
         CU(cudaStreamBeginCaptureToGraph(ctx->stream, bcg, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
         capturing = true;
@@ -362,6 +392,11 @@ int run_stepped(Solver& S, const Problem& P, bool dense, SolverDev* h) {
                 rc = meb_ensure_list(ctx, P.m);
                 if (rc) return rc;
                 int go = h->cg_go;
+                if (go && h->cg_mode == 1) {
+                    rc = seq_cg_persistent(q);
+                    if (rc) return rc;
+                    go = 0;
+                }
                 while (go) {
                     rc = seq_cg_body(q);
                     if (rc) return rc;
@@ -398,6 +433,9 @@ GraphKey make_key(const Solver& S, const Problem& P, bool dense) {
     k.prec = P.prec; k.dense = dense ? 1 : 0; k.m = P.m; k.d = P.d; k.C = P.C; k.ld = P.ld; k.R = P.R;
     for (int b = 0; b < 2; ++b) { k.U[b] = P.U[b]; k.slot[b] = P.slot[b]; k.V[b] = P.V[b]; k.vcap[b] = P.vcap[b]; }
     k.ldv = P.ldv; k.dH = S.dH; k.xn = S.v.xn;
+    k.vlist[0] = P.vlist[0]; k.vlist[1] = P.vlist[1];
+    k.multi = S.par.armijo_multi; k.ag = S.par.ag_outer;
+    k.dW = S.dW; k.wc_cap = S.wc_cap;
     return k;
 }
 
@@ -499,6 +537,10 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             }
             h->slope_floor = (P.prec == MEB_FP32) ? 1e-7 : 2e-15;
             h->abort_margin = ctx->opt[MEB_OPT_NO_ABORT] ? 0.0 : ((P.prec == MEB_FP32) ? 1e-3 : 1e-6);
+            h->pred_margin = (P.prec == MEB_FP32) ? 1e-3 : 1e-6;
+            h->multi_max = (par.armijo_multi > 0 && !small) ? (par.armijo_multi < MEB_MULTI_MAX ? par.armijo_multi : MEB_MULTI_MAX) : 0;
+            h->ag_outer = (par.ag_outer > 0 && !small) ? par.ag_outer : 0;
+            h->ag_inner_max = 500;
             h->stall_max = (P.prec == MEB_FP32) ? 3 : 6;   // the FP32 run only has to deliver a warm start
 #ifdef MEB_TUNING
             if (getenv("MEB_SHRINK_MIN")) h->shrink_min = atof(getenv("MEB_SHRINK_MIN"));
@@ -509,6 +551,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
         h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
+        h->h_cgp = G->h_cgp; h->wc_cap = S.wc_cap;
         h->in_graph = (stepped || small) ? 0 : 1;
         if (first) {
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
@@ -516,7 +559,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         } else {                                                        // resume: constants that may have changed
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(&dev->vcap[0], &h->vcap[0], 2 * sizeof(int64_t),
                                              cudaMemcpyHostToDevice, ctx->stream));
-            MEB_CUDA_OK(ctx, cudaMemcpyAsync(&dev->h_while, &h->h_while, 4 * sizeof(cudaGraphConditionalHandle),
+            MEB_CUDA_OK(ctx, cudaMemcpyAsync(&dev->h_while, &h->h_while, 5 * sizeof(cudaGraphConditionalHandle),
                                              cudaMemcpyHostToDevice, ctx->stream));
             rc = meb_ctrl_resume(ctx, dev);
         }
@@ -566,6 +609,8 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         const double vbytes = (double)h->vrow_reads * (double)S.d * (double)esz(P.prec);   // V rows of balls with u_i > 0
         S.bytes += (double)(h->evals - h->aborted) * G->bytes_per_eval + vbytes;
         S.st->passes_cut += h->aborted;
+        S.st->trials_skipped += h->skipped;
+        S.st->ag_iters += h->ag_total;
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
         S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval + vbytes;
         S.st->pass_count[cls] += (int32_t)h->pass_count;
@@ -590,7 +635,19 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
     return MEB_E_CAPACITY;
 }
 
+bool long_rows(const Problem& P) { return (size_t)P.ld * esz(P.prec) > 1024 || P.d > 256; }
+
 int setup_multipliers(meb_ctx* ctx, Problem& P, int ownU0, int ownS0, int ownV0) {
+    for (int b = 0; b < 2; ++b) {
+        P.vlist[b] = nullptr; P.vcount[b] = nullptr;
+        if (long_rows(P) && ctx->vlist) {
+            int rcv = own_reserve(ctx, OWN_VL0 + b, ((size_t)P.m + 32) * sizeof(int32_t));
+            if (rcv) return rcv;
+            P.vlist[b] = (int32_t*)ctx->own[OWN_VL0 + b];
+            P.vcount[b] = ctx->count_dev + 2 + b;
+        }
+    }
+    if (P.vcount[0]) { cudaError_t e = cudaMemsetAsync(ctx->count_dev + 2, 0, 2 * sizeof(int32_t), ctx->stream); if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; } }
     for (int b = 0; b < 2; ++b) {
         int rc = own_reserve(ctx, ownU0 + b, (size_t)P.m * esz(P.prec));
         if (rc) return rc;
@@ -616,7 +673,7 @@ struct SolveScope {
 
 // buffers of the reduced problem: rows, radii, double-buffered multipliers with a dense V (slot k = k)
 struct Reduced {
-    int64_t cap; int64_t ldr; int32_t d; bool radii;
+    int64_t cap; int64_t ldr; int32_t d; bool radii; bool longrows;
 };
 int reduced_reserve(meb_ctx* ctx, Reduced& Q, int64_t cap, int64_t keep_rows) {
     const size_t row = (size_t)Q.ldr * sizeof(double);
@@ -628,6 +685,8 @@ int reduced_reserve(meb_ctx* ctx, Reduced& Q, int64_t cap, int64_t keep_rows) {
     if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_SREDB, (size_t)cap * sizeof(int32_t), (size_t)keep_rows * sizeof(int32_t));
     if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_VRED0, (size_t)cap * row, (size_t)keep_rows * row);
     if (rc == MEB_OK) rc = own_grow_keep(ctx, OWN_VRED1, (size_t)cap * row, (size_t)keep_rows * row);
+    if (rc == MEB_OK && Q.longrows) rc = own_grow_keep(ctx, OWN_VLRED0, ((size_t)cap + 32) * sizeof(int32_t), (size_t)keep_rows * sizeof(int32_t));
+    if (rc == MEB_OK && Q.longrows) rc = own_grow_keep(ctx, OWN_VLRED1, ((size_t)cap + 32) * sizeof(int32_t), (size_t)keep_rows * sizeof(int32_t));
     if (rc == MEB_OK) Q.cap = cap;
     return rc;
 }
@@ -638,6 +697,10 @@ void reduced_bind(meb_ctx* ctx, const Reduced& Q, Problem& P2) {
     P2.V[0] = ctx->own[OWN_VRED0]; P2.V[1] = ctx->own[OWN_VRED1];
     P2.vcap[0] = P2.vcap[1] = Q.cap;
     P2.own_v[0] = P2.own_v[1] = -1;
+    for (int b = 0; b < 2; ++b) {
+        P2.vlist[b] = Q.longrows ? (int32_t*)ctx->own[OWN_VLRED0 + b] : nullptr;
+        P2.vcount[b] = Q.longrows ? ctx->count_dev + 4 + b : nullptr;
+    }
 }
 
 }  // namespace
@@ -678,16 +741,30 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
         // ---- state vectors on the device ----
         const size_t nH = (d <= 128) ? (size_t)n * n + 8 : 8;
         const size_t nv = ((size_t)n + 7) / 8 * 8;
-        rc = own_reserve(ctx, OWN_STATE, (15 * nv + 2 * MEB_EVAL_NSCALARS + nH) * sizeof(double));
+        rc = own_reserve(ctx, OWN_STATE, (17 * nv + 2 * MEB_EVAL_NSCALARS + nH) * sizeof(double));
         if (rc) break;
         double* base = (double*)ctx->own[OWN_STATE];
         double** vecs[] = {&S.v.xn, &S.v.xbar, &S.v.ab, &S.v.delta, &S.v.g, &S.v.xt, &S.v.x_raw, &S.v.xbar_raw,
-                           &S.v.off, &S.v.grad_t, &S.v.res, &S.v.p, &S.v.Hp, &S.v.xbest};
-        for (size_t i = 0; i < 14; ++i) *vecs[i] = base + i * nv;
-        double* dc0 = base + 14 * nv;
-        S.v.ev_t = base + 15 * nv;
+                           &S.v.off, &S.v.grad_t, &S.v.res, &S.v.p, &S.v.Hp, &S.v.xbest, &S.v.dir_raw};
+        for (size_t i = 0; i < 15; ++i) *vecs[i] = base + i * nv;
+        double* dc0 = base + 15 * nv;
+        S.v.ev_t = base + 17 * nv;
         S.v.ev = S.v.ev_t + MEB_EVAL_NSCALARS;
         S.dH = S.v.ev + MEB_EVAL_NSCALARS;
+        S.dW = nullptr; S.wc_cap = 0; S.rho_c = nullptr; S.cg_bar = nullptr;
+        if (d > 128 || d > S.par.dense_d_max) {
+            // matrix-free Newton path: room for the gathered active rows (up to 256 MB, L2-sized in practice)
+            const size_t dpadw = ((size_t)d + 7) / 8 * 8;
+            int64_t cap = (int64_t)(((size_t)256 << 20) / (dpadw * sizeof(double)));
+            if (cap > m) cap = m;
+            if (cap < 1) cap = 1;
+            rc = own_reserve(ctx, OWN_WC, (size_t)cap * (dpadw + 1) * sizeof(double) + 64);
+            if (rc) break;
+            S.dW = (double*)ctx->own[OWN_WC];
+            S.rho_c = S.dW + (size_t)cap * dpadw;
+            S.cg_bar = (unsigned int*)(S.rho_c + cap);
+            S.wc_cap = cap;
+        }
         // ---- a0: ingest (initial point, validation, FP32 shadow) ----
         float* C32 = nullptr; float* R32 = nullptr;
         const int64_t ld32 = ((int64_t)d + 3) / 4 * 4;
@@ -802,6 +879,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             // ---- reduced problem: gather rows and multipliers ----
             Reduced Q;
             Q.cap = 0; Q.ldr = (d + 1) / 2 * 2; Q.d = d; Q.radii = radii != nullptr;
+            Q.longrows = ((size_t)Q.ldr * 8 > 1024 || d > 256) && ctx->vlist != nullptr;
             {
                 int64_t cap_red = 2 * nred + 1024;           // room for re-introduced balls; grows on demand
                 if (cap_red > m) cap_red = m;
@@ -822,11 +900,14 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             P2.cur = 0; P2.has_mult = true;
             // warm start restricted to I_red.  If the low-precision run did not reach its
             // tolerance (degenerate supports: reading 17) its multipliers are noise: start from zero.
-            if (P1.has_mult && conv1)
+            if (Q.longrows) CUB(cudaMemsetAsync(ctx->count_dev + 4, 0, 2 * sizeof(int32_t), ctx->stream));
+            if (P1.has_mult && conv1) {
                 rc = meb_gather_mult(ctx, (const float*)P1.U[P1.cur], P1.slot[P1.cur], (const float*)P1.V[P1.cur],
                                      P1.ldv, idx, nred, d, (double*)P2.U[0], P2.slot[0], (double*)P2.V[0], ldr);
-            else
+                if (rc == MEB_OK && P2.vlist[0]) rc = meb_build_vlist(ctx, P2.slot[0], nred, P2.vlist[0], P2.vcount[0]);
+            } else {
                 P2.has_mult = false;
+            }
             if (rc) break;
             ab = xn;                                        // reading 11
             for (int rnd = 0; rc == MEB_OK && rnd < S.par.max_rounds; ++rnd) {

@@ -19,6 +19,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <type_traits>
+
 #include "meb_internal.cuh"
 #include "meb_rowops.cuh"
 
@@ -74,6 +76,8 @@ struct TileCfg {
     int sc_tma;            // 1: per-row scalars come with the stage (their arrays are 16-byte aligned)
     int lognchp;           // gradient part: 2^lognchp = lanes that cover one row (>= nch, at most 32); the warp
                            // walks 32 >> lognchp active rows at a time
+    uint32_t off_dir;      // byte offset of the direction Delta c (multi-trial Armijo), same layout as the centre
+    int multi;             // predictions the kernel may be asked for (0: instance without the multi-trial code)
     uint32_t off_tiles;    // byte offsets inside the dynamic shared memory
     uint32_t off_bars;
     uint32_t off_vec;
@@ -86,7 +90,7 @@ struct TileCfg {
 // MAXT = threads per CTA the instance may be launched with: stages of 8 KB and more leave room for at most 12
 // warps, and those launches use the 384-thread instance, which may keep 168 registers per thread (the 512-thread
 // one is held to 128 and rematerialises addresses inside the per-row loops).
-template <typename T, int OP, int G, int CH, bool SHADOW, int MAXT>
+template <typename T, int OP, int G, int CH, bool SHADOW, int MAXT, bool MULTI>
 __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const TileCfg cfg) {
     typedef typename Chunk<T>::type V4;
     constexpr int VEC = Chunk<T>::N;
@@ -126,6 +130,15 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
     if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_start));
     const double* cptr = (OP == OP_INGEST) ? a.c0 : a.x + 1;
     for (int j = threadIdx.x; j < nch * VEC; j += blockDim.x) cs[j] = j < d ? (T)cptr[j] : T(0);
+    // multi-trial Armijo: this pass also predicts Psi at further points along Delta (MebDyn::multi_n), which
+    // needs <b_i, Delta c> per row: Delta c sits in shared memory next to the centre
+    const bool domulti = MULTI && a.dyn != nullptr && a.dyn->multi_n > 0;
+    const int doff4 = (int)(cfg.off_dir / 16);                          // Delta c chunk = centre chunk + doff4
+    if (MULTI) {
+        T* dsm = reinterpret_cast<T*>(smem + cfg.off_dir);
+        for (int j = threadIdx.x; j < nch * VEC; j += blockDim.x) dsm[j] = (domulti && j < d) ? (T)a.dir[1 + j] : T(0);
+    }
+    MultiAcc<MULTI> macc;
     if (lane == 0) {
         for (int s = 0; s < NS; ++s) mbar_init(&bars[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -231,7 +244,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                     if (HASU) ui = Ug[myrow];
                 }
             }
-            T nb2 = T(0), ne2 = T(0), evd = T(0), vv = T(0);
+            T nb2 = T(0), ne2 = T(0), evd = T(0), vv = T(0), pdot = T(0);
             if (haspad) {                                                // zero the padding of the last chunk
                 if (myvalid && g == 0)
                     for (int j = d; j < nch * VEC; ++j) rowp[j] = T(0);
@@ -242,8 +255,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                     T s0 = T(0), s1 = T(0), f0 = T(0);
                     const V4* rp = reinterpret_cast<const V4*>(rowp) + g;
                     const V4* cp = cs4 + g;
-                    uint64_t s01 = 0ull;                                 // FP32: (s0, s1) as one packed pair
-                    auto chunk = [&](const V4* rq, const V4* cq) {
+                    uint64_t s01 = 0ull, p01 = 0ull;                     // FP32: (s0, s1) and the two halves of pdot, packed pairs
+                    T pp = T(0);
+                    auto chunk = [&](auto pm, const V4* rq, const V4* cq) {
+                        constexpr bool PM = decltype(pm)::value;
                         const V4 ev4 = *rq;
                         const V4 cv4 = *cq;
                         if constexpr (sizeof(T) == 4 && OP != OP_INGEST) {
@@ -256,37 +271,55 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                             asm("sub.f32x2 %0, %1, %2;" : "=l"(d1) : "l"(e2[1]), "l"(c2[1]));
                             asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(s01) : "l"(d0));
                             asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(s01) : "l"(d1));
+                            if constexpr (PM) {
+                                const V4 dv4 = *(cq + doff4);
+                                const uint64_t* q2 = reinterpret_cast<const uint64_t*>(&dv4);
+                                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p01) : "l"(d0), "l"(q2[0]));
+                                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(p01) : "l"(d1), "l"(q2[1]));
+                            }
                             return;
                         }
                         const T* e = reinterpret_cast<const T*>(&ev4);
                         const T* cc = reinterpret_cast<const T*>(&cv4);
+                        V4 dv4 = V4();
+                        if constexpr (PM) dv4 = *(cq + doff4);
+                        const T* dd = reinterpret_cast<const T*>(&dv4);
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) {
                             const T ee = e[j] - cc[j];
                             if (j & 1) s1 = fma(ee, ee, s1); else s0 = fma(ee, ee, s0);
                             if (OP == OP_INGEST) f0 = fma(e[j], T(0), f0);   // NaN iff a non-finite entry
+                            if constexpr (PM) pp = fma(ee, dd[j], pp);
                         }
                     };
-                    if (!cfg.rot) {                                      // my chunks g, g + G, ... in order
-                        const V4* rq = rp;
-                        const V4* cq = cp;
-                        int c = 0;
-                        for (; c + 4 <= n_g; c += 4, rq += 4 * G, cq += 4 * G) {
-                            chunk(rq, cq); chunk(rq + G, cq + G); chunk(rq + 2 * G, cq + 2 * G); chunk(rq + 3 * G, cq + 3 * G);
+                    auto walk = [&](auto pm) {
+                        if (!cfg.rot) {                                  // my chunks g, g + G, ... in order
+                            const V4* rq = rp;
+                            const V4* cq = cp;
+                            int c = 0;
+                            for (; c + 4 <= n_g; c += 4, rq += 4 * G, cq += 4 * G) {
+                                chunk(pm, rq, cq); chunk(pm, rq + G, cq + G); chunk(pm, rq + 2 * G, cq + 2 * G); chunk(pm, rq + 3 * G, cq + 3 * G);
+                            }
+                            for (; c < n_g; ++c, rq += G, cq += G) chunk(pm, rq, cq);
+                        } else {                                         // same trip count, start rotated by the row index
+                            int ci = start;
+                            for (int c = 0; c < n_g; ++c) {
+                                chunk(pm, rp + ci * G, cp + ci * G);
+                                ci = (ci + 1 == n_g) ? 0 : ci + 1;
+                            }
                         }
-                        for (; c < n_g; ++c, rq += G, cq += G) chunk(rq, cq);
-                    } else {                                             // same trip count, start rotated by the row index
-                        int ci = start;
-                        for (int c = 0; c < n_g; ++c) {
-                            chunk(rp + ci * G, cp + ci * G);
-                            ci = (ci + 1 == n_g) ? 0 : ci + 1;
-                        }
-                    }
+                    };
+                    if (MULTI && domulti) walk(std::true_type{}); else walk(std::false_type{});
                     if constexpr (sizeof(T) == 4 && OP != OP_INGEST) {
                         float p0, p1;
                         asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(s01));
                         s0 = (T)p0; s1 = (T)p1;
+                        if (MULTI) {
+                            asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(p01));
+                            pp = (T)p0 + (T)p1;
+                        }
                     }
+                    pdot = pp;
                     nb2 = s0 + s1;
                     if (OP == OP_INGEST) ne2 = f0;
                 } else {                                                 // row with a multiplier v_i
@@ -328,6 +361,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                                     const T ee = e[j] - cc[j];                   // padding of the row was zeroed above
                                     const T v = (col + j < d) ? vq[j] : T(0);    // padding of the pool row is not
                                     const T bq = fma(v, inv_sig, ee);
+                                    if (MULTI && domulti) pdot = fma(bq, reinterpret_cast<const T*>(cs4 + doff4)[col + j], pdot);
                                     nb2 = fma(bq, bq, nb2);
                                     ne2 = fma(ee, ee, ne2);
                                     evd = fma(ee, v, evd);
@@ -342,6 +376,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
             for (int o = G >> 1; o > 0; o >>= 1) {                       // combine the G lanes of a row
                 const int ox = o << xsh;
                 nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, ox);
+                if (MULTI && domulti) pdot += __shfl_xor_sync(MEB_FULL_MASK, pdot, ox);
                 if (HASV || OP == OP_INGEST) ne2 += __shfl_xor_sync(MEB_FULL_MASK, ne2, ox);
                 if (HASV) {
                     evd += __shfl_xor_sync(MEB_FULL_MASK, evd, ox);
@@ -351,6 +386,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
             double mylam;
             const bool flag = row_epilogue_core<T, OP>(a, myrow, myvalid && g == 0, myslot >= 0, nb2, ne2, evd, vv,
                                                        r, sig, ri, ui, acc, mylam);
+            if (MULTI && domulti && myvalid && g == 0) multi_row<T>(macc, a, cfg.multi, nb2, pdot, r, sig, ri, ui);
             if (OP != OP_INGEST) {
                 uint32_t bits = __ballot_sync(MEB_FULL_MASK, flag);      // bit of the g = 0 lane of row rl
                 if (G == 1) {
@@ -591,6 +627,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
             pv[j] = sacc;
         }
     }
+    if (MULTI) multi_store(macc, a, W);
     block_reduce_store<OP>(acc, a.part, W);
     if (threadIdx.x == 0) {                 // device time stamps of this CTA (ns), read by the finalize kernel
         long long t_end;
@@ -669,7 +706,10 @@ bool make_cfg(const StreamArgs& a, size_t esize, int cpl, int grid, TileCfg* out
     c.sc_tma = 1;
     const void* ptrs[] = {a.U, a.R, a.v_slot, a.U2[0], a.U2[1], a.slot2[0], a.slot2[1]};
     for (const void* q : ptrs) if (q && !aligned16(q)) c.sc_tma = 0;
-    const size_t cs_bytes = ((size_t)c.nch * 16 + 127) / 128 * 128;
+    const size_t cs1 = ((size_t)c.nch * 16 + 127) / 128 * 128;
+    c.multi = a.multi > 0 ? a.multi : 0;
+    c.off_dir = (uint32_t)cs1;
+    const size_t cs_bytes = cs1 * (c.multi > 0 ? 2 : 1);               // centre, then Delta c for the multi-trial instances
     int W = 16, NS = 0;
     int want_ns = 2;
 #ifdef MEB_TUNING                     // tuning knobs of experimental builds (build.sh -DMEB_TUNING); clamped
@@ -733,16 +773,16 @@ int lanes_per_row(const StreamArgs& a, size_t esize) {
 }
 
 // G is fixed by the row length; CH = 2 only occurs with G = 4 (rows longer than 512 bytes)
-template <typename T, int OP, bool SHADOW>
+template <typename T, int OP, bool SHADOW, bool MULTI>
 int launch_g(meb_ctx* ctx, const StreamArgs& a, bool want_ch, int* grid_out) {
     const int nch = (int)(((size_t)a.d * sizeof(T) + 15) / 16);        // <= 64 (rows of at most 1024 bytes)
     constexpr int VEC = 16 / sizeof(T);
     const int G = lanes_per_row(a, sizeof(T));
-    if (G == 1) return launch_cfg(ctx, tile_kernel<T, OP, 1, 1, SHADOW, 512>, tile_kernel<T, OP, 1, 1, SHADOW, 384>, a, sizeof(T), VEC, grid_out);
-    if (G == 2) return launch_cfg(ctx, tile_kernel<T, OP, 2, 1, SHADOW, 512>, tile_kernel<T, OP, 2, 1, SHADOW, 384>, a, sizeof(T), VEC, grid_out);
+    if (G == 1) return launch_cfg(ctx, tile_kernel<T, OP, 1, 1, SHADOW, 512, MULTI>, tile_kernel<T, OP, 1, 1, SHADOW, 384, MULTI>, a, sizeof(T), VEC, grid_out);
+    if (G == 2) return launch_cfg(ctx, tile_kernel<T, OP, 2, 1, SHADOW, 512, MULTI>, tile_kernel<T, OP, 2, 1, SHADOW, 384, MULTI>, a, sizeof(T), VEC, grid_out);
     if (!want_ch || nch <= 32)
-        return launch_cfg(ctx, tile_kernel<T, OP, 4, 1, SHADOW, 512>, tile_kernel<T, OP, 4, 1, SHADOW, 384>, a, sizeof(T), VEC, grid_out);
-    return launch_cfg(ctx, tile_kernel<T, OP, 4, 2, SHADOW, 512>, tile_kernel<T, OP, 4, 2, SHADOW, 384>, a, sizeof(T), 2 * VEC, grid_out);
+        return launch_cfg(ctx, tile_kernel<T, OP, 4, 1, SHADOW, 512, MULTI>, tile_kernel<T, OP, 4, 1, SHADOW, 384, MULTI>, a, sizeof(T), VEC, grid_out);
+    return launch_cfg(ctx, tile_kernel<T, OP, 4, 2, SHADOW, 512, MULTI>, tile_kernel<T, OP, 4, 2, SHADOW, 384, MULTI>, a, sizeof(T), 2 * VEC, grid_out);
 }
 
 }  // namespace
@@ -759,17 +799,21 @@ bool meb_tile_applicable(int op, int prec, const StreamArgs& a) {
 int meb_launch_tile(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* grid_out) {
     if (prec == MEB_FP64) {
         switch (op) {
-            case OP_EVAL: return launch_g<double, OP_EVAL, false>(ctx, a, true, grid_out);
-            case OP_FEAS: return launch_g<double, OP_FEAS, false>(ctx, a, false, grid_out);
+            case OP_EVAL:
+                if (a.multi > 0) return launch_g<double, OP_EVAL, false, true>(ctx, a, true, grid_out);
+                return launch_g<double, OP_EVAL, false, false>(ctx, a, true, grid_out);
+            case OP_FEAS: return launch_g<double, OP_FEAS, false, false>(ctx, a, false, grid_out);
             case OP_INGEST:
-                if (a.C32) return launch_g<double, OP_INGEST, true>(ctx, a, true, grid_out);
-                return launch_g<double, OP_INGEST, false>(ctx, a, false, grid_out);
+                if (a.C32) return launch_g<double, OP_INGEST, true, false>(ctx, a, true, grid_out);
+                return launch_g<double, OP_INGEST, false, false>(ctx, a, false, grid_out);
             default: return MEB_E_ARG;
         }
     }
     switch (op) {
-        case OP_EVAL: return launch_g<float, OP_EVAL, false>(ctx, a, true, grid_out);
-        case OP_SCREEN: return launch_g<float, OP_SCREEN, false>(ctx, a, false, grid_out);
+        case OP_EVAL:
+            if (a.multi > 0) return launch_g<float, OP_EVAL, false, true>(ctx, a, true, grid_out);
+            return launch_g<float, OP_EVAL, false, false>(ctx, a, true, grid_out);
+        case OP_SCREEN: return launch_g<float, OP_SCREEN, false, false>(ctx, a, false, grid_out);
         default: return MEB_E_ARG;
     }
 }

@@ -151,7 +151,8 @@ def _sandwich(meb, C, R, modes, near_max):
         if sub is None:                                                          # one oracle run serves both modes
             near = np.flatnonzero(reach >= 0.98 * r)
             assert 0 < near.size <= near_max, near.size
-            cs, rs, info = ripalm.meb_solve(C[near], None if R is None else R[near], 1e-10, "fp64")
+            cs, rs, info = ripalm.meb_solve(C[near], None if R is None else R[near], 1e-10, "fp64",
+                                            ripalm.Params(dense_d_max=1024))      # dense Newton up to d = 1000: a path choice
             assert info["converged"]
             sub = (cs, rs)
         cs, rs = sub

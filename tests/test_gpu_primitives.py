@@ -373,3 +373,38 @@ def test_eval_alm_unaligned_scalar_arrays(meb, ctx, prec):
     got = meb.meb_eval_alm(ctx, prec, Cd, Rs, Us, Ss, Vr, dvec(x), dvec(xbar), 2.0, 0.5, per_ball=True)
     assert torch.equal(ref["scalars"], got["scalars"]) and torch.equal(ref["grad"], got["grad"])
     assert torch.equal(ref["t"], got["t"]) and torch.equal(ref["lam"], got["lam"])
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("m,d,ld_pad", [(1000, 10, 0), (4999, 32, 0), (3001, 100, 0), (1031, 128, 0), (777, 1000, 0),
+                                        (70, 2600, 0), (1500, 20, 4)])
+@pytest.mark.parametrize("layout", ["none", "sparse"])
+def test_eval_alm_multi(meb, ctx, prec, m, d, ld_pad, layout):
+    """Multi-trial evaluation: psi at x and at x - gamma_k Delta from ONE pass, against the
+    oracle's plain loop of evaluations.  The expansion ||b + g dc||^2 = ||b||^2 + 2 g <b, dc> + g^2 ||dc||^2 loses
+    a few ulps to cancellation, hence 8 tol_p."""
+    C, R, U, V, x, xbar = make_state(900 + m + d, m, d, with_radii=(m % 2 == 1))
+    if prec == 1:
+        f = lambda a: None if a is None else a.astype(np.float32).astype(np.float64)
+        C, R, U, V = f(C), f(R), f(U), f(V)
+    rng = np.random.default_rng(m + d)
+    direction = np.concatenate([[-0.08 * x[0]], 0.05 * rng.standard_normal(d) / np.sqrt(d)])
+    gammas = [0.5, 0.75, 0.875, 0.9375]
+    Cd, Rd, Ud, slot, Vr = to_device(C, R, U, V, THDT[prec], layout, ld_pad)
+    if layout == "none":
+        U = np.zeros_like(U); V = np.zeros_like(V)
+    if (Cd.stride(0) * Cd.element_size()) % 16 != 0:
+        # rows that are not 16-byte aligned go to the scalar-load kernels, which carry no multi-trial code
+        with pytest.raises(meb.MebError) as ei:
+            meb.meb_eval_alm_multi(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), dvec(xbar), 2.5, 0.7, dvec(direction), gammas)
+        assert ei.value.code == meb.MEB_E_CAPACITY
+        return
+    res = meb.meb_eval_alm_multi(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), dvec(xbar), 2.5, 0.7, dvec(direction), gammas)
+    ref = meb.meb_eval_alm(ctx, prec, Cd, Rd, Ud, slot, Vr, dvec(x), dvec(xbar), 2.5, 0.7)
+    assert torch.equal(res["scalars"][:12], ref["scalars"][:12]) and torch.equal(res["grad"], ref["grad"])
+    want = prim.eval_alm_line(C, R, U, V, x, xbar, 2.5, 0.7, direction, gammas, dtype=NPDT[prec])
+    got = res["psi"].cpu().numpy()
+    for k, (psi, scale) in enumerate(want):
+        assert abs(got[k] - psi) <= 8 * TOL[prec] * scale, (k, got[k], psi, scale)
+    # the points differ: the predictions are not all the same number
+    assert len({float(v) for v in got}) == len(gammas)

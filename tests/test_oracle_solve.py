@@ -201,3 +201,37 @@ def test_paper_instances_mixed_flow():
         assert info["converged"] and info["rounds"] == 1
         assert abs(info["n_red"][0] - table[d][col]) <= 0.25 * table[d][col] + 3
         assert abs(r - r64) <= 1e-8 * r64
+
+
+def test_accelerated_gradient_inner_solver_reaches_the_subproblem_minimiser():
+    """a first-order inner solver minimises the same strongly convex Psi_k as Algorithm 2, so with the
+    stopping tests tightened both must stop at the same point (the minimiser of (4) is unique)."""
+    rng = np.random.default_rng(31)
+    C = rng.standard_normal((400, 6)); R = rng.uniform(0, 0.2, 400)
+    c0, L = ripalm.initial_point(C, R, ripalm.Params())
+    Cn, Rn = (C - c0) / L, R / L
+    x0 = np.zeros(7); x0[0] = 1.0
+    U = np.zeros(400); V = np.zeros((400, 6))
+    par = ripalm.Params(rho=0.0, ag_inner_max=20000)          # rho = 0: condition (5) never fires, only the KKT test does
+    st1, st2 = ripalm.Stats(), ripalm.Stats()
+    xa, eva, sa = ripalm.accelerated_gradient(Cn, Rn, U, V, x0, x0, x0, 4.0, 1.0, -1.0, par, np.float64, L, st1)
+    xs, evs, ss = ripalm.ssn(Cn, Rn, U, V, x0, x0, x0, 4.0, 1.0, -1.0, par, np.float64, L, st2)
+    assert np.linalg.norm(evs["grad"]) <= 1e-9                 # Newton reached the minimiser of Psi_k
+    assert np.linalg.norm(eva["grad"]) <= 1e-6 and st1.evals > st2.evals
+    assert np.linalg.norm(xa - xs) <= 1e-6 * (1 + np.linalg.norm(xs))
+    assert abs(eva["psi_var"] - evs["psi_var"]) <= 1e-10 * abs(evs["psi_var"])
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_first_outer_iterations_by_accelerated_gradient_same_optimum(mode):
+    """The inner solver is a path choice: with the first two outer iterations solved by the accelerated gradient
+    method the unique optimum is the same (closed form: regular simplex, and brute force in the plane)."""
+    par = ripalm.Params(ag_outer=2)
+    n = 9
+    c, r, info = ripalm.meb_solve(np.eye(n), None, 1e-10, mode, par)
+    assert info["converged"] and abs(r - np.sqrt((n - 1) / n)) <= 1e-9
+    rng = np.random.default_rng(32)
+    C = rng.uniform(-1, 1, (7, 2)); R = rng.uniform(0, 0.4, 7)
+    c, r, info = ripalm.meb_solve(C, R, 1e-10, mode, par)
+    cb, rb = bruteforce_meb_2d(C, R)
+    assert abs(r - rb) <= 1e-8 * rb and np.linalg.norm(c - cb) <= 1e-6

@@ -195,6 +195,27 @@ MEB_API int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* centers,
               const double* radii, double tol, int precision_mode, const meb_params* h_params,
               double* h_center_out, double* h_radius_out, meb_stats* h_stats);
 
+/* ---- the same solve with the balls PARTITIONED over several GPUs (the paper's stated
+ * future work; the constraint-wise separable structure that allows it: P:L179, L218) ----
+ * One process per GPU.  This rank holds the contiguous rows [row_offset, row_offset + m_local) of an instance of
+ * m_global balls: centers_local / radii_local are DEVICE arrays of m_local rows.  The (d+1)-sized state and the
+ * controller are replicated; at every reduction point (evaluation, Hessian-vector product or dense Hessian,
+ * initial point, feasibility check) the rank packs its partial into xchg_send (DEVICE, xchg_doubles doubles:
+ * at least meb_shard_record_doubles(d)), calls allgather(user, n), which must place the first n doubles of every
+ * rank's xchg_send at xchg_recv + r * n (DEVICE, nranks * xchg_doubles doubles) for r = 0..nranks-1, ORDERED ON THE
+ * CONTEXT'S STREAM (e.g. ncclAllGather on that stream; return 0 on success), and the second-level kernels add the
+ * nranks records in rank order.  All ranks therefore compute bit-identical iterates.  Records are d + O(10) doubles
+ * ((d+1)^2 for the dense Hessian, d <= 128).  The solve is host-stepped (one decision read-back per evaluation).
+ * Outputs as meb_solve; meb_stats counts this rank's passes and bytes.  Every rank must pass the same tol, mode
+ * and parameters.  m_local >= 1. */
+typedef int (*meb_allgather_fn)(void* user, int64_t n_doubles);
+MEB_API int64_t meb_shard_record_doubles(int32_t d);
+MEB_API int meb_solve_sharded(meb_ctx* ctx, int32_t rank, int32_t nranks, int64_t m_local, int64_t row_offset,
+                      int64_t m_global, int32_t d, const double* centers_local, int64_t ld,
+                      const double* radii_local, double tol, int precision_mode, const meb_params* h_params,
+                      double* xchg_send, double* xchg_recv, int64_t xchg_doubles, meb_allgather_fn allgather,
+                      void* user, double* h_center_out, double* h_radius_out, meb_stats* h_stats);
+
 /* Same, with HOST input buffers: uploads centres (and radii) to device memory owned by the context
  * (host->device copies are part of the call), then solves.  This is the end-to-end entry point. */
 MEB_API int meb_solve_host(meb_ctx* ctx, int64_t m, int32_t d, const double* h_centers, int64_t ld,

@@ -30,7 +30,9 @@ EXPORTS = [
     "meb_version", "meb_solve", "meb_solve_host", "meb_ingest", "meb_eval_alm", "meb_hvp",
     "meb_dense_hessian", "meb_update_multipliers", "meb_screen_compact", "meb_feasibility_check",
     "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch", "meb_set_option", "meb_eval_alm_multi",
+    "meb_solve_sharded", "meb_shard_record_doubles",
 ]
+ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int64)
 
 
 class meb_params(C.Structure):
@@ -99,6 +101,10 @@ def load():
     lib.meb_solve.argtypes = solve_args
     lib.meb_solve_host.argtypes = solve_args
     lib.meb_solve_batch.argtypes = [vp, i32, vp, i32, vp, i64, vp, dbl, C.POINTER(meb_params), vp, vp, vp, vp]
+    lib.meb_shard_record_doubles.argtypes = [i32]
+    lib.meb_shard_record_doubles.restype = i64
+    lib.meb_solve_sharded.argtypes = [vp, i32, i32, i64, i64, i64, i32, vp, i64, vp, dbl, C.c_int, C.POINTER(meb_params),
+                                      vp, vp, i64, ALLGATHER_FN, vp, vp, C.POINTER(dbl), C.POINTER(meb_stats)]
     lib.meb_ingest.argtypes = [vp, i64, i32, vp, i64, vp, i32, vp, vp, vp, i64, vp]
     prob = [vp, C.c_int, i64, i32, vp, i64, vp, vp, vp, vp, i64]
     lib.meb_eval_alm.argtypes = prob + [vp, vp, dbl, dbl, vp, vp, vp, vp, vp, vp, vp]
@@ -112,7 +118,7 @@ def load():
                                           C.POINTER(i32), vp, i64, C.POINTER(i64)]
     for name in EXPORTS:
         fn = getattr(lib, name)
-        if name not in ("meb_strerror", "meb_default_params"):
+        if name not in ("meb_strerror", "meb_default_params", "meb_shard_record_doubles"):
             fn.restype = C.c_int
     _lib = lib
     return lib
@@ -235,6 +241,32 @@ def meb_solve_host(ctx: Context, h_centers, h_radii, tol=1e-8, precision_mode=ME
     allow = (MEB_OK, MEB_W_NOT_CONVERGED) if allow_not_converged else (MEB_OK,)
     _check(code, "meb_solve_host", allow)
     return out_c, out_r.value, st.as_dict()
+
+
+def meb_solve_sharded(ctx: Context, rank, nranks, centers_local, radii_local, row_offset, m_global, xchg_send, xchg_recv,
+                      allgather, tol=1e-8, precision_mode=MEB_MODE_FP64, params=None, allow_not_converged=False):
+    """This rank's rows [row_offset, row_offset + m_local) of an m_global-ball instance (CUDA float64 tensors);
+    xchg_send / xchg_recv: CUDA float64 tensors of meb_shard_record_doubles(d) and nranks times that many doubles;
+    allgather(n) -> 0: gathers the first n doubles of every rank's xchg_send into xchg_recv[r * n : (r + 1) * n],
+    ordered on the context's stream.  Returns (center CPU tensor, radius, stats) -- identical on every rank."""
+    assert centers_local.is_cuda and centers_local.dtype == torch.float64 and centers_local.stride(1) == 1
+    m, d = centers_local.shape
+    out_c = torch.empty(d, dtype=torch.float64)
+    out_r = C.c_double()
+    st = meb_stats()
+    cb = ALLGATHER_FN(lambda user, n: int(allgather(int(n))))
+    code = load().meb_solve_sharded(ctx.h, int(rank), int(nranks), m, int(row_offset), int(m_global), d, _ptr(centers_local),
+                                    centers_local.stride(0), _ptr(radii_local), float(tol), int(precision_mode),
+                                    None if params is None else C.byref(params), _ptr(xchg_send), _ptr(xchg_recv),
+                                    int(xchg_send.numel()), cb, None, C.c_void_p(out_c.data_ptr()), C.byref(out_r),
+                                    C.byref(st))
+    allow = (MEB_OK, MEB_W_NOT_CONVERGED) if allow_not_converged else (MEB_OK,)
+    _check(code, "meb_solve_sharded", allow)
+    return out_c, out_r.value, st.as_dict()
+
+
+def meb_shard_record_doubles(d: int) -> int:
+    return int(load().meb_shard_record_doubles(int(d)))
 
 
 def meb_solve_batch(ctx: Context, centers, radii, row_offsets, tol=1e-8, params=None):

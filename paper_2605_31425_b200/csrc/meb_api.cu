@@ -571,6 +571,10 @@ extern "C" int meb_ingest(meb_ctx* ctx, int64_t m, int32_t d, const double* C, i
     const int S = (int)(m < sample_rows ? m : sample_rows);
     rc = meb_sample_mean(ctx, C, ld, m, d, S, c0_out);
     if (rc != MEB_OK) return rc;
+    if (ctx->shard) {               // sharded solve: c0 = mean of the ranks' sample means weighted by their rows (reading 3)
+        rc = meb_shard_mean(ctx, c0_out, d, m);
+        if (rc != MEB_OK) return rc;
+    }
     StreamArgs s;
     memset(&s, 0, sizeof(s));
     s.C = C; s.ld = ld; s.R = R; s.x = nullptr; s.c0 = c0_out; s.m = m; s.d = d; s.sigma = 1.0;
@@ -580,5 +584,7 @@ extern "C" int meb_ingest(meb_ctx* ctx, int64_t m, int32_t d, const double* C, i
     ctx->cur_class = MEB_PASS_INGEST;
     rc = timed_stream(ctx, OP_INGEST, MEB_FP64, s, bytes, &grid, nullptr);
     if (rc != MEB_OK) return rc;
-    return meb_argmax_finalize(ctx, grid, scalars_out);
+    rc = meb_argmax_finalize(ctx, grid, scalars_out);
+    if (rc == MEB_OK && ctx->shard) rc = meb_shard_argmax(ctx, scalars_out);     // L = max over the ranks, global index
+    return rc;
 }

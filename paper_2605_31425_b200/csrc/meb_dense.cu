@@ -194,14 +194,16 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
                                                              const int32_t* __restrict__ count,
                                                              int dp, int d, const double* __restrict__ ev,
                                                              double sigma, double tau, double* __restrict__ H,
-                                                             const MebDyn* __restrict__ dyn, int rb) {
+                                                             const MebDyn* __restrict__ dyn, int rb, long long pstride) {
     if (dyn) { sigma = dyn->sigma_raw; tau = dyn->tau_eff; }
-    const int ntiles = (*count + rb - 1) / rb;            // CTAs b < ntiles wrote a partial
-    if (nparts > ntiles) nparts = ntiles;
+    if (rb > 0) {
+        const int ntiles = (*count + rb - 1) / rb;        // CTAs b < ntiles wrote a partial
+        if (nparts > ntiles) nparts = ntiles;
+    }
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
     const int n = d + 1;
-    const size_t stride = (size_t)dp * dp + dp;
+    const size_t stride = pstride > 0 ? (size_t)pstride : (size_t)dp * dp + dp;
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n * n; e += gridDim.x * blockDim.x) {
         const int p = e / n, q = e % n;
         double v;
@@ -309,8 +311,19 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
     const int n = c.d + 1;
     int fgrid = (n * n + 255) / 256;
     if (fgrid > 64) fgrid = 64;
+    if (ctx->shard) {                     // sharded solve: records of the ranks' partial matrices, added in rank order
+        rc = meb_shard_pack_mat(ctx, ctx->part_mat, grid, ctx->count_dev, rb, (int64_t)per);
+        if (rc != MEB_OK) return rc;
+        rc = meb_shard_exchange(ctx, (int64_t)per);
+        if (rc != MEB_OK) return rc;
+        ctx->launches++;
+        dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->shard->recv, ctx->shard->nranks, ctx->count_dev, dp, c.d, ev_scalars,
+                                                             c.sigma, c.tau, H, c.gs ? c.gs->dyn : nullptr, 0, (long long)per);
+        MEB_CUDA_OK(ctx, cudaGetLastError());
+        return MEB_OK;
+    }
     ctx->launches++; dense_finalize_kernel<<<fgrid, 256, 0, ctx->stream>>>(ctx->part_mat, grid, ctx->count_dev, dp, c.d, ev_scalars, c.sigma,
-                                                          c.tau, H, c.gs ? c.gs->dyn : nullptr, rb);
+                                                          c.tau, H, c.gs ? c.gs->dyn : nullptr, rb, 0);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

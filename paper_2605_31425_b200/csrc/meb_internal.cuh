@@ -18,6 +18,18 @@
 #define MEB_EVPOOL 4096               // streaming launches of one solve that get an event pair
 #define MEB_MULTI_MAX 4               // step sizes an Armijo trial pass can predict besides its own (meb_params.armijo_multi)
 
+// A sharded solve: this rank holds rows [row_offset, row_offset + m_local) of an
+// m_global-ball instance.  At every reduction point the rank packs its partial into `send` (one record of at most
+// rec_doubles doubles), the caller's all-gather fills `recv` with the records of all ranks in RANK ORDER, and the
+// unchanged second-level kernels add the nranks records in that order: every rank forms bit-identical sums and the
+// replicated controllers take identical decisions.
+struct MebShard {
+    int32_t rank, nranks;
+    int64_t row_offset, m_global;
+    double* send; double* recv; int64_t rec_doubles;
+    meb_allgather_fn allgather; void* user;
+};
+
 struct meb_ctx {
     int device;
     cudaStream_t stream;
@@ -81,6 +93,7 @@ struct meb_ctx {
     double ev_extra_bytes;          // stepped solves: bytes of the multiplier rows the next evaluation pass reads
     int last_path;                  // kernel family of the last streaming launch (PATH_* in meb_api.cu)
     struct MebDyn* dyn_api;         // device MebDyn of the per-primitive multi-trial call
+    MebShard* shard;                // non-null inside meb_solve_sharded
 };
 
 // prints file:line and the CUDA error string to stderr when the context was created with MEB_DEBUG set
@@ -306,6 +319,26 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
 // With S != nullptr the kernel also runs the controller step that follows a Newton solve (first Armijo trial).
 int meb_chol_solve(meb_ctx* ctx, const double* H, const double* g, int n, double scale, double* delta,
                    int* info_dev, SolverDev* S, const SolverVecs* v);
+
+// ---- sharded solves (meb_shard.cu): pack the local partial into the send record, all-gather, return the stride ----
+int meb_shard_exchange(meb_ctx* ctx, int64_t n_doubles);
+// evaluation: per-CTA scalars [grid][MEB_NPART], vector partials [nvec][dpad] (tpb / count: see FinalizeArgs),
+// predictions [grid][MEB_MULTI_MAX] (nullable) -> record [0..11] scalars, [12..15] predictions, [16..16+d) vector
+int meb_shard_pack_eval(meb_ctx* ctx, const double* part, int grid, const double* part_vec, int nvec, int tpb,
+                        const int32_t* count, int dpad, int d, const double* multi_part);
+// hvp: record [0] = sum of the scalar partials, [8 .. 8+d) = sum of the vector partials
+int meb_shard_pack_hvp(meb_ctx* ctx, const double* part_sc, int nsc, const double* part_vec, int nvec, int tpb,
+                       const int32_t* count, int dpad, int d);
+// dense Hessian: record [0 .. per) = sum of the per-CTA partial matrices that were written (CTAs b < ceil(count / rb))
+int meb_shard_pack_mat(meb_ctx* ctx, const double* part_mat, int nparts, const int32_t* count, int rb, int64_t per);
+// small records: n doubles from `src` (device) -> send[0..n)
+int meb_shard_pack_small(meb_ctx* ctx, const double* src, int n);
+// combine the gathered small records (stride rec) on the device: mode 0: (value, index, count) arg-max records ->
+// out[0] = max value, out[1] = its index (smallest on ties), out[2] = sum of counts; mode 1: weighted mean of the
+// d-vectors rec[0..d) with weights rec[d] / sum of weights -> out[0..d)
+int meb_shard_combine(meb_ctx* ctx, int mode, int d, double* out);
+int meb_shard_mean(meb_ctx* ctx, double* c0, int d, int64_t m_local);
+int meb_shard_argmax(meb_ctx* ctx, double* scal3);
 
 // ---- matrix-free Newton direction in one persistent kernel (meb_cg.cu) ----
 int meb_launch_cg(meb_ctx* ctx, const EvalCall& c, double* W, int64_t wc_cap, double* rho_c, unsigned int* bar);

@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
 __global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
     const double* __restrict__ part_vec, int nvec, int tpb, const int32_t* __restrict__ count, int dpad,
     const double* __restrict__ part_sc, const double* __restrict__ ev, const double* __restrict__ q,
-    double sigma, double tau, int d, double* __restrict__ Hq, const MebDyn* __restrict__ dyn, int nsc) {
+    double sigma, double tau, int d, double* __restrict__ Hq, const MebDyn* __restrict__ dyn, int nsc, int sc_stride) {
     if (dyn) { sigma = dyn->sigma_raw; tau = dyn->tau_eff; }
     const double n1 = ev[MEB_EV_N_B1], n3 = ev[MEB_EV_N_B3], srho = ev[MEB_EV_SUM_RHO];
     const double tos = tau / sigma;
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(FBLOCK) hvp_finalize_kernel(
     }
     if (threadIdx.x < 32) {
         double s = 0.0;
-        for (int b = threadIdx.x; b < nsc; b += 32) s += part_sc[b];     // CTAs without list entries wrote 0
+        for (int b = threadIdx.x; b < nsc; b += 32) s += part_sc[(size_t)b * sc_stride];   // CTAs without list entries wrote 0
         s = warp_sum(s);
         if (threadIdx.x == 0) Hq[0] = tos * q[0] + sigma * (n1 * q[0] + 0.5 * (n3 * q[0] + s));
     }
@@ -324,6 +324,18 @@ __global__ void set_kept_kernel(const int32_t* __restrict__ idx, int64_t n, uint
 // ---- host wrappers ---------------------------------------------------------------------------------
 int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f_in) {
     FinalizeArgs f = f_in;
+    if (ctx->shard) {
+        // sharded solve: first level of the reduction here, the ranks' records are added in rank order below
+        int rc = meb_shard_pack_eval(ctx, f.part, f.grid, f.part_vec, f.nvec, f.tpb, f.count, f.dpad, f.d, f.multi_part);
+        if (rc != MEB_OK) return rc;
+        const int64_t rs = 16 + ((int64_t)f.d + 7) / 8 * 8;
+        rc = meb_shard_exchange(ctx, rs);
+        if (rc != MEB_OK) return rc;
+        const double* rv = ctx->shard->recv;
+        f.part = rv; f.grid = ctx->shard->nranks; f.part_stride = (int)rs;
+        f.part_vec = rv + 16; f.nvec = ctx->shard->nranks; f.tpb = 0; f.dpad = (int)rs; f.vec_stride = 0;
+        if (f.multi_part) { f.multi_part = rv + MEB_NPART; f.multi_stride = (int)rs; }
+    }
     if (f.d > 256 && f.nvec > 8) {                 // long vectors: add the partials with many CTAs first
         ctx->launches++;
         reduce_partials_kernel<<<(f.d + 31) / 32, 256, 0, ctx->stream>>>(f.part_vec, f.nvec, f.tpb, f.count, f.dpad, f.d,
@@ -338,6 +350,20 @@ int meb_eval_finalize(meb_ctx* ctx, const FinalizeArgs& f_in) {
 int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, const double* ev,
                      const double* q, double sigma, double tau, int d, double* Hq, const MebDyn* dyn) {
     int tpb = d > 2048 ? 1 : MEB_WARPS;
+    if (ctx->shard) {
+        // sharded solve: this rank's partial goes into its record, the records of all ranks come back in rank order
+        int rc = meb_shard_pack_hvp(ctx, part_sc, nvec, ctx->part_vec, nvec, tpb, ctx->count_dev, dpad, d);
+        if (rc != MEB_OK) return rc;
+        const int64_t rs = 8 + dpad;
+        rc = meb_shard_exchange(ctx, rs);
+        if (rc != MEB_OK) return rc;
+        const double* rv = ctx->shard->recv;
+        ctx->launches++;
+        hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(rv + 8, ctx->shard->nranks, 0, ctx->count_dev, (int)rs, rv, ev, q, sigma, tau, d,
+                                                          Hq, dyn, ctx->shard->nranks, (int)rs);
+        MEB_CUDA_OK(ctx, cudaGetLastError());
+        return MEB_OK;
+    }
     const double* pv = ctx->part_vec;
     int nv = nvec;
     if (d > 128 && nvec > 8) {                     // long vectors: add the partials with many CTAs first
@@ -347,7 +373,7 @@ int meb_hvp_finalize(meb_ctx* ctx, int nvec, int dpad, const double* part_sc, co
         pv = ctx->part_red; nv = 1;
     }
     ctx->launches++; hvp_finalize_kernel<<<1, FBLOCK, 0, ctx->stream>>>(pv, nv, nv == 1 && pv == ctx->part_red ? 0 : tpb, ctx->count_dev, dpad,
-                                                       part_sc, ev, q, sigma, tau, d, Hq, dyn, nvec);
+                                                       part_sc, ev, q, sigma, tau, d, Hq, dyn, nvec, 1);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -501,9 +501,14 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         if (P.off) { rc = upload(ctx, S.v.off, P.off, S.d); if (rc) return rc; }
     }
     bool first = true;
-    bool stepped = ctx->opt[MEB_OPT_STEPPED] != 0;
+    // a sharded solve is host-stepped (the all-gather between the two levels of every reduction is the caller's
+    // collective) and keeps full-size V pools, so that no rank ever stops for capacity on its own
+    bool stepped = ctx->opt[MEB_OPT_STEPPED] != 0 || ctx->shard != nullptr;
+    if (ctx->shard)
+        for (int b = 0; b < 2; ++b)
+            if (P.own_v[b] >= 0 && P.vcap[b] < P.m) { int rcg = grow_pool(ctx, P, b, P.m); if (rcg) return rcg; }
     // small problems (the reduced problem of the mixed mode, small instances): one persistent CTA runs the phase
-    bool small = dense && !ctx->opt[MEB_OPT_NO_SMALL] && meb_small_applicable(P.prec, P.m, P.d);
+    bool small = dense && !ctx->opt[MEB_OPT_NO_SMALL] && !ctx->shard && meb_small_applicable(P.prec, P.m, P.d);
     if (small) {
         for (int b = 0; b < 2 && small; ++b)
             if (P.vcap[b] < P.m) { if (P.own_v[b] < 0 || grow_pool(ctx, P, b, P.m) != MEB_OK) small = false; }
@@ -551,7 +556,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         }
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
         h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
-        h->h_cgp = G->h_cgp; h->wc_cap = S.wc_cap;
+        h->h_cgp = G->h_cgp; h->wc_cap = ctx->shard ? -1 : S.wc_cap;     // sharded: one exchange per CG iteration
         h->in_graph = (stepped || small) ? 0 : 1;
         if (first) {
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
@@ -664,6 +669,23 @@ int setup_multipliers(meb_ctx* ctx, Problem& P, int ownU0, int ownS0, int ownV0)
     return MEB_OK;
 }
 
+// sharded solve: (delta_max, argmax, number of violators) of this rank -> maximum over the ranks, its GLOBAL index,
+// total number of violators (the local count stays in *nv_local)
+int feas_global(meb_ctx* ctx, double* dmax, int32_t* am, int64_t nv_local, int64_t* nv_total) {
+    *nv_total = nv_local;
+    if (!ctx->shard) return MEB_OK;
+    double h3[3] = {*dmax, (double)*am, (double)nv_local};
+    int rc = upload(ctx, ctx->small + SM_AUX, h3, 3);
+    if (rc) return rc;
+    rc = meb_shard_argmax(ctx, ctx->small + SM_AUX);
+    if (rc) return rc;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->small + SM_AUX, 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    rc = sync_stream(ctx);
+    if (rc) return rc;
+    *dmax = ctx->h_pinned[0]; *am = (int32_t)ctx->h_pinned[1]; *nv_total = (int64_t)ctx->h_pinned[2];
+    return MEB_OK;
+}
+
 // resets the per-solve recording state of the context on every way out of meb_solve
 struct SolveScope {
     meb_ctx* ctx; bool timing_was;
@@ -703,11 +725,9 @@ void reduced_bind(meb_ctx* ctx, const Reduced& Q, Problem& P2) {
     }
 }
 
-}  // namespace
-
-extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_t ld,
-                         const double* radii, double tol, int precision_mode, const meb_params* h_params,
-                         double* h_center_out, double* h_radius_out, meb_stats* h_stats) {
+int solve_impl(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_t ld,
+               const double* radii, double tol, int precision_mode, const meb_params* h_params,
+               double* h_center_out, double* h_radius_out, meb_stats* h_stats) {
     if (!ctx || !centers || !h_center_out || !h_radius_out || m < 1 || d < 1 || ld < d) return MEB_E_ARG;
     if (!(tol > 0.0) || (precision_mode != MEB_MODE_FP64 && precision_mode != MEB_MODE_MIXED)) return MEB_E_ARG;
     if (m > ctx->m_max || d > ctx->d_max) return MEB_E_CAPACITY;
@@ -819,6 +839,7 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
             rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, INFINITY, nullptr, &dmax,
                                        &am, nullptr, 0, &nvl);
             if (rc) break;
+            { int64_t nvt = 0; rc = feas_global(ctx, &dmax, &am, nvl, &nvt); if (rc) break; }
             st->passes_fp64_full++;
             S.bytes += ctx->last_pass_bytes;
             for (int j = 0; j < d; ++j) creturn[j] = xr[1 + j];
@@ -929,9 +950,12 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
                 rc = meb_feasibility_check(ctx, m, d, centers, ld, radii, r_alg, S.v.x_raw + 1, eps_feas, kept,
                                            &dmax, &am, idx + nred, m - nred, &nvl);
                 if (rc) break;
+                int64_t nv_total = nvl;                         // sharded: every rank re-adds its own violators, all
+                rc = feas_global(ctx, &dmax, &am, nvl, &nv_total);   // ranks stop together when no rank has any
+                if (rc) break;
                 st->passes_fp64_full++;
                 S.bytes += ctx->last_pass_bytes;
-                if (nvl == 0) break;
+                if (nv_total == 0) break;
                 if (rnd + 1 == S.par.max_rounds) { converged = false; break; }      // round cap: best iterate, not converged
                 // re-introduce the violated balls with zero multipliers (reading 12); the reduced
                 // buffers grow as needed and keep the rows, radii and current multipliers of the balls already there
@@ -992,6 +1016,35 @@ extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* cente
     cudaGetLastError();
     st->kernel_launches = ctx->launches - launches0;
     return converged ? MEB_OK : MEB_W_NOT_CONVERGED;
+}
+
+}  // namespace
+
+extern "C" int meb_solve(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_t ld,
+                         const double* radii, double tol, int precision_mode, const meb_params* h_params,
+                         double* h_center_out, double* h_radius_out, meb_stats* h_stats) {
+    if (!ctx) return MEB_E_ARG;
+    ctx->shard = nullptr;
+    return solve_impl(ctx, m, d, centers, ld, radii, tol, precision_mode, h_params, h_center_out, h_radius_out, h_stats);
+}
+
+extern "C" int meb_solve_sharded(meb_ctx* ctx, int32_t rank, int32_t nranks, int64_t m_local, int64_t row_offset,
+                                 int64_t m_global, int32_t d, const double* centers_local, int64_t ld,
+                                 const double* radii_local, double tol, int precision_mode, const meb_params* h_params,
+                                 double* xchg_send, double* xchg_recv, int64_t xchg_doubles, meb_allgather_fn allgather,
+                                 void* user, double* h_center_out, double* h_radius_out, meb_stats* h_stats) {
+    if (!ctx || nranks < 1 || rank < 0 || rank >= nranks || m_local < 1 || row_offset < 0 || m_global < row_offset + m_local ||
+        !xchg_send || !xchg_recv || (nranks > 1 && !allgather))
+        return MEB_E_ARG;
+    if (xchg_doubles < meb_shard_record_doubles(d)) return MEB_E_CAPACITY;
+    MebShard sh;
+    sh.rank = rank; sh.nranks = nranks; sh.row_offset = row_offset; sh.m_global = m_global;
+    sh.send = xchg_send; sh.recv = xchg_recv; sh.rec_doubles = xchg_doubles; sh.allgather = allgather; sh.user = user;
+    ctx->shard = &sh;
+    const int rc = solve_impl(ctx, m_local, d, centers_local, ld, radii_local, tol, precision_mode, h_params, h_center_out,
+                              h_radius_out, h_stats);
+    ctx->shard = nullptr;
+    return rc;
 }
 
 extern "C" int meb_solve_host(meb_ctx* ctx, int64_t m, int32_t d, const double* h_centers, int64_t ld,

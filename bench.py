@@ -59,6 +59,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the per-config block (configs 1-5, both modes)")
     ap.add_argument("--shard", action="store_true", help="N > 1: partition the balls of one instance over the ranks")
+    ap.add_argument("--paper-grid", action="store_true",
+                    help="the paper's own deterministic instances (P:L289-299, grids of P:L319-320 and L335): one JSON "
+                         "line with device times and the balls kept for the FP64 phase (Table 1, P:L326-333)")
     return ap.parse_args()
 
 
@@ -443,8 +446,39 @@ def run_b200(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_paper_grid():
+    """The paper's own workload: d in {20,30,40,50} x m in {1e3..1e5} (Table 1) and
+    d in {1e2..1e4} x m in {1e3, 5e3}.  Device time of the FP64 and of the mixed solve (best of 3), the
+    number of balls kept for phase 2 and the radius."""
+    import torch
+    import paper_2605_31425_b200 as meb
+    import workloads
+    rows = []
+    grid = [(d, m) for d in (20, 30, 40, 50) for m in (1000, 5000, 10000, 50000, 100000)]
+    grid += [(d, m) for d in (100, 500, 1000, 5000, 10000) for m in (1000, 5000)]
+    for d, m in grid:
+        C, R = workloads.paper_instance(m, d)
+        dC, dR = torch.from_numpy(C).cuda(), torch.from_numpy(R).cuda()
+        rec = {"d": d, "m": m}
+        with meb.Context(m, d) as ctx:
+            for mode, name in ((meb.MEB_MODE_FP64, "fp64"), (meb.MEB_MODE_MIXED, "mixed")):
+                best = None
+                for _ in range(3):
+                    c, r, st = meb.meb_solve(ctx, dC, dR, TOL, mode, allow_not_converged=True)
+                    best = st["ms_total"] if best is None else min(best, st["ms_total"])
+                rec[name + "_ms"] = best
+                rec[name + "_converged"] = st["converged"]
+                rec[name + "_radius"] = r
+                if name == "mixed":
+                    rec["kept"] = st["n_reduced"]
+        rows.append(rec)
+    print(json.dumps({"workload": "paper instances (LCG generator, P:L289-299)", "tol": TOL, "rows": rows}), flush=True)
+
+
 def main():
     args = parse_args()
+    if args.paper_grid:
+        return run_paper_grid()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -91,9 +91,15 @@ typedef struct meb_params {
                                  * below it (trials bound to fail are skipped); 0.5 = plain halving (reading 4)  0.5  */
     int32_t armijo_multi;       /* every Armijo trial pass also evaluates Psi at the next armijo_multi halvings of its
                                  * step (same bytes, one more dot product per row), and halvings already known to fail
-                                 * are skipped (DESIGN reading 19); 0 = off                    4    */
+                                 * are skipped (DESIGN reading 19); 0 = off; -1 = automatic:
+                                 * 4 for rows longer than 1 KB, off for shorter rows, where the per-row cost of the
+                                 * predictions exceeds what the skipped (and anyway cut-short) trials cost         -1   */
     int32_t ag_outer;           /* the first ag_outer outer iterations solve subproblem (4) with the accelerated
                                  * gradient method instead of semismooth Newton (DESIGN reading 20)       0    */
+    double sigma_carry;         /* mixed mode: the FP64 run on the reduced problem starts at
+                                 * sigma = max(sigma0, sigma_carry * sigma reached by the low-precision run) when that
+                                 * run converged (its multipliers are the warm start); 0 = reset to sigma0
+                                 * (DESIGN reading 11)                                                             0    */
 } meb_params;
 
 /* Counters and residuals of one meb_solve (host struct). */

@@ -42,7 +42,7 @@ class meb_params(C.Structure):
                 ("armijo_max_halvings", C.c_int32), ("cg_max", C.c_int32), ("dense_d_max", C.c_int32),
                 ("inner_max", C.c_int32), ("outer_max", C.c_int32), ("max_rounds", C.c_int32),
                 ("sample_rows", C.c_int32), ("outer_max_lo", C.c_int32), ("armijo_shrink_min", C.c_double),
-                ("armijo_multi", C.c_int32), ("ag_outer", C.c_int32)]
+                ("armijo_multi", C.c_int32), ("ag_outer", C.c_int32), ("sigma_carry", C.c_double)]
 
 
 class meb_stats(C.Structure):

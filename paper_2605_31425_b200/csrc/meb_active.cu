@@ -128,6 +128,38 @@ __global__ void __launch_bounds__(MEB_BLOCK, (MODE == MODE_WRITEV && TEAM == 32)
         }
         kstart = n;
     }
+    if (MODE == MODE_ROWSUM && TEAM == MEB_BLOCK) {
+        // Long rows, whole CTA per entry: FOUR entries of the CTA's sequence per sweep over the columns, so that a
+        // thread has eight independent loads in flight per column instead of a load -> shared-memory update chain
+        // per entry (the entries are still added in list order: a fixed chain of four FMAs per column).
+        for (int kb = kstart; kb < n; kb += nteams * 4) {
+            const T* rp[4]; const T* vp[4]; double lam[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const long long k = (long long)kb + (long long)u * nteams;
+                const int i = k < n ? a.list[k] : -1;
+                lam[u] = i >= 0 ? a.rec_lam[i] : 0.0;
+                rp[u] = C + (int64_t)(i >= 0 ? i : 0) * a.ld;
+                const int slot = (i >= 0 && a.v_slot) ? a.v_slot[i] : -1;
+                vp[u] = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
+            }
+#pragma unroll 2
+            for (int j = tt; j < d; j += TEAM) {
+                const T cj = (T)cx[j];
+                T b4[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    b4[u] = rp[u][j] - cj;
+                    if (vp[u]) b4[u] = fma(vp[u][j], inv_sig, b4[u]);
+                }
+                double s = acc[j];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) s = fma(lam[u], (double)b4[u], s);
+                acc[j] = s;
+            }
+        }
+        kstart = n;
+    }
     for (int k = kstart; k < n; k += nteams) {
         const int i = a.list[k];
         const T* rowp = C + (int64_t)i * a.ld;

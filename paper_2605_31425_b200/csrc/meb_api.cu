@@ -66,7 +66,7 @@ extern "C" void meb_default_params(meb_params* p) {
     p->armijo_mu = 1e-4; p->tol_lo = 1e-2; p->tol_red_factor = 0.02;
     p->armijo_max_halvings = 30; p->cg_max = 500; p->dense_d_max = 128; p->inner_max = 50;
     p->outer_max = 200; p->max_rounds = 10; p->sample_rows = 1024; p->outer_max_lo = 30;
-    p->armijo_multi = 4; p->ag_outer = 0;
+    p->armijo_multi = -1; p->ag_outer = 0; p->sigma_carry = 0.0;
 }
 
 extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t m_max, int32_t d_max) {
@@ -364,7 +364,7 @@ __global__ void multi_setup_kernel(MebDyn* dyn, const double* __restrict__ dir, 
         dyn->sigma_raw = sigma; dyn->tau_eff = tau; dyn->cur = 0; dyn->has_mult = has_mult; dyn->s0_abort = 1e300;
         dyn->multi_n = n;
         dyn->multi_gamma[0] = g0; dyn->multi_gamma[1] = g1; dyn->multi_gamma[2] = g2; dyn->multi_gamma[3] = g3;
-        dyn->dir_r = dir[0]; dyn->dir_c2 = t;
+        dyn->dir_r = dir[0]; dyn->dir_c2 = t; dyn->dir_c = sqrt(t);
     }
 }
 // psi_out[k] = r_k + (sigma/2) S_k + (tau/2sigma) ||x_k - xbar||^2 at x_k = x - gamma_k dir (reading 13)

@@ -47,9 +47,14 @@ struct CgArgs {
     SolverDev* S; SolverVecs v;
 };
 
-template <typename T>
+// TEAM = 32: a warp per active row (rows of a few KB); TEAM = CG_THREADS: the whole CTA per row (long rows: one
+// warp would walk 1e4 columns in 300 dependent-latency steps).  Two passes over the row (the second one hits L1/L2):
+// first ||b||^2 with nothing but loads in the loop, then the normalised row is written.
+template <typename T, int TEAM>
 __global__ void __launch_bounds__(CG_THREADS) cg_gather_kernel(const CgArgs a) {
+    __shared__ double red[CG_WARPS];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tt = TEAM == 32 ? lane : (int)threadIdx.x;
     const int n = *a.count < a.wc_cap ? *a.count : (int)a.wc_cap;
     const int cur = a.dyn->cur;
     const bool hm = a.dyn->has_mult != 0;
@@ -59,31 +64,61 @@ __global__ void __launch_bounds__(CG_THREADS) cg_gather_kernel(const CgArgs a) {
     const T inv_sig = T(1) / (T)a.dyn->sigma_raw;
     const double* __restrict__ cx = a.x + 1;
     const int d = a.d;
-    const int nw = gridDim.x * CG_WARPS;
-    for (int k = blockIdx.x * CG_WARPS + warp; k < n; k += nw) {
+    constexpr int TPB = CG_THREADS / TEAM;
+    const int nteams = gridDim.x * TPB;
+    for (int k = blockIdx.x * TPB + (TEAM == 32 ? warp : 0); k < n; k += nteams) {
         const int i = a.list[k];
         const double rho = a.rec_rho[i];
-        double* wrow = a.W + (size_t)k * a.dpad;
+        double* __restrict__ wrow = a.W + (size_t)k * a.dpad;
         if (rho > 1.5) {                                   // B1: P_i = I (counted in n1), no rank-one part
-            for (int j = lane; j < a.dpad; j += 32) wrow[j] = 0.0;
-            if (lane == 0) a.rho_c[k] = 0.0;
+            for (int j = tt; j < a.dpad; j += TEAM) wrow[j] = 0.0;
+            if (tt == 0) a.rho_c[k] = 0.0;
             continue;
         }
-        const T* rowp = C + (int64_t)i * a.ld;
+        const T* __restrict__ rowp = C + (int64_t)i * a.ld;
         const int slot = slotp ? slotp[i] : -1;
-        const T* vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
-        double nb2 = 0.0;
-        for (int j = lane; j < d; j += 32) {
-            T b = rowp[j] - (T)cx[j];
-            if (vrow) b = fma(vrow[j], inv_sig, b);
-            const double bd = (double)b;
-            wrow[j] = bd;
-            nb2 = fma(bd, bd, nb2);
+        const T* __restrict__ vrow = slot >= 0 ? V + (int64_t)slot * a.ldv : nullptr;
+        double nb2 = 0.0, nb2b = 0.0;
+        if (vrow) {
+#pragma unroll 4
+            for (int j = tt; j < d; j += TEAM) {
+                const double bd = (double)fma(vrow[j], inv_sig, rowp[j] - (T)cx[j]);
+                nb2 = fma(bd, bd, nb2);
+            }
+        } else {
+            int j = tt;
+#pragma unroll 1
+            for (; j + 7 * TEAM < d; j += 8 * TEAM) {
+                double bd[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) bd[u] = (double)(rowp[j + u * TEAM] - (T)cx[j + u * TEAM]);
+#pragma unroll
+                for (int u = 0; u < 8; u += 2) { nb2 = fma(bd[u], bd[u], nb2); nb2b = fma(bd[u + 1], bd[u + 1], nb2b); }
+            }
+            for (; j < d; j += TEAM) { const double bd = (double)(rowp[j] - (T)cx[j]); nb2 = fma(bd, bd, nb2); }
+            nb2 += nb2b;
         }
         nb2 = warp_sum(nb2);
+        if (TEAM != 32) {                                  // warps of the CTA in index order
+            __syncthreads();
+            if (lane == 0) red[warp] = nb2;
+            __syncthreads();
+            nb2 = 0.0;
+#pragma unroll
+            for (int w = 0; w < CG_WARPS; ++w) nb2 += red[w];
+        }
         const double inv = 1.0 / sqrt(nb2);                // B3: nb > |a| >= 0
-        for (int j = lane; j < a.dpad; j += 32) wrow[j] = j < d ? wrow[j] * inv : 0.0;
-        if (lane == 0) a.rho_c[k] = rho;
+#pragma unroll 4
+        for (int j = tt; j < a.dpad; j += TEAM) {
+            double wv = 0.0;
+            if (j < d) {
+                T bq = rowp[j] - (T)cx[j];
+                if (vrow) bq = fma(vrow[j], inv_sig, bq);
+                wv = (double)bq * inv;
+            }
+            wrow[j] = wv;
+        }
+        if (tt == 0) a.rho_c[k] = rho;
     }
 }
 
@@ -98,8 +133,7 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* bar, unsigned int tar
         long long spins = 0;
         while (*reinterpret_cast<volatile unsigned int*>(&bar[0]) < target) {
             if (*reinterpret_cast<volatile unsigned int*>(&bar[1]) != 0u) { ok = 0; break; }
-            if (++spins > 400000000LL) { atomicExch(&bar[1], 1u); ok = 0; break; }
-            __nanosleep(20);
+            if (++spins > 2000000000LL) { atomicExch(&bar[1], 1u); ok = 0; break; }
         }
         __threadfence();
         ok_s = ok;
@@ -165,26 +199,66 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         // (a B1 row is stored as zeros: y = 0 and coef w = 0 whatever coef is)
         const double q0 = p_s[0];
         double ys = 0.0;
-        for (int k = r0 + warp; k < r1; k += CG_WARPS) {
-            const double* wrow = a.W + (size_t)k * dpad;
-            double y = 0.0;
-            for (int j = lane; j < d; j += 32) y = fma(wrow[j], p_s[1 + j], y);
-            y = warp_sum(y);
-            if (lane == 0) coef_s[k - r0] = q0 - a.rho_c[k] * y;
-            ys += y;
+        if (d >= 2048) {
+            // long rows (a CTA holds one or two of them): all threads on one row, four loads in flight per thread
+            for (int k = r0; k < r1; ++k) {
+                const double* __restrict__ wrow = a.W + (size_t)k * dpad;
+                double y0 = 0.0, y1 = 0.0, y2 = 0.0, y3 = 0.0;
+                int j = tid;
+                for (; j + 3 * CG_THREADS < d; j += 4 * CG_THREADS) {
+                    const double w0 = wrow[j], w1 = wrow[j + CG_THREADS], w2 = wrow[j + 2 * CG_THREADS], w3 = wrow[j + 3 * CG_THREADS];
+                    y0 = fma(w0, p_s[1 + j], y0); y1 = fma(w1, p_s[1 + j + CG_THREADS], y1);
+                    y2 = fma(w2, p_s[1 + j + 2 * CG_THREADS], y2); y3 = fma(w3, p_s[1 + j + 3 * CG_THREADS], y3);
+                }
+                for (; j < d; j += CG_THREADS) y0 = fma(wrow[j], p_s[1 + j], y0);
+                const double y = cta_sum((y0 + y1) + (y2 + y3), red);
+                if (tid == 0) coef_s[k - r0] = q0 - a.rho_c[k] * y;
+                if (warp == 0) ys += y;                      // counted once (warp 0's slot below)
+            }
+        } else {
+            for (int k = r0 + warp; k < r1; k += CG_WARPS) {
+                const double* __restrict__ wrow = a.W + (size_t)k * dpad;
+                double y0 = 0.0, y1 = 0.0;
+                int j = lane;
+                for (; j + 96 < d; j += 128) {
+                    const double w0 = wrow[j], w1 = wrow[j + 32], w2 = wrow[j + 64], w3 = wrow[j + 96];
+                    y0 = fma(w0, p_s[1 + j], y0); y1 = fma(w1, p_s[1 + j + 32], y1);
+                    y0 = fma(w2, p_s[1 + j + 64], y0); y1 = fma(w3, p_s[1 + j + 96], y1);
+                }
+                for (; j < d; j += 32) y0 = fma(wrow[j], p_s[1 + j], y0);
+                const double y = warp_sum(y0 + y1);
+                if (lane == 0) coef_s[k - r0] = q0 - a.rho_c[k] * y;
+                ys += y;
+            }
         }
         if (lane == 0) ysum_w[warp] = ys;
         __syncthreads();
         // ---- phase B (thread per column): z_j = sum_k coef_k W[k][j], rows in index order ----
-        for (int j = tid; j < d; j += CG_THREADS) {
-            double z = 0.0;
-            for (int k = r0; k < r1; ++k) z = fma(coef_s[k - r0], a.W[(size_t)k * dpad + j], z);
-            zp[j] = z;
+        {
+            const double* __restrict__ Wr = a.W;
+            double* __restrict__ zpr = zp;
+            int j = tid;
+            for (; j + 3 * CG_THREADS < d; j += 4 * CG_THREADS) {     // four columns per thread and sweep: loads first
+                double z0 = 0.0, z1 = 0.0, z2 = 0.0, z3 = 0.0;
+                for (int k = r0; k < r1; ++k) {
+                    const double ck = coef_s[k - r0];
+                    const double* wk = Wr + (size_t)k * dpad + j;
+                    const double w0 = wk[0], w1 = wk[CG_THREADS], w2 = wk[2 * CG_THREADS], w3 = wk[3 * CG_THREADS];
+                    z0 = fma(ck, w0, z0); z1 = fma(ck, w1, z1); z2 = fma(ck, w2, z2); z3 = fma(ck, w3, z3);
+                }
+                zpr[j] = z0; zpr[j + CG_THREADS] = z1; zpr[j + 2 * CG_THREADS] = z2; zpr[j + 3 * CG_THREADS] = z3;
+            }
+            for (; j < d; j += CG_THREADS) {
+                double z = 0.0;
+                for (int k = r0; k < r1; ++k) z = fma(coef_s[k - r0], Wr[(size_t)k * dpad + j], z);
+                zpr[j] = z;
+            }
         }
         if (tid == 0) { double t = 0.0; for (int w = 0; w < CG_WARPS; ++w) t += ysum_w[w]; sp_y[b] = t; }
         if (G > 1) { bars += G; ok = grid_barrier(a.bar, bars); if (!ok) break; } else __syncthreads();
         // ---- my slice of Hp (raw units), <p, Hp> partial ----
         double pHp = 0.0;
+#pragma unroll 2
         for (int e = c0 + tid; e < c1; e += CG_THREADS) {
             double hp;
             if (e == 0) {
@@ -207,11 +281,15 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         for (int bb = 0; bb < G; ++bb) tot += sp_pHp[bb];
         const double alpha = rr / tot;
         double rrn = 0.0;
-        for (int e = c0 + tid; e < c1; e += CG_THREADS) {
-            a.v.delta[e] = fma(alpha, p_s[e], a.v.delta[e]);
-            const double rj = fma(-alpha, a.v.Hp[e], a.v.res[e]);
-            a.v.res[e] = rj;
-            rrn = fma(rj, rj, rrn);
+        {
+            double* __restrict__ dl = a.v.delta; double* __restrict__ rs = a.v.res; const double* __restrict__ hpv = a.v.Hp;
+#pragma unroll 4
+            for (int e = c0 + tid; e < c1; e += CG_THREADS) {
+                dl[e] = fma(alpha, p_s[e], dl[e]);
+                const double rj = fma(-alpha, hpv[e], rs[e]);
+                rs[e] = rj;
+                rrn = fma(rj, rj, rrn);
+            }
         }
         rrn = cta_sum(rrn, red);
         if (tid == 0) sp_rr[b] = rrn;
@@ -219,7 +297,17 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         double rr_new = 0.0;
         for (int bb = 0; bb < G; ++bb) rr_new += sp_rr[bb];
         const double beta = rr_new / rr;
-        for (int j = tid; j < n1d; j += CG_THREADS) p_s[j] = fma(beta, p_s[j], a.v.res[j]);
+        {
+            const double* __restrict__ rs = a.v.res;
+            int j = tid;
+            for (; j + 3 * CG_THREADS < n1d; j += 4 * CG_THREADS) {
+                const double r0v = rs[j], r1v = rs[j + CG_THREADS], r2v = rs[j + 2 * CG_THREADS], r3v = rs[j + 3 * CG_THREADS];
+                p_s[j] = fma(beta, p_s[j], r0v); p_s[j + CG_THREADS] = fma(beta, p_s[j + CG_THREADS], r1v);
+                p_s[j + 2 * CG_THREADS] = fma(beta, p_s[j + 2 * CG_THREADS], r2v);
+                p_s[j + 3 * CG_THREADS] = fma(beta, p_s[j + 3 * CG_THREADS], r3v);
+            }
+            for (; j < n1d; j += CG_THREADS) p_s[j] = fma(beta, p_s[j], rs[j]);
+        }
         rr = rr_new;
         ++it;
         __syncthreads();
@@ -259,8 +347,12 @@ int meb_launch_cg(meb_ctx* ctx, const EvalCall& c, double* W, int64_t wc_cap, do
     const int ggrid = (int)((wc_cap + CG_WARPS - 1) / CG_WARPS < 4 * grid ? ((wc_cap + CG_WARPS - 1) / CG_WARPS) : 4 * grid);
     MEB_CUDA_OK(ctx, cudaMemsetAsync(bar, 0, 2 * sizeof(unsigned int), ctx->stream));
     ctx->launches++;
-    if (c.prec == MEB_FP64) cg_gather_kernel<double><<<ggrid < 1 ? 1 : ggrid, CG_THREADS, 0, ctx->stream>>>(a);
-    else cg_gather_kernel<float><<<ggrid < 1 ? 1 : ggrid, CG_THREADS, 0, ctx->stream>>>(a);
+    if (c.d >= 2048) {                                       // CTA per row
+        const int gg = (int)(wc_cap < 4 * grid ? wc_cap : 4 * grid);
+        if (c.prec == MEB_FP64) cg_gather_kernel<double, CG_THREADS><<<gg < 1 ? 1 : gg, CG_THREADS, 0, ctx->stream>>>(a);
+        else cg_gather_kernel<float, CG_THREADS><<<gg < 1 ? 1 : gg, CG_THREADS, 0, ctx->stream>>>(a);
+    } else if (c.prec == MEB_FP64) cg_gather_kernel<double, 32><<<ggrid < 1 ? 1 : ggrid, CG_THREADS, 0, ctx->stream>>>(a);
+    else cg_gather_kernel<float, 32><<<ggrid < 1 ? 1 : ggrid, CG_THREADS, 0, ctx->stream>>>(a);
     MEB_CUDA_OK(ctx, cudaGetLastError());
     // rows per CTA: 64 KB of W while CTAs are left, wc_cap / grid once all of them take part
     a.rper_cap = (int32_t)(65536 / ((size_t)a.dpad * 8) + 2);

@@ -63,6 +63,8 @@ struct SolverDev {
     double ag_t, ag_Lip;          // momentum parameter t_j, current estimate of the Lipschitz constant of grad Psi
     double ag_psi_y, ag_gg_y;     // Psi(y), ||grad Psi(y)||^2 of the extrapolated point
     int32_t ag_bt, ag_inner_max;  // doublings of Lip at the current y; iteration cap of one inner solve
+    long long m_rows;             // balls of this phase's problem
+    int32_t lowprec, pad_lp;      // 1: low-precision run: it only has to deliver (r_hat, c_hat) for the screening
 };
 
 // (d+1)-vectors of the state, each of length nv = n rounded up to 8, in one device array
@@ -123,9 +125,11 @@ __device__ __forceinline__ void ctrl_to_raw(const SolverDev* S, const SolverVecs
 // written before (by the host, by a set-up kernel, or by the previous phase).  Any CTA size.
 __device__ inline void meb_ctrl_init_dev(SolverDev* S, const SolverVecs v, double sigma0, int cur, int has_mult) {
     const int n = S->n;
+    _Pragma("unroll 4")
     for (int j = threadIdx.x; j < n; j += blockDim.x) v.xbar[j] = v.xn[j];
     ctrl_to_raw(S, v, v.xn, v.x_raw);
     __syncthreads();
+    _Pragma("unroll 4")
     for (int j = threadIdx.x; j < n; j += blockDim.x) v.xbar_raw[j] = v.x_raw[j];
     if (threadIdx.x == 0) {
         S->sigma = sigma0;
@@ -184,6 +188,7 @@ __device__ __forceinline__ void ctrl_arm_multi(SolverDev* S, double eta, int ls,
     for (int k = 0; k < MEB_MULTI_MAX; ++k) { f *= 0.5; S->dyn.multi_gamma[k] = eta * (1.0 - f); }
     S->dyn.dir_r = dir_r;
     S->dyn.dir_c2 = dir_c2;
+    S->dyn.dir_c = sqrt(dir_c2);
 }
 
 // relative KKT residual (reading 7) from the scalars of an evaluation
@@ -214,6 +219,18 @@ __device__ inline void ctrl_after_eval(SolverDev* Sg, SolverDev* S, const Solver
 }
 __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, const double* ev_s, double* sm) {
     __syncthreads();
+    double* __restrict__ xn_ = v.xn;
+    double* __restrict__ xbar_ = v.xbar;
+    double* __restrict__ ab_ = v.ab;
+    double* __restrict__ delta_ = v.delta;
+    double* __restrict__ g_ = v.g;
+    double* __restrict__ xt_ = v.xt;
+    double* __restrict__ x_raw_ = v.x_raw;
+    double* __restrict__ off_ = v.off;
+    double* __restrict__ grad_t_ = v.grad_t;
+    double* __restrict__ res_ = v.res;
+    double* __restrict__ p_ = v.p;
+    double* __restrict__ Hp_ = v.Hp;
     const int n = S->n;
     const int phase = S->phase;
     const double Ls = S->L;
@@ -226,13 +243,14 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         // the pass evaluated Psi and its gradient at y = v.xt: candidate x+ = y - grad Psi(y) / Lip
         double gg = 0.0;
         const double il = 1.0 / S->ag_Lip;
+        _Pragma("unroll 4")
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
-            const double gj = v.grad_t[j], yj = v.xt[j];
-            v.res[j] = gj; v.p[j] = yj;
+            const double gj = grad_t_[j], yj = xt_[j];
+            res_[j] = gj; p_[j] = yj;
             gg = fma(gj, gj, gg);
             const double xj = fma(-il, gj, yj);
-            v.xt[j] = xj;
-            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+            xt_[j] = xj;
+            x_raw_[j] = (j == 0) ? Ls * xj : ((use_off ? off_[j - 1] : 0.0) + Ls * xj);
         }
         gg = ctrl_block_sum(gg, sm);
         if (threadIdx.x == 0) {
@@ -249,10 +267,11 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
         // and re-evaluate at x (the records of this pass are not those of x)
         const bool giveup = S->ag_bt >= 60;
         const double il = 1.0 / (2.0 * S->ag_Lip);
+        _Pragma("unroll 4")
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
-            const double xj = giveup ? v.xn[j] : fma(-il, v.res[j], v.p[j]);
-            v.xt[j] = xj;
-            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
+            const double xj = giveup ? xn_[j] : fma(-il, res_[j], p_[j]);
+            xt_[j] = xj;
+            x_raw_[j] = (j == 0) ? Ls * xj : ((use_off ? off_[j - 1] : 0.0) + Ls * xj);
         }
         __syncthreads();
         if (threadIdx.x == 0) {
@@ -293,8 +312,9 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
             const int np = S->pred_n;
             if (np > 0) {
                 double A = 0.0, B = 0.0, D = 0.0;
+                _Pragma("unroll 4")
                 for (int j = threadIdx.x; j < n; j += blockDim.x) {
-                    const double w = v.xn[j] - v.xbar[j], dj = v.delta[j];
+                    const double w = xn_[j] - xbar_[j], dj = delta_[j];
                     A = fma(w, w, A); B = fma(w, dj, B); D = fma(dj, dj, D);
                 }
                 ctrl_block_sum3(A, B, D, sm);
@@ -304,24 +324,25 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
                 for (int k = 0; k < np; ++k) {
                     ek *= 0.5;
                     if (S->ls + 1 + skip >= S->armijo_max) break;             // the last allowed halving is always evaluated
-                    const double lb = v.xn[0] + ek * v.delta[0] + cs * S->pred_s[k] + cp * (A + ek * (2.0 * B + ek * D));
+                    const double lb = xn_[0] + ek * delta_[0] + cs * S->pred_s[k] + cp * (A + ek * (2.0 * B + ek * D));
                     if (lb > S->psi_cur + S->armijo_mu * ek * S->slope) ++skip; else break;
                 }
                 for (int q = 0; q < skip; ++q) eta *= 0.5;
             }
         }
         double dx2t = 0.0;
+        _Pragma("unroll 4")
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
-            const double xj = v.xn[j] + eta * v.delta[j];
-            v.xt[j] = xj;
-            v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
-            const double dxb = xj - v.xbar[j];
+            const double xj = xn_[j] + eta * delta_[j];
+            xt_[j] = xj;
+            x_raw_[j] = (j == 0) ? Ls * xj : ((use_off ? off_[j - 1] : 0.0) + Ls * xj);
+            const double dxb = xj - xbar_[j];
             dx2t = fma(dxb, dxb, dx2t);
         }
         dx2t = ctrl_block_sum(dx2t, sm);
         __syncthreads();
         if (threadIdx.x == 0) {
-            ctrl_arm_abort(S, !stalled, v.xn[0] + eta * v.delta[0], dx2t);
+            ctrl_arm_abort(S, !stalled, xn_[0] + eta * delta_[0], dx2t);
             if (stalled) { S->phase = PH_REEVAL; } else {
                 S->eta = eta; S->ls += 1 + skip; S->skipped += skip;
                 ctrl_arm_multi(S, eta, S->ls, S->dyn.dir_r, S->dyn.dir_c2);
@@ -337,17 +358,18 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     double agx = 0.0, gg = 0.0, dx2 = 0.0, dotr = 0.0;
     const bool take_xt = phase == PH_ARMIJO || phase == PH_AG_X;
     const bool agmode = S->outer < S->ag_outer;
+    _Pragma("unroll 4")
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
-        const double xj = take_xt ? v.xt[j] : v.xn[j];
-        const double gj = v.grad_t[j];
-        const double abj = v.ab[j], xbj = v.xbar[j];
+        const double xj = take_xt ? xt_[j] : xn_[j];
+        const double gj = grad_t_[j];
+        const double abj = ab_[j], xbj = xbar_[j];
         if (agmode) {                                   // previous iterate, and <grad Psi(y), x+ - x> for the restart test
-            const double xp = v.xn[j];
-            v.Hp[j] = xp;
-            if (phase == PH_AG_X) dotr = fma(v.res[j], xj - xp, dotr);
+            const double xp = xn_[j];
+            Hp_[j] = xp;
+            if (phase == PH_AG_X) dotr = fma(res_[j], xj - xp, dotr);
         }
-        if (take_xt) v.xn[j] = xj;
-        v.g[j] = gj;
+        if (take_xt) xn_[j] = xj;
+        g_[j] = gj;
         agx = fma(abj - xj, gj, agx);
         gg = fma(gj, gj, gg);
         const double dx = xj - xbj;
@@ -411,26 +433,35 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     if (sm[97] != 0.0) {                                    // accelerated gradient: the next point to evaluate
         const bool extrap = sm[97] == 2.0;
         const double beta = sm[98], il = 1.0 / S->ag_Lip;
+        _Pragma("unroll 4")
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
-            const double xj = v.xn[j];
+            const double xj = xn_[j];
             double tj;
-            if (extrap) tj = fma(beta, xj - v.Hp[j], xj);                      // y = x+ + beta (x+ - x)
-            else { const double gj = v.grad_t[j]; v.res[j] = gj; v.p[j] = xj; tj = fma(-il, gj, xj); }
-            v.xt[j] = tj;
-            v.x_raw[j] = (j == 0) ? Ls * tj : ((use_off ? v.off[j - 1] : 0.0) + Ls * tj);
+            if (extrap) tj = fma(beta, xj - Hp_[j], xj);                      // y = x+ + beta (x+ - x)
+            else { const double gj = grad_t_[j]; res_[j] = gj; p_[j] = xj; tj = fma(-il, gj, xj); }
+            xt_[j] = tj;
+            x_raw_[j] = (j == 0) ? Ls * tj : ((use_off ? off_[j - 1] : 0.0) + Ls * tj);
         }
     } else if (S->action == ACT_NEWTON && !S->dense)
+        _Pragma("unroll 4")
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
-            const double gj = v.grad_t[j];
-            v.delta[j] = 0.0;
-            v.res[j] = -gj;
-            v.p[j] = -gj;
+            const double gj = grad_t_[j];
+            delta_[j] = 0.0;
+            res_[j] = -gj;
+            p_[j] = -gj;
         }
 }
 
 // Controller step after a Newton solve (Alg. 2 line 9): slope <g, Delta>, first Armijo trial x + Delta.
 // z: Delta (n doubles, shared or global).  S may live in global or shared memory.  CTA of 256 threads.
 __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs v, const double* z, int n) {
+    double* __restrict__ xn_ = v.xn;
+    double* __restrict__ xbar_ = v.xbar;
+    double* __restrict__ g_ = v.g;
+    double* __restrict__ xt_ = v.xt;
+    double* __restrict__ x_raw_ = v.x_raw;
+    double* __restrict__ off_ = v.off;
+    double* __restrict__ dir_raw_ = v.dir_raw;
     __shared__ double red[8], red2[8];
     const int tid = threadIdx.x;
     const double Ls = S->L;
@@ -439,12 +470,12 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
     double sl = 0.0, dx2t = 0.0, dc2 = 0.0;
     for (int j = tid; j < n; j += 256) {
         const double dj = z[j];
-        sl = fma(v.g[j], dj, sl);
-        const double xj = v.xn[j] + dj;
-        v.xt[j] = xj;
-        v.x_raw[j] = (j == 0) ? Ls * xj : ((use_off ? v.off[j - 1] : 0.0) + Ls * xj);
-        v.dir_raw[j] = Ls * dj;
-        const double dxb = xj - v.xbar[j];
+        sl = fma(g_[j], dj, sl);
+        const double xj = xn_[j] + dj;
+        xt_[j] = xj;
+        x_raw_[j] = (j == 0) ? Ls * xj : ((use_off ? off_[j - 1] : 0.0) + Ls * xj);
+        dir_raw_[j] = Ls * dj;
+        const double dxb = xj - xbar_[j];
         dx2t = fma(dxb, dxb, dx2t);
         if (j > 0) dc2 = fma(dj, dj, dc2);
     }
@@ -456,7 +487,7 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
     if (tid == 0) {
         double t = 0.0, t2 = 0.0, t3 = 0.0;
         for (int w = 0; w < 8; ++w) { t += red[w]; t2 += red2[w]; t3 += red3[w]; }
-        ctrl_arm_abort(S, true, v.xn[0] + z[0], t2);
+        ctrl_arm_abort(S, true, xn_[0] + z[0], t2);
         S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
         S->tiny = (-t <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;
         ctrl_arm_multi(S, 1.0, 0, Ls * z[0], Ls * Ls * t3);
@@ -468,6 +499,14 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
 // logic (reading 18), sigma update, start of the next outer iteration.  Every thread of the CTA
 // calls it; S may live in global or shared memory; nact = number of active balls of the accepted pass.
 __device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs v, long long nact) {
+    double* __restrict__ xn_ = v.xn;
+    double* __restrict__ xbar_ = v.xbar;
+    double* __restrict__ ab_ = v.ab;
+    double* __restrict__ g_ = v.g;
+    double* __restrict__ x_raw_ = v.x_raw;
+    double* __restrict__ xbar_raw_ = v.xbar_raw;
+    double* __restrict__ off_ = v.off;
+    double* __restrict__ xbest_ = v.xbest;
     const int n = S->n;
     const int nxt = S->dyn.has_mult ? 1 - S->dyn.cur : 0;
     const bool fits = nact <= S->vcap[nxt];
@@ -493,19 +532,25 @@ __device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs 
     if (kkt <= S->tol) status = ST_CONVERGED;
     else if (stall >= 3 && best <= S->tol_accept) status = ST_CONVERGED;     // floor of the arithmetic (reading 18)
     else if (stall >= S->stall_max) status = ST_STALLED;
+    // reading 17: a low-precision run whose support is a large part of ALL balls (degenerate: co-spherical points)
+    // cannot resolve multipliers of size 1/|support| and will not reach tol_lo (config 4: its third outer iteration
+    // alone spends 60 passes on line searches in rounding noise): two outer iterations give the (r_hat, c_hat) the
+    // screening needs.  The a-posteriori check makes the result independent of this.
+    else if (S->lowprec && outer1 >= 2 && 10.0 * v.ev[MEB_EV_N_ACTIVE] > (double)S->m_rows) status = ST_STALLED;
     else if (outer1 >= S->outer_max) status = (best <= S->tol_accept) ? ST_CONVERGED : ST_OUTER_CAP;
     const bool take_best = status != ST_RUNNING && !improved && kkt > S->tol;
     __syncthreads();
+    _Pragma("unroll 4")
     for (int j = threadIdx.x; j < n; j += blockDim.x) {
-        const double xj = v.xn[j];
-        v.ab[j] -= sg * v.g[j];
-        if (improved) v.xbest[j] = xj;
-        const double xo = take_best ? v.xbest[j] : xj;
-        if (take_best) v.xn[j] = xo;
-        v.xbar[j] = xo;
-        const double xr = (j == 0) ? S->L * xo : ((S->use_off ? v.off[j - 1] : 0.0) + S->L * xo);
-        v.x_raw[j] = xr;
-        v.xbar_raw[j] = xr;
+        const double xj = xn_[j];
+        ab_[j] -= sg * g_[j];
+        if (improved) xbest_[j] = xj;
+        const double xo = take_best ? xbest_[j] : xj;
+        if (take_best) xn_[j] = xo;
+        xbar_[j] = xo;
+        const double xr = (j == 0) ? S->L * xo : ((S->use_off ? off_[j - 1] : 0.0) + S->L * xo);
+        x_raw_[j] = xr;
+        xbar_raw_[j] = xr;
     }
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -157,6 +157,7 @@ struct MebDyn {
     double multi_gamma[MEB_MULTI_MAX];
     double dir_r;           // Delta r (raw units)
     double dir_c2;          // ||Delta c||^2 (raw units)
+    double dir_c;           // ||Delta c||
 };
 
 // host-side launch helpers implemented in the .cu files -------------------------------------------

@@ -159,7 +159,11 @@ __global__ void __launch_bounds__(LONG_THREADS, 1) long_kernel(const StreamArgs 
     int q = 0;
     // rows per batch: 32 for rows of a few KB, fewer for very long rows (the early stop of a doomed trial is
     // tested once per batch)
-    const int qmax = cfg.data_bytes >= 131072u ? 1 : (131072u / cfg.data_bytes > 32u ? 32 : (int)(131072u / cfg.data_bytes));
+    int qmax = cfg.data_bytes >= 131072u ? 1 : (131072u / cfg.data_bytes > 32u ? 32 : (int)(131072u / cfg.data_bytes));
+    {   // at least four batches per warp, so that a doomed trial of a small problem can still be cut
+        const int64_t per_warp = (m + (int64_t)gridDim.x * W - 1) / ((int64_t)gridDim.x * W);
+        if (per_warp < 4 * (int64_t)qmax) qmax = per_warp >= 4 ? (int)(per_warp / 4) : 1;
+    }
     int64_t my_row = -1;
     T my_nb2 = T(0), my_f0 = T(0), my_p0 = T(0), ri = T(0), ui = T(0);
     int myslot = -1;
@@ -279,7 +283,9 @@ __global__ void __launch_bounds__(LONG_THREADS, 1) long_kernel(const StreamArgs 
 // vlist[0 .. *vcount): ascending indices of the balls with slot >= 0.  CTA b writes its partial to
 // part[(part_base + b) * MEB_NPART ...] (zeros when it has no entry): the finalize kernel adds them after the
 // partials of the streaming kernel.
-template <typename T, bool MULTI>
+// TEAM = 32: warp per entry; TEAM = MEB_BLOCK: the whole CTA per entry (rows of 16 KB and more: one warp would need
+// dozens of dependent-latency rounds per row).
+template <typename T, bool MULTI, int TEAM>
 __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, const int32_t* __restrict__ vlist,
                                                          const int32_t* __restrict__ vcount, int part_base, int multi) {
     typedef typename VecOf<T>::type V4;
@@ -306,8 +312,11 @@ __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, 
                         ((uintptr_t)C % 16 == 0) && ((uintptr_t)V % 16 == 0);
     Acc acc;
     MultiAcc<MULTI> macc;
-    const int nwarps = gridDim.x * MEB_WARPS;
-    for (int k = blockIdx.x * MEB_WARPS + warp; k < n; k += nwarps) {
+    __shared__ double vred[MEB_WARPS][5];
+    constexpr int TPB = MEB_BLOCK / TEAM;
+    const int tt = TEAM == 32 ? lane : (int)threadIdx.x;
+    const int nteams = gridDim.x * TPB;
+    for (int k = blockIdx.x * TPB + (TEAM == 32 ? warp : 0); k < n; k += nteams) {
         const int64_t row = vl[k];
         const int slot = a.v_slot[row];
         if (slot < 0) continue;                    // (a stale list entry cannot happen; defensive)
@@ -322,11 +331,11 @@ __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, 
         };
         if (vec_ok) {
             const int nchunks = d / VEC;
-            for (int c0 = lane; c0 < nchunks; c0 += 32 * 4) {
+            for (int c0 = tt; c0 < nchunks; c0 += TEAM * 4) {
                 V4 e[4], v[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const int c = c0 + 32 * u;
+                    const int c = c0 + TEAM * u;
                     if (c < nchunks) {
                         e[u] = ldg_stream(reinterpret_cast<const V4*>(rowp) + c);
                         v[u] = ldg_stream(reinterpret_cast<const V4*>(vrow) + c);
@@ -334,7 +343,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, 
                 }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const int c = c0 + 32 * u;
+                    const int c = c0 + TEAM * u;
                     if (c < nchunks) {
                         const T* ep = reinterpret_cast<const T*>(&e[u]);
                         const T* vp = reinterpret_cast<const T*>(&v[u]);
@@ -343,9 +352,9 @@ __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, 
                     }
                 }
             }
-            for (int col = nchunks * VEC + lane; col < d; col += 32) elem(__ldg(rowp + col), __ldg(vrow + col), col);
+            for (int col = nchunks * VEC + tt; col < d; col += TEAM) elem(__ldg(rowp + col), __ldg(vrow + col), col);
         } else {
-            for (int col = lane; col < d; col += 32) elem(__ldg(rowp + col), __ldg(vrow + col), col);
+            for (int col = tt; col < d; col += TEAM) elem(__ldg(rowp + col), __ldg(vrow + col), col);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -355,7 +364,17 @@ __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, 
             vv += __shfl_xor_sync(MEB_FULL_MASK, vv, o);
             if (MULTI) p0 += __shfl_xor_sync(MEB_FULL_MASK, p0, o);
         }
-        if (lane == 0) {
+        if (TEAM != 32) {                                   // warps of the CTA in index order
+            __syncthreads();
+            if (lane == 0) { vred[warp][0] = (double)nb2; vred[warp][1] = (double)ne2; vred[warp][2] = (double)evd; vred[warp][3] = (double)vv; vred[warp][4] = (double)p0; }
+            __syncthreads();
+            double t5[5] = {0, 0, 0, 0, 0};
+            for (int w = 0; w < MEB_WARPS; ++w)
+#pragma unroll
+                for (int q5 = 0; q5 < 5; ++q5) t5[q5] += vred[w][q5];
+            nb2 = (T)t5[0]; ne2 = (T)t5[1]; evd = (T)t5[2]; vv = (T)t5[3]; p0 = (T)t5[4];
+        }
+        if (tt == 0) {
             const T ri = Rg ? Rg[row] : T(0);
             const T ui = Ug ? Ug[row] : T(0);
             double mylam;
@@ -505,14 +524,13 @@ int meb_launch_long(meb_ctx* ctx, int op, int prec, const StreamArgs& a, const i
     if (rc != MEB_OK) return rc;
     if (op == OP_EVAL && (a.v_slot != nullptr || a.dyn != nullptr)) {
         const int gv = 32;                                        // 256 warps: supports of a few thousand rows at most
+        const bool wide = c.data_bytes >= 16384u;                 // CTA per entry
         ctx->launches++;
-        if (prec == MEB_FP64) {
-            if (multi > 0) vrow_kernel<double, true><<<gv, MEB_BLOCK, 0, ctx->stream>>>(b, vlist, vcount, grid, multi);
-            else vrow_kernel<double, false><<<gv, MEB_BLOCK, 0, ctx->stream>>>(b, vlist, vcount, grid, 0);
-        } else {
-            if (multi > 0) vrow_kernel<float, true><<<gv, MEB_BLOCK, 0, ctx->stream>>>(b, vlist, vcount, grid, multi);
-            else vrow_kernel<float, false><<<gv, MEB_BLOCK, 0, ctx->stream>>>(b, vlist, vcount, grid, 0);
-        }
+#define MEB_VROW(T, M) do { if (wide) vrow_kernel<T, M, MEB_BLOCK><<<gv, MEB_BLOCK, 0, ctx->stream>>>(b, vlist, vcount, grid, multi); \
+                            else vrow_kernel<T, M, 32><<<gv, MEB_BLOCK, 0, ctx->stream>>>(b, vlist, vcount, grid, multi); } while (0)
+        if (prec == MEB_FP64) { if (multi > 0) MEB_VROW(double, true); else MEB_VROW(double, false); }
+        else { if (multi > 0) MEB_VROW(float, true); else MEB_VROW(float, false); }
+#undef MEB_VROW
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
         grid += gv;

@@ -163,7 +163,7 @@ __device__ __forceinline__ void multi_row(MultiAcc<true>& ma, const StreamArgs& 
     const T dr = (T)a.dyn->dir_r, dc2 = (T)a.dyn->dir_c2;
     {   // balls that stay strictly inside at every predicted point add exactly zero: ||b + g dc|| <= ||b|| + g ||dc||
         const T gmax = (T)a.dyn->multi_gamma[nm - 1];
-        const T reach = t_sqrt<T>(nb2) + gmax * t_sqrt<T>(dc2);
+        const T reach = t_sqrt<T>(nb2) + gmax * (T)a.dyn->dir_c;
         const T amax = av + (dr > T(0) ? gmax * dr : T(0));
         if (reach <= -amax) return;
     }

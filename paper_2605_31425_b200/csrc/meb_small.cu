@@ -104,12 +104,15 @@ __global__ void __launch_bounds__(FBLOCK) eval_finalize_kernel(const FinalizeArg
             dx2 = dx * dx;
         }
     } else {
+        const double* __restrict__ xr = x; const double* __restrict__ xbr = xbar ? xbar : x;
+        double* __restrict__ gr = f.grad;
+#pragma unroll 4
         for (int j = threadIdx.x; j < d; j += FBLOCK) {
             double s = 0.0;
             for (int b = 0; b < nvec; ++b) s += part_vec[(size_t)b * dpad + j];
             const double sv = sigma * s;
-            const double dx = x[1 + j] - (xbar ? xbar[1 + j] : x[1 + j]);
-            f.grad[1 + j] = -sv + tos * dx;
+            const double dx = xr[1 + j] - xbr[1 + j];
+            gr[1 + j] = -sv + tos * dx;
             nv2 = fma(sv, sv, nv2);
             dx2 = fma(dx, dx, dx2);
         }

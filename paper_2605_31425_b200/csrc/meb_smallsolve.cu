@@ -637,7 +637,7 @@ extern "C" int meb_solve_batch(meb_ctx* ctx, int32_t nprob, const int64_t* h_row
     ht.n = n; ht.d = d; ht.inner_max = par.inner_max; ht.outer_max = par.outer_max; ht.armijo_max = par.armijo_max_halvings;
     ht.cg_max = par.cg_max; ht.dense = 1; ht.use_off = 1; ht.in_graph = 0;
     ht.eval_cap = 4 * par.outer_max * (par.inner_max + 2);
-    ht.multi_max = 0; ht.pred_margin = 1e-6; ht.ag_outer = 0;
+    ht.multi_max = 0; ht.pred_margin = 1e-6; ht.ag_outer = 0; ht.lowprec = 0; ht.m_rows = 0;
     MEB_CUDA_OK(ctx, cudaMemcpyAsync(base + o_inst, hi.data(), (size_t)nprob * sizeof(BatchInst), cudaMemcpyHostToDevice, ctx->stream));
     MEB_CUDA_OK(ctx, cudaMemcpyAsync(base + o_tmpl, &ht, sizeof(ht), cudaMemcpyHostToDevice, ctx->stream));
     const BatchInst* dinst = (const BatchInst*)(base + o_inst);

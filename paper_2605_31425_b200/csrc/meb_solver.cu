@@ -165,6 +165,13 @@ int add_conditional(meb_ctx* ctx, cudaGraph_t parent, cudaGraphConditionalHandle
     return MEB_OK;
 }
 
+// predictions per Armijo trial pass (meb_params.armijo_multi; -1: on for long rows only)
+int multi_of(const meb_params& par, const Problem& P) {
+    int n = par.armijo_multi;
+    if (n < 0) n = ((size_t)P.ld * esz(P.prec) > 1024 || P.d > 256) ? MEB_MULTI_MAX : 0;
+    return n > MEB_MULTI_MAX ? MEB_MULTI_MAX : n;
+}
+
 // ---- launch sequences shared by the captured graph and the stepped (host-sequenced) driver ----------
 struct Seq {
     Solver* S; const Problem* P; bool dense;
@@ -181,7 +188,7 @@ void seq_init(Seq& q, Solver& S, const Problem& P, bool dense) {
         q.gs.U2[b] = P.U[b]; q.gs.slot2[b] = P.slot[b]; q.gs.V2[b] = P.V[b]; q.gs.vcap2[b] = P.vcap[b];
         q.gs.vlist2[b] = P.vlist[b]; q.gs.vcount2[b] = P.vcount[b];
     }
-    q.gs.multi = S.par.armijo_multi > 0 ? (S.par.armijo_multi < MEB_MULTI_MAX ? S.par.armijo_multi : MEB_MULTI_MAX) : 0;
+    q.gs.multi = multi_of(S.par, P);
     memset(&q.c, 0, sizeof(q.c));
     q.c.prec = P.prec; q.c.m = P.m; q.c.d = P.d; q.c.C = P.C; q.c.ld = P.ld; q.c.R = P.R; q.c.ldv = P.ldv;
     q.c.x = S.v.x_raw; q.c.xbar = S.v.xbar_raw; q.c.sigma = 1.0; q.c.tau = 1.0; q.c.gs = &q.gs;
@@ -543,7 +550,9 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             h->slope_floor = (P.prec == MEB_FP32) ? 1e-7 : 2e-15;
             h->abort_margin = ctx->opt[MEB_OPT_NO_ABORT] ? 0.0 : ((P.prec == MEB_FP32) ? 1e-3 : 1e-6);
             h->pred_margin = (P.prec == MEB_FP32) ? 1e-3 : 1e-6;
-            h->multi_max = (par.armijo_multi > 0 && !small) ? (par.armijo_multi < MEB_MULTI_MAX ? par.armijo_multi : MEB_MULTI_MAX) : 0;
+            h->m_rows = (ctx->shard && P.full) ? ctx->shard->m_global : P.m;      // (counts in v.ev are global in a sharded solve)
+            h->lowprec = (P.prec == MEB_FP32 && P.full) ? 1 : 0;
+            h->multi_max = small ? 0 : multi_of(par, P);
             h->ag_outer = (par.ag_outer > 0 && !small) ? par.ag_outer : 0;
             h->ag_inner_max = 500;
             h->stall_max = (P.prec == MEB_FP32) ? 3 : 6;   // the FP32 run only has to deliver a warm start
@@ -931,6 +940,9 @@ int solve_impl(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_
             }
             if (rc) break;
             ab = xn;                                        // reading 11
+            S.sigma_start = S.par.sigma0;
+            if (P2.has_mult && S.par.sigma_carry > 0.0 && S.par.sigma_carry * S.sigma_end > S.par.sigma0)
+                S.sigma_start = S.par.sigma_carry * S.sigma_end;
             for (int rnd = 0; rc == MEB_OK && rnd < S.par.max_rounds; ++rnd) {
                 P2.m = nred;
                 st->n_reduced = nred;

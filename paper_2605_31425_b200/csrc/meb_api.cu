@@ -193,24 +193,25 @@ static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, dou
         if (rcl != MEB_OK) return rcl;
         vlist = ctx->vlist; vcount = ctx->count_dev + 1;
     }
+    if (longk) { int rc0 = meb_launch_long(ctx, 0, op, prec, a, vlist, vcount, grid); if (rc0 != MEB_OK) return rc0; }
     if (ctx->time_passes) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     cudaStreamIsCapturing(ctx->stream, &cap);
     const bool pool = ctx->ev_record && !ctx->time_passes && ctx->evn < MEB_EVPOOL && cap == cudaStreamCaptureStatusNone;
     if (pool) MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn], ctx->stream));
     int rc = tile ? meb_launch_tile(ctx, op, prec, a, grid)
-                  : (longk ? meb_launch_long(ctx, op, prec, a, vlist, vcount, grid) : meb_launch_stream(ctx, op, prec, a, grid));
+                  : (longk ? meb_launch_long(ctx, 1, op, prec, a, vlist, vcount, grid) : meb_launch_stream(ctx, op, prec, a, grid));
     if (rc != MEB_OK) return rc;
     ctx->last_path = tile ? PATH_TILE : (longk ? PATH_LONG : PATH_STREAM);
     if (path_out) *path_out = ctx->last_path;
     if (pool) {
         MEB_CUDA_OK(ctx, cudaEventRecord(ctx->evpool[2 * ctx->evn + 1], ctx->stream));
         ctx->evclass[ctx->evn] = ctx->cur_class;
-        ctx->evbytes[ctx->evn] = bytes + (op == OP_EVAL ? ctx->ev_extra_bytes : 0.0);
+        // (long rows: the multiplier rows are read by vrow_kernel, outside the bracket)
+        ctx->evbytes[ctx->evn] = bytes + ((op == OP_EVAL && !longk) ? ctx->ev_extra_bytes : 0.0);
         ctx->evcut[ctx->evn] = false;
         ctx->evn++;
     }
-    ctx->last_grid = *grid;
     ctx->last_pass_bytes = bytes;
     ctx->list_valid = false;
     if (ctx->time_passes && cap == cudaStreamCaptureStatusNone) {
@@ -220,6 +221,11 @@ static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, dou
         MEB_CUDA_OK(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
         ctx->last_pass_ms = ms;
     }
+    if (longk) {                    // balls with a multiplier row: after the bracket, so that the events time the
+        rc = meb_launch_long(ctx, 2, op, prec, a, vlist, vcount, grid);      // streaming kernel alone
+        if (rc != MEB_OK) return rc;
+    }
+    ctx->last_grid = *grid;
     return MEB_OK;
 }
 

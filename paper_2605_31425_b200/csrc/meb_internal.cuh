@@ -216,8 +216,8 @@ int meb_launch_tile(meb_ctx* ctx, int op, int prec, const StreamArgs& a, int* gr
 // are multiples of 16 bytes.  The launcher zeroes a.mask, launches the streaming kernel and (evaluation with
 // multipliers) the kernel that handles the balls on vlist; *grid_out counts the partials of both.
 bool meb_long_applicable(int op, int prec, const StreamArgs& a);
-int meb_launch_long(meb_ctx* ctx, int op, int prec, const StreamArgs& a, const int32_t* vlist, const int32_t* vcount,
-                    int* grid_out);
+int meb_launch_long(meb_ctx* ctx, int phase, int op, int prec, const StreamArgs& a, const int32_t* vlist,
+                    const int32_t* vcount, int* grid_out);
 int meb_build_vlist(meb_ctx* ctx, const int32_t* slot, int64_t m, int32_t* vlist, int32_t* vcount);
 int meb_copy_vlist(meb_ctx* ctx, const int32_t* list, const int32_t* count, const MebDyn* dyn, int32_t* v0, int32_t* v1,
                    int32_t* c0, int32_t* c1, int64_t cap);

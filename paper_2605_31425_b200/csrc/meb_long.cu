@@ -481,9 +481,10 @@ bool meb_long_applicable(int op, int prec, const StreamArgs& a) {
     return make_long_cfg(a, esize, 0, &c);
 }
 
-// The mask must be zero before the launch (flags are OR-ed in).  Launches the streaming kernel and, for an
-// evaluation with multiplier rows, vrow_kernel over `vlist`; *grid_out = number of per-CTA partials written.
-int meb_launch_long(meb_ctx* ctx, int op, int prec, const StreamArgs& a, const int32_t* vlist, const int32_t* vcount,
+// Three steps, so that the caller can bracket the streaming kernel ALONE with its CUDA events:
+//   phase 0: zero the mask (flags are OR-ed in);  phase 1: the streaming kernel, *grid_out = its CTAs;
+//   phase 2: for an evaluation with multipliers, vrow_kernel over `vlist`; *grid_out += its CTAs (in: the grid of phase 1).
+int meb_launch_long(meb_ctx* ctx, int phase, int op, int prec, const StreamArgs& a, const int32_t* vlist, const int32_t* vcount,
                     int* grid_out) {
     const size_t esize = prec == MEB_FP64 ? 8 : 4;
     int multi = (op == OP_EVAL) ? a.multi : 0;
@@ -492,36 +493,43 @@ int meb_launch_long(meb_ctx* ctx, int op, int prec, const StreamArgs& a, const i
     if (multi == 0 && !make_long_cfg(a, esize, 0, &c)) return MEB_E_CAPACITY;
     StreamArgs b = a;
     b.multi = multi;
-    if (op != OP_INGEST) {
-        const size_t nwords = (size_t)(a.m + 31) / 32;
-        cudaError_t e = cudaMemsetAsync(a.mask, 0, nwords * sizeof(uint32_t), ctx->stream);
-        if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
-    }
-    int grid = 0, rc = MEB_E_ARG;
-    if (prec == MEB_FP64) {
-        switch (op) {
-            case OP_EVAL:
-                rc = multi > 0 ? launch_long(ctx, long_kernel<double, OP_EVAL, false, true>, b, c, &grid)
-                               : launch_long(ctx, long_kernel<double, OP_EVAL, false, false>, b, c, &grid);
-                break;
-            case OP_FEAS: rc = launch_long(ctx, long_kernel<double, OP_FEAS, false, false>, b, c, &grid); break;
-            case OP_INGEST:
-                rc = a.C32 ? launch_long(ctx, long_kernel<double, OP_INGEST, true, false>, b, c, &grid)
-                           : launch_long(ctx, long_kernel<double, OP_INGEST, false, false>, b, c, &grid);
-                break;
-            default: return MEB_E_ARG;
+    if (phase == 0) {
+        if (op != OP_INGEST) {
+            const size_t nwords = (size_t)(a.m + 31) / 32;
+            cudaError_t e = cudaMemsetAsync(a.mask, 0, nwords * sizeof(uint32_t), ctx->stream);
+            if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
         }
-    } else {
-        switch (op) {
-            case OP_EVAL:
-                rc = multi > 0 ? launch_long(ctx, long_kernel<float, OP_EVAL, false, true>, b, c, &grid)
-                               : launch_long(ctx, long_kernel<float, OP_EVAL, false, false>, b, c, &grid);
-                break;
-            case OP_SCREEN: rc = launch_long(ctx, long_kernel<float, OP_SCREEN, false, false>, b, c, &grid); break;
-            default: return MEB_E_ARG;
-        }
+        return MEB_OK;
     }
-    if (rc != MEB_OK) return rc;
+    if (phase == 1) {
+        int grid = 0, rc = MEB_E_ARG;
+        if (prec == MEB_FP64) {
+            switch (op) {
+                case OP_EVAL:
+                    rc = multi > 0 ? launch_long(ctx, long_kernel<double, OP_EVAL, false, true>, b, c, &grid)
+                                   : launch_long(ctx, long_kernel<double, OP_EVAL, false, false>, b, c, &grid);
+                    break;
+                case OP_FEAS: rc = launch_long(ctx, long_kernel<double, OP_FEAS, false, false>, b, c, &grid); break;
+                case OP_INGEST:
+                    rc = a.C32 ? launch_long(ctx, long_kernel<double, OP_INGEST, true, false>, b, c, &grid)
+                               : launch_long(ctx, long_kernel<double, OP_INGEST, false, false>, b, c, &grid);
+                    break;
+                default: return MEB_E_ARG;
+            }
+        } else {
+            switch (op) {
+                case OP_EVAL:
+                    rc = multi > 0 ? launch_long(ctx, long_kernel<float, OP_EVAL, false, true>, b, c, &grid)
+                                   : launch_long(ctx, long_kernel<float, OP_EVAL, false, false>, b, c, &grid);
+                    break;
+                case OP_SCREEN: rc = launch_long(ctx, long_kernel<float, OP_SCREEN, false, false>, b, c, &grid); break;
+                default: return MEB_E_ARG;
+            }
+        }
+        if (rc == MEB_OK) *grid_out = grid;
+        return rc;
+    }
+    int grid = *grid_out;
     if (op == OP_EVAL && (a.v_slot != nullptr || a.dyn != nullptr)) {
         const int gv = 32;                                        // 256 warps: supports of a few thousand rows at most
         const bool wide = c.data_bytes >= 16384u;                 // CTA per entry

@@ -324,6 +324,22 @@ MEB_API int meb_feasibility_check(meb_ctx* ctx, int64_t m, int32_t d, const doub
                           const uint8_t* kept_mask, double* h_delta_max, int32_t* h_argmax,
                           int32_t* viol_idx, int64_t cap, int64_t* h_n_viol);
 
+/* ---- a8': the feasibility maximum WITHOUT any allocation ---------------------------
+ *   out2 (DEVICE, 2 doubles): out2[0] = max_i (r_i + ||c - c_i|| - r), out2[1] = its smallest index.
+ * For callers that cannot call cudaMalloc (under CUDA graph capture, serving loops): no context, no
+ * workspace; nothing is allocated or freed, nothing is synchronised.  The scratch of the two-level
+ * reduction is a file-scope __device__ array of MEB_STATIC_MAX_TILES (value, index) pairs = 1 MiB that
+ * every GPU holding the library keeps until exit, so m <= MEB_STATIC_MAX_ROWS (else MEB_E_CAPACITY).
+ * C (m x d FP64, row stride ld), R (nullable = points), c: DEVICE pointers on the CURRENT device;
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream); the kernels are queued on it and the call
+ * returns without waiting.  All calls share the scratch: calls ordered on one stream are safe, calls
+ * that overlap on the GPU (other streams, other host threads) race.  Not thread-safe on first use per
+ * device.  Errors: MEB_E_ARG (null pointer, m < 1, d < 1, ld < d), MEB_E_CAPACITY, MEB_E_CUDA. */
+#define MEB_STATIC_MAX_TILES 65536
+#define MEB_STATIC_MAX_ROWS (256LL * MEB_STATIC_MAX_TILES)      /* 16,777,216 balls */
+MEB_API int meb_feasibility_max_static(void* cuda_stream, int64_t m, int32_t d, const double* C, int64_t ld,
+                                       const double* R, double r, const double* c, double* out2);
+
 /* ---- measurement helper ------------------------------------------------------------------------
  * Device time (ms, CUDA events on the context's stream) and algorithmic bytes of the most recent
  * streaming-pass launch made through this context (eval/hvp-classify/screen/feasibility/ingest). */

@@ -29,6 +29,7 @@ EXPORTS = [
     "meb_create", "meb_destroy", "meb_strerror", "meb_last_cuda_error", "meb_default_params",
     "meb_version", "meb_solve", "meb_solve_host", "meb_ingest", "meb_eval_alm", "meb_hvp",
     "meb_dense_hessian", "meb_update_multipliers", "meb_screen_compact", "meb_feasibility_check",
+    "meb_feasibility_max_static",
     "meb_last_pass_info", "meb_set_pass_timing", "meb_solve_batch", "meb_set_option", "meb_eval_alm_multi",
     "meb_solve_sharded", "meb_shard_record_doubles",
 ]
@@ -114,6 +115,7 @@ def load():
     lib.meb_update_multipliers.argtypes = prob + [vp, dbl, vp, vp, vp, i64, i64, C.POINTER(i64), C.POINTER(dbl)]
     lib.meb_screen_compact.argtypes = [vp, i64, i32, vp, i64, vp, flt, vp, flt, vp, i64, C.POINTER(i64), vp,
                                        C.c_int]
+    lib.meb_feasibility_max_static.argtypes = [vp, i64, i32, vp, i64, vp, dbl, vp, vp]
     lib.meb_feasibility_check.argtypes = [vp, i64, i32, vp, i64, vp, dbl, vp, dbl, vp, C.POINTER(dbl),
                                           C.POINTER(i32), vp, i64, C.POINTER(i64)]
     for name in EXPORTS:
@@ -410,3 +412,20 @@ def meb_feasibility_check(ctx: Context, Cm, R, r, c, eps_feas, kept_mask=None, c
                                         _ptr(kept_mask), C.byref(dm), C.byref(am), _ptr(idx), cap, C.byref(n))
     _check(code, "meb_feasibility_check", (MEB_OK, MEB_E_CAPACITY))
     return dict(delta_max=dm.value, argmax=am.value, viol_idx=idx[:min(n.value, cap)], n_viol=n.value, code=code)
+
+
+MEB_STATIC_MAX_ROWS = 256 * 65536
+
+
+def meb_feasibility_max_static(Cm, R, r, c, out2, stream=None):
+    """Allocation-free feasibility maximum (include/meb.h a8'): the kernels are queued on ``stream`` (default: torch's
+    current stream) and write (Delta_max, arg-max as a double) into the caller's device tensor ``out2``; nothing is
+    allocated, copied to the host or synchronised here.  Returns the status code (MEB_E_CAPACITY beyond
+    MEB_STATIC_MAX_ROWS balls).  Calls share one static device scratch: do not overlap them on the GPU."""
+    m, d, ld, _ = _problem(MEB_FP64, Cm, R, None, None, None)
+    assert out2.is_cuda and out2.dtype == torch.float64 and out2.is_contiguous() and out2.numel() >= 2
+    assert c.is_cuda and c.dtype == torch.float64 and c.is_contiguous() and c.numel() == d
+    st = torch.cuda.current_stream(Cm.device) if stream is None else stream
+    code = load().meb_feasibility_max_static(C.c_void_p(st.cuda_stream), m, d, _ptr(Cm), ld, _ptr(R), float(r), _ptr(c),
+                                             _ptr(out2))
+    return _check(code, "meb_feasibility_max_static", (MEB_OK, MEB_E_CAPACITY))

@@ -57,6 +57,9 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  : "memory");
 }
 
+// a row of zeros stands in for the multiplier row of a ball that has none (rows of at most 1024 bytes)
+__device__ __align__(32) const double tile_zero_row[128] = {};
+
 template <typename T> struct Chunk;
 template <> struct Chunk<double> { typedef double2 type; static constexpr int N = 2; };
 template <> struct Chunk<float>  { typedef float4 type;  static constexpr int N = 4; };
@@ -250,8 +253,11 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                     for (int j = d; j < nch * VEC; ++j) rowp[j] = T(0);
                 __syncwarp();
             }
+            // a sub-tile with multiplier rows runs ONE loop for all its lanes (v = 0 where a row has none): two
+            // divergent loops, one per kind of row, cost more than the few extra multiplications
+            const bool wv = HASV && __any_sync(MEB_FULL_MASK, myvalid && myslot >= 0);
             if (myvalid) {
-                if (myslot < 0) {
+                if (!wv) {
                     T s0 = T(0), s1 = T(0), f0 = T(0);
                     const V4* rp = reinterpret_cast<const V4*>(rowp) + g;
                     const V4* cp = cs4 + g;
@@ -322,54 +328,75 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                     pdot = pp;
                     nb2 = s0 + s1;
                     if (OP == OP_INGEST) ne2 = f0;
-                } else {                                                 // row with a multiplier v_i
-                    // 16-byte chunks of the V row straight from global memory (rows of the pool are in
-                    // ascending ball order, so neighbouring lanes read neighbouring pool rows)
-                    const V4* vrow4 = reinterpret_cast<const V4*>(Vg + (int64_t)myslot * a.ldv);
+                } else {                                                 // sub-tile with multiplier rows v_i
+                    // 16-byte chunks of the V row straight from global memory (rows of the pool are in ascending
+                    // ball order, so neighbouring lanes read neighbouring pool rows); a lane whose row has no v_i
+                    // reads a row of zeros instead (one broadcast sector), which keeps the loop free of predicates.
+                    // The V loads of a batch of 8 chunks are issued together (one exposed latency per batch), then
+                    // the arithmetic runs on registers.  Chunk order rotated by the row index like the rows
+                    // without multipliers (lanes of a quarter warp would otherwise read the same banks).
                     const V4* rp = reinterpret_cast<const V4*>(rowp);
                     const bool v16 = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
-                    // my chunks g, g + G, ...: the V loads of a batch of 8 are issued together (one exposed latency
-                    // per batch instead of one per chunk), then the arithmetic runs on registers
-                    for (int k0 = 0; k0 < n_g; k0 += 8) {
-                        V4 vb[8];
+                    const bool hasrow = myslot >= 0;
+                    const T* vrowT = hasrow ? Vg + (int64_t)myslot * a.ldv : reinterpret_cast<const T*>(tile_zero_row);
+                    const V4* vrow4 = reinterpret_cast<const V4*>(vrowT);
+                    // FAST: whole batches, no column padding, aligned pool rows, power-of-two chunk count
+                    auto vwalk = [&](auto fast) {
+                        constexpr bool FAST = decltype(fast)::value;
+                        for (int k0 = 0; k0 < n_g; k0 += 8) {
+                            V4 vb[8];
+                            int cidx[8];
 #pragma unroll
-                        for (int u = 0; u < 8; ++u) {
-                            const int c = g + ((k0 + u) << LG);
-                            if (k0 + u < n_g) {
-                                if (v16) {
+                            for (int u = 0; u < 8; ++u) {
+                                int ci = start + k0 + u;
+                                if (FAST) ci &= n_g - 1; else if (ci >= n_g) ci -= n_g;
+                                cidx[u] = g + (ci << LG);
+                            }
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                const int c = cidx[u];
+                                if (FAST) {
                                     vb[u] = __ldg(vrow4 + c);
                                 } else {
-                                    T* vq = reinterpret_cast<T*>(&vb[u]);
+                                    vb[u] = V4();
+                                    if (k0 + u < n_g) {
+                                        if (v16) {
+                                            vb[u] = __ldg(vrow4 + c);
+                                        } else {
+                                            T* vq = reinterpret_cast<T*>(&vb[u]);
 #pragma unroll
-                                    for (int j = 0; j < VEC; ++j)
-                                        vq[j] = (c * VEC + j < d) ? __ldg(Vg + (int64_t)myslot * a.ldv + c * VEC + j) : T(0);
+                                            for (int j = 0; j < VEC; ++j) vq[j] = (c * VEC + j < d) ? __ldg(vrowT + c * VEC + j) : T(0);
+                                        }
+                                    }
+                                }
+                            }
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                const int c = cidx[u];
+                                if (FAST || k0 + u < n_g) {
+                                    const V4 ev4 = rp[c];
+                                    const V4 cv4 = cs4[c];
+                                    const T* e = reinterpret_cast<const T*>(&ev4);
+                                    const T* cc = reinterpret_cast<const T*>(&cv4);
+                                    const T* vq = reinterpret_cast<const T*>(&vb[u]);
+                                    const int col = c * VEC;
+#pragma unroll
+                                    for (int j = 0; j < VEC; ++j) {
+                                        const T ee = e[j] - cc[j];               // padding of the row was zeroed above
+                                        const T v = (FAST || col + j < d) ? vq[j] : T(0);   // padding of the pool row is not
+                                        const T bq = fma(v, inv_sig, ee);
+                                        if (MULTI && domulti) pdot = fma(bq, reinterpret_cast<const T*>(cs4 + doff4)[col + j], pdot);
+                                        nb2 = fma(bq, bq, nb2);
+                                        ne2 = fma(ee, ee, ne2);
+                                        evd = fma(ee, v, evd);
+                                        vv = fma(v, v, vv);
+                                    }
                                 }
                             }
                         }
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) {
-                            const int c = g + ((k0 + u) << LG);
-                            if (k0 + u < n_g) {
-                                const V4 ev4 = rp[c];
-                                const V4 cv4 = cs4[c];
-                                const T* e = reinterpret_cast<const T*>(&ev4);
-                                const T* cc = reinterpret_cast<const T*>(&cv4);
-                                const T* vq = reinterpret_cast<const T*>(&vb[u]);
-                                const int col = c * VEC;
-#pragma unroll
-                                for (int j = 0; j < VEC; ++j) {
-                                    const T ee = e[j] - cc[j];                   // padding of the row was zeroed above
-                                    const T v = (col + j < d) ? vq[j] : T(0);    // padding of the pool row is not
-                                    const T bq = fma(v, inv_sig, ee);
-                                    if (MULTI && domulti) pdot = fma(bq, reinterpret_cast<const T*>(cs4 + doff4)[col + j], pdot);
-                                    nb2 = fma(bq, bq, nb2);
-                                    ne2 = fma(ee, ee, ne2);
-                                    evd = fma(ee, v, evd);
-                                    vv = fma(v, v, vv);
-                                }
-                            }
-                        }
-                    }
+                    };
+                    if (!haspad && v16 && (n_g & 7) == 0 && (n_g & (n_g - 1)) == 0) vwalk(std::true_type{});
+                    else vwalk(std::false_type{});
                 }
             }
 #pragma unroll
@@ -403,161 +430,135 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                     }
                 }
                 if (OP == OP_EVAL && bits != 0u) {
-                    // gradient vector part: sum over the ACTIVE rows of lam_i b_i, from shared memory.  lam_i (and
-                    // the slot of v_i) of the sub-tile's rows go through a warp-private shared array; group `grp`
-                    // of the warp then walks the active rows grp, grp + RP, ..., lane `cl` of the group owning
-                    // the 16-byte chunks cl, cl + 32 of every row.
+                    // gradient vector part: sum over the ACTIVE rows of lam_i b_i, from shared memory.  The active
+                    // rows of the sub-tile are first compacted (ascending) into a warp-private list of (row, lam_i,
+                    // slot of v_i); group `grp` of the warp then walks the entries grp, grp + RP, ..., lane `cl` of
+                    // the group owning the 16-byte chunks cl, cl + 32 of every row.  Work is proportional to the
+                    // number of active rows (a loop over all 32 rows that skipped the inactive ones cost a third of
+                    // the pass's instructions on config 4, where every second row is active).
                     __shared__ double lam_w[16][32];
                     __shared__ int32_t slot_w[16][32];
-                    if (g == 0) { lam_w[warp][rl] = mylam; slot_w[warp][rl] = myslot; }
+                    __shared__ uint8_t row_w[16][32];
+                    if (flag) {                                          // flag only on the g = 0 lane of a row
+                        const int o = __popc(bits & ((1u << lane) - 1u));
+                        lam_w[warp][o] = mylam; slot_w[warp][o] = myslot; row_w[warp][o] = (uint8_t)rl;
+                    }
                     __syncwarp();
+                    const int nact = __popc(bits);
                     const bool v16a = (a.ldv * (int64_t)sizeof(T)) % 16 == 0 && (reinterpret_cast<uintptr_t>(Vg) % 16) == 0;
-                    // one row with lam != 0 and possibly a multiplier row v_i in the pool
-                    auto grad_row = [&](const V4* rp4, double lam, int slot, double (&va)[CH][VEC]) {
+                    auto load_v = [&](int slot, int ch) -> V4 {          // chunk ch of pool row `slot` (zero if none)
+                        V4 vb = V4();
+                        if (slot >= 0) {
+                            const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
+                            if (v16a) {
+                                vb = __ldg(reinterpret_cast<const V4*>(vrow));
+                            } else {
+                                T* vq = reinterpret_cast<T*>(&vb);
 #pragma unroll
-                        for (int q = 0; q < CH; ++q) {
-                            const int ch = cl + 32 * q;
-                            if (ch < nch) {
-                                V4 vb = V4();
-                                if (slot >= 0) {
-                                    const T* vrow = Vg + (int64_t)slot * a.ldv + ch * VEC;
-                                    if (v16a) {
-                                        vb = __ldg(reinterpret_cast<const V4*>(vrow));
-                                    } else {
-                                        T* vq = reinterpret_cast<T*>(&vb);
-#pragma unroll
-                                        for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
-                                    }
-                                }
-                                const V4 ev4 = rp4[ch];
-                                const T* e = reinterpret_cast<const T*>(&ev4);
-                                const T* vq = reinterpret_cast<const T*>(&vb);
-#pragma unroll
-                                for (int j = 0; j < VEC; ++j) {
-                                    T bj = e[j] - creg[q][j];
-                                    if (slot >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
-                                    va[q][j] = fma(lam, (double)bj, va[q][j]);
-                                }
+                                for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
                             }
                         }
+                        return vb;
                     };
-                    // (384-thread instance only: the extra registers of the batch spill in the 512-thread one)
-                    const bool anyv = MAXT == 384 && HASV && __any_sync(MEB_FULL_MASK, myslot >= 0 && mylam != 0.0);
-                    if (anyv) {
-                        // active rows with a multiplier row v_i: b_i = c_i - c + v_i / sigma.  The pool rows come
-                        // from global memory; the loads of FOUR rows of my group are issued before any of them is
-                        // used (one dependent load per row made the pass latency-bound: config 4, every second
-                        // row).  Rows alternate between the two accumulation chains exactly as in the loop below.
-                        for (int rs = grp; rs < RPT; rs += 4 * RP) {
-                            double lam4[4];
-                            int sl4[4];
-                            V4 vb[4][CH];
+                    const bool anyv = HASV && __any_sync(MEB_FULL_MASK, flag && myslot >= 0);
+                    if (anyv && MAXT == 384) {
+                        // rows with a multiplier row v_i: b_i = c_i - c + v_i / sigma.  The pool rows come from
+                        // global memory (L1 / L2: the norm part has just read them); the loads of FOUR entries of
+                        // my group are issued before any of them is used.  Entries alternate between the two
+                        // accumulation chains.  (384-thread instance only: the batch spills in the 512-thread one.)
+                        // FAST: every lane of a group owns a chunk, no column padding, aligned pool rows; an entry
+                        // without v_i (or past the end of the list) reads the row of zeros.
+                        auto gwalk = [&](auto fast) {
+                            constexpr bool FAST = decltype(fast)::value;
+                            for (int k0 = grp; k0 < nact; k0 += 4 * RP) {
+                                double lam4[4];
+                                int sl4[4], r4[4];
+                                V4 vb[4][CH];
 #pragma unroll
-                            for (int u = 0; u < 4; ++u) {
-                                const int rq = rs + u * RP;
-                                lam4[u] = rq < RPT ? lam_w[warp][rq] : 0.0;
-                                sl4[u] = lam4[u] != 0.0 ? slot_w[warp][rq] : -1;
-                            }
+                                for (int u = 0; u < 4; ++u) {
+                                    const int kq = k0 + u * RP;
+                                    const bool on = kq < nact;
+                                    lam4[u] = on ? lam_w[warp][kq] : 0.0;
+                                    sl4[u] = on ? slot_w[warp][kq] : -1;
+                                    r4[u] = on ? (int)row_w[warp][kq] : (FAST ? (int)row_w[warp][k0] : -1);
+                                }
 #pragma unroll
-                            for (int u = 0; u < 4; ++u) {
+                                for (int u = 0; u < 4; ++u)
 #pragma unroll
-                                for (int q = 0; q < CH; ++q) {
-                                    const int ch = cl + 32 * q;
-                                    vb[u][q] = V4();
-                                    if (sl4[u] >= 0 && ch < nch) {
-                                        const T* vrow = Vg + (int64_t)sl4[u] * a.ldv + ch * VEC;
-                                        if (v16a) {
-                                            vb[u][q] = __ldg(reinterpret_cast<const V4*>(vrow));
+                                    for (int q = 0; q < CH; ++q) {
+                                        const int ch = cl + 32 * q;
+                                        if (FAST) {
+                                            const T* vrow = sl4[u] >= 0 ? Vg + (int64_t)sl4[u] * a.ldv : reinterpret_cast<const T*>(tile_zero_row);
+                                            vb[u][q] = __ldg(reinterpret_cast<const V4*>(vrow) + ch);
                                         } else {
-                                            T* vq = reinterpret_cast<T*>(&vb[u][q]);
+                                            vb[u][q] = load_v(ch < nch ? sl4[u] : -1, ch);
+                                        }
+                                    }
 #pragma unroll
-                                            for (int j = 0; j < VEC; ++j) vq[j] = (ch * VEC + j < d) ? __ldg(vrow + j) : T(0);
+                                for (int u = 0; u < 4; ++u) {
+                                    if (!FAST && r4[u] < 0) continue;    // (FAST: lam = 0 on a valid row adds exactly zero)
+                                    const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + r4[u]) * ldT);
+#pragma unroll
+                                    for (int q = 0; q < CH; ++q) {
+                                        const int ch = cl + 32 * q;
+                                        if (FAST || ch < nch) {
+                                            const V4 ev4 = rp4[ch];
+                                            const T* e = reinterpret_cast<const T*>(&ev4);
+                                            const T* vq = reinterpret_cast<const T*>(&vb[u][q]);
+#pragma unroll
+                                            for (int j = 0; j < VEC; ++j) {
+                                                T bj = e[j] - creg[q][j];
+                                                if (FAST) bj = fma(vq[j], inv_sig, bj);
+                                                else if (sl4[u] >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
+                                                if (u & 1) vaccB[q][j] = fma(lam4[u], (double)bj, vaccB[q][j]);
+                                                else vacc[q][j] = fma(lam4[u], (double)bj, vacc[q][j]);
+                                            }
                                         }
                                     }
                                 }
                             }
-#pragma unroll
-                            for (int u = 0; u < 4; ++u) {
-                                if (lam4[u] == 0.0) continue;
-                                const V4* rp4 = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs + u * RP) * ldT);
-#pragma unroll
-                                for (int q = 0; q < CH; ++q) {
-                                    const int ch = cl + 32 * q;
-                                    if (ch < nch) {
-                                        const V4 ev4 = rp4[ch];
-                                        const T* e = reinterpret_cast<const T*>(&ev4);
-                                        const T* vq = reinterpret_cast<const T*>(&vb[u][q]);
-#pragma unroll
-                                        for (int j = 0; j < VEC; ++j) {
-                                            T bj = e[j] - creg[q][j];
-                                            if (sl4[u] >= 0 && ch * VEC + j < d) bj = fma(vq[j], inv_sig, bj);
-                                            if (u & 1) vaccB[q][j] = fma(lam4[u], (double)bj, vaccB[q][j]);
-                                            else vacc[q][j] = fma(lam4[u], (double)bj, vacc[q][j]);
-                                        }
-                                    }
-                                }
-                            }
-                        }
+                        };
+                        if (CH == 1 && !haspad && v16a && nch == (1 << lognchp)) gwalk(std::true_type{});
+                        else gwalk(std::false_type{});
                     } else {
-                        const int rstep = RP * (ldT / VEC);               // 16-byte units between rows rs and rs + RP
-                        for (int rs = grp; rs < RPT; rs += 2 * RP) {      // two rows of my group per step
-                            const int rsB = rs + RP;
-                            const double lamA = lam_w[warp][rs];
-                            const double lamB = rsB < RPT ? lam_w[warp][rsB] : 0.0;
-                            if (lamA == 0.0 && lamB == 0.0) continue;
-                            const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rs) * ldT);
-                            const V4* rpB = rpA + rstep;
-                            const int slotA = (HASV && lamA != 0.0) ? slot_w[warp][rs] : -1;
-                            const int slotB = (HASV && lamB != 0.0) ? slot_w[warp][rsB] : -1;
-                            if (slotA >= 0 || slotB >= 0) {               // rows with a multiplier row
-                                if (CH == 1 && v16a) {                    // both pool loads before either is used
-                                    const int ch = cl;
-                                    if (ch < nch) {
-                                        V4 vA = V4(), vB = V4(), eA = V4(), eB = V4();
-                                        if (slotA >= 0) vA = __ldg(reinterpret_cast<const V4*>(Vg + (int64_t)slotA * a.ldv) + ch);
-                                        if (slotB >= 0) vB = __ldg(reinterpret_cast<const V4*>(Vg + (int64_t)slotB * a.ldv) + ch);
-                                        if (lamA != 0.0) eA = rpA[ch];
-                                        if (lamB != 0.0) eB = rpB[ch];
-                                        const T* ea = reinterpret_cast<const T*>(&eA);
-                                        const T* eb = reinterpret_cast<const T*>(&eB);
-                                        const T* va = reinterpret_cast<const T*>(&vA);
-                                        const T* vbq = reinterpret_cast<const T*>(&vB);
-#pragma unroll
-                                        for (int j = 0; j < VEC; ++j) {
-                                            T bA = ea[j] - creg[0][j], bB = eb[j] - creg[0][j];
-                                            if (slotA >= 0 && ch * VEC + j < d) bA = fma(va[j], inv_sig, bA);
-                                            if (slotB >= 0 && ch * VEC + j < d) bB = fma(vbq[j], inv_sig, bB);
-                                            vacc[0][j] = fma(lamA, (double)bA, vacc[0][j]);
-                                            vaccB[0][j] = fma(lamB, (double)bB, vaccB[0][j]);
-                                        }
-                                    }
-                                } else {
-                                    if (lamA != 0.0) grad_row(rpA, lamA, slotA, vacc);
-                                    if (lamB != 0.0) grad_row(rpB, lamB, slotB, vaccB);
-                                }
-                                continue;
-                            }
-                            // a row with lam = 0 adds exactly zero, without being read (shared memory behind the
-                            // last row of the data is stale)
+                        // two entries of my group per step (chains A and B); a missing second entry repeats the
+                        // first row with lam = 0 and adds exactly zero
+                        for (int k0 = grp; k0 < nact; k0 += 2 * RP) {
+                            const int kB = k0 + RP;
+                            const bool hasB = kB < nact;
+                            const double lamA = lam_w[warp][k0];
+                            const double lamB = hasB ? lam_w[warp][kB] : 0.0;
+                            const int rA = row_w[warp][k0];
+                            const int rB = hasB ? (int)row_w[warp][kB] : rA;
+                            const int slotA = anyv ? slot_w[warp][k0] : -1;
+                            const int slotB = (anyv && hasB) ? slot_w[warp][kB] : -1;
+                            const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rA) * ldT);
+                            const V4* rpB = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rB) * ldT);
 #pragma unroll
                             for (int q = 0; q < CH; ++q) {
                                 const int ch = cl + 32 * q;
                                 if (ch < nch) {
-                                    V4 eA = V4(), eB = V4();
-                                    if (lamA != 0.0) eA = rpA[ch];
-                                    if (lamB != 0.0) eB = rpB[ch];
+                                    V4 vA = V4(), vB = V4();
+                                    if (anyv) { vA = load_v(slotA, ch); vB = load_v(slotB, ch); }
+                                    const V4 eA = rpA[ch];
+                                    const V4 eB = rpB[ch];
                                     const T* ea = reinterpret_cast<const T*>(&eA);
                                     const T* eb = reinterpret_cast<const T*>(&eB);
+                                    const T* va = reinterpret_cast<const T*>(&vA);
+                                    const T* vbq = reinterpret_cast<const T*>(&vB);
 #pragma unroll
                                     for (int j = 0; j < VEC; ++j) {
-                                        vacc[q][j] = fma(lamA, (double)(ea[j] - creg[q][j]), vacc[q][j]);
-                                        vaccB[q][j] = fma(lamB, (double)(eb[j] - creg[q][j]), vaccB[q][j]);
+                                        T bA = ea[j] - creg[q][j], bB = eb[j] - creg[q][j];
+                                        if (anyv && slotA >= 0 && ch * VEC + j < d) bA = fma(va[j], inv_sig, bA);
+                                        if (anyv && slotB >= 0 && ch * VEC + j < d) bB = fma(vbq[j], inv_sig, bB);
+                                        vacc[q][j] = fma(lamA, (double)bA, vacc[q][j]);
+                                        vaccB[q][j] = fma(lamB, (double)bB, vaccB[q][j]);
                                     }
                                 }
                             }
                         }
                     }
-                    __syncwarp();                                        // lam_w is rewritten by the next sub-tile
+                    __syncwarp();                                        // the lists are rewritten by the next sub-tile
                 }
             }
             if (SHADOW) {                       // FP32 shadow of the centred rows (reading 8)
@@ -769,7 +770,7 @@ int launch_cfg(meb_ctx* ctx, KernelT kernel512, KernelT kernel384, const StreamA
 
 int lanes_per_row(const StreamArgs& a, size_t esize) {
     const size_t rb = (size_t)a.ld * esize;
-    return rb <= 256 ? 1 : (rb <= 416 ? 2 : 4);              // sub-tile of at most ~8 KB
+    return rb <= (getenv("MEB_G1MAX") ? (size_t)atoi(getenv("MEB_G1MAX")) : 256) ? 1 : (rb <= 416 ? 2 : 4);              // sub-tile of at most ~8 KB
 }
 
 // G is fixed by the row length; CH = 2 only occurs with G = 4 (rows longer than 512 bytes)

@@ -241,6 +241,100 @@ __global__ void __launch_bounds__(MEB_BLOCK, (MODE == MODE_WRITEV && TEAM == 32)
     }
 }
 
+// MODE_WRITEV for SHORT rows (d <= 32): eight lanes per list entry, four consecutive entries per warp and step, lane l8 of
+// an entry owning the columns l8, l8 + 8, ...  A warp per entry spent 130 instructions on a row of 32 numbers and kept
+// one row per warp in flight; here the instructions are shared by four rows and UB steps (16 rows per warp) are loaded
+// level by level (list -> slot, lam, t -> rows of C and V) before any is used.  Consecutive entries are neighbouring
+// balls and consecutive rows of the new pool, so the four rows of a step are read and written as one run.
+// Same arithmetic per entry as the generic loop (fma(0, 1/sigma, b) = b for a row without v_i); ||v+||^2 is added over
+// the eight lanes by an xor tree, entries in the fixed order of the static partition.
+template <typename T>
+__global__ void __launch_bounds__(MEB_BLOCK, 2) writev_short_kernel(const ActiveArgs a_in) {
+    ActiveArgs a = a_in;
+    meb_resolve_dyn(a);
+    __shared__ double sc_red[MEB_WARPS];
+    constexpr int UB = 4, EL = 4;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane >> 3, l8 = lane & 7;
+    const int d = a.d;
+    const int n = *a.count;
+    const T* __restrict__ C = static_cast<const T*>(a.C);
+    const T* __restrict__ V = static_cast<const T*>(a.V);
+    const T inv_sig = T(1) / (T)a.sigma;
+    T cxe[EL];
+#pragma unroll
+    for (int e = 0; e < EL; ++e) cxe[e] = (l8 + 8 * e) < d ? (T)a.x[1 + l8 + 8 * e] : T(0);
+    const long long NW = (long long)gridDim.x * MEB_WARPS;
+    double sc = 0.0;
+    for (long long q0 = (long long)blockIdx.x * MEB_WARPS + warp; q0 * 4 < n; q0 += NW * UB) {
+        int ii[UB], sl[UB];
+        long long kk[UB];
+        double lam[UB], tv[UB];
+        T cv[UB][EL], vv[UB][EL];
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            kk[u] = (q0 + (long long)u * NW) * 4 + sub;
+            ii[u] = kk[u] < n ? a.list[kk[u]] : -1;
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int i = ii[u];
+            sl[u] = (i >= 0 && a.v_slot) ? a.v_slot[i] : -1;
+            lam[u] = i >= 0 ? a.rec_lam[i] : 0.0;
+            tv[u] = i >= 0 ? a.rec_t[i] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const T* rowp = C + (int64_t)(ii[u] >= 0 ? ii[u] : 0) * a.ld;
+            const T* vrow = V + (int64_t)(sl[u] >= 0 ? sl[u] : 0) * a.ldv;
+#pragma unroll
+            for (int e = 0; e < EL; ++e) {
+                const int j = l8 + 8 * e;
+                cv[u][e] = (ii[u] >= 0 && j < d) ? rowp[j] : T(0);
+                vv[u][e] = (sl[u] >= 0 && j < d) ? vrow[j] : T(0);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const bool on = ii[u] >= 0;
+            const T sl_ = (T)(a.sigma * lam[u]);
+            T* vout = static_cast<T*>(a.V_out) + (int64_t)kk[u] * a.ldv_out;
+            const bool store = on && kk[u] < a.cap_rows;
+            double nb2 = 0.0;
+#pragma unroll
+            for (int e = 0; e < EL; ++e) {
+                const int j = l8 + 8 * e;
+                if (j < d) {
+                    T b = cv[u][e] - cxe[e];
+                    b = fma(vv[u][e], inv_sig, b);
+                    const T vp = sl_ * b;
+                    if (store) vout[j] = vp;
+                    nb2 = fma((double)vp, (double)vp, nb2);
+                }
+            }
+            nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, 1);
+            nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, 2);
+            nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, 4);
+            if (on && l8 == 0) {
+                const T up = (T)a.sigma * (T)tv[u];
+                static_cast<T*>(a.U_out)[ii[u]] = up;
+                a.slot_out[ii[u]] = store ? (int32_t)kk[u] : -1;
+                sc += (double)up * (double)up + nb2;
+            }
+        }
+    }
+    // scalar partial: the four entries of a warp, then the warps, in index order
+    sc += __shfl_xor_sync(MEB_FULL_MASK, sc, 8);
+    sc += __shfl_xor_sync(MEB_FULL_MASK, sc, 16);
+    if (lane == 0) sc_red[warp] = sc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < MEB_WARPS; ++w) t += sc_red[w];
+        a.part_sc[blockIdx.x] = t;
+    }
+}
+
 template <typename T, int MODE>
 int launch_active_t(meb_ctx* ctx, const ActiveArgs& a, int* grid_out) {
     const bool wide = a.d > 2048;
@@ -254,7 +348,12 @@ int launch_active_t(meb_ctx* ctx, const ActiveArgs& a, int* grid_out) {
         if (grid > 1024) grid = 1024;
     }
     cudaError_t e;
-    if (wide) {
+    if (MODE == MODE_WRITEV && a.d <= 32) {
+        grid = ctx->sm_count * 2;
+        ctx->launches++;
+        writev_short_kernel<T><<<grid, MEB_BLOCK, 0, ctx->stream>>>(a);
+        e = cudaSuccess;
+    } else if (wide) {
         auto kern = active_kernel<T, MEB_BLOCK, MODE>;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) { ctx->launches++; kern<<<grid, MEB_BLOCK, smem, ctx->stream>>>(a); }

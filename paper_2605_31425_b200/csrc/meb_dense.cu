@@ -190,6 +190,154 @@ __global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a_in, 
     }
 }
 
+// Rows of at most 48 columns (DP = 8 B): the variant the large active sets of short-row instances run (config 4: 5e6
+// rows of 32 numbers per Hessian).  Differences to syrk_kernel, which spent 180 warp instructions per row there:
+//  * fill: EIGHT lanes per row (lane l8 owns the columns l8, l8 + 8, ...), so a warp normalises its four rows of the
+//    tile at once -- a quarter of the loads, shuffles and rsqrt sequences per row;
+//  * the fill also stores rho_i w_i next to w_i and accumulates s = sum w_i, which takes 4 multiplications and the
+//    additions of s out of the inner loop of every thread;
+//  * only the blocks on and below the diagonal are accumulated (B (B + 1) / 2 of B^2 FMAs per thread and row; the
+//    finalize kernel reads H from the lower triangle).
+// Same three-level software pipeline of the gather, same static partition and fixed-order combination.
+template <typename T, int B>
+__global__ void __launch_bounds__(MEB_BLOCK) syrk8_kernel(const ActiveArgs a_in, double* __restrict__ part_mat) {
+    constexpr int TD = 8, DP = TD * B, KS = SyrkShape<TD>::KS, RB = SyrkShape<TD>::RB;
+    static_assert(RB == 4 * MEB_WARPS, "four rows per warp and tile");
+    ActiveArgs a = a_in;
+    meb_resolve_dyn(a);
+    extern __shared__ __align__(16) double sm[];             // W[RB][DP], Wr[RB][DP], then red[DP*DP + DP]
+    double* W = sm;
+    double* Wr = sm + (size_t)RB * DP;
+    double* red = sm + 2 * (size_t)RB * DP;
+    const int tx = threadIdx.x % TD, ty = (threadIdx.x / TD) % TD, kg = threadIdx.x / (TD * TD);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane >> 3, l8 = lane & 7;
+    const int rr = warp * 4 + sub;                           // my row of a tile in the fill phase
+    const int d = a.d;
+    const T* __restrict__ C = static_cast<const T*>(a.C);
+    const T* __restrict__ V = static_cast<const T*>(a.V);
+    const T inv_sig = T(1) / (T)a.sigma;
+    const int n = *a.count;
+    if (blockIdx.x * RB >= n) return;                        // no tile for this CTA: the finalize skips it
+    double acc[B][B];
+    double accs[B];                                          // fill lanes: my columns of s = sum of the w rows I normalised
+#pragma unroll
+    for (int i = 0; i < B; ++i) {
+        accs[i] = 0.0;
+#pragma unroll
+        for (int j = 0; j < B; ++j) acc[i][j] = 0.0;
+    }
+    T cxr[B];
+#pragma unroll
+    for (int e = 0; e < B; ++e) cxr[e] = (l8 + 8 * e) < d ? (T)a.x[1 + l8 + 8 * e] : T(0);
+    int i_a;                                                 // level 1: list entry (tile t+3)
+    int i_b, slot_b; double rho_b;                           // level 2: (rho, slot) of tile t+2
+    T cq[B], vq[B]; double rho_c;                            // level 3: raw row of tile t+1
+    auto level1 = [&](int k0) {
+        const int k = k0 + rr;
+        i_a = (k0 >= 0 && k < n) ? a.list[k] : -1;
+    };
+    auto level2 = [&]() {
+        const int i = i_a;
+        i_b = i;
+        rho_b = i >= 0 ? a.rec_rho[i] : 2.0;                 // B1 rows (rho = 2): P_i = I, no SYRK term
+        slot_b = (i >= 0 && a.v_slot) ? a.v_slot[i] : -1;
+    };
+    auto level3 = [&]() {
+        const int i = i_b;
+        const bool use = i >= 0 && rho_b < 1.5;
+        rho_c = use ? rho_b : 2.0;
+        const T* rowp = C + (int64_t)(use ? i : 0) * a.ld;
+        const T* vrow = V + (int64_t)(slot_b >= 0 ? slot_b : 0) * a.ldv;
+#pragma unroll
+        for (int e = 0; e < B; ++e) {
+            const int j = l8 + 8 * e;
+            cq[e] = (use && j < d) ? rowp[j] : T(0);
+            vq[e] = (use && slot_b >= 0 && j < d) ? vrow[j] : T(0);
+        }
+    };
+    const int kstep = gridDim.x * RB;
+    int k0 = blockIdx.x * RB;
+    auto tile_at = [&](int q) {                              // first list entry of the q-th tile after k0, or -1
+        const long long k = (long long)k0 + (long long)q * kstep;
+        return k < n ? (int)k : -1;
+    };
+    level1(k0); level2(); level3();
+    level1(tile_at(1)); level2();
+    level1(tile_at(2));
+    for (; k0 < n; k0 += kstep) {
+        __syncthreads();
+        {   // normalise my row of this tile (level 3 registers) into shared memory
+            const bool use = rho_c < 1.5;
+            double bd[B];
+            double nb2 = 0.0;
+#pragma unroll
+            for (int e = 0; e < B; ++e) {
+                T b = cq[e] - cxr[e];
+                b = fma(vq[e], inv_sig, b);
+                bd[e] = (use && l8 + 8 * e < d) ? (double)b : 0.0;
+                nb2 = fma(bd[e], bd[e], nb2);
+            }
+            nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, 1);
+            nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, 2);
+            nb2 += __shfl_xor_sync(MEB_FULL_MASK, nb2, 4);
+            const double inv = use ? rsqrt(nb2) : 0.0;
+            const double rho = use ? rho_c : 0.0;
+#pragma unroll
+            for (int e = 0; e < B; ++e) {
+                const double w = bd[e] * inv;
+                W[(size_t)rr * DP + l8 + 8 * e] = w;
+                Wr[(size_t)rr * DP + l8 + 8 * e] = rho * w;
+                accs[e] += w;
+            }
+        }
+        __syncthreads();
+        level3();                                            // row of the next tile
+        level2();                                            // (rho, slot) of the tile after it
+        level1(tile_at(3));                                  // list entry three tiles ahead
+#pragma unroll 4
+        for (int r2 = kg; r2 < RB; r2 += KS) {
+            const double* w = W + (size_t)r2 * DP;
+            const double* wr = Wr + (size_t)r2 * DP;
+            double wq[B], wp[B];
+#pragma unroll
+            for (int j = 0; j < B; ++j) wq[j] = w[tx + TD * j];
+#pragma unroll
+            for (int i = 0; i < B; ++i) wp[i] = wr[ty + TD * i];
+#pragma unroll
+            for (int i = 0; i < B; ++i)
+#pragma unroll
+                for (int j = 0; j <= i; ++j) acc[i][j] = fma(wp[i], wq[j], acc[i][j]);
+        }
+    }
+    // per-CTA partial: [DP*DP] matrix (lower blocks; the others stay zero) then [DP] vector.  Row groups are added
+    // in index order; s: the 32 fill rows (warp, sub) in index order.
+    double* pm = part_mat + (size_t)blockIdx.x * ((size_t)DP * DP + DP);
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < B; ++e) W[(size_t)rr * DP + l8 + 8 * e] = accs[e];
+    for (int gk = 0; gk < KS; ++gk) {
+        __syncthreads();
+        if (kg == gk) {
+#pragma unroll
+            for (int i = 0; i < B; ++i)
+#pragma unroll
+                for (int j = 0; j < B; ++j) {
+                    const int e = (ty + TD * i) * DP + tx + TD * j;
+                    red[e] = (gk == 0 ? 0.0 : red[e]) + acc[i][j];
+                }
+        }
+    }
+    if (threadIdx.x < DP) {
+        double s = 0.0;
+#pragma unroll 4
+        for (int q = 0; q < RB; ++q) s += W[(size_t)q * DP + threadIdx.x];
+        red[DP * DP + threadIdx.x] = s;
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < DP * DP + DP; e += MEB_BLOCK) pm[e] = red[e];
+}
+
 __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __restrict__ part_mat, int nparts,
                                                              const int32_t* __restrict__ count,
                                                              int dp, int d, const double* __restrict__ ev,
@@ -216,7 +364,8 @@ __global__ void __launch_bounds__(256) dense_finalize_kernel(const double* __res
             v = 0.5 * sigma * s;
         } else {
             double s = 0.0;
-            for (int b = 0; b < nparts; ++b) s += part_mat[b * stride + (size_t)(p - 1) * dp + (q - 1)];
+            const int hi = (p > q ? p : q) - 1, lo = (p > q ? q : p) - 1;       // lower triangle (syrk8 fills no other)
+            for (int b = 0; b < nparts; ++b) s += part_mat[b * stride + (size_t)hi * dp + lo];
             v = -0.5 * sigma * s;
             if (p == q) v += tos + sigma * (n1 + 0.5 * (n3 + srho));
         }
@@ -270,15 +419,18 @@ int launch_syrk(meb_ctx* ctx, const ActiveArgs& a, int dp, double* part_mat, int
     const int bs = dp / 16;
     const int td = bs <= 3 ? 8 : 16;
     const int rb = td == 8 ? SyrkShape<8>::RB : SyrkShape<16>::RB;
-    const size_t smem = ((size_t)rb * dp + rb + (td == 8 ? (size_t)dp * dp + dp : 0)) * sizeof(double);
+    const size_t smem = td == 8 ? (2 * (size_t)rb * dp + (size_t)dp * dp + dp) * sizeof(double)
+                                : ((size_t)rb * dp + rb) * sizeof(double);
     *rb_out = rb;
 #define MEB_SYRK_CASE(BSV, TD, B) case BSV: ctx->launches++; syrk_kernel<T, TD, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat); break;
+#define MEB_SYRK8_CASE(BSV, B) case BSV: ctx->launches++; syrk8_kernel<T, B><<<grid, MEB_BLOCK, smem, ctx->stream>>>(a, part_mat); break;
     switch (bs) {
-        MEB_SYRK_CASE(1, 8, 2) MEB_SYRK_CASE(2, 8, 4) MEB_SYRK_CASE(3, 8, 6) MEB_SYRK_CASE(4, 16, 4)
+        MEB_SYRK8_CASE(1, 2) MEB_SYRK8_CASE(2, 4) MEB_SYRK8_CASE(3, 6) MEB_SYRK_CASE(4, 16, 4)
         MEB_SYRK_CASE(5, 16, 5) MEB_SYRK_CASE(6, 16, 6) MEB_SYRK_CASE(7, 16, 7) MEB_SYRK_CASE(8, 16, 8)
         default: return MEB_E_CAPACITY;
     }
 #undef MEB_SYRK_CASE
+#undef MEB_SYRK8_CASE
     MEB_CUDA_OK(ctx, cudaGetLastError());
     return MEB_OK;
 }

@@ -453,7 +453,7 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
 }
 
 // Controller step after a Newton solve (Alg. 2 line 9): slope <g, Delta>, first Armijo trial x + Delta.
-// z: Delta (n doubles, shared or global).  S may live in global or shared memory.  CTA of 256 threads.
+// z: Delta (n doubles, shared or global).  S may live in global or shared memory.  Any CTA size (whole warps).
 __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs v, const double* z, int n) {
     double* __restrict__ xn_ = v.xn;
     double* __restrict__ xbar_ = v.xbar;
@@ -462,13 +462,13 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
     double* __restrict__ x_raw_ = v.x_raw;
     double* __restrict__ off_ = v.off;
     double* __restrict__ dir_raw_ = v.dir_raw;
-    __shared__ double red[8], red2[8];
+    __shared__ double red[32], red2[32];
     const int tid = threadIdx.x;
     const double Ls = S->L;
     const bool use_off = S->use_off != 0;
-    __shared__ double red3[8];
+    __shared__ double red3[32];
     double sl = 0.0, dx2t = 0.0, dc2 = 0.0;
-    for (int j = tid; j < n; j += 256) {
+    for (int j = tid; j < n; j += blockDim.x) {
         const double dj = z[j];
         sl = fma(g_[j], dj, sl);
         const double xj = xn_[j] + dj;
@@ -486,7 +486,8 @@ __device__ inline void meb_ctrl_after_newton_dev(SolverDev* S, const SolverVecs 
     __syncthreads();
     if (tid == 0) {
         double t = 0.0, t2 = 0.0, t3 = 0.0;
-        for (int w = 0; w < 8; ++w) { t += red[w]; t2 += red2[w]; t3 += red3[w]; }
+        const int nw = (blockDim.x + 31) >> 5;
+        for (int w = 0; w < nw; ++w) { t += red[w]; t2 += red2[w]; t3 += red3[w]; }
         ctrl_arm_abort(S, true, xn_[0] + z[0], t2);
         S->slope = t; S->eta = 1.0; S->ls = 0; S->phase = PH_ARMIJO; S->action = ACT_TRIAL;
         S->tiny = (-t <= S->slope_floor * fabs(S->psi_cur)) ? 1 : 0;

@@ -356,6 +356,10 @@ void meb_free_graph_cache(meb_ctx* ctx);
 size_t meb_solver_dev_size();
 
 // ---- single-CTA solver of small problems (meb_smallsolve.cu) ----
+bool meb_wide_applicable(int prec, int64_t m, int32_t d);
+int meb_launch_wide_solve(meb_ctx* ctx, const void* C, int64_t ld, const void* R, int64_t m, int32_t d, int64_t ldv,
+                          void* const U2[2], int32_t* const slot2[2], void* const V2[2], SolverDev* S,
+                          const SolverVecs& v, double* W);
 bool meb_small_applicable(int prec, int64_t m, int32_t d);
 int meb_launch_small_solve(meb_ctx* ctx, const void* C, int64_t ld, const void* R, int64_t m, int32_t d, int64_t ldv,
                            void* const U2[2], int32_t* const slot2[2], void* const V2[2], SolverDev* S,

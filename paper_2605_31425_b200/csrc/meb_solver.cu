@@ -520,14 +520,23 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         for (int b = 0; b < 2 && small; ++b)
             if (P.vcap[b] < P.m) { if (P.own_v[b] < 0 || grow_pool(ctx, P, b, P.m) != MEB_OK) small = false; }
     }
-    if (small) stepped = false;
+    // few balls with long rows (the reduced problem of a high-dimensional instance): one persistent CTA too,
+    // matrix-free Newton steps on the gathered rows (meb_wide.cu)
+    bool wide = !small && !dense && !ctx->opt[MEB_OPT_NO_SMALL] && !ctx->shard && S.dW != nullptr && S.wc_cap >= P.m &&
+                meb_wide_applicable(P.prec, P.m, P.d);
+    if (wide) {
+        for (int b = 0; b < 2 && wide; ++b)
+            if (P.vcap[b] < P.m) { if (P.own_v[b] < 0 || grow_pool(ctx, P, b, P.m) != MEB_OK) wide = false; }
+    }
+    const bool one_cta = small || wide;
+    if (one_cta) stepped = false;
     int64_t stepped_launches = 0;
     (void)stepped_launches;
     SolveGraph stepped_info;
     memset(&stepped_info, 0, sizeof(stepped_info));
     for (int attempt = 0; attempt < 64; ++attempt) {
         SolveGraph* G = &stepped_info;
-        if (small) {
+        if (one_cta) {
             stepped_info.k_eval = 0; stepped_info.k_newton = 0; stepped_info.k_cg = 0; stepped_info.k_update = 0;
             stepped_info.bytes_per_eval = (double)P.m * (P.d * 8.0 + (P.R ? 8 : 0) + 12.0);
         } else if (!stepped) {
@@ -552,8 +561,8 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             h->pred_margin = (P.prec == MEB_FP32) ? 1e-3 : 1e-6;
             h->m_rows = (ctx->shard && P.full) ? ctx->shard->m_global : P.m;      // (counts in v.ev are global in a sharded solve)
             h->lowprec = (P.prec == MEB_FP32 && P.full) ? 1 : 0;
-            h->multi_max = small ? 0 : multi_of(par, P);
-            h->ag_outer = (par.ag_outer > 0 && !small) ? par.ag_outer : 0;
+            h->multi_max = one_cta ? 0 : multi_of(par, P);
+            h->ag_outer = (par.ag_outer > 0 && !one_cta) ? par.ag_outer : 0;
             h->ag_inner_max = 500;
             h->stall_max = (P.prec == MEB_FP32) ? 3 : 6;   // the FP32 run only has to deliver a warm start
 #ifdef MEB_TUNING
@@ -566,7 +575,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         h->vcap[0] = P.vcap[0]; h->vcap[1] = P.vcap[1];
         h->h_while = G->h_while; h->h_newton = G->h_newton; h->h_update = G->h_update; h->h_cg = G->h_cg;
         h->h_cgp = G->h_cgp; h->wc_cap = ctx->shard ? -1 : S.wc_cap;     // sharded: one exchange per CG iteration
-        h->in_graph = (stepped || small) ? 0 : 1;
+        h->in_graph = (stepped || one_cta) ? 0 : 1;
         if (first) {
             MEB_CUDA_OK(ctx, cudaMemcpyAsync(dev, h, sizeof(*h), cudaMemcpyHostToDevice, ctx->stream));
             rc = meb_ctrl_init(ctx, dev, S.v, S.sigma_start, P.cur, P.has_mult ? 1 : 0);
@@ -581,6 +590,9 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         first = false;
         if (small) {
             rc = meb_launch_small_solve(ctx, P.C, P.ld, P.R, P.m, P.d, P.ldv, P.U, P.slot, P.V, dev, S.v);
+            if (rc) return rc;
+        } else if (wide) {
+            rc = meb_launch_wide_solve(ctx, P.C, P.ld, P.R, P.m, P.d, P.ldv, P.U, P.slot, P.V, dev, S.v, S.dW);
             if (rc) return rc;
         } else if (stepped) {
             const int64_t l0 = ctx->launches;
@@ -628,7 +640,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
         S.st->pass_bytes[cls] += (double)h->pass_count * G->bytes_per_eval + vbytes;
         S.st->pass_count[cls] += (int32_t)h->pass_count;
-        if (!stepped && !small)   // kernels launched by the graph: counted from the device-side iteration counters
+        if (!stepped && !one_cta)   // kernels launched by the graph: counted from the device-side iteration counters
             ctx->launches += (int64_t)h->evals * G->k_eval + (int64_t)h->newton_total * G->k_newton +
                              (int64_t)h->cg_total * G->k_cg + (int64_t)h->outer * G->k_update;
         S.st->n_support = h->n_support;

@@ -246,3 +246,29 @@ def test_accelerated_gradient_first_outer_iterations(meb, k, m, d, mode):
     assert st["converged"] == 1 and st["ag_iters"] > 0, st
     assert abs(r - ro) <= 1e-8 * ro and np.linalg.norm(c - co) <= 1e-5 * (1 + ro)
     assert _violation(C, R, c, r) <= 1e-10 * (1 + r)
+
+
+@pytest.mark.parametrize("m,d,with_radii", [(1, 127, True), (5, 1000, True), (40, 300, False), (200, 517, True), (256, 130, False)])
+def test_cluster_solver_matches_graph_path_and_oracle(meb, m, d, with_radii):
+    """Few balls with long rows (m <= 256, d > 126) run in ONE thread-block cluster (csrc/meb_wide.cu); MEB_OPT_NO_SMALL
+    sends the same instance through the graph of grid kernels.  Same optimum, far fewer launches; oracle parity as usual."""
+    rng = np.random.default_rng(5000 + m + d)
+    C = rng.standard_normal((m, d)) * np.linspace(0.2, 2.0, d)
+    R = rng.lognormal(-2.0, 1.0, size=m) if with_radii else None
+    dC = torch.from_numpy(C).cuda()
+    dR = None if R is None else torch.from_numpy(R).cuda()
+    with meb.Context(m, d) as c1:
+        ca, ra, sta = meb.meb_solve(c1, dC, dR, 1e-8, meb.MEB_MODE_FP64)
+        ca2, ra2, sta2 = meb.meb_solve(c1, dC, dR, 1e-8, meb.MEB_MODE_FP64)
+    with meb.Context(m, d) as c2:
+        meb.meb_set_option(c2, meb.OPT["NO_SMALL"], True)
+        cb, rb, stb = meb.meb_solve(c2, dC, dR, 1e-8, meb.MEB_MODE_FP64)
+    assert sta["converged"] == 1 and stb["converged"] == 1
+    assert ra == ra2 and torch.equal(ca, ca2)                          # deterministic
+    assert abs(ra - rb) <= 1e-9 * (1 + rb) and np.linalg.norm(ca.numpy() - cb.numpy()) <= 1e-6 * (1 + rb)
+    if m > 1:
+        assert sta["kernel_launches"] < stb["kernel_launches"]
+    co, ro, _ = ripalm.meb_solve(C, R, 1e-10, "fp64", ripalm.Params(dense_d_max=4096))
+    assert abs(ra - ro) <= 1e-8 * (1 + ro)
+    assert np.linalg.norm(ca.numpy() - co) <= 1e-5 * (1 + ro)
+    assert _violation(C, R, ca.numpy(), ra) <= 1e-10 * (1 + ra)

@@ -522,41 +522,59 @@ __global__ void __launch_bounds__(MAXT, 1) tile_kernel(const StreamArgs a, const
                         else gwalk(std::false_type{});
                     } else {
                         // two entries of my group per step (chains A and B); a missing second entry repeats the
-                        // first row with lam = 0 and adds exactly zero
-                        for (int k0 = grp; k0 < nact; k0 += 2 * RP) {
-                            const int kB = k0 + RP;
-                            const bool hasB = kB < nact;
-                            const double lamA = lam_w[warp][k0];
-                            const double lamB = hasB ? lam_w[warp][kB] : 0.0;
-                            const int rA = row_w[warp][k0];
-                            const int rB = hasB ? (int)row_w[warp][kB] : rA;
-                            const int slotA = anyv ? slot_w[warp][k0] : -1;
-                            const int slotB = (anyv && hasB) ? slot_w[warp][kB] : -1;
-                            const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rA) * ldT);
-                            const V4* rpB = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rB) * ldT);
+                        // first row with lam = 0 and adds exactly zero.  FAST as above (then an entry without v_i
+                        // reads the row of zeros and the loop has no predicates).
+                        auto gwalk2 = [&](auto fast, auto withv) {
+                            constexpr bool FAST = decltype(fast)::value;
+                            constexpr bool WV = decltype(withv)::value;
+                            for (int k0 = grp; k0 < nact; k0 += 2 * RP) {
+                                const int kB = k0 + RP;
+                                const bool hasB = kB < nact;
+                                const double lamA = lam_w[warp][k0];
+                                const double lamB = hasB ? lam_w[warp][kB] : 0.0;
+                                const int rA = row_w[warp][k0];
+                                const int rB = hasB ? (int)row_w[warp][kB] : rA;
+                                const int slotA = WV ? slot_w[warp][k0] : -1;
+                                const int slotB = (WV && hasB) ? slot_w[warp][kB] : -1;
+                                const V4* rpA = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rA) * ldT);
+                                const V4* rpB = reinterpret_cast<const V4*>(stage + (size_t)(rs0 + rB) * ldT);
 #pragma unroll
-                            for (int q = 0; q < CH; ++q) {
-                                const int ch = cl + 32 * q;
-                                if (ch < nch) {
-                                    V4 vA = V4(), vB = V4();
-                                    if (anyv) { vA = load_v(slotA, ch); vB = load_v(slotB, ch); }
-                                    const V4 eA = rpA[ch];
-                                    const V4 eB = rpB[ch];
-                                    const T* ea = reinterpret_cast<const T*>(&eA);
-                                    const T* eb = reinterpret_cast<const T*>(&eB);
-                                    const T* va = reinterpret_cast<const T*>(&vA);
-                                    const T* vbq = reinterpret_cast<const T*>(&vB);
+                                for (int q = 0; q < CH; ++q) {
+                                    const int ch = cl + 32 * q;
+                                    if (FAST || ch < nch) {
+                                        V4 vA = V4(), vB = V4();
+                                        if (WV && FAST) {
+                                            const T* pa = slotA >= 0 ? Vg + (int64_t)slotA * a.ldv : reinterpret_cast<const T*>(tile_zero_row);
+                                            const T* pb = slotB >= 0 ? Vg + (int64_t)slotB * a.ldv : reinterpret_cast<const T*>(tile_zero_row);
+                                            vA = __ldg(reinterpret_cast<const V4*>(pa) + ch);
+                                            vB = __ldg(reinterpret_cast<const V4*>(pb) + ch);
+                                        } else if (WV) {
+                                            vA = load_v(slotA, ch); vB = load_v(slotB, ch);
+                                        }
+                                        const V4 eA = rpA[ch];
+                                        const V4 eB = rpB[ch];
+                                        const T* ea = reinterpret_cast<const T*>(&eA);
+                                        const T* eb = reinterpret_cast<const T*>(&eB);
+                                        const T* va = reinterpret_cast<const T*>(&vA);
+                                        const T* vbq = reinterpret_cast<const T*>(&vB);
 #pragma unroll
-                                    for (int j = 0; j < VEC; ++j) {
-                                        T bA = ea[j] - creg[q][j], bB = eb[j] - creg[q][j];
-                                        if (anyv && slotA >= 0 && ch * VEC + j < d) bA = fma(va[j], inv_sig, bA);
-                                        if (anyv && slotB >= 0 && ch * VEC + j < d) bB = fma(vbq[j], inv_sig, bB);
-                                        vacc[q][j] = fma(lamA, (double)bA, vacc[q][j]);
-                                        vaccB[q][j] = fma(lamB, (double)bB, vaccB[q][j]);
+                                        for (int j = 0; j < VEC; ++j) {
+                                            T bA = ea[j] - creg[q][j], bB = eb[j] - creg[q][j];
+                                            if (WV && FAST) { bA = fma(va[j], inv_sig, bA); bB = fma(vbq[j], inv_sig, bB); }
+                                            else if (WV) {
+                                                if (slotA >= 0 && ch * VEC + j < d) bA = fma(va[j], inv_sig, bA);
+                                                if (slotB >= 0 && ch * VEC + j < d) bB = fma(vbq[j], inv_sig, bB);
+                                            }
+                                            vacc[q][j] = fma(lamA, (double)bA, vacc[q][j]);
+                                            vaccB[q][j] = fma(lamB, (double)bB, vaccB[q][j]);
+                                        }
                                     }
                                 }
                             }
-                        }
+                        };
+                        const bool fastg = CH == 1 && !haspad && v16a && nch == (1 << lognchp);
+                        if (anyv) { if (fastg) gwalk2(std::true_type{}, std::true_type{}); else gwalk2(std::false_type{}, std::true_type{}); }
+                        else { if (fastg) gwalk2(std::true_type{}, std::false_type{}); else gwalk2(std::false_type{}, std::false_type{}); }
                     }
                     __syncwarp();                                        // the lists are rewritten by the next sub-tile
                 }

@@ -44,6 +44,8 @@ struct CgArgs {
     double* spart;                         // [3][grid] per-CTA partials: sum y, <p, Hp>, ||res||^2
     unsigned int* bar;                     // [2]: arrival counter, error flag
     int32_t rper_cap;                      // rows a CTA can be given (size of its coefficient array)
+    int32_t wcache_cap;                    // doubles of shared memory behind the coefficients: the CTA's block of W is
+                                           // copied there once per solve when it fits (every CG iteration reads it twice)
     SolverDev* S; SolverVecs v;
 };
 
@@ -125,17 +127,20 @@ __global__ void __launch_bounds__(CG_THREADS) cg_gather_kernel(const CgArgs a) {
 // all threads of the CTA call it; returns false if the watchdog fired (the caller leaves the loop)
 __device__ __forceinline__ bool grid_barrier(unsigned int* bar, unsigned int target) {
     __shared__ int ok_s;
-    __syncthreads();
+    __syncthreads();                                         // the CTA's writes happen before thread 0's release
     if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(&bar[0], 1u);
+        // arrive: release (cumulative over the CTA's writes through the barrier above); wait: acquire loads, which
+        // also drop this SM's stale L1 lines before the others read what the other CTAs wrote
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
         int ok = 1;
         long long spins = 0;
-        while (*reinterpret_cast<volatile unsigned int*>(&bar[0]) < target) {
+        for (;;) {
+            unsigned int v;
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+            if (v >= target) break;
             if (*reinterpret_cast<volatile unsigned int*>(&bar[1]) != 0u) { ok = 0; break; }
             if (++spins > 2000000000LL) { atomicExch(&bar[1], 1u); ok = 0; break; }
         }
-        __threadfence();
         ok_s = ok;
     }
     __syncthreads();
@@ -181,6 +186,17 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         return;
     }
     const int r0 = b * rper, r1 = (r0 + rper < n) ? r0 + rper : n;
+    // my block of W: in shared memory when it fits, else where the gather left it (L2)
+    const double* Wl = a.W + (size_t)r0 * dpad;
+    if (r1 > r0 && (long long)(r1 - r0) * dpad <= (long long)a.wcache_cap) {
+        double* wc = coef_s + ((a.rper_cap + 1) & ~1);
+        const double2* src = reinterpret_cast<const double2*>(Wl);      // rows start at multiples of 64 bytes
+        double2* dst = reinterpret_cast<double2*>(wc);
+        const int n2 = (r1 - r0) * (dpad / 2);
+#pragma unroll 4
+        for (int q = tid; q < n2; q += CG_THREADS) dst[q] = src[q];
+        Wl = wc;
+    }
     const int cper = ((n1d + G - 1) / G + 3) & ~3;
     const int c0 = b * cper, c1 = (c0 + cper < n1d) ? c0 + cper : n1d;
     double* zp = a.zpart + (size_t)b * dpad;
@@ -202,7 +218,7 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         if (d >= 2048) {
             // long rows (a CTA holds one or two of them): all threads on one row, four loads in flight per thread
             for (int k = r0; k < r1; ++k) {
-                const double* __restrict__ wrow = a.W + (size_t)k * dpad;
+                const double* __restrict__ wrow = Wl + (size_t)(k - r0) * dpad;
                 double y0 = 0.0, y1 = 0.0, y2 = 0.0, y3 = 0.0;
                 int j = tid;
                 for (; j + 3 * CG_THREADS < d; j += 4 * CG_THREADS) {
@@ -217,7 +233,7 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
             }
         } else {
             for (int k = r0 + warp; k < r1; k += CG_WARPS) {
-                const double* __restrict__ wrow = a.W + (size_t)k * dpad;
+                const double* __restrict__ wrow = Wl + (size_t)(k - r0) * dpad;
                 double y0 = 0.0, y1 = 0.0;
                 int j = lane;
                 for (; j + 96 < d; j += 128) {
@@ -235,14 +251,14 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         __syncthreads();
         // ---- phase B (thread per column): z_j = sum_k coef_k W[k][j], rows in index order ----
         {
-            const double* __restrict__ Wr = a.W;
+            const double* __restrict__ Wr = Wl;
             double* __restrict__ zpr = zp;
             int j = tid;
             for (; j + 3 * CG_THREADS < d; j += 4 * CG_THREADS) {     // four columns per thread and sweep: loads first
                 double z0 = 0.0, z1 = 0.0, z2 = 0.0, z3 = 0.0;
                 for (int k = r0; k < r1; ++k) {
                     const double ck = coef_s[k - r0];
-                    const double* wk = Wr + (size_t)k * dpad + j;
+                    const double* wk = Wr + (size_t)(k - r0) * dpad + j;
                     const double w0 = wk[0], w1 = wk[CG_THREADS], w2 = wk[2 * CG_THREADS], w3 = wk[3 * CG_THREADS];
                     z0 = fma(ck, w0, z0); z1 = fma(ck, w1, z1); z2 = fma(ck, w2, z2); z3 = fma(ck, w3, z3);
                 }
@@ -250,7 +266,7 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
             }
             for (; j < d; j += CG_THREADS) {
                 double z = 0.0;
-                for (int k = r0; k < r1; ++k) z = fma(coef_s[k - r0], Wr[(size_t)k * dpad + j], z);
+                for (int k = r0; k < r1; ++k) z = fma(coef_s[k - r0], Wr[(size_t)(k - r0) * dpad + j], z);
                 zpr[j] = z;
             }
         }
@@ -357,8 +373,12 @@ int meb_launch_cg(meb_ctx* ctx, const EvalCall& c, double* W, int64_t wc_cap, do
     // rows per CTA: 64 KB of W while CTAs are left, wc_cap / grid once all of them take part
     a.rper_cap = (int32_t)(65536 / ((size_t)a.dpad * 8) + 2);
     if ((wc_cap + grid - 1) / grid + 1 > a.rper_cap) a.rper_cap = (int32_t)((wc_cap + grid - 1) / grid + 1);
-    const size_t smem = ((size_t)a.dpad + 8 + (size_t)a.rper_cap + 8) * sizeof(double);
-    if (smem > 200 * 1024) return MEB_E_CAPACITY;
+    const size_t base = ((size_t)a.dpad + 8 + (size_t)a.rper_cap + 8) * sizeof(double);
+    if (base > 200 * 1024) return MEB_E_CAPACITY;
+    size_t wcache = 65536 + (size_t)a.dpad * 8;               // a CTA's block: 64 KB, rounded up to whole rows
+    if (base + wcache > 200 * 1024) wcache = 200 * 1024 - base;
+    a.wcache_cap = (int32_t)(wcache / sizeof(double));
+    const size_t smem = base + wcache;
     MEB_CUDA_OK(ctx, cudaFuncSetAttribute(cg_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ctx->launches++;
     cg_solve_kernel<<<grid, CG_THREADS, smem, ctx->stream>>>(a);

@@ -44,6 +44,8 @@ struct CgArgs {
     double* spart;                         // [3][grid] per-CTA partials: sum y, <p, Hp>, ||res||^2
     unsigned int* bar;                     // [2]: arrival counter, error flag
     int32_t rper_cap;                      // rows a CTA can be given (size of its coefficient array)
+    int32_t full_vec;                      // 1: every CTA keeps res and delta whole in shared memory and updates them
+                                           // redundantly (same order, same bits): no third barrier per iteration
     int32_t wcache_cap;                    // doubles of shared memory behind the coefficients: the CTA's block of W is
                                            // copied there once per solve when it fits (every CG iteration reads it twice)
     SolverDev* S; SolverVecs v;
@@ -172,7 +174,10 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
     const int b = blockIdx.x;
     if (b >= G) return;
     double* p_s = cg_sm;                    // p_s[0] = p_0, p_s[1 + j] = p_1[j]
-    double* coef_s = cg_sm + (dpad + 8);    // [rper_cap] coefficients of my rows
+    const bool full = a.full_vec != 0;
+    double* res_s = cg_sm + (dpad + 8);     // [dpad + 8] (full only)
+    double* del_s = res_s + (dpad + 8);     // [dpad + 8] (full only)
+    double* coef_s = cg_sm + (full ? 3 : 1) * (dpad + 8);    // [rper_cap] coefficients of my rows
     const double sigma = a.dyn->sigma_raw, tau = a.dyn->tau_eff;
     const double tos = tau / sigma;
     const double Ls = S->L;
@@ -203,6 +208,8 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
     double* sp_y = a.spart, *sp_pHp = a.spart + gridDim.x, *sp_rr = a.spart + 2 * gridDim.x;
     // start: delta = 0, res = p = -g (written by the controller), rr = ||g||^2, tolerance: S->cg_tol
     for (int j = tid; j < n1d; j += CG_THREADS) p_s[j] = a.v.p[j];
+    if (full)
+        for (int j = tid; j < n1d; j += CG_THREADS) { res_s[j] = a.v.res[j]; del_s[j] = 0.0; }
     double rr = S->cg_rr;
     const double tol = S->cg_tol;
     const int itmax = S->cg_max;
@@ -297,6 +304,26 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         for (int bb = 0; bb < G; ++bb) tot += sp_pHp[bb];
         const double alpha = rr / tot;
         double rrn = 0.0;
+        if (full) {
+            // every CTA updates the WHOLE residual and direction sum from the Hp slices the others published before
+            // the barrier above: ||res||^2 and the next p follow without another exchange
+            const double* hpv = a.v.Hp;
+#pragma unroll 4
+            for (int e = tid; e < n1d; e += CG_THREADS) {
+                del_s[e] = fma(alpha, p_s[e], del_s[e]);
+                const double rj = fma(-alpha, hpv[e], res_s[e]);
+                res_s[e] = rj;
+                rrn = fma(rj, rj, rrn);
+            }
+            const double rr_new = cta_sum(rrn, red);
+            const double beta = rr_new / rr;
+#pragma unroll 4
+            for (int e = tid; e < n1d; e += CG_THREADS) p_s[e] = fma(beta, p_s[e], res_s[e]);
+            rr = rr_new;
+            ++it;
+            __syncthreads();
+            continue;
+        }
         {
             double* __restrict__ dl = a.v.delta; double* __restrict__ rs = a.v.res; const double* __restrict__ hpv = a.v.Hp;
 #pragma unroll 4
@@ -328,6 +355,8 @@ __global__ void __launch_bounds__(CG_THREADS, 1) cg_solve_kernel(const CgArgs a)
         ++it;
         __syncthreads();
     }
+    if (full && b == 0)
+        for (int e = tid; e < n1d; e += CG_THREADS) { a.v.delta[e] = del_s[e]; a.v.res[e] = res_s[e]; }
     if (b == 0 && tid == 0) {
         S->cg_rr = rr;
         S->cg_it = it;
@@ -373,8 +402,10 @@ int meb_launch_cg(meb_ctx* ctx, const EvalCall& c, double* W, int64_t wc_cap, do
     // rows per CTA: 64 KB of W while CTAs are left, wc_cap / grid once all of them take part
     a.rper_cap = (int32_t)(65536 / ((size_t)a.dpad * 8) + 2);
     if ((wc_cap + grid - 1) / grid + 1 > a.rper_cap) a.rper_cap = (int32_t)((wc_cap + grid - 1) / grid + 1);
-    const size_t base = ((size_t)a.dpad + 8 + (size_t)a.rper_cap + 8) * sizeof(double);
+    size_t base = ((size_t)a.dpad + 8 + (size_t)a.rper_cap + 8) * sizeof(double);
     if (base > 200 * 1024) return MEB_E_CAPACITY;
+    a.full_vec = (base + 2 * ((size_t)a.dpad + 8) * sizeof(double) + 65536 <= 200 * 1024) ? 1 : 0;
+    if (a.full_vec) base += 2 * ((size_t)a.dpad + 8) * sizeof(double);
     size_t wcache = 65536 + (size_t)a.dpad * 8;               // a CTA's block: 64 KB, rounded up to whole rows
     if (base + wcache > 200 * 1024) wcache = 200 * 1024 - base;
     a.wcache_cap = (int32_t)(wcache / sizeof(double));

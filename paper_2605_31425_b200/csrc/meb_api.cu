@@ -107,7 +107,7 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     TRY_ALLOC(c->part_red, dpad * sizeof(double));
     {
         const size_t dpm = (size_t)((d_max < 128 ? d_max : 128) + 15) / 16 * 16;
-        c->part_mat_len = (size_t)c->vec_rows * (dpm * dpm + dpm);
+        c->part_mat_len = (size_t)(c->vec_rows * 3 / 2) * (dpm * dpm + dpm);      // up to three SYRK CTAs per SM
     }
     TRY_ALLOC(c->part_mat, c->part_mat_len * sizeof(double));
     TRY_ALLOC(c->count_dev, 8 * sizeof(int32_t));

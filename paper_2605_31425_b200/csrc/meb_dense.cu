@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(MEB_BLOCK) syrk_kernel(const ActiveArgs a_in, 
 //    finalize kernel reads H from the lower triangle).
 // Same three-level software pipeline of the gather, same static partition and fixed-order combination.
 template <typename T, int B>
-__global__ void __launch_bounds__(MEB_BLOCK) syrk8_kernel(const ActiveArgs a_in, double* __restrict__ part_mat) {
+__global__ void __launch_bounds__(MEB_BLOCK, B <= 4 ? 3 : 2) syrk8_kernel(const ActiveArgs a_in, double* __restrict__ part_mat) {
     constexpr int TD = 8, DP = TD * B, KS = SyrkShape<TD>::KS, RB = SyrkShape<TD>::RB;
     static_assert(RB == 4 * MEB_WARPS, "four rows per warp and tile");
     ActiveArgs a = a_in;
@@ -444,7 +444,7 @@ int meb_dense_from_records(meb_ctx* ctx, const EvalCall& c, const double* ev_sca
     const int dp = (c.d + 15) / 16 * 16;
     const size_t per = (size_t)dp * dp + dp;
     const size_t avail = ctx->part_mat_len;
-    int grid = ctx->sm_count * 2;
+    int grid = ctx->sm_count * (dp <= 32 ? 3 : 2);      // (d <= 32: the 80-register instance of syrk8, three CTAs per SM)
     if ((size_t)grid * per > avail) grid = (int)(avail / per);
     if (grid < 1) return MEB_E_CAPACITY;
     ActiveArgs a;

@@ -161,7 +161,9 @@ def test_hvp(meb, ctx, prec, m, d, ld_pad):
 
 
 @pytest.mark.parametrize("prec", [0, 1])
-@pytest.mark.parametrize("m,d", [(1000, 10), (4999, 32), (3001, 100), (600, 128), (257, 33)])
+@pytest.mark.parametrize("m,d", [(1000, 10), (4999, 32), (3001, 100), (600, 128), (257, 33),
+                                 # syrk8_kernel (d <= 48): B = 2, 4, 6 with ragged column counts, many tiles per CTA
+                                 (90_001, 16), (70_003, 27), (50_000, 48), (5, 3)])
 def test_dense_hessian(meb, ctx, prec, m, d):
     C, R, U, V, x, xbar = make_state(400 + m + d, m, d)
     if prec == 1:
@@ -176,7 +178,10 @@ def test_dense_hessian(meb, ctx, prec, m, d):
 
 
 @pytest.mark.parametrize("prec", [0, 1])
-@pytest.mark.parametrize("m,d", [(1000, 10), (3001, 100), (300, 1000), (40, 2600), (257, 33)])
+@pytest.mark.parametrize("m,d", [(1000, 10), (3001, 100), (300, 1000), (40, 2600), (257, 33),
+                                 # d <= 32: eight lanes per entry, four entries per warp and step (writev_short_kernel);
+                                 # 120,001 balls are several sweeps of the grid and a ragged last step
+                                 (4999, 32), (1203, 5), (999, 16), (120_001, 20), (3, 1)])
 def test_update_multipliers(meb, ctx, prec, m, d):
     C, R, U, V, x, xbar = make_state(500 + m + d, m, d)
     if prec == 1:

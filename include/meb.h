@@ -188,7 +188,10 @@ enum {
                             *    CUDA-event pair, meb_stats.pass_ev_*) */
     MEB_OPT_NO_SMALL = 1,  /* 1: small (reduced) problems run through the general kernels, not the single-CTA solver */
     MEB_OPT_NO_ABORT = 2,  /* 1: doomed Armijo trials are not cut short (results are bit-identical either way) */
-    MEB_OPT_NCOUNT = 3
+    MEB_OPT_NO_FUSED_SCREEN = 3,   /* 1: the screening of the mixed mode always runs as its own pass (long rows normally
+                                    * take the retain rule from the last evaluation pass of the low-precision run; same
+                                    * kept set either way) */
+    MEB_OPT_NCOUNT = 4
 };
 MEB_API int meb_set_option(meb_ctx* ctx, int option, int value);    /* MEB_E_ARG for an unknown option */
 

@@ -20,7 +20,7 @@ MEB_E_ARG, MEB_E_INPUT, MEB_E_ALLOC, MEB_E_CUDA, MEB_E_CAPACITY = -1, -2, -3, -4
 MEB_FP64, MEB_FP32 = 0, 1
 MEB_MODE_FP64, MEB_MODE_MIXED = 0, 1
 MEB_EVAL_NSCALARS = 16
-OPT = dict(STEPPED=0, NO_SMALL=1, NO_ABORT=2)
+OPT = dict(STEPPED=0, NO_SMALL=1, NO_ABORT=2, NO_FUSED_SCREEN=3)
 PASS = dict(INGEST=0, EVAL_FP64=1, EVAL_FP32=2, SCREEN=3, FEAS=4, EVAL_REDUCED=5)
 EV = dict(PSI=0, SUM_UPLUS=1, SUM_PROJ2=2, SUM_DMULT2=3, N_B1=4, N_B3=5, MAX_PFEAS=6, MAX_COMPL=7,
           MAX_DFEAS=8, SUM_RHO=9, NORM_SUM_VPLUS=10, N_ACTIVE=11)

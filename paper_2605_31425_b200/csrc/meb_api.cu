@@ -19,7 +19,7 @@ static size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 static void ctx_free_all(meb_ctx* c) {
     if (!c) return;
-    cudaFree(c->vmask); cudaFree(c->vlist); cudaFree(c->part_multi); cudaFree(c->dyn_api);
+    cudaFree(c->vmask); cudaFree(c->vlist); cudaFree(c->part_multi); cudaFree(c->dyn_api); cudaFree(c->smask);
     cudaFree(c->mask); cudaFree(c->rec_lam); cudaFree(c->rec_rho); cudaFree(c->rec_t);
     cudaFree(c->list); cudaFree(c->blocksum); cudaFree(c->part_scalar); cudaFree(c->part_vec);
     cudaFree(c->part_mat); cudaFree(c->part_red); cudaFree(c->count_dev); cudaFree(c->part_sc); cudaFree(c->small);
@@ -91,6 +91,7 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     c->h_pinned_len = 12 * (int64_t)dpad + 256;     // [0, 4 dpad + 256): read-backs; then 8 upload slots of dpad
 #define TRY_ALLOC(ptr, bytes) if (e == cudaSuccess) e = cudaMalloc((void**)&(ptr), (bytes))
     TRY_ALLOC(c->mask, nwords * sizeof(uint32_t));
+    TRY_ALLOC(c->smask, nwords * sizeof(uint32_t));
     if ((size_t)d_max * 8 > 1024) {                  // long rows (meb_long.cu): list of the balls with a multiplier row
         TRY_ALLOC(c->vmask, nwords * sizeof(uint32_t));
         TRY_ALLOC(c->vlist, ((size_t)m_max + 32) * sizeof(int32_t));
@@ -130,6 +131,7 @@ extern "C" int meb_create(meb_ctx** out, int device, void* cuda_stream, int64_t 
     c->opt[MEB_OPT_STEPPED] = getenv("MEB_NO_GRAPH") ? 1 : 0;
     c->opt[MEB_OPT_NO_SMALL] = getenv("MEB_NO_SMALL") ? 1 : 0;
     c->opt[MEB_OPT_NO_ABORT] = getenv("MEB_NO_ABORT") ? 1 : 0;
+    c->opt[MEB_OPT_NO_FUSED_SCREEN] = 0;
     c->debug = getenv("MEB_DEBUG") != nullptr;
     c->cur_class = MEB_PASS_NCLASS - 1;
     if (e == cudaSuccess) e = cudaMemsetAsync(c->count_dev, 0, 8 * sizeof(int32_t), c->stream);
@@ -182,7 +184,25 @@ static int check_problem(const meb_ctx* ctx, int64_t m, int32_t d, const void* C
 
 // one streaming launch, optionally timed with CUDA events on the context's stream.  Short aligned rows
 // go to the TMA-staged tile kernels (meb_tile.cu), everything else to the register-mapped kernels.
-enum { PATH_TILE = 0, PATH_LONG = 1, PATH_STREAM = 2 };
+// which kernel family an evaluation of this problem uses (the dispatch of timed_stream)
+int meb_eval_path(const meb_ctx* ctx, int prec, const void* C, int64_t ld, int64_t m, int32_t d) {
+    StreamArgs a;
+    memset(&a, 0, sizeof(a));
+    a.C = C; a.ld = ld; a.m = m; a.d = d; a.part_vec = ctx->part_vec;
+    if (meb_tile_applicable(OP_EVAL, prec, a)) return PATH_TILE;
+    if (ctx->vlist != nullptr && meb_long_applicable(OP_EVAL, prec, a)) return PATH_LONG;
+    return PATH_STREAM;
+}
+// the ascending list of the set bits of `mask` into idx_out[cap]; *h_count (host) = how many (MEB_E_CAPACITY if > cap)
+int meb_compact_mask(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* idx_out, int64_t cap, int64_t* h_count) {
+    int rc = meb_launch_compact_cap(ctx, mask, m, idx_out, cap, ctx->count_dev);
+    if (rc != MEB_OK) return rc;
+    MEB_CUDA_OK(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->count_dev, sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    MEB_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    const int64_t n = *(int32_t*)ctx->h_pinned;
+    if (h_count) *h_count = n;
+    return n > cap ? MEB_E_CAPACITY : MEB_OK;
+}
 static int timed_stream(meb_ctx* ctx, int op, int prec, const StreamArgs& a, double bytes, int* grid, int* path_out) {
     const bool tile = meb_tile_applicable(op, prec, a);
     const bool longk = !tile && ctx->vlist != nullptr && meb_long_applicable(op, prec, a);
@@ -272,6 +292,7 @@ int meb_eval_internal(meb_ctx* ctx, const EvalCall& c, double* out_scalars, doub
             s.vlist2[b] = c.gs->vlist2[b]; s.vcount2[b] = c.gs->vcount2[b];
         }
         any_mult = true;
+        s.smask = ctx->smask;                    // written only while MebDyn::screen_on (low-precision run of a mixed solve)
         if (c.gs->multi > 0 && (c.gs->v || c.gs->dir)) {
             s.multi = c.gs->multi; s.dir = c.gs->dir ? c.gs->dir : c.gs->v->dir_raw; s.multi_part = ctx->part_multi;
         }

@@ -43,7 +43,9 @@ struct SolverDev {
     cudaGraphConditionalHandle h_while, h_newton, h_update, h_cg;
     cudaGraphConditionalHandle h_cgp;   // matrix-free Newton solve in one persistent kernel (meb_cg.cu)
     long long wc_cap;                   // active rows the gathered matrix W of that kernel can hold
-    int32_t cg_mode, pad_cg;            // 1: persistent kernel, 0: one launch per CG iteration (more active rows than W holds)
+    int32_t cg_mode;                    // 1: persistent kernel, 0: one launch per CG iteration (more active rows than W holds)
+    int32_t screen_valid;               // 1: the last evaluation pass ran at the current x (its fused screening mask is the
+                                        // retain rule at x); cleared by every pass at another point and by a fall-back to xbest
     double tol_accept, best_kkt, best_terms[5];   // best outer iterate so far (reading 18)
     double abort_margin;          // relative slack of MebDyn::s0_abort (rounding of the partial sums); 0: early stop off
     int32_t aborted, pad3;        // Armijo trials cut short
@@ -219,6 +221,7 @@ __device__ inline void ctrl_after_eval(SolverDev* Sg, SolverDev* S, const Solver
 }
 __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, const double* ev_s, double* sm) {
     __syncthreads();
+    if (threadIdx.x == 0) S->screen_valid = 0;              // (set below if this pass becomes the evaluation at x)
     double* __restrict__ xn_ = v.xn;
     double* __restrict__ xbar_ = v.xbar;
     double* __restrict__ ab_ = v.ab;
@@ -381,6 +384,7 @@ __device__ inline void ctrl_after_eval_body(SolverDev* S, const SolverVecs v, co
     if (agmode && phase == PH_AG_X) dotr = ctrl_block_sum(dotr, sm);        // (touches sm[0..31] only)
     if (threadIdx.x == 0) {
         sm[97] = 0.0;                                   // AG continuation: 0 none, 1 step from y = x, 2 extrapolate (sm[98] = beta)
+        S->screen_valid = 1;                            // the pass ran at what is now x
         S->evals++;
         S->psi_cur = psi_t;
         double terms[5];
@@ -563,7 +567,7 @@ __device__ inline void meb_ctrl_after_update_dev(SolverDev* S, const SolverVecs 
         if (improved) { S->best_kkt = kkt; for (int i = 0; i < 5; ++i) S->best_terms[i] = S->terms[i]; }
         if (status != ST_RUNNING) {
             S->done = 1; S->status = status;
-            if (take_best) { S->kkt = S->best_kkt; for (int i = 0; i < 5; ++i) S->terms[i] = S->best_terms[i]; }
+            if (take_best) { S->screen_valid = 0; S->kkt = S->best_kkt; for (int i = 0; i < 5; ++i) S->terms[i] = S->best_terms[i]; }
         } else {
             const double s2 = fmin(S->sigma_max, S->kappa * sg);
             S->sigma = s2;

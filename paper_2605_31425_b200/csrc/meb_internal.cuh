@@ -42,6 +42,7 @@ struct meb_ctx {
     uint32_t* vmask;        // [ceil(m/32)] scratch: balls with a multiplier row (meb_build_vlist)
     int32_t* vlist;         // [m] ascending list of the balls with a multiplier row, per-primitive calls (long rows)
     double* part_multi;     // [MEB_MAX_GRID * MEB_MULTI_MAX] per-CTA partials of the predicted step sizes
+    uint32_t* smask;        // bit mask of the fused screening (same size as mask)
     double* rec_lam;        // [m] lam_i of active balls (dense-indexed, sparse writes)
     double* rec_rho;        // [m] rho_i = a/nb (2.0 marks B1)
     double* rec_t;          // [m] t_i of active balls
@@ -153,11 +154,16 @@ struct MebDyn {
     // Multi-trial Armijo (DESIGN reading 19): a trial pass at x_t = x + eta Delta also forms
     // sum_i ||Pi(z_i)||^2 at the multi_n further points x_t - gamma_k Delta (gamma_k = eta (1 - 2^-k): the next
     // halvings of eta) from ||b_i||^2, <b_i, Delta c> and ||Delta c||^2 -- no extra bytes.  0: not a trial pass.
-    int32_t multi_n, pad_multi;
+    int32_t multi_n;
+    // Screening fused into the evaluation passes of the low-precision run: with screen_on the pass also
+    // sets, in StreamArgs::smask, the bit of every ball with r - r_i - ||c - c_i|| <= screen_factor * r -- the
+    // retain rule at the point it evaluates; after the last accepted evaluation that is the rule at (r_hat, c_hat).
+    int32_t screen_on;
     double multi_gamma[MEB_MULTI_MAX];
     double dir_r;           // Delta r (raw units)
     double dir_c2;          // ||Delta c||^2 (raw units)
     double dir_c;           // ||Delta c||
+    double screen_factor;   // tol_red / r_hat (meb_params.tol_red_factor)
 };
 
 // host-side launch helpers implemented in the .cu files -------------------------------------------
@@ -190,6 +196,7 @@ struct StreamArgs {
     // multi-trial Armijo: direction Delta (device, (d+1), raw units), host-side switch (0: kernel without it),
     // per-CTA partials [grid][MEB_MULTI_MAX]
     const double* dir; int32_t multi; double* multi_part;
+    uint32_t* smask;             // nullable: bit mask of the fused screening (MebDyn::screen_on), [ceil(m / 32)]
 };
 
 // resolves the device-resident parameters of a solve graph into the plain fields
@@ -356,6 +363,9 @@ void meb_free_graph_cache(meb_ctx* ctx);
 size_t meb_solver_dev_size();
 
 // ---- single-CTA solver of small problems (meb_smallsolve.cu) ----
+enum { PATH_TILE = 0, PATH_LONG = 1, PATH_STREAM = 2 };
+int meb_eval_path(const meb_ctx* ctx, int prec, const void* C, int64_t ld, int64_t m, int32_t d);
+int meb_compact_mask(meb_ctx* ctx, const uint32_t* mask, int64_t m, int32_t* idx_out, int64_t cap, int64_t* h_count);
 bool meb_wide_applicable(int prec, int64_t m, int32_t d);
 int meb_launch_wide_solve(meb_ctx* ctx, const void* C, int64_t ld, const void* R, int64_t m, int32_t d, int64_t ldv,
                           void* const U2[2], int32_t* const slot2[2], void* const V2[2], SolverDev* S,

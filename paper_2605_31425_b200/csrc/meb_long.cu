@@ -121,6 +121,8 @@ __global__ void __launch_bounds__(LONG_THREADS, 1) long_kernel(const StreamArgs 
 
     const T r = (OP == OP_INGEST) ? T(0) : (T)a.x[0];
     const T sig = (T)sigma_d;
+    const bool screen_on = OP == OP_EVAL && a.smask != nullptr && a.dyn != nullptr && a.dyn->screen_on != 0;
+    const T screen_eps = screen_on ? (T)(a.dyn->screen_factor * a.x[0]) : T(0);
     Acc acc;
     MultiAcc<MULTI> macc;
     const V4* cs4 = reinterpret_cast<const V4*>(cs);
@@ -172,6 +174,10 @@ __global__ void __launch_bounds__(LONG_THREADS, 1) long_kernel(const StreamArgs 
             double mylam;
             const bool flag = row_epilogue_core<T, OP>(a, my_row, true, false, my_nb2, my_f0, T(0), T(0), r, sig, ri, ui, acc, mylam);
             if (OP != OP_INGEST && flag) atomicOr(&a.mask[my_row >> 5], 1u << (my_row & 31));
+            if (OP == OP_EVAL && screen_on) {                           // fused screening, as OP_SCREEN
+                const T sslack = (r - ri) - t_sqrt<T>(my_nb2);
+                if (sslack <= screen_eps) atomicOr(&a.smask[my_row >> 5], 1u << (my_row & 31));
+            }
             if (MULTI) multi_row<T>(macc, a, cfg.multi, my_nb2, my_p0, r, sig, ri, ui);
         }
         q = 0;
@@ -380,6 +386,10 @@ __global__ void __launch_bounds__(MEB_BLOCK) vrow_kernel(const StreamArgs a_in, 
             double mylam;
             const bool flag = row_epilogue_core<T, OP_EVAL>(a, row, true, true, nb2, ne2, evd, vv, r, sig, ri, ui, acc, mylam);
             if (flag) atomicOr(&a.mask[row >> 5], 1u << (row & 31));
+            if (a.smask != nullptr && a.dyn != nullptr && a.dyn->screen_on != 0) {      // fused screening: ||c_i - c||^2 = ne2
+                const T sslack = (r - ri) - t_sqrt<T>(ne2);
+                if (sslack <= (T)(a.dyn->screen_factor * a.x[0])) atomicOr(&a.smask[row >> 5], 1u << (row & 31));
+            }
             if (MULTI) multi_row<T>(macc, a, multi, nb2, p0, r, sig, ri, ui);
         }
     }
@@ -497,6 +507,8 @@ int meb_launch_long(meb_ctx* ctx, int phase, int op, int prec, const StreamArgs&
         if (op != OP_INGEST) {
             const size_t nwords = (size_t)(a.m + 31) / 32;
             cudaError_t e = cudaMemsetAsync(a.mask, 0, nwords * sizeof(uint32_t), ctx->stream);
+            if (e == cudaSuccess && op == OP_EVAL && a.smask != nullptr)
+                e = cudaMemsetAsync(a.smask, 0, nwords * sizeof(uint32_t), ctx->stream);    // (screening flags are OR-ed in too)
             if (e != cudaSuccess) { ctx->last_cuda_error = (int)e; return MEB_E_CUDA; }
         }
         return MEB_OK;

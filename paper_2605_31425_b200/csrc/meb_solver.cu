@@ -70,6 +70,8 @@ struct Solver {
     meb_ctx* ctx; meb_params par; meb_stats* st;
     double sigma_start;            // sigma_0 of the next phase (normalised units)
     double sigma_end;              // sigma reached by the last phase
+    bool screen_arm;               // the phase about to run fuses the screening into its evaluation passes
+    bool screen_valid;             // ... and its last pass ran at the iterate it returned
     int32_t d; double L;
     double* dH;                    // device (d+1)^2: dense Newton system
     double* dW; int64_t wc_cap;    // device [wc_cap][dpad] gathered active rows of the matrix-free Newton solve, then
@@ -561,6 +563,8 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
             h->pred_margin = (P.prec == MEB_FP32) ? 1e-3 : 1e-6;
             h->m_rows = (ctx->shard && P.full) ? ctx->shard->m_global : P.m;      // (counts in v.ev are global in a sharded solve)
             h->lowprec = (P.prec == MEB_FP32 && P.full) ? 1 : 0;
+            h->dyn.screen_on = (S.screen_arm && !one_cta) ? 1 : 0;
+            h->dyn.screen_factor = par.tol_red_factor;
             h->multi_max = one_cta ? 0 : multi_of(par, P);
             h->ag_outer = (par.ag_outer > 0 && !one_cta) ? par.ag_outer : 0;
             h->ag_inner_max = 500;
@@ -635,6 +639,7 @@ int ripalm(Solver& S, Problem& P, std::vector<double>& xn, std::vector<double>& 
         const double vbytes = (double)h->vrow_reads * (double)S.d * (double)esz(P.prec);   // V rows of balls with u_i > 0
         S.bytes += (double)(h->evals - h->aborted) * G->bytes_per_eval + vbytes;
         S.st->passes_cut += h->aborted;
+        S.screen_valid = h->dyn.screen_on != 0 && h->screen_valid != 0 && h->status != ST_NEED_CAPACITY;
         S.st->trials_skipped += h->skipped;
         S.st->ag_iters += h->ag_total;
         S.st->pass_ms[cls] += (double)h->pass_ns * 1e-6;
@@ -757,6 +762,7 @@ int solve_impl(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_
     memset(st, 0, sizeof(*st));
     Solver S;
     S.ctx = ctx; S.st = st; S.d = d; S.bytes = 0.0; S.sigma_start = 0.0; S.sigma_end = 0.0;
+    S.screen_arm = false; S.screen_valid = false;
     if (h_params) S.par = *h_params; else meb_default_params(&S.par);
     if (!(S.par.rho >= 0.0 && S.par.rho < 1.0) || !(S.par.sigma0 > 0.0) || !(S.par.tau > 0.0) ||
         !(S.par.kappa >= 1.0) || S.par.sample_rows < 1)
@@ -874,6 +880,12 @@ int solve_impl(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_
             if (rc) break;
             bool conv1 = false;
             double kkt1, terms1[5];
+            // long rows (meb_long.cu): the evaluation passes of this run also apply the retain rule of the screening at
+            // the point they evaluate, which saves the screening pass (8 GB on config 5) when the run ends at the point
+            // of its last pass.  Short rows keep the separate pass: it is 1-2 % of their solve and the extra per-row work
+            // in the instruction-bound tile kernel would cost as much.
+            S.screen_arm = !ctx->shard && !ctx->opt[MEB_OPT_NO_FUSED_SCREEN] && meb_eval_path(ctx, MEB_FP32, C32, ld32, m, d) == PATH_LONG;
+            S.screen_valid = false;
             rc = ripalm(S, P1, xn, ab, S.par.tol_lo, S.par.tol_lo, &conv1, &kkt1, terms1,
                         S.par.outer_max_lo > 0 ? S.par.outer_max_lo : S.par.outer_max);
             if (rc) break;
@@ -888,11 +900,18 @@ int solve_impl(meb_ctx* ctx, int64_t m, int32_t d, const double* centers, int64_
             rc = upload(ctx, S.v.xt, xs.data(), n);
             if (rc) break;
             int64_t nred = 0;
-            rc = meb_screen_compact(ctx, m, d, C32, ld32, R32, (float)xs[0], S.v.xt + 1,
-                                    (float)(S.par.tol_red_factor * xs[0]), idx, m, &nred, nullptr, 0);
-            if (rc) break;
-            st->passes_fp32_full++;
-            S.bytes += ctx->last_pass_bytes;
+            S.screen_arm = false;
+            if (S.screen_valid) {
+                // the last pass of the low-precision run evaluated at (r_hat, c_hat): its mask IS the screening
+                rc = meb_compact_mask(ctx, ctx->smask, m, idx, m, &nred);
+                if (rc) break;
+            } else {
+                rc = meb_screen_compact(ctx, m, d, C32, ld32, R32, (float)xs[0], S.v.xt + 1,
+                                        (float)(S.par.tol_red_factor * xs[0]), idx, m, &nred, nullptr, 0);
+                if (rc) break;
+                st->passes_fp32_full++;
+                S.bytes += ctx->last_pass_bytes;
+            }
             Problem P2;
             memset(&P2, 0, sizeof(P2));
             P2.prec = MEB_FP64; P2.d = d; P2.off = c0.data(); P2.full = false;

@@ -272,3 +272,22 @@ def test_cluster_solver_matches_graph_path_and_oracle(meb, m, d, with_radii):
     assert abs(ra - ro) <= 1e-8 * (1 + ro)
     assert np.linalg.norm(ca.numpy() - co) <= 1e-5 * (1 + ro)
     assert _violation(C, R, ca.numpy(), ra) <= 1e-10 * (1 + ra)
+
+
+@pytest.mark.parametrize("k,m,d", [(3, 20_000, 1000), (5, 3_000, 4000)])
+def test_fused_screening_keeps_the_same_balls(meb, k, m, d):
+    """Long rows: the retain rule of the screening is applied by the LAST evaluation pass of the low-precision
+    run instead of a pass of its own.  Same arithmetic on the same point: the kept set, and with it every later iterate,
+    is bit-identical; one FP32 pass fewer."""
+    C, R = workloads.config(k, m, d)[:2]
+    dC, dR = torch.from_numpy(C).cuda(), torch.from_numpy(R).cuda()
+    out = []
+    for off in (False, True):
+        with meb.Context(m, d) as ctx:
+            meb.meb_set_option(ctx, meb.OPT["NO_FUSED_SCREEN"], off)
+            out.append(meb.meb_solve(ctx, dC, dR, 1e-8, meb.MEB_MODE_MIXED))
+    (ca, ra, sa), (cb, rb, sb) = out
+    assert sa["converged"] == 1 and sb["converged"] == 1
+    assert sa["n_reduced"] == sb["n_reduced"] and ra == rb and torch.equal(ca, cb)
+    assert sa["passes_fp32_full"] == sb["passes_fp32_full"] - 1
+    assert sa["pass_count"][meb.PASS["SCREEN"]] == 0 and sb["pass_count"][meb.PASS["SCREEN"]] == 1

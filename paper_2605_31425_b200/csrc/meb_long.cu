@@ -121,8 +121,6 @@ __global__ void __launch_bounds__(LONG_THREADS, 1) long_kernel(const StreamArgs 
 
     const T r = (OP == OP_INGEST) ? T(0) : (T)a.x[0];
     const T sig = (T)sigma_d;
-    const bool screen_on = OP == OP_EVAL && a.smask != nullptr && a.dyn != nullptr && a.dyn->screen_on != 0;
-    const T screen_eps = screen_on ? (T)(a.dyn->screen_factor * a.x[0]) : T(0);
     Acc acc;
     MultiAcc<MULTI> macc;
     const V4* cs4 = reinterpret_cast<const V4*>(cs);
@@ -174,9 +172,11 @@ __global__ void __launch_bounds__(LONG_THREADS, 1) long_kernel(const StreamArgs 
             double mylam;
             const bool flag = row_epilogue_core<T, OP>(a, my_row, true, false, my_nb2, my_f0, T(0), T(0), r, sig, ri, ui, acc, mylam);
             if (OP != OP_INGEST && flag) atomicOr(&a.mask[my_row >> 5], 1u << (my_row & 31));
-            if (OP == OP_EVAL && screen_on) {                           // fused screening, as OP_SCREEN
+            if (OP == OP_EVAL && a.smask != nullptr && a.dyn != nullptr && a.dyn->screen_on != 0) {
+                // fused screening, the arithmetic of OP_SCREEN (the switch and the threshold are re-read
+                // here, once per batch of rows, rather than kept in registers across the streaming loop)
                 const T sslack = (r - ri) - t_sqrt<T>(my_nb2);
-                if (sslack <= screen_eps) atomicOr(&a.smask[my_row >> 5], 1u << (my_row & 31));
+                if (sslack <= (T)(a.dyn->screen_factor * a.x[0])) atomicOr(&a.smask[my_row >> 5], 1u << (my_row & 31));
             }
             if (MULTI) multi_row<T>(macc, a, cfg.multi, my_nb2, my_p0, r, sig, ri, ui);
         }

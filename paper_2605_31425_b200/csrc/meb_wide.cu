@@ -495,9 +495,29 @@ size_t wide_smem_bytes(int m, int d) {
 
 }  // namespace
 
-// FP64 problems with at most 256 balls and rows too long for the dense Newton path: one cluster runs the phase.
+// FP64 problems with at most 256 balls and rows too long for the dense Newton path: one cluster runs the phase --
+// if the device can place such a cluster at all (asked once per shape class; a partitioned or busy GPU may not).
 bool meb_wide_applicable(int prec, int64_t m, int32_t d) {
-    return prec == MEB_FP64 && m >= 1 && m <= WD_M_MAX && d > 126 && wide_smem_bytes((int)m, d) <= 200 * 1024;
+    if (!(prec == MEB_FP64 && m >= 1 && m <= WD_M_MAX && d > 126)) return false;
+    const size_t smem = wide_smem_bytes((int)m, d);
+    if (smem > 200 * 1024) return false;
+    if (cudaFuncSetAttribute(wide_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(WD_NC, 1, 1);
+    cfg.blockDim = dim3(WD_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = WD_NC; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int nclusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&nclusters, wide_solve_kernel, &cfg) != cudaSuccess) { cudaGetLastError(); return false; }
+    return nclusters >= 1;
 }
 
 // W: device buffer of at least m * dpad doubles (dpad = d rounded up to 8).  V pools must hold m rows each.

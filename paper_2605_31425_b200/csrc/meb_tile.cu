@@ -788,7 +788,9 @@ int launch_cfg(meb_ctx* ctx, KernelT kernel512, KernelT kernel384, const StreamA
 
 int lanes_per_row(const StreamArgs& a, size_t esize) {
     const size_t rb = (size_t)a.ld * esize;
-    return rb <= (getenv("MEB_G1MAX") ? (size_t)atoi(getenv("MEB_G1MAX")) : 256) ? 1 : (rb <= 416 ? 2 : 4);              // sub-tile of at most ~8 KB
+    // sub-tile of at most ~8 KB.  (Two lanes per row for 256-byte rows, i.e. stages of 4 KB, were measured on config 4:
+    // the pass slows from 0.60 to 0.90 ms -- the kernel is bound by per-stage instruction overhead.)
+    return rb <= 256 ? 1 : (rb <= 416 ? 2 : 4);
 }
 
 // G is fixed by the row length; CH = 2 only occurs with G = 4 (rows longer than 512 bytes)
